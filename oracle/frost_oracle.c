@@ -1,0 +1,494 @@
+/*
+ * frost_oracle.c -- the CPU ORACLE for the HHS-FSI hot path.  TEST INFRASTRUCTURE ONLY.
+ *
+ * This file is a plain, slow, obviously-correct restatement of what the paper
+ * (Rantala, Naab & Springel, "FROST", arXiv 2011.14984; /root/reference/PAPER.md) says the hot
+ * path computes.  It exists so that the CUDA library can be checked element by element, and so
+ * that bench.py can time "the oracle as it stands" as the cpu_baseline.  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may call it.  It
+ * shares NO code, header, table or constant with paper_2011_14984_b200/csrc/ and neither side
+ * includes the other.
+ *
+ * Style: one loop nest per definition, in the paper's order and notation; no blocking, fusion
+ * or reordering.  Sums over pairs are accumulated in `long double` (x87 80-bit on x86-64) with
+ * j ascending and rounded to double once at the end, so that the oracle's own rounding error
+ * (~1e-19 relative per term) is far below the 1e-12 / 1e-10 parity tolerances.  The time-step
+ * criterion, kick and drift are computed in plain double, because the method itself is an fp64
+ * method and the slow/fast decision tau_i >= tau_pivot must be taken in that precision on both
+ * sides.  Compile with -ffp-contract=off (oracle/build.py does) so no FMA contraction happens.
+ * OpenMP parallelises over sinks only: each sink's sum is sequential, so results do not depend
+ * on the number of threads.
+ *
+ * Pins (tests/test_oracle_pins.py; every function below is pinned unless it says otherwise):
+ *   O1 oracle_forces ACC   : autograd / finite differences of U (Eq. 23), two-body closed form,
+ *                            sum m a = 0, Plummer mean field (Eq. A2).
+ *   O2 oracle_forces GRAD  : autograd / finite differences of G_P = -sum m |a|^2 (Eq. 17, 39),
+ *                            two-body closed form g = 4 G (m1+m2) r^-3 a (Eq. 25-26), sum m g = 0.
+ *   O3 oracle_timesteps    : circular binary tau = eta P / 2 pi (Eq. 52), s(q) values and
+ *                            symmetries (Eq. 49, Fig. 2), brute-force scalar re-evaluation.
+ *                            The choice "eta inside q" (reading 9) is PARITY UNPINNED:
+ *                            nothing the paper prints separates it from "q without eta".
+ *                            Softened time-steps (reading 14) are PARITY UNPINNED.
+ *   O5 oracle_fsi_step     : 4th-order convergence against the Kepler closed form, time reversal.
+ *   O6 oracle_hhs_step     : 4th-order convergence with a frozen partition on a star+planets
+ *                            system, momentum at roundoff, five-body Solar system (Tables A1/A2).
+ *   O7 oracle_diagnostics  : textbook definitions (Eq. 23); used by the pins.
+ *
+ * Array convention (same as include/frost.h, restated independently): positions, velocities,
+ * accelerations are three SoA planes, component c of particle i at p[c*ld + i]; index arrays
+ * are int32, NULL means "all particles 0..n-1".
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORACLE_ACC 1
+#define ORACLE_GRAD 2
+#define ORACLE_MUTUAL 4
+
+#define ORACLE_OK 0
+#define ORACLE_EINVAL (-1)
+#define ORACLE_ENOMEM (-3)
+#define ORACLE_EDEPTH (-4)
+
+#define ORACLE_MAX_LEVELS 64
+
+typedef long double ld_t;
+
+typedef struct {
+    int32_t depth;                          /* deepest level entered with a non-empty set */
+    int32_t reserved;
+    int64_t entries[ORACLE_MAX_LEVELS];     /* non-empty entries of hhs_fsi at level k */
+    int64_t n_slow[ORACLE_MAX_LEVELS];      /* sum of |S| over those entries */
+    int64_t n_fast[ORACLE_MAX_LEVELS];      /* sum of |F| over those entries */
+    int64_t pairs_newton;                   /* ordered pairs swept by Eq. 24 / 42 */
+    int64_t pairs_gradient;                 /* ordered pairs swept by Eq. 27 / 43 / 44 */
+    int64_t pairs_timestep;                 /* ordered pairs swept by Eq. 49-54 */
+} oracle_hhs_stats;
+
+int oracle_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void oracle_set_num_threads(int t) {
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+
+static inline int pick(const int32_t *idx, int k) { return idx ? idx[k] : k; }
+
+/* ---------------------------------------------------------------------------------------------
+ * O1.  Newtonian acceleration, Eq. (24) PAPER.md:216-219 (self) and Eq. (42)
+ * (inter-level), with the Plummer-softening substitution r -> (r^2+eps_p^2)^(1/2) of PAPER.md:250:
+ *     a_i = G * sum_{j in J, s_ij^2 > 0} m_j x_ji / s_ij^3,   x_ji = x_j - x_i,
+ *     s_ij^2 = |x_ji|^2 + eps2.
+ * "j != i" is expressed as s_ij^2 > 0 (reading 11).
+ * ------------------------------------------------------------------------------------------- */
+static void newton_one_direction(int ld, const double *pos, const double *mass,
+                                 const int32_t *I, int nI, const int32_t *J, int nJ,
+                                 double G, double eps2, double *acc) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < nI; ++a) {
+        const int i = pick(I, a);
+        const ld_t xi = pos[i], yi = pos[ld + i], zi = pos[2 * ld + i];
+        ld_t ax = 0, ay = 0, az = 0;
+        for (int b = 0; b < nJ; ++b) {
+            const int j = pick(J, b);
+            const ld_t dx = (ld_t)pos[j] - xi;
+            const ld_t dy = (ld_t)pos[ld + j] - yi;
+            const ld_t dz = (ld_t)pos[2 * ld + j] - zi;
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) {
+                const ld_t s = sqrtl(s2);
+                const ld_t w = (ld_t)mass[j] / (s2 * s);
+                ax += w * dx;
+                ay += w * dy;
+                az += w * dz;
+            }
+        }
+        acc[i] = (double)((ld_t)G * ax);
+        acc[ld + i] = (double)((ld_t)G * ay);
+        acc[2 * ld + i] = (double)((ld_t)G * az);
+    }
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O2.  Gradient acceleration, Eq. (27) PAPER.md:234-239 (self) and Eq. (43)-(44)
+ * PAPER.md:373-387 (inter-level):
+ *     g_i = 2 G * sum_{j in J, s>0} m_j / s^5 * ( s^2 a_ji - 3 (x_ji . a_ji) x_ji ),
+ *     a_ji = a_j - a_i,  x_ji = x_j - x_i.
+ * `acc` must hold, for every i in I and j in J, the acceleration generated by the same pair set
+ * (reading O2).  The prefactor 2 is the one printed in Eq. (27); Eq. (28)'s G eps^2/24
+ * is 2/48.
+ * ------------------------------------------------------------------------------------------- */
+static void gradient_one_direction(int ld, const double *pos, const double *mass,
+                                   const int32_t *I, int nI, const int32_t *J, int nJ,
+                                   double G, double eps2, const double *acc, double *grad) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < nI; ++a) {
+        const int i = pick(I, a);
+        const ld_t xi = pos[i], yi = pos[ld + i], zi = pos[2 * ld + i];
+        const ld_t axi = acc[i], ayi = acc[ld + i], azi = acc[2 * ld + i];
+        ld_t gx = 0, gy = 0, gz = 0;
+        for (int b = 0; b < nJ; ++b) {
+            const int j = pick(J, b);
+            const ld_t dx = (ld_t)pos[j] - xi;
+            const ld_t dy = (ld_t)pos[ld + j] - yi;
+            const ld_t dz = (ld_t)pos[2 * ld + j] - zi;
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) {
+                const ld_t dax = (ld_t)acc[j] - axi;
+                const ld_t day = (ld_t)acc[ld + j] - ayi;
+                const ld_t daz = (ld_t)acc[2 * ld + j] - azi;
+                const ld_t s = sqrtl(s2);
+                const ld_t s5 = s2 * s2 * s;
+                const ld_t xa = dx * dax + dy * day + dz * daz;
+                const ld_t w = (ld_t)mass[j] / s5;
+                gx += w * (s2 * dax - 3 * xa * dx);
+                gy += w * (s2 * day - 3 * xa * dy);
+                gz += w * (s2 * daz - 3 * xa * dz);
+            }
+        }
+        grad[i] = (double)(2 * (ld_t)G * gx);
+        grad[ld + i] = (double)(2 * (ld_t)G * gy);
+        grad[2 * ld + i] = (double)(2 * (ld_t)G * gz);
+    }
+}
+
+/* compute_acc_newton / compute_acc_gradient (Alg. 2) when I == J; one direction of
+ * acc_sf_newton / acc_sf_gradient (Alg. 3) when I != J; both directions under
+ * ORACLE_MUTUAL.  Entries of acc/grad outside I (and J under MUTUAL) are not touched. */
+int oracle_forces(int n, int ld, const double *pos, const double *mass,
+                  const int32_t *sink_idx, int n_sink, const int32_t *source_idx, int n_source,
+                  double G, double eps2, double *acc, double *grad, int flags) {
+    if (n < 0 || ld < n || !pos || !mass || !acc) return ORACLE_EINVAL;
+    if (!sink_idx) n_sink = n;
+    if (!source_idx) n_source = n;
+    if ((flags & ORACLE_GRAD) && !grad) return ORACLE_EINVAL;
+    if (flags & ORACLE_ACC) {
+        newton_one_direction(ld, pos, mass, sink_idx, n_sink, source_idx, n_source, G, eps2, acc);
+        if (flags & ORACLE_MUTUAL)
+            newton_one_direction(ld, pos, mass, source_idx, n_source, sink_idx, n_sink, G, eps2, acc);
+    }
+    if (flags & ORACLE_GRAD) {
+        gradient_one_direction(ld, pos, mass, sink_idx, n_sink, source_idx, n_source, G, eps2, acc, grad);
+        if (flags & ORACLE_MUTUAL)
+            gradient_one_direction(ld, pos, mass, source_idx, n_source, sink_idx, n_sink, G, eps2, acc, grad);
+    }
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O3.  Symmetrised free-fall / fly-by time-steps, Eq. (49)-(54) PAPER.md:429-474, over the
+ * particles of ONE hierarchy level: sinks = sources = idx.
+ * ------------------------------------------------------------------------------------------- */
+
+/* Harmonic symmetrisation factor of Eq. (49), PAPER.md:431:
+ *     s(q) = [ q + sqrt(1+q^2) - 1 ] / q ,   q = d tau / dt,
+ * written in the algebraically identical form 1 + q / (1 + sqrt(1+q^2)) which has no 0/0 at q=0
+ * and no cancellation (reading 10). */
+double oracle_sym_factor(double q) { return 1.0 + q / (1.0 + sqrt(1.0 + q * q)); }
+
+/* The symmetrised step candidates of one ordered pair (i <- j).  out[0] = free-fall candidate,
+ * out[1] = fly-by candidate (+inf if the pair gives none).  r = x_j - x_i, v = v_j - v_i. */
+void oracle_pair_timestep(const double xi[3], const double vi[3], double mi,
+                          const double xj[3], const double vj[3], double mj,
+                          double G, double eta_ff, double eta_fb, int eta_in_q, double out[2]) {
+    const double rx = xj[0] - xi[0], ry = xj[1] - xi[1], rz = xj[2] - xi[2];
+    const double vx = vj[0] - vi[0], vy = vj[1] - vi[1], vz = vj[2] - vi[2];
+    const double r2 = rx * rx + ry * ry + rz * rz;
+    const double v2 = vx * vx + vy * vy + vz * vz;
+    out[0] = INFINITY;
+    out[1] = INFINITY;
+    if (!(r2 > 0.0)) return;                    /* coincident pair / self: ignored (reading 11) */
+    const double r = sqrt(r2);
+    const double mu = G * (mi + mj);
+    const double rv = rx * vx + ry * vy + rz * vz;
+    /* Eq. (50): t_ff = ( r^3 / (G (m_i+m_j)) )^(1/2) */
+    const double t_ff = sqrt(r2 * r / mu);
+    /* Eq. (53): d t_ff/dt = (3/2) (r.v)/r^2 t_ff */
+    const double dt_ff = 1.5 * (rv / r2) * t_ff;
+    const double q_ff = eta_in_q ? eta_ff * dt_ff : dt_ff;
+    out[0] = oracle_sym_factor(q_ff) * (eta_ff * t_ff);
+    if (v2 > 0.0) {                             /* v = 0: no fly-by candidate (reading 11) */
+        /* Eq. (51): t_fb = r / v */
+        const double t_fb = r / sqrt(v2);
+        /* Eq. (54), two-body approximation: d t_fb/dt = (r.v)/r^2 [ 1 + G(m_i+m_j)/(v^2 r) ] t_fb */
+        const double dt_fb = (rv / r2) * (1.0 + mu / (v2 * r)) * t_fb;
+        const double q_fb = eta_in_q ? eta_fb * dt_fb : dt_fb;
+        out[1] = oracle_sym_factor(q_fb) * (eta_fb * t_fb);
+    }
+}
+
+/* bin = smallest k >= 0 with tau_pivot * 2^-k <= tau (include/frost.h restates this). */
+static int32_t bin_of(double tau, double tau_pivot) {
+    int32_t k = 0;
+    double p = tau_pivot;
+    if (!(tau > 0.0)) return 2000;
+    while (p > tau && k < 2000) {
+        p *= 0.5;
+        ++k;
+    }
+    return k;
+}
+
+/* assign_timesteps: tau_i = min_j min( tau_ff_sym, tau_fb_sym ).
+ * A level with a single particle gets tau = +inf. */
+int oracle_timesteps(int n, int ld, const double *pos, const double *vel, const double *mass,
+                     const int32_t *idx, int n_idx, double G, double eta_ff, double eta_fb,
+                     int eta_in_q, double tau_pivot, double *out_tau, int32_t *out_bin) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !out_tau) return ORACLE_EINVAL;
+    if (!idx) n_idx = n;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < n_idx; ++a) {
+        const int i = pick(idx, a);
+        const double xi[3] = {pos[i], pos[ld + i], pos[2 * ld + i]};
+        const double vi[3] = {vel[i], vel[ld + i], vel[2 * ld + i]};
+        double tau = INFINITY;
+        for (int b = 0; b < n_idx; ++b) {
+            const int j = pick(idx, b);
+            if (j == i) continue;
+            const double xj[3] = {pos[j], pos[ld + j], pos[2 * ld + j]};
+            const double vj[3] = {vel[j], vel[ld + j], vel[2 * ld + j]};
+            double c[2];
+            oracle_pair_timestep(xi, vi, mass[i], xj, vj, mass[j], G, eta_ff, eta_fb, eta_in_q, c);
+            if (c[0] < tau) tau = c[0];
+            if (c[1] < tau) tau = c[1];
+        }
+        out_tau[i] = tau;
+        if (out_bin) out_bin[i] = bin_of(tau, tau_pivot);
+    }
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O4.  kick and drift, Eq. (6); Alg. 2; kick_sf PAPER.md:596-597.
+ *     kick : v_i <- v_i + c (a_i + kappa g_i)      (kappa = eps^2/48 forms a~ of Eq. 28, or 0)
+ *     drift: x_i <- x_i + c v_i
+ * ------------------------------------------------------------------------------------------- */
+int oracle_kick(int n, int ld, double *vel, const double *acc, const double *grad,
+                const int32_t *idx, int n_idx, double c, double kappa) {
+    if (n < 0 || ld < n || !vel || !acc) return ORACLE_EINVAL;
+    if (!idx) n_idx = n;
+    for (int a = 0; a < n_idx; ++a) {
+        const int i = pick(idx, a);
+        for (int k = 0; k < 3; ++k) {
+            double at = acc[k * ld + i];
+            if (grad && kappa != 0.0) at = at + kappa * grad[k * ld + i];
+            vel[k * ld + i] = vel[k * ld + i] + c * at;
+        }
+    }
+    return ORACLE_OK;
+}
+
+int oracle_drift(int n, int ld, double *pos, const double *vel, const int32_t *idx, int n_idx,
+                 double c) {
+    if (n < 0 || ld < n || !pos || !vel) return ORACLE_EINVAL;
+    if (!idx) n_idx = n;
+    for (int a = 0; a < n_idx; ++a) {
+        const int i = pick(idx, a);
+        for (int k = 0; k < 3; ++k) pos[k * ld + i] = pos[k * ld + i] + c * vel[k * ld + i];
+    }
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O5.  FSI, Eq. (21); Alg. 2 PAPER.md:554:
+ *   a <- newton; kick dt/6; drift dt/2; (a, g) <- newton + gradient; kick 2dt/3 with
+ *   a~ = a + dt^2 g / 48 (Eq. 28; eps = this operator's own step, reading 7);
+ *   drift dt/2; a <- newton; kick dt/6.   Empty set: no-op.
+ * `acc`, `grad` are caller-provided scratch planes [3][ld].
+ * ------------------------------------------------------------------------------------------- */
+static int fsi_on_set(int n, int ld, double *pos, double *vel, const double *mass,
+                      const int32_t *idx, int n_idx, double dt, double G, double eps2,
+                      double *acc, double *grad, oracle_hhs_stats *st) {
+    if (!idx) n_idx = n;
+    if (n_idx == 0) return ORACLE_OK;
+    const int64_t np = (int64_t)n_idx * n_idx;
+    oracle_forces(n, ld, pos, mass, idx, n_idx, idx, n_idx, G, eps2, acc, NULL, ORACLE_ACC);
+    oracle_kick(n, ld, vel, acc, NULL, idx, n_idx, dt / 6.0, 0.0);
+    oracle_drift(n, ld, pos, vel, idx, n_idx, dt / 2.0);
+    oracle_forces(n, ld, pos, mass, idx, n_idx, idx, n_idx, G, eps2, acc, grad, ORACLE_ACC | ORACLE_GRAD);
+    oracle_kick(n, ld, vel, acc, grad, idx, n_idx, 2.0 * dt / 3.0, dt * dt / 48.0);
+    oracle_drift(n, ld, pos, vel, idx, n_idx, dt / 2.0);
+    oracle_forces(n, ld, pos, mass, idx, n_idx, idx, n_idx, G, eps2, acc, NULL, ORACLE_ACC);
+    oracle_kick(n, ld, vel, acc, NULL, idx, n_idx, dt / 6.0, 0.0);
+    if (st) {
+        st->pairs_newton += 3 * np;
+        st->pairs_gradient += np;
+    }
+    return ORACLE_OK;
+}
+
+int oracle_fsi_step(int n, int ld, double *pos, double *vel, const double *mass,
+                    const int32_t *idx, int n_idx, double dt, double G, double eps2) {
+    if (n < 0 || ld < n || !pos || !vel || !mass) return ORACLE_EINVAL;
+    double *acc = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    double *grad = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    if (!acc || !grad) {
+        free(acc);
+        free(grad);
+        return ORACLE_ENOMEM;
+    }
+    const int rc = fsi_on_set(n, ld, pos, vel, mass, idx, n_idx, dt, G, eps2, acc, grad, NULL);
+    free(acc);
+    free(grad);
+    return rc;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O6.  HHS-FSI, Eq. (41); Alg. 3, line by line.
+ * `frozen_level` (may be NULL): if given, particle i is slow at the first level k with
+ * k >= frozen_level[i] instead of by its time-step -- the "frozen partition" used only by the
+ * convergence-order pin (with adaptive steps the partition changes with tau and the error is no
+ * longer a smooth function of the step).
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+    int n, ld;
+    double *pos, *vel;
+    const double *mass;
+    double G, eps2, eta_ff, eta_fb;
+    int eta_in_q, max_depth;
+    const int32_t *frozen_level;
+    double *acc, *grad, *tau;
+    oracle_hhs_stats *st;
+} hhs_env;
+
+static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_pivot, int level) {
+    if (n_set == 0) return ORACLE_OK;                          /* "if set != empty" */
+    if (level >= e->max_depth || level >= ORACLE_MAX_LEVELS) return ORACLE_EDEPTH;
+    const int n = e->n, ld = e->ld;
+    /* {tau_i} <- assign_timesteps(set): only this level's members */
+    oracle_timesteps(n, ld, e->pos, e->vel, e->mass, set, n_set, e->G, e->eta_ff, e->eta_fb,
+                     e->eta_in_q, tau_pivot, e->tau, NULL);
+    /* partition (Eq. 29): slow iff tau_i >= tau_pivot; stable order */
+    int32_t *S = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_set + 1));
+    int32_t *F = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_set + 1));
+    if (!S || !F) {
+        free(S);
+        free(F);
+        return ORACLE_ENOMEM;
+    }
+    int nS = 0, nF = 0;
+    for (int a = 0; a < n_set; ++a) {
+        const int i = set[a];
+        int slow;
+        if (e->frozen_level) slow = (level >= e->frozen_level[i]);
+        else slow = (e->tau[i] >= tau_pivot);
+        if (slow) S[nS++] = i;
+        else F[nF++] = i;
+    }
+    oracle_hhs_stats *st = e->st;
+    if (st) {
+        if (level > st->depth) st->depth = level;
+        st->entries[level] += 1;
+        st->n_slow[level] += nS;
+        st->n_fast[level] += nF;
+        st->pairs_timestep += (int64_t)n_set * n_set;
+    }
+    const int64_t cross = 2 * (int64_t)nS * nF;
+    int rc = ORACLE_OK;
+    const double h = 0.5 * tau_pivot;
+    /* acc_sf_newton (Eq. 42); kick_sf by tau/6 */
+    oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+    oracle_kick(n, ld, e->vel, e->acc, NULL, S, nS, tau_pivot / 6.0, 0.0);
+    oracle_kick(n, ld, e->vel, e->acc, NULL, F, nF, tau_pivot / 6.0, 0.0);
+    /* fsi(S, tau/2); hhs_fsi(F, tau/2) */
+    rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
+    if (rc == ORACLE_OK) rc = hhs_recursive(e, F, nF, h, level + 1);
+    if (rc == ORACLE_OK) {
+        /* acc_sf_gradient (Eq. 43-44) with the inter-level a of Eq. 42; kick_sf by 2 tau/3 with
+         * a~ = a + tau_pivot^2 g / 48 (eps = this level's step, reading 7) */
+        oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, e->grad,
+                      ORACLE_ACC | ORACLE_GRAD | ORACLE_MUTUAL);
+        oracle_kick(n, ld, e->vel, e->acc, e->grad, S, nS, 2.0 * tau_pivot / 3.0, tau_pivot * tau_pivot / 48.0);
+        oracle_kick(n, ld, e->vel, e->acc, e->grad, F, nF, 2.0 * tau_pivot / 3.0, tau_pivot * tau_pivot / 48.0);
+        /* hhs_fsi(F, tau/2); fsi(S, tau/2) */
+        rc = hhs_recursive(e, F, nF, h, level + 1);
+    }
+    if (rc == ORACLE_OK)
+        rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
+    if (rc == ORACLE_OK) {
+        /* acc_sf_newton; kick_sf by tau/6 */
+        oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+        oracle_kick(n, ld, e->vel, e->acc, NULL, S, nS, tau_pivot / 6.0, 0.0);
+        oracle_kick(n, ld, e->vel, e->acc, NULL, F, nF, tau_pivot / 6.0, 0.0);
+        if (st) {
+            st->pairs_newton += 3 * cross;
+            st->pairs_gradient += cross;
+        }
+    }
+    free(S);
+    free(F);
+    return rc;
+}
+
+int oracle_hhs_step(int n, int ld, double *pos, double *vel, const double *mass, double dt_top,
+                    double G, double eps2, double eta_ff, double eta_fb, int eta_in_q,
+                    int max_depth, const int32_t *frozen_level, oracle_hhs_stats *stats) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !(dt_top > 0.0)) return ORACLE_EINVAL;
+    hhs_env e;
+    e.n = n; e.ld = ld; e.pos = pos; e.vel = vel; e.mass = mass;
+    e.G = G; e.eps2 = eps2; e.eta_ff = eta_ff; e.eta_fb = eta_fb;
+    e.eta_in_q = eta_in_q; e.max_depth = max_depth; e.frozen_level = frozen_level;
+    e.acc = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    e.grad = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    e.tau = (double *)calloc((size_t)ld + 1, sizeof(double));
+    int32_t *all = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n + 1));
+    if (stats) memset(stats, 0, sizeof(*stats));
+    e.st = stats;
+    int rc = ORACLE_ENOMEM;
+    if (e.acc && e.grad && e.tau && all) {
+        for (int i = 0; i < n; ++i) all[i] = i;
+        rc = hhs_recursive(&e, all, n, dt_top, 0);
+    }
+    free(e.acc); free(e.grad); free(e.tau); free(all);
+    return rc;
+}
+
+/* ---------------------------------------------------------------------------------------------
+ * O7.  Diagnostics (Eq. 23):
+ *   out[0] = T = 1/2 sum m v^2,  out[1] = U = -G sum_{i<j} m_i m_j / s_ij,
+ *   out[2..4] = P = sum m v,  out[5..7] = L = sum m x cross v.
+ * ------------------------------------------------------------------------------------------- */
+int oracle_diagnostics(int n, int ld, const double *pos, const double *vel, const double *mass,
+                       double G, double eps2, double *out) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !out) return ORACLE_EINVAL;
+    ld_t T = 0, U = 0, P[3] = {0, 0, 0}, L[3] = {0, 0, 0};
+    for (int i = 0; i < n; ++i) {
+        const ld_t m = mass[i];
+        const ld_t x = pos[i], y = pos[ld + i], z = pos[2 * ld + i];
+        const ld_t vx = vel[i], vy = vel[ld + i], vz = vel[2 * ld + i];
+        T += 0.5L * m * (vx * vx + vy * vy + vz * vz);
+        P[0] += m * vx; P[1] += m * vy; P[2] += m * vz;
+        L[0] += m * (y * vz - z * vy);
+        L[1] += m * (z * vx - x * vz);
+        L[2] += m * (x * vy - y * vx);
+    }
+#pragma omp parallel for schedule(dynamic, 16) reduction(+ : U)
+    for (int i = 0; i < n; ++i) {
+        ld_t u = 0;
+        for (int j = i + 1; j < n; ++j) {
+            const ld_t dx = (ld_t)pos[j] - pos[i];
+            const ld_t dy = (ld_t)pos[ld + j] - pos[ld + i];
+            const ld_t dz = (ld_t)pos[2 * ld + j] - pos[2 * ld + i];
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) u += (ld_t)mass[j] / sqrtl(s2);
+        }
+        U += -(ld_t)G * (ld_t)mass[i] * u;
+    }
+    out[0] = (double)T; out[1] = (double)U;
+    for (int k = 0; k < 3; ++k) { out[2 + k] = (double)P[k]; out[5 + k] = (double)L[k]; }
+    return ORACLE_OK;
+}

@@ -1,0 +1,475 @@
+"""Pins for the CPU oracle (oracle/frost_oracle.c) against what the paper and the mathematics fix.
+
+None of these tests re-types an oracle formula and compares it with itself: accelerations are
+pinned to derivatives of the potentials (autograd and finite differences), to two-body closed
+forms, to conservation laws, to the Plummer mean field; the time-step pieces to Eq. (52), to the
+printed symmetrisation factor and to finite differences of the timescale *definitions* along the
+two-body flow; the operator sequences to their convergence order against the Kepler solution.
+Citations are PAPER.md line numbers.
+"""
+import math
+
+import numpy as np
+import pytest
+import torch
+
+import frost_inputs as fi
+
+pytestmark = pytest.mark.filterwarnings("ignore")
+
+
+def _random_system(n, seed, mass_ratio=10.0):
+    rng = np.random.default_rng(seed)
+    pos = np.ascontiguousarray(rng.normal(size=(3, n)))
+    vel = np.ascontiguousarray(rng.normal(size=(3, n)) * 0.3)
+    mass = rng.uniform(1.0, mass_ratio, n) / n
+    return pos, vel, mass
+
+
+def _pairs_mask(n, kind, A=None):
+    """Unordered pair set P as a boolean (n,n) upper-triangular mask."""
+    M = np.zeros((n, n), dtype=bool)
+    for i in range(n):
+        for j in range(i + 1, n):
+            if kind == "self":
+                M[i, j] = True
+            elif kind == "bipartite":          # U_SF: one member in A (=S), the other not
+                M[i, j] = (i in A) != (j in A)
+            elif kind == "active":             # at least one member active (config 4)
+                M[i, j] = (i in A) or (j in A)
+    return M
+
+
+def _autograd_a_g(pos, mass, G, eps2, mask):
+    """a = -(1/m) dU_P/dx (Eq. 24/42) and g = -(1/m) dG_P/dx, G_P = -sum m |a|^2 (Eq. 17, 39),
+    by automatic differentiation of the potential written as in Eq. (23)."""
+    x = torch.tensor(pos.T.copy(), dtype=torch.float64, requires_grad=True)   # (n,3)
+    m = torch.tensor(mass, dtype=torch.float64)
+    iu, ju = np.nonzero(mask)
+    d = x[ju] - x[iu]
+    s = torch.sqrt((d * d).sum(1) + eps2)
+    U = -(G * m[iu] * m[ju] / s).sum()
+    (dU,) = torch.autograd.grad(U, x, create_graph=True)
+    a = -dU / m[:, None]
+    Gpot = -(m[:, None] * a * a).sum()
+    (dG,) = torch.autograd.grad(Gpot, x)
+    g = -dG / m[:, None]
+    return a.detach().numpy().T, g.numpy().T
+
+
+# --------------------------------------------------------------------------- O1 / O2: a_i, g_i
+
+@pytest.mark.parametrize("eps2", [0.0, 0.01])
+def test_self_acc_and_grad_match_autograd(oracle, eps2):
+    n, G = 7, 1.7
+    pos, _, mass = _random_system(n, 11)
+    a_ref, g_ref = _autograd_a_g(pos, mass, G, eps2, _pairs_mask(n, "self"))
+    a, g = oracle.forces(pos, mass, G=G, eps2=eps2)
+    np.testing.assert_allclose(a, a_ref, rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(g, g_ref, rtol=1e-11, atol=1e-12)
+
+
+@pytest.mark.parametrize("eps2", [0.0, 0.02])
+def test_bipartite_sf_acc_and_grad_match_autograd(oracle, eps2):
+    """Inter-level terms Eq. (42)-(44): only S-F pairs, a's are inter-level a's."""
+    n, G = 8, 0.9
+    pos, _, mass = _random_system(n, 5)
+    S = np.array([0, 3, 4], dtype=np.int32)
+    F = np.array([1, 2, 5, 6, 7], dtype=np.int32)
+    a_ref, g_ref = _autograd_a_g(pos, mass, G, eps2, _pairs_mask(n, "bipartite", set(S.tolist())))
+    a, g = oracle.forces(pos, mass, sink_idx=S, source_idx=F, G=G, eps2=eps2,
+                         flags=oracle.ACC | oracle.GRAD | oracle.MUTUAL)
+    np.testing.assert_allclose(a, a_ref, rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(g, g_ref, rtol=1e-11, atol=1e-12)
+
+
+def test_active_vs_all_pair_set_matches_autograd(oracle):
+    """Config 4's pair set {(i,j): i in A or j in A}: A<-all and (all\\A)<-A, then the gradient of
+    the same pair set (reading O2)."""
+    n, G = 8, 1.0
+    pos, _, mass = _random_system(n, 8)
+    A = np.array([2, 5], dtype=np.int32)
+    rest = np.array([i for i in range(n) if i not in A], dtype=np.int32)
+    a_ref, g_ref = _autograd_a_g(pos, mass, G, 0.0, _pairs_mask(n, "active", set(A.tolist())))
+    acc = np.zeros((3, n)); grad = np.zeros((3, n))
+    oracle.forces(pos, mass, sink_idx=A, source_idx=None, G=G, flags=oracle.ACC, acc=acc, grad=grad)
+    oracle.forces(pos, mass, sink_idx=rest, source_idx=A, G=G, flags=oracle.ACC, acc=acc, grad=grad)
+    oracle.forces(pos, mass, sink_idx=A, source_idx=None, G=G, flags=oracle.GRAD, acc=acc, grad=grad)
+    oracle.forces(pos, mass, sink_idx=rest, source_idx=A, G=G, flags=oracle.GRAD, acc=acc, grad=grad)
+    np.testing.assert_allclose(acc, a_ref, rtol=1e-12, atol=1e-13)
+    np.testing.assert_allclose(grad, g_ref, rtol=1e-11, atol=1e-12)
+    # momentum-conserving: sum m a = 0 and sum m g = 0 over this pair set
+    assert np.abs((mass * acc).sum(1)).max() < 1e-15
+    assert np.abs((mass * grad).sum(1)).max() < 1e-13
+
+
+def test_grad_matches_central_finite_difference_of_G(oracle):
+    """north_star pin: g_i = -(1/m_i) dG/dx_i with G = -sum_k m_k |a_k|^2 (Eq. 17),
+    by central differences on N = 6 using the (already pinned) oracle accelerations."""
+    n, G = 6, 1.0
+    pos, _, mass = _random_system(n, 3)
+    _, g = oracle.forces(pos, mass, G=G)
+
+    def Gpot(p):
+        a, _ = oracle.forces(np.ascontiguousarray(p), mass, G=G, flags=oracle.ACC)
+        return -(mass * (a * a).sum(0)).sum()
+
+    h = 1e-5
+    for i in range(n):
+        for c in range(3):
+            pp, pm = pos.copy(), pos.copy()
+            pp[c, i] += h; pm[c, i] -= h
+            fd = -(Gpot(pp) - Gpot(pm)) / (2 * h) / mass[i]
+            assert abs(fd - g[c, i]) <= 2e-7 * np.abs(g[:, i]).max() + 1e-9
+
+
+def test_acc_matches_central_finite_difference_of_U(oracle):
+    n, G = 6, 2.0
+    pos, vel, mass = _random_system(n, 4)
+    a, _ = oracle.forces(pos, mass, G=G, flags=oracle.ACC)
+    h = 1e-6
+    for i in range(n):
+        for c in range(3):
+            pp, pm = pos.copy(), pos.copy()
+            pp[c, i] += h; pm[c, i] -= h
+            Up = oracle.diagnostics(pp, vel, mass, G=G)["U"]
+            Um = oracle.diagnostics(pm, vel, mass, G=G)["U"]
+            fd = -(Up - Um) / (2 * h) / mass[i]
+            assert abs(fd - a[c, i]) <= 1e-8 * np.abs(a[:, i]).max()
+
+
+def test_potential_energy_is_textbook_pair_sum(oracle):
+    """O7 pinned to Eq. (23) written out with numpy broadcasting."""
+    pos, vel, mass = _random_system(9, 21)
+    d = pos[:, :, None] - pos[:, None, :]
+    r = np.sqrt((d * d).sum(0)) + np.eye(9)
+    U = -0.5 * (np.outer(mass, mass) / r * (1 - np.eye(9))).sum() * 1.3
+    dg = oracle.diagnostics(pos, vel, mass, G=1.3)
+    assert abs(dg["U"] - U) < 1e-14 * abs(U)
+    assert abs(dg["T"] - 0.5 * (mass * (vel ** 2).sum(0)).sum()) < 1e-15
+    np.testing.assert_allclose(dg["P"], (mass * vel).sum(1), atol=1e-16)
+    np.testing.assert_allclose(dg["L"], (mass * np.cross(pos.T, vel.T).T).sum(1), atol=1e-15)
+
+
+def test_two_body_closed_forms(oracle):
+    """a_1 = G m_2 x_21 / r^3 (Eq. 24) and g_1 = [4 G (m_1+m_2) / r^3] a_1 -- Eq. (25)-(26),
+    PAPER.md:221-230 (g = 2 t_dyn^-2 a with t_dyn^-2 = 2GM/r^3, reading 3)."""
+    G, m1, m2 = 1.3, 0.7, 2.1
+    pos = np.ascontiguousarray(np.array([[0.3, -1.1], [0.2, 0.9], [-0.5, 0.4]]))
+    mass = np.array([m1, m2])
+    a, g = oracle.forces(pos, mass, G=G)
+    x21 = pos[:, 1] - pos[:, 0]
+    r = np.linalg.norm(x21)
+    np.testing.assert_allclose(a[:, 0], G * m2 * x21 / r ** 3, rtol=1e-15)
+    np.testing.assert_allclose(a[:, 1], -G * m1 * x21 / r ** 3, rtol=1e-15)
+    fac = 4 * G * (m1 + m2) / r ** 3
+    np.testing.assert_allclose(g[:, 0], fac * a[:, 0], rtol=1e-14)
+    np.testing.assert_allclose(g[:, 1], fac * a[:, 1], rtol=1e-14)
+    # modified acceleration of Eq. (26): a~ = [1 + (eps/t_dyn)^2 / 24] a, t_dyn^-2 = 2 G M / r^3
+    eps = 0.37
+    at = a + eps ** 2 / 48 * g
+    np.testing.assert_allclose(at[:, 0], (1 + eps ** 2 * 2 * G * (m1 + m2) / r ** 3 / 24) * a[:, 0],
+                               rtol=1e-14)
+
+
+def test_newton_third_law(oracle):
+    """sum m a = 0 to roundoff; exactly 0 for two equal masses."""
+    pos, _, mass = fi.plummer(512, 0)
+    a, g = oracle.forces(pos, mass)
+    scale = (mass * np.abs(a)).sum(1)
+    assert np.abs((mass * a).sum(1)).max() < 1e-15 * scale.max()
+    gscale = (mass * np.abs(g)).sum(1)
+    assert np.abs((mass * g).sum(1)).max() < 1e-14 * gscale.max()
+    p2, _, m2, _ = fi.kepler_binary(10.0, 10.0, 10.0, 0.9)
+    a2, g2 = oracle.forces(p2, m2)
+    assert ((m2 * a2).sum(1) == 0.0).all() and ((m2 * g2).sum(1) == 0.0).all()
+
+
+def test_plummer_mean_field(oracle):
+    """|a_r| ~ G M(r)/r^2 with M(r) of Eq. (A2), statistically at N = 16384."""
+    n = 16384
+    pos, _, mass = fi.plummer(n, 1)
+    a, _ = oracle.forces(pos, mass, flags=oracle.ACC)
+    r = np.linalg.norm(pos, axis=0)
+    a_r = -(a * pos).sum(0) / r                       # inward radial component
+    order = np.argsort(r)
+    a0 = fi.PLUMMER_A
+    for lo in range(2000, n - 2000, 2000):
+        sel = order[lo:lo + 2000]
+        rr = r[sel]
+        expected = ((1 + a0 ** 2 / rr ** 2) ** -1.5 / 0.999 / rr ** 2).mean()
+        assert abs(a_r[sel].mean() - expected) < 0.08 * expected
+
+
+def test_self_pair_and_empty_sets(oracle):
+    pos, _, mass = _random_system(5, 2)
+    e = np.zeros(0, dtype=np.int32)
+    acc = np.full((3, 5), 7.0); grad = np.full((3, 5), 7.0)
+    oracle.forces(pos, mass, sink_idx=e, source_idx=None, acc=acc, grad=grad)
+    assert (acc == 7.0).all() and (grad == 7.0).all()           # untouched outside I
+    one = np.array([3], dtype=np.int32)
+    oracle.forces(pos, mass, sink_idx=one, source_idx=one, acc=acc, grad=grad)
+    assert (acc[:, 3] == 0).all() and (grad[:, 3] == 0).all()   # only the self pair: ignored
+    assert (np.delete(acc, 3, axis=1) == 7.0).all()
+
+
+# --------------------------------------------------------------------------- O3: time-steps
+
+def test_sym_factor_values_and_symmetries(oracle):
+    """Eq. (49) harmonic factor, evaluated as printed for |q| not small:
+    [q + sqrt(1+q^2) - 1]/q; golden-ratio values at q = +-2; anti-symmetry about (0, tau) and
+    <= arithmetic factor."""
+    for q in [-2.0, -1.0, -0.3, 0.3, 1.0, 2.0, 7.5, -40.0]:
+        printed = (q + math.sqrt(1 + q * q) - 1) / q
+        assert abs(oracle.sym_factor(q) - printed) < 1e-15 * max(1, abs(printed))
+    assert abs(oracle.sym_factor(2.0) - (1 + math.sqrt(5)) / 2) < 1e-15
+    assert abs(oracle.sym_factor(-2.0) - (3 - math.sqrt(5)) / 2) < 1e-15
+    assert oracle.sym_factor(0.0) == 1.0
+    assert abs(oracle.sym_factor(1e-9) - (1 + 0.5e-9)) < 1e-16        # no cancellation at q -> 0
+    for q in np.linspace(-5, 1.9, 40):
+        s = oracle.sym_factor(q)
+        assert abs((s - 1) + (oracle.sym_factor(-q) - 1)) < 1e-15     # odd about (0, 1)
+        assert s <= 1 / (1 - q / 2) + 1e-15                           # harmonic <= arithmetic
+        assert s > 0
+
+
+def test_harmonic_factor_solves_its_defining_equation(oracle):
+    """tau_sym = 2 [1/tau + 1/(tau + tau_sym q)]^-1 (Eq. 47 with Eq. 48)."""
+    for q in [-3.0, -0.5, 0.2, 1.0, 4.0]:
+        s = oracle.sym_factor(q)
+        assert abs(s - 2.0 / (1.0 + 1.0 / (1.0 + s * q))) < 1e-14
+
+
+def test_circular_binary_timestep_is_eta_P_over_2pi(oracle):
+    """Eq. (52): both criteria give tau/P = eta/2pi on a circular orbit."""
+    G, eta = 2.5, 0.05
+    pos, vel, mass, P = fi.kepler_binary(3.0, 1.0, 2.0, 0.0, G=G)
+    ff, fb = oracle.pair_timestep(pos[:, 0], vel[:, 0], mass[0], pos[:, 1], vel[:, 1], mass[1],
+                                  G=G, eta_ff=eta, eta_fb=eta)
+    assert abs(ff / P - eta / (2 * math.pi)) < 1e-15
+    assert abs(fb / P - eta / (2 * math.pi)) < 1e-15
+    tau, bins = oracle.timesteps(pos, vel, mass, G=G, eta_ff=eta, eta_fb=eta, tau_pivot=P)
+    np.testing.assert_allclose(tau, eta * P / (2 * math.pi), rtol=1e-15)
+    k = int(bins[0])
+    assert P * 2.0 ** -k <= tau[0] < P * 2.0 ** -(k - 1) and bins[0] == bins[1]
+
+
+def _q_from_candidate(c, eta, t):
+    """Invert s(q) = 1 + q/(1+sqrt(1+q^2)):  u = s-1 = tan(theta/2), q = tan(theta) = 2u/(1-u^2)."""
+    u = c / (eta * t) - 1.0
+    return 2 * u / (1 - u * u)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_timescale_derivatives_match_finite_differences_along_two_body_flow(oracle, seed):
+    """Eq. (53)-(54), pinned to the *definitions* Eq. (50)-(51): d t/dt by
+    central differences with r(t+-h) = r +- v h, v(t+-h) = v +- a h, a = -mu r / r^3 (the
+    two-body approximation the paper states).  Pins sign, 3/2, and [1 + mu/(v^2 r)]."""
+    rng = np.random.default_rng(seed)
+    G, eta = 1.4, 0.3
+    xi, xj = rng.normal(size=3), rng.normal(size=3)
+    vi, vj = rng.normal(size=3), rng.normal(size=3)
+    mi, mj = 0.6, 1.9
+    mu = G * (mi + mj)
+    r0, v0 = xj - xi, vj - vi
+
+    def t_ff(r, v): return math.sqrt(np.linalg.norm(r) ** 3 / mu)
+    def t_fb(r, v): return np.linalg.norm(r) / np.linalg.norm(v)
+
+    def ddt(f):
+        out = []
+        for h in (1e-4,):
+            acc = lambda r: -mu * r / np.linalg.norm(r) ** 3
+            rp, vp = r0 + v0 * h + 0.5 * acc(r0) * h * h, v0 + acc(r0) * h
+            rm, vm = r0 - v0 * h + 0.5 * acc(r0) * h * h, v0 - acc(r0) * h
+            out.append((f(rp, vp) - f(rm, vm)) / (2 * h))
+        return out[0]
+
+    ff, fb = oracle.pair_timestep(xi, vi, mi, xj, vj, mj, G=G, eta_ff=eta, eta_fb=eta)
+    q_ff = _q_from_candidate(ff, eta, t_ff(r0, v0))
+    q_fb = _q_from_candidate(fb, eta, t_fb(r0, v0))
+    assert abs(q_ff - eta * ddt(t_ff)) < 1e-6 * max(1.0, abs(q_ff))
+    assert abs(q_fb - eta * ddt(t_fb)) < 1e-6 * max(1.0, abs(q_fb))
+    # the other documented reading (q without eta, reading 9) differs exactly by eta
+    ff2, fb2 = oracle.pair_timestep(xi, vi, mi, xj, vj, mj, G=G, eta_ff=eta, eta_fb=eta,
+                                    eta_in_q=False)
+    assert abs(_q_from_candidate(ff2, eta, t_ff(r0, v0)) - ddt(t_ff)) < 1e-6 * max(1, abs(q_ff / eta))
+    assert abs(_q_from_candidate(fb2, eta, t_fb(r0, v0)) - ddt(t_fb)) < 1e-6 * max(1, abs(q_fb / eta))
+
+
+def test_timesteps_are_min_over_level_members_only(oracle):
+    """tau_i = min_j over the same level's members; brute force on N = 8."""
+    pos, vel, mass = _random_system(8, 13)
+    idx = np.array([0, 2, 3, 6, 7], dtype=np.int32)
+    tau, bins = oracle.timesteps(pos, vel, mass, idx=idx, eta_ff=0.2, eta_fb=0.1, tau_pivot=0.5)
+    for i in idx:
+        best = math.inf
+        for j in idx:
+            if i != j:
+                c = oracle.pair_timestep(pos[:, i], vel[:, i], mass[i], pos[:, j], vel[:, j],
+                                         mass[j], eta_ff=0.2, eta_fb=0.1)
+                best = min(best, *c)
+        assert tau[i] == best
+        k = int(bins[i])
+        assert 0.5 * 2.0 ** -k <= tau[i] and (k == 0 or tau[i] < 0.5 * 2.0 ** -(k - 1))
+    others = [i for i in range(8) if i not in idx]
+    assert np.isinf(tau[others]).all()                       # untouched (initialised to +inf)
+    # pairwise symmetric criterion: the closest pair shares its step when it is mutual-minimum
+    lone, _ = oracle.timesteps(pos, vel, mass, idx=np.array([4], dtype=np.int32))
+    assert np.isinf(lone[4])                                 # a level of one particle: +inf
+
+
+def test_zero_relative_velocity_gives_free_fall_only(oracle):
+    G, eta = 1.0, 0.2
+    ff, fb = oracle.pair_timestep([0, 0, 0], [0, 0, 0], 1.0, [2.0, 0, 0], [0, 0, 0], 3.0, G=G,
+                                  eta_ff=eta, eta_fb=eta)
+    assert math.isinf(fb)
+    assert abs(ff - eta * math.sqrt(8.0 / 4.0)) < 1e-15      # q = 0: s = 1, t_ff = sqrt(r^3/mu)
+
+
+# --------------------------------------------------------------------------- O4-O6: integrators
+
+def _kepler_state(m1, m2, a, e, t, G=1.0):
+    """Closed-form relative two-body state at time t after apocentre (textbook Kepler solution)."""
+    mt = m1 + m2
+    nmean = math.sqrt(G * mt / a ** 3)
+    M = math.pi + nmean * t
+    E = M
+    for _ in range(80):
+        E -= (E - e * math.sin(E) - M) / (1 - e * math.cos(E))
+    b = math.sqrt(1 - e * e)
+    x, y = a * (math.cos(E) - e), a * b * math.sin(E)
+    rr = a * (1 - e * math.cos(E))
+    vx, vy = -a * a * nmean * math.sin(E) / rr, a * a * nmean * b * math.cos(E) / rr
+    return np.array([x, y, 0.0]), np.array([vx, vy, 0.0])
+
+
+def _fsi_kepler_error(oracle, nsteps, e=0.5):
+    m1, m2, a = 0.6, 0.4, 1.0
+    pos, vel, mass, P = fi.kepler_binary(m1, m2, a, e)
+    # kepler_binary starts at apocentre on the +x side for body 2: relative x = -(-r) ... align
+    T = 0.25 * P
+    dt = T / nsteps
+    E0 = oracle.diagnostics(pos, vel, mass)["E"]
+    emax = 0.0
+    for _ in range(nsteps):
+        oracle.fsi_step(pos, vel, mass, dt)
+        emax = max(emax, abs(oracle.diagnostics(pos, vel, mass)["E"] / E0 - 1))
+    xr, vr = _kepler_state(m1, m2, a, e, T)
+    rel = pos[:, 1] - pos[:, 0]
+    # apocentre of the relative orbit is at x = -a(1+e) in _kepler_state's frame; kepler_binary
+    # puts body 2 at +r, so mirror x and y (rotation by pi keeps the sense of revolution)
+    return np.linalg.norm(rel - (-xr)), emax
+
+
+def test_fsi_is_fourth_order_against_kepler_closed_form(oracle):
+    """Alg. 2 coefficients 1/6, 2/3, 1/6; 1/2, 1/2; a~ = a + dt^2 g/48 (Eq. 21, 28): the position
+    error against the Kepler solution and max |dE/E| fall 16x per step halving."""
+    e1, d1 = _fsi_kepler_error(oracle, 64)
+    e2, d2 = _fsi_kepler_error(oracle, 128)
+    e3, d3 = _fsi_kepler_error(oracle, 256)
+    for r in (e1 / e2, e2 / e3, d1 / d2, d2 / d3):
+        assert 14.0 < r < 18.0, (e1, e2, e3, d1, d2, d3)
+
+
+def test_fsi_time_reversal_and_exact_momentum(oracle):
+    pos, vel, mass, P = fi.kepler_binary(10.0, 10.0, 10.0, 0.9)
+    p0, v0 = pos.copy(), vel.copy()
+    dt = P / 400
+    for _ in range(100):
+        oracle.fsi_step(pos, vel, mass, dt)
+    assert ((mass * vel).sum(1) == 0.0).all()               # Delta P = 0 exactly
+    vel *= -1
+    for _ in range(100):
+        oracle.fsi_step(pos, vel, mass, dt)
+    np.testing.assert_allclose(pos, p0, atol=1e-11 * 19.0)
+    np.testing.assert_allclose(-vel, v0, atol=1e-11 * np.abs(v0).max())
+
+
+def _star_planets():
+    """Star + 3 planets on well separated circular-ish orbits (G = 1)."""
+    mass = np.array([1.0, 1e-3, 5e-4, 2e-4])
+    pos = np.zeros((3, 4)); vel = np.zeros((3, 4))
+    for k, (a, ph) in enumerate([(0.3, 0.4), (1.0, 2.1), (3.2, 4.0)], start=1):
+        pos[0, k], pos[1, k] = a * math.cos(ph), a * math.sin(ph)
+        v = math.sqrt(1.0 / a)
+        vel[0, k], vel[1, k] = -v * math.sin(ph), v * math.cos(ph)
+        pos[2, k] = 0.02 * a * k
+    pos -= (pos * mass).sum(1, keepdims=True) / mass.sum()
+    vel -= (vel * mass).sum(1, keepdims=True) / mass.sum()
+    return np.ascontiguousarray(pos), np.ascontiguousarray(vel), mass
+
+
+def _hhs_frozen_error(oracle, nsteps, ref):
+    pos, vel, mass = _star_planets()
+    frozen = np.array([2, 2, 1, 0], dtype=np.int32)          # outer planet slow, star+inner fastest
+    T = 0.4
+    for _ in range(nsteps):
+        oracle.hhs_step(pos, vel, mass, T / nsteps, frozen_level=frozen)
+    return np.abs(pos - ref[0]).max(), pos, vel, mass
+
+
+def test_hhs_fsi_is_fourth_order_with_frozen_partition(oracle):
+    """Alg. 3 / Eq. (41) with three levels: 16x per halving requires the middle kick_sf to use
+    eps = tau_pivot and fsi(S, tau/2) to use tau/2 (reading 7)."""
+    pos, vel, mass = _star_planets()
+    frozen = np.array([2, 2, 1, 0], dtype=np.int32)
+    nref = 512
+    for _ in range(nref):
+        oracle.hhs_step(pos, vel, mass, 0.4 / nref, frozen_level=frozen)
+    ref = (pos.copy(), vel.copy())
+    e1, *_ = _hhs_frozen_error(oracle, 8, ref)
+    e2, *_ = _hhs_frozen_error(oracle, 16, ref)
+    e3, p3, v3, m3 = _hhs_frozen_error(oracle, 32, ref)
+    assert 13.0 < e1 / e2 < 19.0 and 13.0 < e2 / e3 < 19.0, (e1, e2, e3)
+    assert np.abs((m3 * v3).sum(1)).max() < 1e-17           # momentum at roundoff
+
+
+def test_hhs_level_bookkeeping_and_equivalence_to_fsi_when_single_level(oracle):
+    """All particles slow at level 0  =>  hhs_fsi(tau) == fsi(tau/2) o fsi(tau/2) exactly
+    (F empty: every inter-level term vanishes; Alg. 3)."""
+    pos, vel, mass = _random_system(6, 17)
+    p1, v1 = pos.copy(), vel.copy()
+    st = oracle.hhs_step(pos, vel, mass, 1e-3, frozen_level=np.zeros(6, dtype=np.int32))
+    oracle.fsi_step(p1, v1, mass, 0.5e-3); oracle.fsi_step(p1, v1, mass, 0.5e-3)
+    assert (pos == p1).all() and (vel == v1).all()
+    assert st["depth"] == 0 and st["entries"] == [1] and st["n_slow"] == [6] and st["n_fast"] == [0]
+    assert st["pairs_newton"] == 2 * 3 * 36 and st["pairs_gradient"] == 2 * 36
+    assert st["pairs_timestep"] == 36
+
+
+def test_hhs_solar_system_adaptive(oracle):
+    """Five-body Solar system of Tables A1/A2: several hierarchy levels are
+    populated, momentum stays at roundoff (|dP| < 1e-15), energy error is small and
+    falls steeply with eta."""
+    errs = []
+    for eta in (0.2, 0.05):
+        pos, vel, mass, G = fi.solar_system()
+        vel -= (vel * mass).sum(1, keepdims=True) / mass.sum()
+        d0 = oracle.diagnostics(pos, vel, mass, G=G)
+        depth = 0
+        for _ in range(4):
+            st = oracle.hhs_step(pos, vel, mass, 512.0, G=G, eta_ff=eta, eta_fb=eta)
+            depth = max(depth, st["depth"])
+        d1 = oracle.diagnostics(pos, vel, mass, G=G)
+        errs.append(abs(d1["E"] / d0["E"] - 1))
+        assert np.abs(d1["P"] - d0["P"]).max() < 1e-17
+        assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-12 * np.linalg.norm(d0["L"])
+        assert depth >= 2 and sum(1 for s in st["n_slow"] if s > 0) >= 2
+    assert errs[0] < 1e-6 and errs[1] < errs[0] / 20
+
+
+def test_small_plummer_run_conserves_as_the_paper_reports(oracle):
+    """north_star pin: |dE/E| small and ~dt^4, linear/angular momentum drift at roundoff on a
+    small Plummer run (config 1's shape at N = 256 so the CPU suite stays fast)."""
+    res = []
+    for dt, steps in ((1 / 512, 4), (1 / 1024, 8)):
+        pos, vel, mass = fi.plummer(256, 0)
+        d0 = oracle.diagnostics(pos, vel, mass, eps2=1e-4)
+        for _ in range(steps):
+            oracle.fsi_step(pos, vel, mass, dt, eps2=1e-4)
+        d1 = oracle.diagnostics(pos, vel, mass, eps2=1e-4)
+        res.append(abs(d1["E"] / d0["E"] - 1))
+        assert np.abs(d1["P"] - d0["P"]).max() < 1e-16
+        assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-14
+    assert res[1] < 1e-8 and res[1] < res[0] / 6
