@@ -1,0 +1,355 @@
+// frost_api.cu -- the C-ABI of include/frost.h: argument checks, scratch, and the host-side
+// sequencing of Alg. 2 (fsi) and Alg. 3 (hhs_fsi).  All arithmetic is in the kernels of
+// frost_sweeps.cu / frost_update.cu.
+#include <new>
+
+#include "frost_common.cuh"
+
+using namespace frost;
+
+static int pad1024(int n) { return round_up(n > 0 ? n : 1, 1024); }
+
+extern "C" {
+
+int frost_create(frost_ctx **out, int device, void *stream) {
+    if (!out) return FROST_EINVAL;
+    *out = nullptr;
+    int count = 0;
+    if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return FROST_ECUDA;
+    if (cudaSetDevice(device) != cudaSuccess) return FROST_ECUDA;
+    frost_ctx *c = new (std::nothrow) frost_ctx();
+    if (!c) return FROST_ENOMEM;
+    c->device = device;
+    c->stream = (cudaStream_t)stream;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete c; return FROST_ECUDA; }
+    c->num_sms = prop.multiProcessorCount;
+    if (cudaMallocHost((void **)&c->pinned_counts, 4 * sizeof(int32_t)) != cudaSuccess) {
+        delete c;
+        return FROST_ENOMEM;
+    }
+    *out = c;
+    return FROST_OK;
+}
+
+int frost_destroy(frost_ctx *c) {
+    if (!c) return FROST_EINVAL;
+    cudaSetDevice(c->device);
+    cudaStreamSynchronize(c->stream);
+    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->iota,
+                   &c->acc, &c->grad, &c->tau, &c->blockcnt};
+    for (Buf *b : bufs) if (b->p) cudaFree(b->p);
+    for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
+    for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
+        if (c->lvlS[k].p) cudaFree(c->lvlS[k].p);
+        if (c->lvlF[k].p) cudaFree(c->lvlF[k].p);
+    }
+    if (c->pinned_counts) cudaFreeHost(c->pinned_counts);
+    delete c;
+    return FROST_OK;
+}
+
+int frost_set_params(frost_ctx *c, double G, double eps2, double eta_ff, double eta_fb, int max_depth) {
+    if (!c || !(eps2 >= 0.0) || !(eta_ff > 0.0) || !(eta_fb > 0.0) || max_depth < 1) return FROST_EINVAL;
+    c->G = G; c->eps2 = eps2; c->eta_ff = eta_ff; c->eta_fb = eta_fb;
+    c->max_depth = max_depth < FROST_MAX_LEVELS ? max_depth : FROST_MAX_LEVELS;
+    return FROST_OK;
+}
+
+int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices) {
+    if (!c) return FROST_EINVAL;
+    if (!(sinks_per_thread == 0 || sinks_per_thread == 1 || sinks_per_thread == 2 || sinks_per_thread == 4))
+        return FROST_EINVAL;
+    if (source_slices < 0) return FROST_EINVAL;
+    c->tune_k = sinks_per_thread;
+    c->tune_slices = source_slices;
+    return FROST_OK;
+}
+
+int64_t frost_launch_count(const frost_ctx *c) { return c ? c->launches : -1; }
+int frost_last_cuda_error(const frost_ctx *c) { return c ? c->last_cuda : 0; }
+const char *frost_version(void) { return "frost-b200 0.1 (sm_100a)"; }
+
+const char *frost_strerror(int status) {
+    switch (status) {
+        case FROST_OK: return "ok";
+        case FROST_EINVAL: return "invalid argument";
+        case FROST_ECUDA: return "CUDA error (see frost_last_cuda_error)";
+        case FROST_ENOMEM: return "out of memory";
+        case FROST_EDEPTH: return "hierarchy deeper than max_depth";
+        case FROST_ENONFINITE: return "non-finite input";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"
+
+// zero the padding records [n, n_pad) of a packed vector stream
+static int zero_tail(frost_ctx *c, double *rec, int n, int n_pad) {
+    if (n_pad > n)
+        FROST_CUDA(c, cudaMemsetAsync(rec + 4 * (size_t)n, 0, (size_t)(n_pad - n) * kRecBytes, c->stream));
+    return FROST_OK;
+}
+
+static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+                       const int32_t *I, int nI, const int32_t *J, int nJ, double *acc, double *grad,
+                       int flags) {
+    if (!I) nI = n;
+    if (!J) nJ = n;
+    const bool mutual = (flags & FROST_MUTUAL) != 0;
+    const bool self = (I == J) && (nI == nJ);
+    if (nI <= 0 && !(mutual && nJ > 0)) return FROST_OK;
+    const int padA = pad1024(nI), padB = pad1024(nJ);
+    FROST_TRY(ensure(c, c->recA_xm, (size_t)padA * kRecBytes));
+    FROST_TRY(ensure(c, c->recA_v, (size_t)padA * kRecBytes));
+    double *Axm = (double *)c->recA_xm.p, *Av = (double *)c->recA_v.p;
+    double *Bxm = Axm, *Bv = Av;
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, I, nI, padA, Axm));
+    if (!self) {
+        FROST_TRY(ensure(c, c->recB_xm, (size_t)padB * kRecBytes));
+        FROST_TRY(ensure(c, c->recB_v, (size_t)padB * kRecBytes));
+        Bxm = (double *)c->recB_xm.p; Bv = (double *)c->recB_v.p;
+        FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm));
+    }
+    if (flags & FROST_ACC) {
+        FROST_TRY(zero_tail(c, Av, nI, padA));
+        FROST_TRY(sweep_newton(c, Axm, nI, Bxm, nJ, I, ld, acc, Av));
+        if (mutual && !self) {
+            FROST_TRY(zero_tail(c, Bv, nJ, padB));
+            FROST_TRY(sweep_newton(c, Bxm, nJ, Axm, nI, J, ld, acc, Bv));
+        }
+    }
+    if (flags & FROST_GRAD) {
+        if (!(flags & FROST_ACC)) FROST_TRY(launch_pack_vec(c, ld, acc, I, nI, padA, Av));
+        if (!self && !((flags & FROST_ACC) && mutual))
+            FROST_TRY(launch_pack_vec(c, ld, acc, J, nJ, padB, Bv));
+        FROST_TRY(sweep_gradient(c, Axm, Av, nI, Bxm, Bv, nJ, I, ld, grad));
+        if (mutual && !self) FROST_TRY(sweep_gradient(c, Bxm, Bv, nJ, Axm, Av, nI, J, ld, grad));
+    }
+    return FROST_OK;
+}
+
+static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
+                          const double *mass, const int32_t *idx, int n_idx, double tau_pivot,
+                          double *out_tau, int32_t *out_bin) {
+    if (!idx) n_idx = n;
+    if (n_idx <= 0) return FROST_OK;
+    const int pad = pad1024(n_idx);
+    FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+    FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
+    double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm));
+    FROST_TRY(launch_pack_vec(c, ld, vel, idx, n_idx, pad, v));
+    return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
+}
+
+static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                    const int32_t *idx, int n_idx, double dt, frost_hhs_stats *st) {
+    if (!idx) n_idx = n;
+    if (n_idx <= 0) return FROST_OK;
+    FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
+    FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
+    double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
+    FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, nullptr, FROST_ACC));
+    FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0));
+    FROST_TRY(launch_drift(c, ld, pos, vel, idx, n_idx, dt / 2.0));
+    FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, grad, FROST_ACC | FROST_GRAD));
+    FROST_TRY(launch_kick(c, ld, vel, acc, grad, idx, n_idx, 2.0 * dt / 3.0, dt * dt / 48.0));
+    FROST_TRY(launch_drift(c, ld, pos, vel, idx, n_idx, dt / 2.0));
+    FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, nullptr, FROST_ACC));
+    FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0));
+    if (st) {
+        const int64_t np = (int64_t)n_idx * n_idx;
+        st->pairs_newton += 3 * np;
+        st->pairs_gradient += np;
+    }
+    return FROST_OK;
+}
+
+static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st) {
+    if (n_set <= 0) return FROST_OK;
+    if (level >= c->max_depth || level >= FROST_MAX_LEVELS) return FROST_EDEPTH;
+    double *tau = (double *)c->tau.p, *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
+    FROST_TRY(timesteps_impl(c, n, ld, pos, vel, mass, set, n_set, tau_pivot, tau, nullptr));
+    FROST_TRY(ensure(c, c->lvlS[level], (size_t)n_set * sizeof(int32_t)));
+    FROST_TRY(ensure(c, c->lvlF[level], (size_t)n_set * sizeof(int32_t)));
+    int32_t *S = (int32_t *)c->lvlS[level].p, *F = (int32_t *)c->lvlF[level].p;
+    int32_t cnt[2];
+    FROST_TRY(launch_partition(c, tau, set, n_set, tau_pivot, S, F, cnt));
+    const int nS = cnt[0], nF = cnt[1];
+    if (st) {
+        if (level > st->depth) st->depth = level;
+        st->entries[level] += 1;
+        st->n_slow[level] += nS;
+        st->n_fast[level] += nF;
+        st->pairs_timestep += (int64_t)n_set * n_set;
+    }
+    const bool cross = nS > 0 && nF > 0;
+    const double h = 0.5 * tau_pivot;
+    if (cross) {
+        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, S, nS, tau_pivot / 6.0, 0.0));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, F, nF, tau_pivot / 6.0, 0.0));
+    }
+    FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
+    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
+    if (cross) {
+        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad,
+                              FROST_ACC | FROST_GRAD | FROST_MUTUAL));
+        const double kap = tau_pivot * tau_pivot / 48.0;
+        FROST_TRY(launch_kick(c, ld, vel, acc, grad, S, nS, 2.0 * tau_pivot / 3.0, kap));
+        FROST_TRY(launch_kick(c, ld, vel, acc, grad, F, nF, 2.0 * tau_pivot / 3.0, kap));
+    }
+    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
+    FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
+    if (cross) {
+        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, S, nS, tau_pivot / 6.0, 0.0));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, F, nF, tau_pivot / 6.0, 0.0));
+    }
+    if (st) {
+        const int64_t cr = 2 * (int64_t)nS * nF;
+        st->pairs_newton += 3 * cr;
+        st->pairs_gradient += cr;
+    }
+    return FROST_OK;
+}
+
+static bool bad_planes(int n, int ld) { return n < 0 || ld < n; }
+
+extern "C" {
+
+int frost_forces(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
+                 const double *mass, const int32_t *sink_idx, int n_sink,
+                 const int32_t *source_idx, int n_source, double *out_acc, double *out_grad,
+                 int flags) {
+    (void)vel;
+    if (!c || bad_planes(n, ld) || !pos || !mass || !out_acc) return FROST_EINVAL;
+    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~7)) return FROST_EINVAL;
+    if ((flags & FROST_GRAD) && !out_grad) return FROST_EINVAL;
+    if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
+    if ((sink_idx && n_sink < 0) || (source_idx && n_source < 0)) return FROST_EINVAL;
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return forces_impl(c, n, ld, pos, mass, sink_idx, n_sink, source_idx, n_source, out_acc, out_grad, flags);
+}
+
+int frost_forces_host(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+                      const int32_t *sink_idx, int n_sink, const int32_t *source_idx,
+                      int n_source, double *out_acc, double *out_grad, int flags) {
+    if (!c || bad_planes(n, ld) || !pos || !mass || !out_acc) return FROST_EINVAL;
+    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~7)) return FROST_EINVAL;
+    if ((flags & FROST_GRAD) && !out_grad) return FROST_EINVAL;
+    if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    const size_t pb = (size_t)3 * ld * sizeof(double);
+    FROST_TRY(ensure(c, c->host_stage[0], pb));
+    FROST_TRY(ensure(c, c->host_stage[1], (size_t)n * sizeof(double)));
+    FROST_TRY(ensure(c, c->host_stage[2], pb));
+    FROST_TRY(ensure(c, c->host_stage[3], pb));
+    double *dpos = (double *)c->host_stage[0].p, *dmass = (double *)c->host_stage[1].p;
+    double *dacc = (double *)c->host_stage[2].p, *dgrad = (double *)c->host_stage[3].p;
+    int32_t *dI = nullptr, *dJ = nullptr;
+    if (sink_idx) {
+        FROST_TRY(ensure(c, c->host_stage[4], (size_t)(n_sink + 1) * sizeof(int32_t)));
+        dI = (int32_t *)c->host_stage[4].p;
+        FROST_CUDA(c, cudaMemcpyAsync(dI, sink_idx, (size_t)n_sink * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+    }
+    if (source_idx) {
+        if (source_idx == sink_idx && n_source == n_sink) dJ = dI;
+        else {
+            FROST_TRY(ensure(c, c->host_stage[5], (size_t)(n_source + 1) * sizeof(int32_t)));
+            dJ = (int32_t *)c->host_stage[5].p;
+            FROST_CUDA(c, cudaMemcpyAsync(dJ, source_idx, (size_t)n_source * sizeof(int32_t), cudaMemcpyHostToDevice, c->stream));
+        }
+    }
+    FROST_CUDA(c, cudaMemcpyAsync(dpos, pos, pb, cudaMemcpyHostToDevice, c->stream));
+    FROST_CUDA(c, cudaMemcpyAsync(dmass, mass, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    // out_acc is an input when the gradient is requested on caller-provided accelerations, and
+    // entries outside the swept sets must come back untouched
+    FROST_CUDA(c, cudaMemcpyAsync(dacc, out_acc, pb, cudaMemcpyHostToDevice, c->stream));
+    if (flags & FROST_GRAD)
+        FROST_CUDA(c, cudaMemcpyAsync(dgrad, out_grad, pb, cudaMemcpyHostToDevice, c->stream));
+    FROST_TRY(forces_impl(c, n, ld, dpos, dmass, dI, n_sink, dJ, n_source, dacc, dgrad, flags));
+    if (flags & FROST_ACC)
+        FROST_CUDA(c, cudaMemcpyAsync(out_acc, dacc, pb, cudaMemcpyDeviceToHost, c->stream));
+    if (flags & FROST_GRAD)
+        FROST_CUDA(c, cudaMemcpyAsync(out_grad, dgrad, pb, cudaMemcpyDeviceToHost, c->stream));
+    FROST_CUDA(c, cudaStreamSynchronize(c->stream));
+    return FROST_OK;
+}
+
+int frost_timesteps(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
+                    const double *mass, const int32_t *idx, int n_idx, double tau_pivot,
+                    double *out_tau, int32_t *out_bin) {
+    if (!c || bad_planes(n, ld) || !pos || !vel || !mass || !out_tau) return FROST_EINVAL;
+    if (idx && n_idx < 0) return FROST_EINVAL;
+    if (out_bin && !(tau_pivot > 0.0)) return FROST_EINVAL;
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return timesteps_impl(c, n, ld, pos, vel, mass, idx, n_idx, tau_pivot, out_tau, out_bin);
+}
+
+int frost_partition(frost_ctx *c, int n, const double *tau, const int32_t *idx, int n_idx,
+                    double tau_pivot, int32_t *out_slow, int32_t *out_fast, int32_t *counts) {
+    if (!c || n < 0 || !tau || !out_slow || !out_fast || !counts) return FROST_EINVAL;
+    if (!idx) n_idx = n;
+    if (n_idx < 0) return FROST_EINVAL;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return launch_partition(c, tau, idx, n_idx, tau_pivot, out_slow, out_fast, counts);
+}
+
+int frost_kick(frost_ctx *c, int n, int ld, double *vel, const double *acc, const double *grad,
+               const int32_t *idx, int n_idx, double cc, double kappa) {
+    if (!c || bad_planes(n, ld) || !vel || !acc) return FROST_EINVAL;
+    if (kappa != 0.0 && !grad) return FROST_EINVAL;
+    if (!idx) n_idx = n;
+    if (n_idx < 0) return FROST_EINVAL;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return launch_kick(c, ld, vel, acc, grad, idx, n_idx, cc, kappa);
+}
+
+int frost_drift(frost_ctx *c, int n, int ld, double *pos, const double *vel, const int32_t *idx,
+                int n_idx, double cc) {
+    if (!c || bad_planes(n, ld) || !pos || !vel) return FROST_EINVAL;
+    if (!idx) n_idx = n;
+    if (n_idx < 0) return FROST_EINVAL;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return launch_drift(c, ld, pos, vel, idx, n_idx, cc);
+}
+
+int frost_fsi_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                   const int32_t *idx, int n_idx, double dt) {
+    if (!c || bad_planes(n, ld) || !pos || !vel || !mass) return FROST_EINVAL;
+    if (idx && n_idx < 0) return FROST_EINVAL;
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return fsi_impl(c, n, ld, pos, vel, mass, idx, n_idx, dt, nullptr);
+}
+
+int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                   double dt_top, frost_hhs_stats *stats) {
+    if (!c || bad_planes(n, ld) || !pos || !vel || !mass || !(dt_top > 0.0)) return FROST_EINVAL;
+    if (stats) *stats = frost_hhs_stats{};
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
+    FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
+    FROST_TRY(ensure(c, c->tau, (size_t)ld * sizeof(double)));
+    const int rc = hhs_rec(c, n, ld, pos, vel, mass, nullptr, n, dt_top, 0, stats);
+    cudaStreamSynchronize(c->stream);
+    return rc;
+}
+
+int frost_gather_pack(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+                      const int32_t *idx, int n_idx, int n_pad, double *out_records) {
+    if (!c || bad_planes(n, ld) || !pos || !mass || !out_records) return FROST_EINVAL;
+    if (!idx) n_idx = n;
+    if (n_idx < 0 || n_pad < n_idx) return FROST_EINVAL;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    return launch_pack_xm(c, ld, pos, mass, idx, n_idx, n_pad, out_records);
+}
+
+}  // extern "C"

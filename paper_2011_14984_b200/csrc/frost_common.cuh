@@ -1,0 +1,179 @@
+// frost_common.cuh -- context, scratch management and PTX helpers shared by the CUDA translation
+// units of libfrost_b200.so.  (Product code: shares nothing with oracle/.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/frost.h"
+
+namespace frost {
+
+// ---- geometry of the pair sweeps -------------------------------------------------------------
+constexpr int kTile = 256;        // source records per shared-memory stage
+constexpr int kStages = 3;        // ring depth of the TMA bulk-copy pipeline
+constexpr int kRecBytes = 32;     // one packed record: 4 doubles
+
+struct Buf {
+    void *p = nullptr;
+    size_t cap = 0;
+};
+
+}  // namespace frost
+
+struct frost_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    double G = 1.0, eps2 = 0.0, eta_ff = 0.2, eta_fb = 0.2;
+    int max_depth = 64;
+    int tune_k = 0, tune_slices = 0;
+    int num_sms = 148;
+    int last_cuda = 0;
+    int64_t launches = 0;
+    // scratch (grow-only)
+    frost::Buf recA_xm, recB_xm;   // packed {x,y,z,m} streams of set A (sinks) and set B (sources)
+    frost::Buf recA_v, recB_v;     // packed {ax,ay,az,0} or {vx,vy,vz,0}
+    frost::Buf partial;            // [slices][3][n_pad] partial sums / [slices][n_pad] partial minima
+    frost::Buf iota;               // unused placeholder for identity lists
+    frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
+    frost::Buf blockcnt;           // partition scratch
+    frost::Buf host_stage[6];      // device staging for frost_forces_host
+    frost::Buf lvlS[FROST_MAX_LEVELS], lvlF[FROST_MAX_LEVELS];
+    int32_t *pinned_counts = nullptr;  // host pinned int32[4]
+};
+
+namespace frost {
+
+#define FROST_CUDA(ctx, call)                         \
+    do {                                              \
+        cudaError_t e_ = (call);                      \
+        if (e_ != cudaSuccess) {                      \
+            (ctx)->last_cuda = (int)e_;               \
+            return FROST_ECUDA;                       \
+        }                                             \
+    } while (0)
+
+#define FROST_TRY(expr)                \
+    do {                               \
+        int rc_ = (expr);              \
+        if (rc_ != FROST_OK) return rc_; \
+    } while (0)
+
+inline int ensure(frost_ctx *c, Buf &b, size_t bytes) {
+    if (bytes <= b.cap) return FROST_OK;
+    if (b.p) {
+        // the buffer may still be in use by enqueued work: drain the stream before freeing
+        cudaStreamSynchronize(c->stream);
+        cudaFree(b.p);
+        b.p = nullptr;
+        b.cap = 0;
+    }
+    size_t want = bytes + bytes / 4 + 256;
+    cudaError_t e = cudaMalloc(&b.p, want);
+    if (e != cudaSuccess) {
+        c->last_cuda = (int)e;
+        b.p = nullptr;
+        return FROST_ENOMEM;
+    }
+    b.cap = want;
+    return FROST_OK;
+}
+
+inline int check_launch(frost_ctx *c) {
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        c->last_cuda = (int)e;
+        return FROST_ECUDA;
+    }
+    return FROST_OK;
+}
+
+inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+// ---- launchers implemented in the other translation units ------------------------------------
+// frost_update.cu
+int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
+                   int n_idx, int n_pad, double *out);
+int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
+                    int n_pad, double *out);
+int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
+                const int32_t *idx, int n_idx, double cc, double kappa);
+int launch_drift(frost_ctx *c, int ld, double *pos, const double *vel, const int32_t *idx,
+                 int n_idx, double cc);
+int launch_partition(frost_ctx *c, const double *tau, const int32_t *idx, int n_idx,
+                     double tau_pivot, int32_t *out_slow, int32_t *out_fast, int32_t *counts_host);
+// frost_sweeps.cu
+// One direction: sinks = stream A (n_snk real records, padded), sources = stream B.
+int sweep_newton(frost_ctx *c, const double *snk_xm, int n_snk, const double *src_xm, int n_src,
+                 const int32_t *snk_idx, int ld, double *out_acc, double *snk_a_packed);
+int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int n_snk,
+                   const double *src_xm, const double *src_a, int n_src, const int32_t *snk_idx,
+                   int ld, double *out_grad);
+int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set,
+                   const int32_t *idx, double tau_pivot, double *out_tau, int32_t *out_bin);
+
+// ---- device-side PTX helpers ------------------------------------------------------------------
+#ifdef __CUDACC__
+__device__ __forceinline__ uint32_t smem_u32(const void *p) {
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_fence_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)),
+        "r"(parity)
+        : "memory");
+}
+// 1-D TMA bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, uint32_t bytes,
+                                         uint64_t *bar) {
+    asm volatile(
+        "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::
+            "r"(smem_u32(dst_smem)),
+        "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
+        : "memory");
+}
+
+// fp64 reciprocal square root seed: MUFU.RSQ64H on the high word (rel. error ~2^-22), low word 0.
+// Returns exactly 0 when x is zero or subnormal (exponent field 0), which is how a coincident /
+// self pair is made to contribute nothing without an FP64-pipe compare.
+__device__ __forceinline__ double rsqrt_seed_or_zero(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const int hx = __double2hiint(x);
+    const int hy = __double2hiint(y);
+    return __hiloint2double(hx < 0x00100000 ? 0 : hy, 0);
+}
+// Full-precision 1/sqrt(x) from the seed by one cubic (Householder order 3) step: 5 FP64 slots.
+//   e = 1 - x y^2 ;  y' = y + y e (1/2 + 3/8 e)          (error ~ (5/16) e^3 ~ 2^-66 + rounding)
+__device__ __forceinline__ double rsqrt_full_or_zero(double x) {
+    const double y = rsqrt_seed_or_zero(x);
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double ye = y * e;
+    return fma(ye, p, y);
+}
+#endif
+
+}  // namespace frost

@@ -1,0 +1,191 @@
+// frost_update.cu -- the O(N), HBM-bound kernels of the path: gather/pack of the source and sink
+// streams (step 1), kick / kick_sf and drift (Eq. 6), and the stable
+// slow/fast partition (Eq. 29).
+#include "frost_common.cuh"
+
+namespace frost {
+
+// out[k] = {x,y,z,m} of particle idx[k]; zero records for n_idx <= k < n_pad.  One 32-byte record
+// per thread: two 16-byte stores, fully coalesced on the write side; reads are coalesced when idx
+// is NULL or ascending-dense.
+__global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__restrict__ mass, int ld,
+                               const int32_t *__restrict__ idx, int n_idx, int n_pad,
+                               double4 *__restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_pad) return;
+    double4 r = make_double4(0.0, 0.0, 0.0, 0.0);
+    if (k < n_idx) {
+        const int i = idx ? idx[k] : k;
+        r = make_double4(pos[i], pos[(size_t)ld + i], pos[2 * (size_t)ld + i], mass[i]);
+    }
+    out[k] = r;
+}
+
+// out[k] = {p_x, p_y, p_z, 1} of particle idx[k] (accelerations or velocities); zero padding.
+// The 1 marks a real record (the time-step sweep skips records whose flag is 0).
+__global__ void pack_vec_kernel(const double *__restrict__ planes, int ld,
+                                const int32_t *__restrict__ idx, int n_idx, int n_pad,
+                                double4 *__restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_pad) return;
+    double4 r = make_double4(0.0, 0.0, 0.0, 0.0);
+    if (k < n_idx) {
+        const int i = idx ? idx[k] : k;
+        r = make_double4(planes[i], planes[(size_t)ld + i], planes[2 * (size_t)ld + i], 1.0);
+    }
+    out[k] = r;
+}
+
+__global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__ acc,
+                            const double *__restrict__ grad, int ld, const int32_t *__restrict__ idx,
+                            int n_idx, double c, double kappa) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_idx) return;
+    const int i = idx ? idx[k] : k;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const size_t o = (size_t)d * ld + i;
+        double a = acc[o];
+        if (grad) a = fma(kappa, grad[o], a);
+        vel[o] = fma(c, a, vel[o]);
+    }
+}
+
+__global__ void drift_kernel(double *__restrict__ pos, const double *__restrict__ vel, int ld,
+                             const int32_t *__restrict__ idx, int n_idx, double c) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_idx) return;
+    const int i = idx ? idx[k] : k;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const size_t o = (size_t)d * ld + i;
+        pos[o] = fma(c, vel[o], pos[o]);
+    }
+}
+
+// ---- stable partition: count per block -> scan of block counts -> scatter ----------------------
+constexpr int kPartBlock = 1024;
+
+__device__ __forceinline__ int block_exclusive_scan_1024(int v, int *total) {
+    __shared__ int warp_sums[32];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) warp_sums[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int s = warp_sums[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, s, o);
+            if (lane >= o) s += t;
+        }
+        warp_sums[lane] = s;
+    }
+    __syncthreads();
+    const int base = (w > 0) ? warp_sums[w - 1] : 0;
+    *total = warp_sums[31];
+    __syncthreads();
+    return base + inc - v;
+}
+
+__global__ void __launch_bounds__(kPartBlock)
+part_count_kernel(const double *__restrict__ tau, const int32_t *__restrict__ idx, int n_idx,
+                  double pivot, int *__restrict__ block_counts) {
+    const int k = blockIdx.x * kPartBlock + threadIdx.x;
+    int slow = 0;
+    if (k < n_idx) slow = tau[idx ? idx[k] : k] >= pivot;
+    const int c = __syncthreads_count(slow);
+    if (threadIdx.x == 0) block_counts[blockIdx.x] = c;
+}
+
+// single block: exclusive scan of block_counts in place; counts[0] = |S|, counts[1] = |F|
+__global__ void __launch_bounds__(kPartBlock)
+part_scan_kernel(int *__restrict__ block_counts, int n_blocks, int n_idx, int *__restrict__ counts) {
+    int carry = 0;
+    for (int b0 = 0; b0 < n_blocks; b0 += kPartBlock) {
+        const int b = b0 + threadIdx.x;
+        const int v = (b < n_blocks) ? block_counts[b] : 0;
+        int total;
+        const int ex = block_exclusive_scan_1024(v, &total);
+        if (b < n_blocks) block_counts[b] = carry + ex;
+        carry += total;
+    }
+    if (threadIdx.x == 0) { counts[0] = carry; counts[1] = n_idx - carry; }
+}
+
+__global__ void __launch_bounds__(kPartBlock)
+part_scatter_kernel(const double *__restrict__ tau, const int32_t *__restrict__ idx, int n_idx,
+                    double pivot, const int *__restrict__ block_offsets,
+                    int32_t *__restrict__ out_slow, int32_t *__restrict__ out_fast) {
+    const int k = blockIdx.x * kPartBlock + threadIdx.x;
+    int slow = 0, i = 0;
+    if (k < n_idx) { i = idx ? idx[k] : k; slow = tau[i] >= pivot; }
+    int total;
+    const int ex = block_exclusive_scan_1024(slow, &total);
+    if (k < n_idx) {
+        const int slow_before = block_offsets[blockIdx.x] + ex;
+        if (slow) out_slow[slow_before] = i;
+        else out_fast[k - slow_before] = i;
+    }
+}
+
+// ---- launchers ---------------------------------------------------------------------------------
+int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
+                   int n_idx, int n_pad, double *out) {
+    if (n_pad <= 0) return FROST_OK;
+    pack_xm_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(pos, mass, ld, idx, n_idx, n_pad,
+                                                             (double4 *)out);
+    return check_launch(c);
+}
+
+int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
+                    int n_pad, double *out) {
+    if (n_pad <= 0) return FROST_OK;
+    pack_vec_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(planes, ld, idx, n_idx, n_pad,
+                                                              (double4 *)out);
+    return check_launch(c);
+}
+
+int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
+                const int32_t *idx, int n_idx, double cc, double kappa) {
+    if (n_idx <= 0) return FROST_OK;
+    kick_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(vel, acc, kappa != 0.0 ? grad : nullptr,
+                                                          ld, idx, n_idx, cc, kappa);
+    return check_launch(c);
+}
+
+int launch_drift(frost_ctx *c, int ld, double *pos, const double *vel, const int32_t *idx,
+                 int n_idx, double cc) {
+    if (n_idx <= 0) return FROST_OK;
+    drift_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(pos, vel, ld, idx, n_idx, cc);
+    return check_launch(c);
+}
+
+int launch_partition(frost_ctx *c, const double *tau, const int32_t *idx, int n_idx,
+                     double tau_pivot, int32_t *out_slow, int32_t *out_fast, int32_t *counts_host) {
+    if (n_idx <= 0) { counts_host[0] = counts_host[1] = 0; return FROST_OK; }
+    const int nb = (n_idx + kPartBlock - 1) / kPartBlock;
+    FROST_TRY(ensure(c, c->blockcnt, (size_t)(nb + 2) * sizeof(int)));
+    int *bc = (int *)c->blockcnt.p;
+    int *dcounts = bc + nb;
+    part_count_kernel<<<nb, kPartBlock, 0, c->stream>>>(tau, idx, n_idx, tau_pivot, bc);
+    FROST_TRY(check_launch(c));
+    part_scan_kernel<<<1, kPartBlock, 0, c->stream>>>(bc, nb, n_idx, dcounts);
+    FROST_TRY(check_launch(c));
+    part_scatter_kernel<<<nb, kPartBlock, 0, c->stream>>>(tau, idx, n_idx, tau_pivot, bc, out_slow,
+                                                        out_fast);
+    FROST_TRY(check_launch(c));
+    FROST_CUDA(c, cudaMemcpyAsync(c->pinned_counts, dcounts, 2 * sizeof(int), cudaMemcpyDeviceToHost,
+                                  c->stream));
+    FROST_CUDA(c, cudaStreamSynchronize(c->stream));
+    counts_host[0] = c->pinned_counts[0];
+    counts_host[1] = c->pinned_counts[1];
+    return FROST_OK;
+}
+
+}  // namespace frost

@@ -1,0 +1,220 @@
+"""Parity of the CUDA path (through the C-ABI binding) against the CPU oracle, element by element
+on the same seeded inputs.  Tolerances are north_star's, read per particle against the vector norm
+(reading 19): |da_k| <= 1e-12 |a_i|, |dg_k| <= 1e-10 |g_i|; bins identical; index work
+bit-exact."""
+import numpy as np
+import pytest
+import torch
+
+import frost_inputs as fi
+
+pytestmark = pytest.mark.gpu
+
+TOL_A, TOL_G, TOL_TAU = 1e-12, 1e-10, 1e-13
+
+
+@pytest.fixture(scope="module")
+def fr():
+    import paper_2011_14984_b200 as frost
+    f = frost.Frost()
+    yield f
+    f.close()
+
+
+def dev(a, dtype=None):
+    return torch.as_tensor(np.ascontiguousarray(a), dtype=dtype).cuda()
+
+
+def vec_err(x, ref):
+    """max over particles of max_k |dx_k| / |ref_i|_2 (particles with ref == 0 must match exactly)."""
+    nrm = np.linalg.norm(ref, axis=0)
+    d = np.abs(x - ref).max(axis=0)
+    ok0 = (nrm == 0)
+    assert (d[ok0] == 0).all()
+    return float((d[~ok0] / nrm[~ok0]).max()) if (~ok0).any() else 0.0
+
+
+def check_forces(fr, oracle, pos, mass, I=None, J=None, flags=3, G=1.0, eps2=0.0, acc0=None):
+    fr.set_params(G=G, eps2=eps2)
+    n = mass.size
+    a0 = np.zeros((3, n)) if acc0 is None else acc0.copy()
+    a_ref, g_ref = oracle.forces(pos, mass, sink_idx=I, source_idx=J, G=G, eps2=eps2, flags=flags,
+                                 acc=a0.copy(), grad=np.full((3, n), 5.0))
+    a_gpu = dev(a0)
+    g_gpu = torch.full((3, n), 5.0, dtype=torch.float64, device="cuda")
+    fr.forces(dev(pos), dev(mass), None if I is None else dev(I), None if J is None else dev(J),
+              out_acc=a_gpu, out_grad=g_gpu, flags=flags)
+    torch.cuda.synchronize()
+    a, g = a_gpu.cpu().numpy(), g_gpu.cpu().numpy()
+    ea = vec_err(a, a_ref)
+    eg = vec_err(g, g_ref) if flags & 2 else 0.0
+    assert ea <= TOL_A, ea
+    assert eg <= TOL_G, eg
+    return a, g, a_ref, g_ref
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 255, 256, 257, 1024, 3000])
+def test_self_forces_small_and_ragged(fr, oracle, n):
+    pos, vel, mass = fi.plummer(max(n, 2), 0)
+    pos, mass = np.ascontiguousarray(pos[:, :n]), mass[:n].copy()
+    check_forces(fr, oracle, pos, mass)
+
+
+@pytest.mark.parametrize("k,slices", [(1, 1), (1, 5), (2, 1), (2, 3), (4, 2), (0, 0)])
+def test_every_kernel_variant_and_slice_count(fr, oracle, k, slices):
+    pos, vel, mass = fi.plummer(5000, 7)
+    fr.set_tuning(k, slices)
+    try:
+        check_forces(fr, oracle, pos, mass, eps2=1e-6)
+    finally:
+        fr.set_tuning(0, 0)
+
+
+def test_softened_and_scaled_G(fr, oracle):
+    pos, vel, mass = fi.plummer(2048, 3)
+    check_forces(fr, oracle, pos, mass, G=6.674e-3, eps2=1e-4)
+
+
+def test_config1_plummer_1024_acc_grad(fr, oracle):
+    pos, vel, mass = fi.plummer(1024, 0)
+    a, g, _, _ = check_forces(fr, oracle, pos, mass)
+    assert np.abs((mass * a).sum(1)).max() < 1e-15 * (mass * np.abs(a)).sum(1).max()
+    assert np.abs((mass * g).sum(1)).max() < 1e-13 * (mass * np.abs(g)).sum(1).max()
+
+
+def test_sink_subset_vs_all_and_reverse_config4_shape(fr, oracle):
+    """Config 4's structure at N = 20000: A<-all, (all\\A)<-A, then both gradients; momentum of
+    the resulting kick vanishes to roundoff."""
+    n = 20000
+    pos, vel, mass = fi.plummer(n, 3)
+    for frac in (0.001, 0.01, 0.1):
+        A = fi.active_subset(n, frac, 3)
+        rest = np.setdiff1d(np.arange(n, dtype=np.int32), A).astype(np.int32)
+        a, _, a_ref, _ = check_forces(fr, oracle, pos, mass, I=A, J=None, flags=1)
+        a2, _, a_ref2, _ = check_forces(fr, oracle, pos, mass, I=rest, J=A, flags=1, acc0=a_ref)
+        _, g, _, g_ref = check_forces(fr, oracle, pos, mass, I=A, J=None, flags=2, acc0=a_ref2)
+        _, g2, _, _ = check_forces(fr, oracle, pos, mass, I=rest, J=A, flags=2, acc0=a_ref2)
+        gt = g.copy(); gt[:, rest] = g2[:, rest]
+        assert np.abs((mass * a2).sum(1)).max() < 1e-14 * (mass * np.abs(a2)).sum(1).max()
+        assert np.abs((mass * gt).sum(1)).max() < 1e-12 * (mass * np.abs(gt)).sum(1).max()
+
+
+def test_mutual_slow_fast_sets(fr, oracle):
+    n = 3000
+    pos, vel, mass = fi.plummer(n, 5)
+    rng = np.random.default_rng(1)
+    perm = rng.permutation(n).astype(np.int32)
+    S, F = np.sort(perm[:700]), np.sort(perm[700:2500])      # 500 particles in neither set
+    a, g, a_ref, g_ref = check_forces(fr, oracle, pos, mass, I=S, J=F, flags=7)
+    out = np.sort(perm[2500:])
+    assert (a[:, out] == 0).all() and (g[:, out] == 5.0).all()   # untouched outside S u F
+
+
+def test_empty_and_degenerate_sets(fr, oracle):
+    pos, vel, mass = fi.plummer(300, 2)
+    e = np.zeros(0, dtype=np.int32)
+    one = np.array([17], dtype=np.int32)
+    check_forces(fr, oracle, pos, mass, I=e, J=None, flags=3)
+    check_forces(fr, oracle, pos, mass, I=one, J=one, flags=3)
+    check_forces(fr, oracle, pos, mass, I=one, J=e, flags=1)
+    # two coincident unsoftened particles are ignored pairwise (reading 11)
+    p2 = pos.copy(); p2[:, 5] = p2[:, 9]
+    check_forces(fr, oracle, p2, mass)
+
+
+def test_run_to_run_bitwise_determinism(fr):
+    pos, vel, mass = fi.plummer(40000, 9)
+    p, m = dev(pos), dev(mass)
+    a1, g1 = fr.forces(p, m)
+    a2, g2 = fr.forces(p, m)
+    torch.cuda.synchronize()
+    assert torch.equal(a1, a2) and torch.equal(g1, g2)
+
+
+@pytest.mark.parametrize("n", [2, 100, 1000, 4097])
+def test_timesteps_and_bins(fr, oracle, n):
+    pos, vel, mass = fi.plummer(n, 4)
+    fr.set_params(G=1.0, eta_ff=0.2, eta_fb=0.2)
+    pivot = 1.0 / 64
+    tau_ref, bin_ref = oracle.timesteps(pos, vel, mass, tau_pivot=pivot)
+    tau, bins = fr.timesteps(dev(pos), dev(vel), dev(mass), tau_pivot=pivot)
+    tau, bins = tau.cpu().numpy(), bins.cpu().numpy()
+    np.testing.assert_allclose(tau, tau_ref, rtol=TOL_TAU)
+    bad = np.nonzero(bins != bin_ref)[0]
+    for i in bad:      # accepted only within 1e-13 of a bin edge (reading 20); expected count 0
+        edge = pivot * 2.0 ** -min(bins[i], bin_ref[i])
+        assert abs(tau_ref[i] / edge - 1) < 1e-13
+    assert bad.size == 0
+
+
+def test_timesteps_on_level_subset_and_partition(fr, oracle):
+    n = 5000
+    pos, vel, mass = fi.plummer(n, 6)
+    idx = fi.active_subset(n, 0.3, 6)
+    fr.set_params(eta_ff=0.1, eta_fb=0.3)
+    tau_ref, _ = oracle.timesteps(pos, vel, mass, idx=idx, eta_ff=0.1, eta_fb=0.3)
+    tau, _ = fr.timesteps(dev(pos), dev(vel), dev(mass), idx=dev(idx), want_bins=False)
+    t = tau.cpu().numpy()
+    np.testing.assert_allclose(t[idx], tau_ref[idx], rtol=TOL_TAU)
+    assert np.isinf(np.delete(t, idx)).all()
+    fr.set_params()
+    pivot = float(np.median(tau_ref[idx]))
+    slow, fast = fr.partition(dev(tau_ref), pivot, idx=dev(idx))
+    s_ref = idx[tau_ref[idx] >= pivot]; f_ref = idx[tau_ref[idx] < pivot]
+    assert np.array_equal(slow.cpu().numpy(), s_ref) and np.array_equal(fast.cpu().numpy(), f_ref)
+    slow, fast = fr.partition(dev(tau_ref), 0.0)                 # all slow, idx = None
+    assert slow.numel() == n and fast.numel() == 0
+    assert np.array_equal(slow.cpu().numpy(), np.arange(n))
+
+
+def test_kick_drift_gather(fr, oracle):
+    n = 3333
+    rng = np.random.default_rng(0)
+    pos, vel, mass = fi.plummer(n, 8)
+    acc = np.ascontiguousarray(rng.normal(size=(3, n))); grad = np.ascontiguousarray(rng.normal(size=(3, n)))
+    idx = fi.active_subset(n, 0.5, 8)
+    for ii in (None, idx):
+        v_ref, p_ref = vel.copy(), pos.copy()
+        oracle.kick(v_ref, acc, grad, idx=ii, c=0.37, kappa=0.011)
+        oracle.drift(p_ref, v_ref, idx=ii, c=0.21)
+        v, p = dev(vel), dev(pos)
+        fr.kick(v, dev(acc), dev(grad), idx=None if ii is None else dev(ii), c=0.37, kappa=0.011)
+        fr.drift(p, v, idx=None if ii is None else dev(ii), c=0.21)
+        np.testing.assert_allclose(v.cpu().numpy(), v_ref, rtol=0, atol=4e-16 * np.abs(v_ref).max())
+        np.testing.assert_allclose(p.cpu().numpy(), p_ref, rtol=0, atol=4e-16 * np.abs(p_ref).max())
+    rec = fr.gather_pack(dev(pos), dev(mass), idx=dev(idx), n_pad=idx.size + 7).cpu().numpy()
+    assert np.array_equal(rec[: idx.size, :3], pos[:, idx].T) and np.array_equal(rec[: idx.size, 3], mass[idx])
+    assert (rec[idx.size:] == 0).all()
+
+
+def test_config1_ten_fsi_steps(fr, oracle):
+    """Config 1: N = 1024, 10 fixed-step FSI steps with dt = 1/1024."""
+    pos, vel, mass = fi.plummer(1024, 0)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    fr.set_params()
+    pr, vr = pos.copy(), vel.copy()
+    d0 = oracle.diagnostics(pos, vel, mass)
+    for _ in range(10):
+        fr.fsi_step(p, v, m, 1.0 / 1024)
+        oracle.fsi_step(pr, vr, mass, 1.0 / 1024)
+    pg, vg = p.cpu().numpy(), v.cpu().numpy()
+    assert np.abs(pg - pr).max() < 1e-11 and np.abs(vg - vr).max() < 1e-10
+    d1 = oracle.diagnostics(pg, vg, mass)
+    assert np.abs(d1["P"] - d0["P"]).max() < 1e-15
+    assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-13
+
+
+def test_hhs_step_small_cluster(fr, oracle):
+    """Reduced-N replica of config 5: level sets, bookkeeping and the trajectory must match."""
+    n = 1024
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    pr, vr = pos.copy(), vel.copy()
+    st_ref = oracle.hhs_step(pr, vr, mass, 1.0 / 256)
+    p, v = dev(pos), dev(vel)
+    st = fr.hhs_step(p, v, dev(mass), 1.0 / 256)
+    assert st == st_ref
+    assert st["depth"] >= 3
+    pg, vg = p.cpu().numpy(), v.cpu().numpy()
+    assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
+    assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
