@@ -100,6 +100,8 @@ def _idx(t: Optional[torch.Tensor], name: str):
         return None, 0
     if not (t.is_cuda and t.dtype == torch.int32 and t.dim() == 1 and t.is_contiguous()):
         raise FrostError(f"{name}: expected a contiguous CUDA int32 vector or None")
+    if t.numel() == 0:      # an empty list is not "all particles": pass a non-NULL pointer, count 0
+        return torch.zeros(1, dtype=torch.int32, device=t.device), 0
     return t, t.numel()
 
 
