@@ -164,15 +164,31 @@ __device__ __forceinline__ double rsqrt_seed_or_zero(double x) {
     const int hy = __double2hiint(y);
     return __hiloint2double(hx < 0x00100000 ? 0 : hy, 0);
 }
+// Unguarded seed (caller guarantees x is a positive normal number).
+__device__ __forceinline__ double rsqrt_seed(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return y;
+}
+// x += w*dx; y += w*dy; z += w*dz as three adjacent DFMAs with w in the same operand slot.
+__device__ __forceinline__ void fma3_shared(double &x, double &y, double &z, double w, double dx,
+                                            double dy, double dz) {
+    asm("fma.rn.f64 %0, %3, %4, %0;\n\t"
+        "fma.rn.f64 %1, %3, %5, %1;\n\t"
+        "fma.rn.f64 %2, %3, %6, %2;"
+        : "+d"(x), "+d"(y), "+d"(z)
+        : "d"(w), "d"(dx), "d"(dy), "d"(dz));
+}
 // Full-precision 1/sqrt(x) from the seed by one cubic (Householder order 3) step: 5 FP64 slots.
-//   e = 1 - x y^2 ;  y' = y + y e (1/2 + 3/8 e)          (error ~ (5/16) e^3 ~ 2^-66 + rounding)
+//   e = 1 - x y^2 ;  y' = y + y (e (1/2 + 3/8 e))        (error ~ (5/16) e^3 ~ 2^-66 + rounding)
+// The last FMA reads only two distinct register pairs (y twice), so it issues in 2 cycles.
 __device__ __forceinline__ double rsqrt_full_or_zero(double x) {
     const double y = rsqrt_seed_or_zero(x);
     const double t = x * y;
     const double e = fma(-t, y, 1.0);
     const double p = fma(0.375, e, 0.5);
-    const double ye = y * e;
-    return fma(ye, p, y);
+    const double ep = e * p;
+    return fma(y, ep, y);
 }
 #endif
 

@@ -40,13 +40,18 @@ struct NewtonPolicy {
         s.x = r.x; s.y = r.y; s.z = r.z;
     }
     __device__ static __forceinline__ void init(Acc &a) { a.x = a.y = a.z = 0.0; }
-    // Eq. (24): a_i += m_j x_ji / s^3.  16 FP64-pipe instructions + 1 MUFU + 1 ISETP + 1 SEL.
+    // Eq. (24): a_i += m_j x_ji / s^3.  16 FP64-pipe instructions + 1 MUFU, nothing else.
     // w = m y^3 (1-e)^(-3/2) with e = 1 - s2 y^2 ~ 2^-22: series to e^2 (next term 35/16 e^3).
+    // p.eps2 is floored at 2^-400 by the launcher, so s2 > 0 and the MUFU seed is finite without
+    // any guard: the self pair then has dx = dy = dz = 0 exactly and a finite w, and adds 0.
+    // The three accumulating FMAs share w in the same operand slot and are kept adjacent so that
+    // the operand-reuse cache serves it (a DFMA reading three distinct register pairs costs 3
+    // issue cycles instead of 2 on sm_100a -- DESIGN.md "FP64 issue model").
     __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
                                                 const double4 &, const SweepParams &p) {
         const double dx = j0.x - s.x, dy = j0.y - s.y, dz = j0.z - s.z;
         const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
-        const double y = rsqrt_seed_or_zero(s2);
+        const double y = rsqrt_seed(s2);
         const double y2 = y * y;
         const double e = fma(-s2, y2, 1.0);
         const double ym = y * j0.w;
@@ -54,9 +59,7 @@ struct NewtonPolicy {
         const double q = fma(1.875, e, 1.5);
         const double qe = q * e;
         const double w = fma(w0, qe, w0);
-        a.x = fma(w, dx, a.x);
-        a.y = fma(w, dy, a.y);
-        a.z = fma(w, dz, a.z);
+        fma3_shared(a.x, a.y, a.z, w, dx, dy, dz);
     }
     __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
         part[i] = a.x; part[n_pad + i] = a.y; part[2 * n_pad + i] = a.z;
@@ -87,10 +90,9 @@ struct GradientPolicy {
         const double w3 = mr * q;
         const double t = q * dot;
         const double u = t * -3.0;
-        const double vx = fma(u, dx, ax), vy = fma(u, dy, ay), vz = fma(u, dz, az);
-        g.x = fma(w3, vx, g.x);
-        g.y = fma(w3, vy, g.y);
-        g.z = fma(w3, vz, g.z);
+        double vx = ax, vy = ay, vz = az;
+        fma3_shared(vx, vy, vz, u, dx, dy, dz);
+        fma3_shared(g.x, g.y, g.z, w3, vx, vy, vz);
     }
     __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
         part[i] = a.x; part[n_pad + i] = a.y; part[2 * n_pad + i] = a.z;
@@ -200,7 +202,7 @@ sweep_kernel(const SweepParams prm) {
         mbar_wait(&full[s], (uint32_t)(t / kStages) & 1u);
         const double4 *t0 = tiles + (size_t)s * P::kRecs * kTile;
         const double4 *t1 = t0 + (P::kRecs == 2 ? kTile : 0);
-#pragma unroll 2
+#pragma unroll 4
         for (int j = 0; j < kTile; ++j) {
             const double4 j0 = t0[j];
             const double4 j1 = (P::kRecs == 2) ? t1[j] : j0;
@@ -333,7 +335,9 @@ int sweep_newton(frost_ctx *c, const double *snk_xm, int n_snk, const double *sr
     prm.snk1 = nullptr; prm.src1 = nullptr;
     prm.partial = (double *)c->partial.p; prm.n_pad = n_pad;
     prm.n_tiles = pl.n_tiles; prm.tiles_per_slice = pl.tiles_per_slice;
-    prm.eps2 = c->eps2; prm.G = c->G; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+    // floor: keeps the unguarded rsqrt seed finite for the self pair (see NewtonPolicy::pair)
+    prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
+    prm.G = c->G; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
     if (n_src <= 0) { prm.n_tiles = 0; }
     FROST_TRY(launch_sweep<NewtonPolicy>(c, prm, pl));
     reduce_vec_kernel<<<(n_snk + 255) / 256, 256, 0, c->stream>>>(
