@@ -273,10 +273,12 @@ static Plan make_plan(const frost_ctx *c, int n_snk, int n_src, int max_k) {
     Plan pl;
     pl.n_tiles = (n_src + kTile - 1) / kTile;
     if (pl.n_tiles < 1) pl.n_tiles = 1;
-    // sinks per thread: more register blocking once the sink set fills the machine several times
+    // sinks per thread: register blocking amortises the per-source LDS/loop/MUFU issue slots
+    // (measured on B200: K=4 wins from ~32k sinks, K=2 from ~8k; below that K=1 with 128-thread
+    // CTAs wastes the fewest lanes in the last sink block)
     int k = 1;
-    const long long per_wave1 = (long long)c->num_sms * 4 * 128;
-    if (n_snk >= 4 * per_wave1) k = 2;
+    if (n_snk >= 8192) k = 2;
+    if (n_snk >= 32768) k = 4;
     if (c->tune_k > 0) k = c->tune_k;
     if (k > max_k) k = max_k;
     pl.k = k;
