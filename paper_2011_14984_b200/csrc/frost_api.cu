@@ -138,7 +138,7 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
     double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
-    FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm));
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, c->G, 1));   // .w = G m, NaN padding
     FROST_TRY(launch_pack_vec(c, ld, vel, idx, n_idx, pad, v));
     return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
 }

@@ -92,8 +92,9 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 // ---- launchers implemented in the other translation units ------------------------------------
 // frost_update.cu
+// wscale multiplies the mass written to .w; nan_pad != 0 pads with NaN positions instead of zeros
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
-                   int n_idx, int n_pad, double *out);
+                   int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0);
 int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
                     int n_pad, double *out);
 int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
@@ -189,6 +190,24 @@ __device__ __forceinline__ double rsqrt_full_or_zero(double x) {
     const double p = fma(0.375, e, 0.5);
     const double ep = e * p;
     return fma(y, ep, y);
+}
+// Unguarded full-precision 1/sqrt(x): x = 0 gives NaN (MUFU(0) = +inf, 0*inf), NaN propagates.
+__device__ __forceinline__ double rsqrt_full(double x) {
+    const double y = rsqrt_seed(x);
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double ep = e * p;
+    return fma(y, ep, y);
+}
+// Full-precision 1/x for x in the normal range: MUFU.RCP64H seed + one cubic step
+//   e = 1 - x y ;  y' = y + y (e + e^2)                   (error ~ e^3 ~ 2^-66 + rounding)
+__device__ __forceinline__ double rcp_full(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    const double ee = fma(e, e, e);
+    return fma(y, ee, y);
 }
 #endif
 

@@ -100,25 +100,33 @@ struct GradientPolicy {
 };
 
 // Harmonic symmetrisation factor of Eq. (49) in the cancellation-free form 1 + q/(1+sqrt(1+q^2))
-// (reading 10).
+// (reading 10), without IEEE sqrt/div sequences: with u = 1/sqrt(1+q^2) in (0,1],
+//   q/(1+sqrt(1+q^2)) = q u / (1 + u);  1/(1+u) by MUFU.RCP64H + one cubic step.  13 FP64 instr.
 __device__ __forceinline__ double sym_factor(double q) {
-    return 1.0 + q / (1.0 + sqrt(fma(q, q, 1.0)));
+    const double h = fma(q, q, 1.0);
+    const double u = rsqrt_full(h);
+    const double qu = q * u;
+    const double d = u + 1.0;
+    const double rd = rcp_full(d);
+    return fma(qu, rd, 1.0);
 }
 
 struct TimestepPolicy {
     static constexpr int kRecs = 2;
     static constexpr int kPlanes = 1;
-    struct Sink { double x, y, z, m, vx, vy, vz; };
+    struct Sink { double x, y, z, gm, vx, vy, vz; };
     struct Acc { double tau; };
     __device__ static __forceinline__ void load(Sink &s, const SweepParams &p, int i) {
         const double4 r = p.snk0[i];
         const double4 v = p.snk1[i];
-        s.x = r.x; s.y = r.y; s.z = r.z; s.m = r.w; s.vx = v.x; s.vy = v.y; s.vz = v.z;
+        s.x = r.x; s.y = r.y; s.z = r.z; s.gm = r.w; s.vx = v.x; s.vy = v.y; s.vz = v.z;
     }
     __device__ static __forceinline__ void init(Acc &a) { a.tau = __longlong_as_double(0x7ff0000000000000LL); }
     // Eq. (50)-(54) + Eq. (49) per ordered pair, min over the candidates.
-    // The velocity record carries a validity flag in .w (1 for a real particle, 0 for padding), so
-    // zero padding is skipped without constraining real masses.
+    // The position record carries G*m in .w.  No branch and no compare: the self pair (r2 = 0), a
+    // padding record (NaN position) and a pair at rest (v2 = 0, fly-by only) turn into NaN through
+    // MUFU(0) = +inf and 0*inf, and fmin() returns its non-NaN operand, so such candidates drop out
+    // exactly as DESIGN.md reading 11 requires.  ~77 FP64 instructions + 7 MUFU per pair.
     __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
                                                 const double4 &j1, const SweepParams &p) {
         const double rx = j0.x - s.x, ry = j0.y - s.y, rz = j0.z - s.z;
@@ -126,22 +134,20 @@ struct TimestepPolicy {
         const double r2 = fma(rz, rz, fma(ry, ry, rx * rx));
         const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
         const double rv = fma(rz, vz, fma(ry, vy, rx * vx));
-        const bool live = (__double2hiint(r2) >= 0x00100000) && (j1.w != 0.0);
-        if (live) {
-            const double r = sqrt(r2);
-            const double mu = p.G * (s.m + j0.w);
-            const double rvr2 = rv / r2;
-            const double t_ff = sqrt(r2 * r / mu);
-            const double q_ff = p.eta_ff * (1.5 * rvr2 * t_ff);
-            const double c_ff = sym_factor(q_ff) * (p.eta_ff * t_ff);
-            a.tau = fmin(a.tau, c_ff);
-            if (v2 > 0.0) {
-                const double t_fb = r / sqrt(v2);
-                const double q_fb = p.eta_fb * (rvr2 * (1.0 + mu / (v2 * r)) * t_fb);
-                const double c_fb = sym_factor(q_fb) * (p.eta_fb * t_fb);
-                a.tau = fmin(a.tau, c_fb);
-            }
-        }
+        const double mu = s.gm + j0.w;                 // G (m_i + m_j)
+        const double ir = rsqrt_full(r2);              // 1/r       (NaN for r2 = 0)
+        const double iv = rsqrt_full(v2);              // 1/v       (NaN for v2 = 0)
+        const double ir2 = ir * ir;
+        const double mir = mu * ir;
+        const double t_ff = rsqrt_full(mir * ir2);     // Eq. 50: (r^3/mu)^(1/2) = (mu/r^3)^(-1/2)
+        const double t_fb = (r2 * ir) * iv;            // Eq. 51: r / v
+        const double rvr2 = rv * ir2;                  // (r.v)/r^2
+        const double q_ff = (rvr2 * t_ff) * (1.5 * p.eta_ff);                 // eta * Eq. 53
+        const double f = rvr2 * t_fb;
+        const double q_fb = fma(f, mir * (iv * iv), f) * p.eta_fb;            // eta * Eq. 54
+        const double c_ff = sym_factor(q_ff) * (t_ff * p.eta_ff);
+        const double c_fb = sym_factor(q_fb) * (t_fb * p.eta_fb);
+        a.tau = fmin(a.tau, fmin(c_ff, c_fb));
     }
     __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
         part[i] = a.tau;

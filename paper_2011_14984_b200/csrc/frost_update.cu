@@ -10,13 +10,14 @@ namespace frost {
 // is NULL or ascending-dense.
 __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__restrict__ mass, int ld,
                                const int32_t *__restrict__ idx, int n_idx, int n_pad,
-                               double4 *__restrict__ out) {
+                               double4 *__restrict__ out, double wscale, int nan_pad) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_pad) return;
-    double4 r = make_double4(0.0, 0.0, 0.0, 0.0);
+    const double fill = nan_pad ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
+    double4 r = make_double4(fill, fill, fill, 0.0);
     if (k < n_idx) {
         const int i = idx ? idx[k] : k;
-        r = make_double4(pos[i], pos[(size_t)ld + i], pos[2 * (size_t)ld + i], mass[i]);
+        r = make_double4(pos[i], pos[(size_t)ld + i], pos[2 * (size_t)ld + i], mass[i] * wscale);
     }
     out[k] = r;
 }
@@ -136,10 +137,10 @@ part_scatter_kernel(const double *__restrict__ tau, const int32_t *__restrict__ 
 
 // ---- launchers ---------------------------------------------------------------------------------
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
-                   int n_idx, int n_pad, double *out) {
+                   int n_idx, int n_pad, double *out, double wscale, int nan_pad) {
     if (n_pad <= 0) return FROST_OK;
     pack_xm_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(pos, mass, ld, idx, n_idx, n_pad,
-                                                             (double4 *)out);
+                                                             (double4 *)out, wscale, nan_pad);
     return check_launch(c);
 }
 
