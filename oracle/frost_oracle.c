@@ -272,6 +272,38 @@ int oracle_timesteps(int n, int ld, const double *pos, const double *vel, const 
     return ORACLE_OK;
 }
 
+/* Same definition, evaluated only for the sinks listed in `sel` (a subset of the level `idx`):
+ * tau_i = min over ALL other members j of the level.  Lets the tests check sampled outputs of a
+ * level too large for a full O(n^2) oracle pass. */
+int oracle_timesteps_sampled(int n, int ld, const double *pos, const double *vel,
+                             const double *mass, const int32_t *idx, int n_idx,
+                             const int32_t *sel, int n_sel, double G, double eta_ff,
+                             double eta_fb, int eta_in_q, double tau_pivot, double *out_tau,
+                             int32_t *out_bin) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !out_tau || !sel) return ORACLE_EINVAL;
+    if (!idx) n_idx = n;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int a = 0; a < n_sel; ++a) {
+        const int i = sel[a];
+        const double xi[3] = {pos[i], pos[ld + i], pos[2 * ld + i]};
+        const double vi[3] = {vel[i], vel[ld + i], vel[2 * ld + i]};
+        double tau = INFINITY;
+        for (int b = 0; b < n_idx; ++b) {
+            const int j = pick(idx, b);
+            if (j == i) continue;
+            const double xj[3] = {pos[j], pos[ld + j], pos[2 * ld + j]};
+            const double vj[3] = {vel[j], vel[ld + j], vel[2 * ld + j]};
+            double c[2];
+            oracle_pair_timestep(xi, vi, mass[i], xj, vj, mass[j], G, eta_ff, eta_fb, eta_in_q, c);
+            if (c[0] < tau) tau = c[0];
+            if (c[1] < tau) tau = c[1];
+        }
+        out_tau[i] = tau;
+        if (out_bin) out_bin[i] = bin_of(tau, tau_pivot);
+    }
+    return ORACLE_OK;
+}
+
 /* ---------------------------------------------------------------------------------------------
  * O4.  kick and drift, Eq. (6); Alg. 2; kick_sf PAPER.md:596-597.
  *     kick : v_i <- v_i + c (a_i + kappa g_i)      (kappa = eps^2/48 forms a~ of Eq. 28, or 0)

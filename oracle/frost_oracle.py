@@ -110,6 +110,24 @@ def timesteps(pos, vel, mass, idx=None, G=1.0, eta_ff=0.2, eta_fb=0.2, tau_pivot
     return tau, bins
 
 
+def timesteps_sampled(pos, vel, mass, sel, idx=None, G=1.0, eta_ff=0.2, eta_fb=0.2, tau_pivot=1.0,
+                      eta_in_q=True):
+    """tau and bin of the sinks in `sel` only, each against every member of the level `idx`."""
+    ld = pos.shape[1]
+    n = mass.shape[0]
+    tau = np.full(ld, np.inf)
+    bins = np.zeros(ld, dtype=np.int32)
+    ii, ni = _i(idx)
+    ss, nsel = _i(sel)
+    rc = lib().oracle_timesteps_sampled(C.c_int(n), C.c_int(ld), _d(pos), _d(vel), _d(mass),
+                                        _ptr(ii), C.c_int(ni), _ptr(ss), C.c_int(nsel),
+                                        C.c_double(G), C.c_double(eta_ff), C.c_double(eta_fb),
+                                        C.c_int(1 if eta_in_q else 0), C.c_double(tau_pivot),
+                                        _d(tau), _ptr(bins))
+    _check(rc, "oracle_timesteps_sampled")
+    return tau, bins
+
+
 def pair_timestep(xi, vi, mi, xj, vj, mj, G=1.0, eta_ff=0.2, eta_fb=0.2, eta_in_q=True):
     out = (C.c_double * 2)()
     arr = lambda v: (C.c_double * 3)(*[float(t) for t in v])

@@ -1,0 +1,154 @@
+"""Parity at BASELINE.json's full sizes, in the launch configuration bench.py times (planner on
+auto).  Where the oracle cannot finish a full pass in seconds, sampled sinks are compared one by one
+(each sink's sum is a pure function of the inputs, so a sample is exact evidence for those
+outputs) and size-independent properties (momentum, bitwise determinism) cover the rest."""
+import numpy as np
+import pytest
+import torch
+
+import frost_inputs as fi
+
+pytestmark = pytest.mark.gpu
+TOL_A, TOL_G, TOL_TAU = 1e-12, 1e-10, 1e-13
+
+
+@pytest.fixture(scope="module")
+def fr():
+    import paper_2011_14984_b200 as frost
+    f = frost.Frost()
+    yield f
+    f.close()
+
+
+def dev(a):
+    return torch.as_tensor(np.ascontiguousarray(a)).cuda()
+
+
+def rel(x, ref):
+    return float((np.abs(x - ref).max(0) / np.linalg.norm(ref, axis=0)).max())
+
+
+def test_config2_full_pass_n65536(fr, oracle):
+    """Config 2: N = 65536, full self acc+gradient pass plus the pairwise time-step pass, every
+    output compared."""
+    n = 65536
+    pos, vel, mass = fi.plummer(n, 1)
+    fr.set_params()
+    a, g = fr.forces(dev(pos), dev(mass))
+    tau, bins = fr.timesteps(dev(pos), dev(vel), dev(mass), tau_pivot=1.0 / 128)
+    torch.cuda.synchronize()
+    a_ref, g_ref = oracle.forces(pos, mass)
+    tau_ref, bin_ref = oracle.timesteps(pos, vel, mass, tau_pivot=1.0 / 128)
+    a, g = a.cpu().numpy(), g.cpu().numpy()
+    assert rel(a, a_ref) <= TOL_A and rel(g, g_ref) <= TOL_G
+    np.testing.assert_allclose(tau.cpu().numpy(), tau_ref, rtol=TOL_TAU)
+    assert np.array_equal(bins.cpu().numpy(), bin_ref)
+    assert np.abs((mass * a).sum(1)).max() < 1e-15 * (mass * np.abs(a)).sum(1).max()
+    assert np.abs((mass * g).sum(1)).max() < 1e-13 * (mass * np.abs(g)).sum(1).max()
+
+
+def test_config3_headline_pass_n2pow20_sampled(fr, oracle):
+    """Config 3: N = 2^20 full pass; 384 random sinks compared one by one.  The oracle's gradient
+    sum is fed the GPU's full acceleration array (step 3 is a pure function of (x, m, a)), the
+    acceleration sample itself is checked end to end."""
+    n = 1 << 20
+    pos, vel, mass = fi.plummer(n, 2)
+    fr.set_params()
+    p, m = dev(pos), dev(mass)
+    a, g = fr.forces(p, m)
+    a2, g2 = fr.forces(p, m)
+    torch.cuda.synchronize()
+    assert torch.equal(a, a2) and torch.equal(g, g2)                  # bitwise reproducible
+    a, g = a.cpu().numpy(), g.cpu().numpy()
+    s = fi.active_subset(n, 384 / n, 77)
+    a_ref = np.zeros((3, n)); g_ref = np.zeros((3, n))
+    oracle.forces(pos, mass, sink_idx=s, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+    assert rel(a[:, s], a_ref[:, s]) <= TOL_A
+    a_in = a.copy()
+    oracle.forces(pos, mass, sink_idx=s, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+    assert rel(g[:, s], g_ref[:, s]) <= TOL_G
+    assert np.abs((mass * a).sum(1)).max() < 1e-14 * (mass * np.abs(a)).sum(1).max()
+    assert np.abs((mass * g).sum(1)).max() < 1e-12 * (mass * np.abs(g)).sum(1).max()
+
+
+@pytest.mark.parametrize("frac", [0.001, 0.01, 0.1])
+def test_config4_active_subsets_n2pow20(fr, oracle, frac):
+    """Config 4: active set A (0.1 %, 1 %, 10 % of N = 2^20) against all sources, the reverse
+    (all \\ A) <- A, both gradients, then the momentum-conserving kick of every particle."""
+    n = 1 << 20
+    pos, vel, mass = fi.plummer(n, 3)
+    A = fi.active_subset(n, frac, 3)
+    rest = np.setdiff1d(np.arange(n, dtype=np.int32), A).astype(np.int32)
+    fr.set_params()
+    p, m, v = dev(pos), dev(mass), dev(vel)
+    dA, dR = dev(A), dev(rest)
+    acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+    import paper_2011_14984_b200 as frost
+    fr.forces(p, m, sink_idx=dA, source_idx=None, out_acc=acc, out_grad=grad, flags=frost.ACC)
+    fr.forces(p, m, sink_idx=dR, source_idx=dA, out_acc=acc, out_grad=grad, flags=frost.ACC)
+    fr.forces(p, m, sink_idx=dA, source_idx=None, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+    fr.forces(p, m, sink_idx=dR, source_idx=dA, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+    dt = 1.0 / 1024
+    fr.kick(v, acc, grad, idx=None, c=2 * dt / 3, kappa=dt * dt / 48)
+    torch.cuda.synchronize()
+    a, g, vk = acc.cpu().numpy(), grad.cpu().numpy(), v.cpu().numpy()
+    # sampled parity: 128 sinks of A (sources: all) and 128 of the rest (sources: A)
+    sA, sR = A[:: max(1, A.size // 128)][:128], rest[:: rest.size // 128][:128]
+    a_ref = np.zeros((3, n)); g_ref = np.zeros((3, n))
+    oracle.forces(pos, mass, sink_idx=sA, source_idx=None, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+    oracle.forces(pos, mass, sink_idx=sR, source_idx=A, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+    assert rel(a[:, sA], a_ref[:, sA]) <= TOL_A and rel(a[:, sR], a_ref[:, sR]) <= TOL_A
+    a_in = a.copy()
+    oracle.forces(pos, mass, sink_idx=sA, source_idx=None, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+    oracle.forces(pos, mass, sink_idx=sR, source_idx=A, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+    assert rel(g[:, sA], g_ref[:, sA]) <= TOL_G and rel(g[:, sR], g_ref[:, sR]) <= TOL_G
+    # pairwise (momentum-conserving) kick: sum m dv = 0 to roundoff
+    dP = (mass * (vk - vel)).sum(1)
+    scale = (mass * np.abs(vk - vel)).sum(1).max()
+    assert np.abs(dP).max() < 1e-13 * scale
+
+
+def test_config5_first_level_n262144(fr, oracle):
+    """Config 5 at full size: the first hierarchy entry -- time-steps of all N = 262144 particles
+    (sampled sinks), their bins, and the slow/fast partition at dt_top = 2^-7 (bit-exact given
+    tau) -- plus the first inter-level sweep S<->F (sampled)."""
+    n = 262144
+    pos, vel, mass, pairs = fi.star_cluster(n, 4)
+    pivot = 2.0 ** -7
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    tau, bins = fr.timesteps(p, v, m, tau_pivot=pivot)
+    slow, fast = fr.partition(tau, pivot)
+    torch.cuda.synchronize()
+    tau_h, bins_h = tau.cpu().numpy(), bins.cpu().numpy()
+    s = np.concatenate([[0], pairs[:64].ravel(), fi.active_subset(n, 256 / n, 9)]).astype(np.int32)
+    # sampled sinks (central mass, binary members, random stars), each against the whole level
+    tau_ref, bin_ref = oracle.timesteps_sampled(pos, vel, mass, s, tau_pivot=pivot)
+    np.testing.assert_allclose(tau_h[s], tau_ref[s], rtol=TOL_TAU)
+    assert np.array_equal(bins_h[s], bin_ref[s])
+    k = bins_h.astype(np.float64)
+    ok = np.isfinite(tau_h)
+    assert (pivot * 2.0 ** -k[ok] <= tau_h[ok]).all()
+    assert ((k[ok] == 0) | (tau_h[ok] < pivot * 2.0 ** -(k[ok] - 1))).all()
+    idx = np.arange(n, dtype=np.int32)
+    assert np.array_equal(slow.cpu().numpy(), idx[tau_h >= pivot])
+    assert np.array_equal(fast.cpu().numpy(), idx[tau_h < pivot])
+    assert fast.numel() >= 2 * pairs.shape[0] * 0.9 and bins_h.max() >= 10
+    # first inter-level sweep, both directions, sampled
+    import paper_2011_14984_b200 as frost
+    S, F = slow.cpu().numpy(), fast.cpu().numpy()
+    acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+    fr.forces(p, m, sink_idx=slow, source_idx=fast, out_acc=acc, out_grad=grad,
+              flags=frost.ACC | frost.GRAD | frost.MUTUAL)
+    torch.cuda.synchronize()
+    a, g = acc.cpu().numpy(), grad.cpu().numpy()
+    sS, sF = S[:: S.size // 64][:64], F[:: F.size // 64][:64]
+    a_ref = np.zeros((3, n)); g_ref = np.zeros((3, n))
+    oracle.forces(pos, mass, sink_idx=sS, source_idx=F, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+    oracle.forces(pos, mass, sink_idx=sF, source_idx=S, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+    assert rel(a[:, sS], a_ref[:, sS]) <= TOL_A and rel(a[:, sF], a_ref[:, sF]) <= TOL_A
+    a_in = a.copy()
+    oracle.forces(pos, mass, sink_idx=sS, source_idx=F, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+    oracle.forces(pos, mass, sink_idx=sF, source_idx=S, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+    assert rel(g[:, sS], g_ref[:, sS]) <= TOL_G and rel(g[:, sF], g_ref[:, sF]) <= TOL_G
+    assert np.abs((mass * a).sum(1)).max() < 1e-13 * (mass * np.abs(a)).sum(1).max()

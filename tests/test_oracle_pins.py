@@ -319,6 +319,15 @@ def test_timesteps_are_min_over_level_members_only(oracle):
     assert np.isinf(lone[4])                                 # a level of one particle: +inf
 
 
+def test_sampled_timesteps_equal_full_level_pass(oracle):
+    pos, vel, mass = fi.plummer(300, 12)
+    idx = fi.active_subset(300, 0.6, 12)
+    full, fb = oracle.timesteps(pos, vel, mass, idx=idx, tau_pivot=0.01)
+    sel = idx[::7]
+    part, pb = oracle.timesteps_sampled(pos, vel, mass, sel, idx=idx, tau_pivot=0.01)
+    assert np.array_equal(part[sel], full[sel]) and np.array_equal(pb[sel], fb[sel])
+
+
 def test_zero_relative_velocity_gives_free_fall_only(oracle):
     G, eta = 1.0, 0.2
     ff, fb = oracle.pair_timestep([0, 0, 0], [0, 0, 0], 1.0, [2.0, 0, 0], [0, 0, 0], 3.0, G=G,
