@@ -63,7 +63,7 @@ def load_library():
     lib.frost_create.argtypes = [C.POINTER(vp), i32, vp]
     lib.frost_destroy.argtypes = [vp]
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
-    lib.frost_set_tuning.argtypes = [vp, i32, i32]
+    lib.frost_set_tuning.argtypes = [vp, i32, i32, i32]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_timesteps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, vp, vp]
@@ -143,8 +143,9 @@ class Frost:
         self._check(self.lib.frost_set_params(self.h, G, eps2, eta_ff, eta_fb, max_depth),
                     "frost_set_params")
 
-    def set_tuning(self, sinks_per_thread=0, source_slices=0):
-        self._check(self.lib.frost_set_tuning(self.h, sinks_per_thread, source_slices),
+    def set_tuning(self, sinks_per_thread=0, source_slices=0, small_set_max=-1):
+        self._check(self.lib.frost_set_tuning(self.h, sinks_per_thread, source_slices,
+                                              small_set_max),
                     "frost_set_tuning")
 
     def launch_count(self) -> int:

@@ -37,7 +37,7 @@ int frost_destroy(frost_ctx *c) {
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
     Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->iota,
-                   &c->acc, &c->grad, &c->tau, &c->blockcnt};
+                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
     for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
@@ -56,8 +56,10 @@ int frost_set_params(frost_ctx *c, double G, double eps2, double eta_ff, double 
     return FROST_OK;
 }
 
-int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices) {
+int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices, int small_set_max) {
     if (!c) return FROST_EINVAL;
+    if (small_set_max < -1 || small_set_max > small_max()) return FROST_EINVAL;
+    c->tune_small = small_set_max;
     if (!(sinks_per_thread == 0 || sinks_per_thread == 1 || sinks_per_thread == 2 || sinks_per_thread == 4))
         return FROST_EINVAL;
     if (source_slices < 0) return FROST_EINVAL;
@@ -143,10 +145,14 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
 }
 
+static int small_threshold(const frost_ctx *c) { return c->tune_small < 0 ? small_max() : c->tune_small; }
+
 static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                     const int32_t *idx, int n_idx, double dt, frost_hhs_stats *st) {
     if (!idx) n_idx = n;
     if (n_idx <= 0) return FROST_OK;
+    if (n_idx <= small_threshold(c))     // one CTA, set resident in shared memory (row 11)
+        return launch_small(c, 1, ld, pos, vel, mass, idx, n_idx, dt, 0, st ? c->dev_stats.p : nullptr);
     FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
     double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
@@ -170,6 +176,8 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
                    const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st) {
     if (n_set <= 0) return FROST_OK;
     if (level >= c->max_depth || level >= FROST_MAX_LEVELS) return FROST_EDEPTH;
+    if (n_set <= small_threshold(c))     // the whole subtree on the device, asynchronously (row 11)
+        return launch_small(c, 0, ld, pos, vel, mass, set, n_set, tau_pivot, level, c->dev_stats.p);
     double *tau = (double *)c->tau.p, *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
     FROST_TRY(timesteps_impl(c, n, ld, pos, vel, mass, set, n_set, tau_pivot, tau, nullptr));
     FROST_TRY(ensure(c, c->lvlS[level], (size_t)n_set * sizeof(int32_t)));
@@ -338,8 +346,26 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->tau, (size_t)ld * sizeof(double)));
-    const int rc = hhs_rec(c, n, ld, pos, vel, mass, nullptr, n, dt_top, 0, stats);
-    cudaStreamSynchronize(c->stream);
+    FROST_TRY(ensure(c, c->dev_stats, small_stats_bytes()));
+    FROST_CUDA(c, cudaMemsetAsync(c->dev_stats.p, 0, small_stats_bytes(), c->stream));
+    frost_hhs_stats local = frost_hhs_stats{};
+    local.depth = -1;
+    int rc = hhs_rec(c, n, ld, pos, vel, mass, nullptr, n, dt_top, 0, &local);
+    // merge what the device-resident subtrees counted (also carries their status)
+    struct { long long e[FROST_MAX_LEVELS], s[FROST_MAX_LEVELS], f[FROST_MAX_LEVELS], pn, pg, pt; int depth, status; } d;
+    static_assert(sizeof(d) >= 1, "");
+    if (sizeof(d) != small_stats_bytes()) return FROST_EINVAL;
+    FROST_CUDA(c, cudaMemcpyAsync(&d, c->dev_stats.p, sizeof(d), cudaMemcpyDeviceToHost, c->stream));
+    FROST_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (rc == FROST_OK && d.status) rc = d.status;
+    // the device kernel records depth = -1 when it never entered a level
+    for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
+        local.entries[k] += d.e[k]; local.n_slow[k] += d.s[k]; local.n_fast[k] += d.f[k];
+    }
+    local.pairs_newton += d.pn; local.pairs_gradient += d.pg; local.pairs_timestep += d.pt;
+    if (d.depth > local.depth) local.depth = d.depth;
+    if (local.depth < 0) local.depth = 0;
+    if (stats) *stats = local;
     return rc;
 }
 

@@ -25,7 +25,7 @@ struct frost_ctx {
     cudaStream_t stream = nullptr;
     double G = 1.0, eps2 = 0.0, eta_ff = 0.2, eta_fb = 0.2;
     int max_depth = 64;
-    int tune_k = 0, tune_slices = 0;
+    int tune_k = 0, tune_slices = 0, tune_small = -1;   // -1: auto threshold for the subtree kernel
     int num_sms = 148;
     int last_cuda = 0;
     int64_t launches = 0;
@@ -36,6 +36,7 @@ struct frost_ctx {
     frost::Buf iota;               // unused placeholder for identity lists
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
     frost::Buf blockcnt;           // partition scratch
+    frost::Buf dev_stats;          // SmallStats accumulated by the subtree kernel
     frost::Buf host_stage[6];      // device staging for frost_forces_host
     frost::Buf lvlS[FROST_MAX_LEVELS], lvlF[FROST_MAX_LEVELS];
     int32_t *pinned_counts = nullptr;  // host pinned int32[4]
@@ -112,6 +113,12 @@ int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int 
                    int ld, double *out_grad);
 int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set,
                    const int32_t *idx, double tau_pivot, double *out_tau, int32_t *out_bin);
+
+// frost_small.cu: one-CTA device-resident hhs_fsi subtree (mode 0) or fsi step (mode 1)
+int small_max();
+size_t small_stats_bytes();
+int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats);
 
 // ---- device-side PTX helpers ------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -1,0 +1,382 @@
+// frost_small.cu -- SURVEY.md §8(a) row 11: the whole hhs_fsi(F, tau) subtree (Alg. 3,
+// PAPER.md:572-587) of a small particle set executed by ONE CTA with the set resident in shared
+// memory and an explicit level stack -- no host round trip, no launch per operator.  This is the
+// B200-native stand-in for the paper's "serial CPU code ... when N <~ a few hundred particles"
+// (PAPER.md:545): deep hierarchy levels hold a handful of particles and are entered 2^k times per
+// top-level step, where ~20 launches plus a count read-back per entry would dominate.
+//
+// The arithmetic is the same pair code as the streaming sweeps (frost_pairs.cuh).  A sink is
+// served by L = 1..32 adjacent lanes that split the source list and combine with warp shuffles, so
+// small sink sets still use the whole CTA; the combination order is fixed (deterministic).
+#include "frost_pairs.cuh"
+
+namespace frost {
+
+constexpr int kSmallMax = 1024;     // particles the subtree kernel accepts
+constexpr int kSmallThreads = 512;
+
+struct SmallStats {                 // device-side mirror of frost_hhs_stats (+ status)
+    long long entries[FROST_MAX_LEVELS], n_slow[FROST_MAX_LEVELS], n_fast[FROST_MAX_LEVELS];
+    long long pairs_newton, pairs_gradient, pairs_timestep;
+    int depth, status;
+};
+
+struct SmallParams {
+    const int32_t *idx;             // global indices of the set (NULL = 0..n-1)
+    int n, ld;
+    double *pos, *vel;
+    const double *mass;
+    double tau_pivot;               // pivot step of the subtree's root
+    double dt_fsi;                  // mode 1: plain fsi(set, dt_fsi) instead of hhs_fsi
+    int mode;                       // 0 = hhs_fsi subtree, 1 = fsi step
+    int level0, max_depth;
+    double G, eps2, eta_ff, eta_fb;
+    SmallStats *stats;
+};
+
+struct SmallSmem {
+    double4 xm[kSmallMax];          // x, y, z, m
+    double4 vv[kSmallMax];          // vx, vy, vz, 1
+    double4 aa[kSmallMax];          // ax, ay, az, 1
+    double4 gg[kSmallMax];          // gx, gy, gz, -
+    double tau[kSmallMax];
+    int perm[kSmallMax];            // the level sets are contiguous segments of this list
+    int tmp[kSmallMax];
+    int scan[kSmallThreads / 32 + 1];
+    // explicit recursion stack
+    int f_start[FROST_MAX_LEVELS], f_n[FROST_MAX_LEVELS], f_ns[FROST_MAX_LEVELS], f_stage[FROST_MAX_LEVELS];
+    double f_tau[FROST_MAX_LEVELS];
+    int sp, err;
+    long long st_entries[FROST_MAX_LEVELS], st_slow[FROST_MAX_LEVELS], st_fast[FROST_MAX_LEVELS];
+    long long st_pn, st_pg, st_pt;
+    int st_depth;
+};
+
+// lanes per sink: largest power of two <= 32 with nA * L <= blockDim
+__device__ __forceinline__ int lanes_per_sink(int nA) {
+    int L = 1;
+    while (L < 32 && nA * (L * 2) <= kSmallThreads) L *= 2;
+    return L;
+}
+
+__device__ __forceinline__ double shfl_sum(double v, int L) {
+    for (int o = L >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ double shfl_min(double v, int L) {
+    for (int o = L >> 1; o > 0; o >>= 1) v = fmin(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// a_i = G sum_{j in B} ...  for i in segment A (Eq. 24 / 42).  Segments are [a0, a0+nA) and
+// [b0, b0+nB) of sm.perm.  All threads must call (uniform control flow, shuffles).
+__device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
+    const int L = lanes_per_sink(nA);
+    const int per = kSmallThreads / L;
+    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    for (int base = 0; base < nA; base += per) {
+        const int a = base + slot;
+        const bool live = a < nA;
+        const int i = sm.perm[a0 + (live ? a : 0)];
+        NewtonPolicy::Sink s;
+        const double4 r = sm.xm[i];
+        s.x = r.x; s.y = r.y; s.z = r.z;
+        NewtonPolicy::Acc acc; NewtonPolicy::init(acc);
+        for (int b = sub; b < nB; b += L) {
+            const double4 j0 = sm.xm[sm.perm[b0 + b]];
+            NewtonPolicy::pair(s, acc, j0, j0, prm);
+        }
+        acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
+        if (live && sub == 0) sm.aa[i] = make_double4(acc.x * prm.G, acc.y * prm.G, acc.z * prm.G, 1.0);
+    }
+    __syncthreads();
+}
+
+// g_i = 2G sum_{j in B} ... using sm.aa of sinks and sources (Eq. 27 / 43 / 44).
+__device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
+    const int L = lanes_per_sink(nA);
+    const int per = kSmallThreads / L;
+    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    for (int base = 0; base < nA; base += per) {
+        const int a = base + slot;
+        const bool live = a < nA;
+        const int i = sm.perm[a0 + (live ? a : 0)];
+        GradientPolicy::Sink s;
+        const double4 r = sm.xm[i], ai = sm.aa[i];
+        s.x = r.x; s.y = r.y; s.z = r.z; s.ax = ai.x; s.ay = ai.y; s.az = ai.z;
+        GradientPolicy::Acc acc; GradientPolicy::init(acc);
+        for (int b = sub; b < nB; b += L) {
+            const int j = sm.perm[b0 + b];
+            GradientPolicy::pair(s, acc, sm.xm[j], sm.aa[j], prm);
+        }
+        acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
+        const double k2g = 2.0 * prm.G;
+        if (live && sub == 0) sm.gg[i] = make_double4(acc.x * k2g, acc.y * k2g, acc.z * k2g, 0.0);
+    }
+    __syncthreads();
+}
+
+// tau_i = min over the other members of the level (Eq. 49-54); a level of one particle: +inf.
+__device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int nA) {
+    const int L = lanes_per_sink(nA);
+    const int per = kSmallThreads / L;
+    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    for (int base = 0; base < nA; base += per) {
+        const int a = base + slot;
+        const bool live = a < nA;
+        const int i = sm.perm[a0 + (live ? a : 0)];
+        TimestepPolicy::Sink s;
+        const double4 r = sm.xm[i], v = sm.vv[i];
+        s.x = r.x; s.y = r.y; s.z = r.z; s.gm = r.w * prm.G; s.vx = v.x; s.vy = v.y; s.vz = v.z;
+        TimestepPolicy::Acc acc; TimestepPolicy::init(acc);
+        for (int b = sub; b < nA; b += L) {
+            const int j = sm.perm[a0 + b];
+            double4 j0 = sm.xm[j];
+            j0.w *= prm.G;
+            TimestepPolicy::pair(s, acc, j0, sm.vv[j], prm);
+        }
+        acc.tau = shfl_min(acc.tau, L);
+        if (live && sub == 0) sm.tau[i] = acc.tau;
+    }
+    __syncthreads();
+}
+
+// v_i += c (a_i + kappa g_i) ; x_i += c v_i  on a segment (Eq. 6).
+__device__ void cta_kick(SmallSmem &sm, int a0, int nA, double c, double kappa, bool with_g) {
+    for (int a = threadIdx.x; a < nA; a += kSmallThreads) {
+        const int i = sm.perm[a0 + a];
+        double4 v = sm.vv[i];
+        const double4 ac = sm.aa[i];
+        double ax = ac.x, ay = ac.y, az = ac.z;
+        if (with_g) {
+            const double4 g = sm.gg[i];
+            ax = fma(kappa, g.x, ax); ay = fma(kappa, g.y, ay); az = fma(kappa, g.z, az);
+        }
+        v.x = fma(c, ax, v.x); v.y = fma(c, ay, v.y); v.z = fma(c, az, v.z);
+        sm.vv[i] = v;
+    }
+    __syncthreads();
+}
+
+__device__ void cta_drift(SmallSmem &sm, int a0, int nA, double c) {
+    for (int a = threadIdx.x; a < nA; a += kSmallThreads) {
+        const int i = sm.perm[a0 + a];
+        double4 x = sm.xm[i];
+        const double4 v = sm.vv[i];
+        x.x = fma(c, v.x, x.x); x.y = fma(c, v.y, x.y); x.z = fma(c, v.z, x.z);
+        sm.xm[i] = x;
+    }
+    __syncthreads();
+}
+
+// Stable in-place partition of the segment [a0, a0+n) of sm.perm: slow (tau >= pivot) first.
+// Returns |S| (Eq. 29).
+__device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    constexpr int kWarps = kSmallThreads / 32;
+    int nS = 0;
+    for (int base = 0; base < n; base += kSmallThreads) {
+        const int k = base + threadIdx.x;
+        const int f = (k < n) ? (sm.tau[sm.perm[a0 + k]] >= pivot) : 0;
+        nS += __syncthreads_count(f);
+    }
+    int carry = 0;
+    for (int base = 0; base < n; base += kSmallThreads) {
+        const int k = base + threadIdx.x;
+        const int i = (k < n) ? sm.perm[a0 + k] : 0;
+        const int f = (k < n) ? (sm.tau[i] >= pivot) : 0;
+        int inc = f;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) sm.scan[w] = inc;
+        __syncthreads();
+        int wbase = 0, total = 0;
+        for (int q = 0; q < kWarps; ++q) {
+            const int v = sm.scan[q];
+            if (q < w) wbase += v;
+            total += v;
+        }
+        const int slow_before = carry + wbase + inc - f;
+        if (k < n) {
+            if (f) sm.tmp[slow_before] = i;
+            else sm.tmp[nS + (k - slow_before)] = i;
+        }
+        carry += total;
+        __syncthreads();
+    }
+    for (int k = threadIdx.x; k < n; k += kSmallThreads) sm.perm[a0 + k] = sm.tmp[k];
+    __syncthreads();
+    return nS;
+}
+
+// fsi(set, dt): Alg. 2 on the segment [a0, a0+nA).
+__device__ void cta_fsi(SmallSmem &sm, const SweepParams &pN, const SweepParams &pG, int a0, int nA,
+                        double dt) {
+    if (nA <= 0) return;
+    cta_newton(sm, pN, a0, nA, a0, nA);
+    cta_kick(sm, a0, nA, dt / 6.0, 0.0, false);
+    cta_drift(sm, a0, nA, dt / 2.0);
+    cta_newton(sm, pN, a0, nA, a0, nA);
+    cta_gradient(sm, pG, a0, nA, a0, nA);
+    cta_kick(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true);
+    cta_drift(sm, a0, nA, dt / 2.0);
+    cta_newton(sm, pN, a0, nA, a0, nA);
+    cta_kick(sm, a0, nA, dt / 6.0, 0.0, false);
+    if (threadIdx.x == 0) {
+        const long long np = (long long)nA * nA;
+        sm.st_pn += 3 * np;
+        sm.st_pg += np;
+    }
+}
+
+__global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const SmallParams P) {
+    extern __shared__ __align__(16) unsigned char small_raw[];
+    SmallSmem &sm = *reinterpret_cast<SmallSmem *>(small_raw);
+    const int n = P.n, ld = P.ld;
+    for (int k = threadIdx.x; k < n; k += kSmallThreads) {
+        const int i = P.idx ? P.idx[k] : k;
+        sm.xm[k] = make_double4(P.pos[i], P.pos[(size_t)ld + i], P.pos[2 * (size_t)ld + i], P.mass[i]);
+        sm.vv[k] = make_double4(P.vel[i], P.vel[(size_t)ld + i], P.vel[2 * (size_t)ld + i], 1.0);
+        sm.perm[k] = k;
+    }
+    for (int k = threadIdx.x; k < FROST_MAX_LEVELS; k += kSmallThreads) {
+        sm.st_entries[k] = 0; sm.st_slow[k] = 0; sm.st_fast[k] = 0;
+    }
+    if (threadIdx.x == 0) {
+        sm.sp = 0; sm.err = 0; sm.st_pn = sm.st_pg = sm.st_pt = 0; sm.st_depth = -1;
+        sm.f_start[0] = 0; sm.f_n[0] = n; sm.f_ns[0] = 0; sm.f_stage[0] = 0; sm.f_tau[0] = P.tau_pivot;
+    }
+    SweepParams pN{}, pG{};
+    pN.G = pG.G = P.G; pN.eta_ff = pG.eta_ff = P.eta_ff; pN.eta_fb = pG.eta_fb = P.eta_fb;
+    pG.eps2 = P.eps2;
+    pN.eps2 = P.eps2 > 0x1p-400 ? P.eps2 : 0x1p-400;     // see NewtonPolicy::pair
+    __syncthreads();
+
+    if (P.mode == 1) {
+        cta_fsi(sm, pN, pG, 0, n, P.dt_fsi);
+    } else {
+        while (true) {
+            __syncthreads();
+            const int sp = sm.sp;
+            if (sp < 0 || sm.err) break;
+            const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
+            const double tau = sm.f_tau[sp];
+            const int level = P.level0 + sp;
+            if (stage == 0) {
+                if (cnt <= 0) {
+                    __syncthreads();
+                    if (threadIdx.x == 0) sm.sp = sp - 1;
+                    continue;
+                }
+                if (level >= P.max_depth || sp >= FROST_MAX_LEVELS - 1) {
+                    __syncthreads();
+                    if (threadIdx.x == 0) sm.err = FROST_EDEPTH;
+                    continue;
+                }
+                cta_timesteps(sm, pG, start, cnt);
+                const int nS = cta_partition(sm, start, cnt, tau);
+                const int nF = cnt - nS;
+                if (nS > 0 && nF > 0) {
+                    cta_newton(sm, pN, start, nS, start + nS, nF);
+                    cta_newton(sm, pN, start + nS, nF, start, nS);
+                    cta_kick(sm, start, cnt, tau / 6.0, 0.0, false);
+                }
+                cta_fsi(sm, pN, pG, start, nS, 0.5 * tau);
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    sm.f_ns[sp] = nS;
+                    sm.st_entries[level] += 1; sm.st_slow[level] += nS; sm.st_fast[level] += nF;
+                    sm.st_pt += (long long)cnt * cnt;
+                    if (level > sm.st_depth) sm.st_depth = level;
+                    sm.f_stage[sp] = 1;
+                    if (nF > 0) {
+                        sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
+                        sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                        sm.sp = sp + 1;
+                    }
+                }
+            } else if (stage == 1) {
+                const int nS = sm.f_ns[sp], nF = cnt - nS;
+                if (nS > 0 && nF > 0) {
+                    cta_newton(sm, pN, start, nS, start + nS, nF);
+                    cta_newton(sm, pN, start + nS, nF, start, nS);
+                    cta_gradient(sm, pG, start, nS, start + nS, nF);
+                    cta_gradient(sm, pG, start + nS, nF, start, nS);
+                    cta_kick(sm, start, cnt, 2.0 * tau / 3.0, tau * tau / 48.0, true);
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    sm.f_stage[sp] = 2;
+                    if (nF > 0) {
+                        sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
+                        sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                        sm.sp = sp + 1;
+                    }
+                }
+            } else {
+                const int nS = sm.f_ns[sp], nF = cnt - nS;
+                cta_fsi(sm, pN, pG, start, nS, 0.5 * tau);
+                if (nS > 0 && nF > 0) {
+                    cta_newton(sm, pN, start, nS, start + nS, nF);
+                    cta_newton(sm, pN, start + nS, nF, start, nS);
+                    cta_kick(sm, start, cnt, tau / 6.0, 0.0, false);
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    const long long cr = 2LL * nS * nF;
+                    sm.st_pn += 3 * cr; sm.st_pg += cr;
+                    sm.sp = sp - 1;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    for (int k = threadIdx.x; k < n; k += kSmallThreads) {
+        const int i = P.idx ? P.idx[k] : k;
+        const double4 x = sm.xm[k], v = sm.vv[k];
+        P.pos[i] = x.x; P.pos[(size_t)ld + i] = x.y; P.pos[2 * (size_t)ld + i] = x.z;
+        P.vel[i] = v.x; P.vel[(size_t)ld + i] = v.y; P.vel[2 * (size_t)ld + i] = v.z;
+    }
+    if (P.stats) {
+        for (int k = threadIdx.x; k < FROST_MAX_LEVELS; k += kSmallThreads) {
+            P.stats->entries[k] += sm.st_entries[k];
+            P.stats->n_slow[k] += sm.st_slow[k];
+            P.stats->n_fast[k] += sm.st_fast[k];
+        }
+        if (threadIdx.x == 0) {
+            P.stats->pairs_newton += sm.st_pn; P.stats->pairs_gradient += sm.st_pg;
+            P.stats->pairs_timestep += sm.st_pt;
+            if (sm.st_depth > P.stats->depth) P.stats->depth = sm.st_depth;
+            if (sm.err && !P.stats->status) P.stats->status = sm.err;
+        }
+    }
+}
+
+int small_max() { return kSmallMax; }
+
+// mode 0: hhs_fsi(set, tau) subtree rooted at hierarchy level `level0`; mode 1: fsi(set, dt).
+int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats) {
+    if (n <= 0) return FROST_OK;
+    if (n > kSmallMax) return FROST_EINVAL;
+    static bool attr_done = false;
+    if (!attr_done) {
+        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           (int)sizeof(SmallSmem)));
+        attr_done = true;
+    }
+    SmallParams P{};
+    P.idx = idx; P.n = n; P.ld = ld; P.pos = pos; P.vel = vel; P.mass = mass;
+    P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0;
+    P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
+    P.stats = (SmallStats *)dev_stats;
+    hhs_small_kernel<<<1, kSmallThreads, sizeof(SmallSmem), c->stream>>>(P);
+    return check_launch(c);
+}
+
+size_t small_stats_bytes() { return sizeof(SmallStats); }
+
+}  // namespace frost

@@ -63,11 +63,11 @@ def test_self_forces_small_and_ragged(fr, oracle, n):
 @pytest.mark.parametrize("k,slices", [(1, 1), (1, 5), (2, 1), (2, 3), (4, 2), (0, 0)])
 def test_every_kernel_variant_and_slice_count(fr, oracle, k, slices):
     pos, vel, mass = fi.plummer(5000, 7)
-    fr.set_tuning(k, slices)
+    fr.set_tuning(k, slices, -1)
     try:
         check_forces(fr, oracle, pos, mass, eps2=1e-6)
     finally:
-        fr.set_tuning(0, 0)
+        fr.set_tuning(0, 0, -1)
 
 
 def test_softened_and_scaled_G(fr, oracle):
@@ -187,16 +187,22 @@ def test_kick_drift_gather(fr, oracle):
     assert (rec[idx.size:] == 0).all()
 
 
-def test_config1_ten_fsi_steps(fr, oracle):
-    """Config 1: N = 1024, 10 fixed-step FSI steps with dt = 1/1024."""
+@pytest.mark.parametrize("small", [-1, 0])
+def test_config1_ten_fsi_steps(fr, oracle, small):
+    """Config 1: N = 1024, 10 fixed-step FSI steps with dt = 1/1024 -- through the one-CTA
+    device-resident kernel (small = -1) and through the streaming sweeps (small = 0)."""
     pos, vel, mass = fi.plummer(1024, 0)
     p, v, m = dev(pos), dev(vel), dev(mass)
     fr.set_params()
+    fr.set_tuning(0, 0, small)
     pr, vr = pos.copy(), vel.copy()
     d0 = oracle.diagnostics(pos, vel, mass)
-    for _ in range(10):
-        fr.fsi_step(p, v, m, 1.0 / 1024)
-        oracle.fsi_step(pr, vr, mass, 1.0 / 1024)
+    try:
+        for _ in range(10):
+            fr.fsi_step(p, v, m, 1.0 / 1024)
+            oracle.fsi_step(pr, vr, mass, 1.0 / 1024)
+    finally:
+        fr.set_tuning(0, 0, -1)
     pg, vg = p.cpu().numpy(), v.cpu().numpy()
     assert np.abs(pg - pr).max() < 1e-11 and np.abs(vg - vr).max() < 1e-10
     d1 = oracle.diagnostics(pg, vg, mass)
@@ -204,17 +210,44 @@ def test_config1_ten_fsi_steps(fr, oracle):
     assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-13
 
 
-def test_hhs_step_small_cluster(fr, oracle):
-    """Reduced-N replica of config 5: level sets, bookkeeping and the trajectory must match."""
-    n = 1024
+@pytest.mark.parametrize("n,small", [(1024, -1), (1024, 0), (1024, 48), (3000, -1), (3000, 100)])
+def test_hhs_step_small_cluster(fr, oracle, n, small):
+    """Reduced-N replica of config 5: level sets, bookkeeping and the trajectory must match the
+    oracle whether the recursion runs on the host (small = 0), in the device-resident subtree
+    kernel (whole problem for n <= 1024) or in a mix of both."""
     pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
     fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    fr.set_tuning(0, 0, small)
     pr, vr = pos.copy(), vel.copy()
     st_ref = oracle.hhs_step(pr, vr, mass, 1.0 / 256)
     p, v = dev(pos), dev(vel)
-    st = fr.hhs_step(p, v, dev(mass), 1.0 / 256)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), 1.0 / 256)
+    finally:
+        fr.set_tuning(0, 0, -1)
     assert st == st_ref
     assert st["depth"] >= 3
     pg, vg = p.cpu().numpy(), v.cpu().numpy()
     assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
     assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
+
+
+def test_hhs_tiny_systems_and_depth_limit(fr, oracle):
+    """Five-body Solar system (Tables A1/A2) entirely inside the subtree kernel; a hard binary with
+    a far too long top step must stop with FROST_EDEPTH instead of recursing forever."""
+    import paper_2011_14984_b200 as frost
+    pos, vel, mass, G = fi.solar_system()
+    vel = vel - (vel * mass).sum(1, keepdims=True) / mass.sum()
+    fr.set_params(G=G, eta_ff=0.05, eta_fb=0.05)
+    pr, vr = pos.copy(), np.ascontiguousarray(vel.copy())
+    p, v = dev(pos), dev(vel)
+    for _ in range(3):
+        st_ref = oracle.hhs_step(pr, vr, mass, 512.0, G=G, eta_ff=0.05, eta_fb=0.05)
+        st = fr.hhs_step(p, v, dev(mass), 512.0)
+        assert st == st_ref
+    assert np.abs(p.cpu().numpy() - pr).max() < 1e-11 * 30 and st["depth"] >= 2
+    b_pos, b_vel, b_mass, P = fi.kepler_binary(1.0, 1.0, 1e-6, 0.0)
+    fr.set_params(G=1.0, max_depth=12)
+    with pytest.raises(frost.FrostError, match="deeper"):
+        fr.hhs_step(dev(b_pos), dev(b_vel), dev(b_mass), 1.0)
+    fr.set_params()
