@@ -23,7 +23,7 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
 ]
 
 
@@ -64,6 +64,7 @@ def load_library():
     lib.frost_destroy.argtypes = [vp]
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
     lib.frost_set_tuning.argtypes = [vp, i32, i32, i32]
+    lib.frost_set_symmetric.argtypes = [vp, i32]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_timesteps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, vp, vp]
@@ -147,6 +148,10 @@ class Frost:
         self._check(self.lib.frost_set_tuning(self.h, sinks_per_thread, source_slices,
                                               small_set_max),
                     "frost_set_tuning")
+
+    def set_symmetric(self, mode=0):
+        """0 = auto, 1 = one-sided sweeps only, 2 = pair-symmetric sweeps whenever applicable."""
+        self._check(self.lib.frost_set_symmetric(self.h, mode), "frost_set_symmetric")
 
     def launch_count(self) -> int:
         return int(self.lib.frost_launch_count(self.h))

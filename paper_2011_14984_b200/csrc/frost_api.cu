@@ -36,7 +36,7 @@ int frost_destroy(frost_ctx *c) {
     if (!c) return FROST_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->iota,
+    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->iota,
                    &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
@@ -68,6 +68,12 @@ int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices, int 
     return FROST_OK;
 }
 
+int frost_set_symmetric(frost_ctx *c, int mode) {
+    if (!c || mode < 0 || mode > 2) return FROST_EINVAL;
+    c->tune_sym = mode;
+    return FROST_OK;
+}
+
 int64_t frost_launch_count(const frost_ctx *c) { return c ? c->launches : -1; }
 int frost_last_cuda_error(const frost_ctx *c) { return c ? c->last_cuda : 0; }
 const char *frost_version(void) { return "frost-b200 0.1 (sm_100a)"; }
@@ -93,6 +99,15 @@ static int zero_tail(frost_ctx *c, double *rec, int n, int n_pad) {
     return FROST_OK;
 }
 
+// Whether a sweep with nA register-resident particles against nB streamed ones goes through the
+// pair-symmetric kernels: they need enough tile pairs to fill the GPU (A tiles of 1024, B tiles of
+// 256 particles); below that the one-sided sweeps with source slices win.
+static bool use_sym(const frost_ctx *c, int nA, int nB) {
+    if (c->tune_sym == 1) return false;
+    if (c->tune_sym == 2) return nA > 0 && nB > 0;
+    return nA >= 16384 && nB >= 4096;
+}
+
 static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
                        const int32_t *I, int nI, const int32_t *J, int nJ, double *acc, double *grad,
                        int flags) {
@@ -112,6 +127,30 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
         FROST_TRY(ensure(c, c->recB_v, (size_t)padB * kRecBytes));
         Bxm = (double *)c->recB_xm.p; Bv = (double *)c->recB_v.p;
         FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm));
+    }
+    // pair-symmetric sweeps (frost_sym.cu) serve both directions of every pair with one evaluation:
+    // the self case, and the mutual case with the larger set as the register-resident A side
+    const bool sym_self = self && use_sym(c, nI, nI);
+    const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI);
+    if (sym_self || sym_mut) {
+        const bool swap = sym_mut && nJ > nI;            // A = the larger set
+        const double *Pxm = swap ? Bxm : Axm, *Qxm = swap ? Axm : Bxm;
+        double *Pv = swap ? Bv : Av, *Qv = swap ? Av : Bv;
+        const int32_t *Pi = swap ? J : I, *Qi = swap ? I : J;
+        const int nP = swap ? nJ : nI, nQ = swap ? nI : nJ;
+        if (flags & FROST_ACC) {
+            FROST_TRY(zero_tail(c, Av, nI, padA));
+            if (!self) FROST_TRY(zero_tail(c, Bv, nJ, padB));
+            FROST_TRY(sym_newton(c, Pxm, nP, Qxm, nQ, self, Pi, Qi, ld, acc, Pv, self ? nullptr : Qv));
+        }
+        if (flags & FROST_GRAD) {
+            if (!(flags & FROST_ACC)) {
+                FROST_TRY(launch_pack_vec(c, ld, acc, I, nI, padA, Av));
+                if (!self) FROST_TRY(launch_pack_vec(c, ld, acc, J, nJ, padB, Bv));
+            }
+            FROST_TRY(sym_gradient(c, Pxm, Pv, nP, Qxm, Qv, nQ, self, Pi, Qi, ld, grad));
+        }
+        return FROST_OK;
     }
     if (flags & FROST_ACC) {
         FROST_TRY(zero_tail(c, Av, nI, padA));
@@ -142,6 +181,7 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
     FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, c->G, 1));   // .w = G m, NaN padding
     FROST_TRY(launch_pack_vec(c, ld, vel, idx, n_idx, pad, v));
+    if (use_sym(c, n_idx, n_idx)) return sym_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
     return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
 }
 

@@ -26,6 +26,7 @@ struct frost_ctx {
     double G = 1.0, eps2 = 0.0, eta_ff = 0.2, eta_fb = 0.2;
     int max_depth = 64;
     int tune_k = 0, tune_slices = 0, tune_small = -1;   // -1: auto threshold for the subtree kernel
+    int tune_sym = 0;              // pair-symmetric sweeps: 0 auto, 1 never, 2 whenever applicable
     int num_sms = 148;
     int last_cuda = 0;
     int64_t launches = 0;
@@ -33,6 +34,7 @@ struct frost_ctx {
     frost::Buf recA_xm, recB_xm;   // packed {x,y,z,m} streams of set A (sinks) and set B (sources)
     frost::Buf recA_v, recB_v;     // packed {ax,ay,az,0} or {vx,vy,vz,0}
     frost::Buf partial;            // [slices][3][n_pad] partial sums / [slices][n_pad] partial minima
+    frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
     frost::Buf iota;               // unused placeholder for identity lists
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
     frost::Buf blockcnt;           // partition scratch
@@ -113,6 +115,16 @@ int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int 
                    int ld, double *out_grad);
 int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set,
                    const int32_t *idx, double tau_pivot, double *out_tau, int32_t *out_bin);
+
+// frost_sym.cu: pair-symmetric sweeps (one evaluation serves i<-j and j<-i).  self: B == A.
+int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
+               const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
+               double *A_a_packed, double *B_a_packed);
+int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
+                 const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
+                 int ld, double *out_grad);
+int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
+                 double tau_pivot, double *out_tau, int32_t *out_bin);
 
 // frost_small.cu: one-CTA device-resident hhs_fsi subtree (mode 0) or fsi step (mode 1)
 int small_max();

@@ -1,0 +1,449 @@
+// frost_sym.cu -- pair-symmetric variants of the three all-pairs sweeps: Newtonian
+// accelerations (Eq. 24/42), gradient accelerations (Eq. 27/43/44), time-step criterion
+// (Eq. 49-54).  Every quantity a pair (i, j) needs -- x_ji, s^-3, the tidal contraction, the
+// symmetrised time-step candidate -- is either symmetric or antisymmetric under i <-> j
+// ("the force-gradient term ... obeys Newton's third law"), so one evaluation
+// can serve both ordered pairs (i <- j) and (j <- i): 20 instead of 2 x 16 FP64 instructions for
+// the Newton pair, 29 instead of 2 x 28 for the gradient pair, one candidate instead of two for
+// the time step.  The one-sided sweeps of frost_sweeps.cu cannot exploit this because their
+// sources are broadcast to all lanes; here both particles of a pair live in registers:
+//
+//   * a CTA owns an A tile of NT*KA particles (KA per thread, resident for the CTA's life) and
+//     streams B tiles of NT particles through a TMA bulk-copy ring (as frost_sweeps.cu);
+//   * each warp takes one 32-particle chunk of the B tile at a time; lane l starts with B particle
+//     l as its "traveller" and the travellers rotate one lane per step (accumulators by SHFL,
+//     coordinates re-read from shared memory at the rotated index), so after 32 steps every A
+//     particle of the warp has met every B particle of the chunk and the traveller accumulators
+//     are back in their home lane;
+//   * the NT/32 warps visit the chunks round-robin (warp w takes chunk (w + r) mod W in round r,
+//     one __syncthreads per round), so the B-side sums of a tile are combined in shared memory in
+//     a fixed order, without atomics, and leave the CTA once per (A tile, B tile);
+//   * A-side sums leave once per CTA (segment of the B list), B-side sums once per tile pair; a
+//     second kernel adds both kinds in a fixed order -- results are bitwise reproducible.
+//
+// For the self case (A list == B list) only B tiles at or beyond the A tile are visited: the
+// diagonal block is evaluated one-sided (its B-side sums are dropped), everything beyond it
+// two-sided.  For the bipartite case (slow/fast sets of Alg. 3) every tile pair
+// is two-sided and one sweep yields both directions of acc_sf_*.
+#include "frost_pairs.cuh"
+
+namespace frost {
+
+struct SymParams {
+    const double4 *a0, *a1;   // A records {x,y,z,m} and {ax,ay,az,.} / {vx,vy,vz,.}
+    const double4 *b0, *b1;   // B records
+    double *partA;            // [segments][planes][na_pad]
+    double *partB;            // per A tile: [planes][row length]   (see partB_row)
+    int na_pad, nb_pad;
+    int self;                 // A list == B list: visit only B tiles >= the A tile
+    int nb_tiles;             // B tiles of NT records
+    int seg_tiles;            // B tiles per CTA
+    double eps2, eta_ff, eta_fb;
+};
+
+// B-side partial sums of A tile I: self case rows are triangular (particles beyond the A tile).
+__host__ __device__ inline size_t partB_row_offset(int self, int planes, int I, int TA, int nb_pad) {
+    if (self) return (size_t)planes * ((size_t)I * nb_pad - (size_t)TA * ((size_t)I * (I + 1) / 2));
+    return (size_t)planes * (size_t)I * nb_pad;
+}
+__host__ __device__ inline int partB_row_len(int self, int I, int TA, int nb_pad) {
+    return self ? nb_pad - TA * (I + 1) : nb_pad;
+}
+__host__ __device__ inline int partB_row_first(int self, int I, int TA) { return self ? TA * (I + 1) : 0; }
+
+// ------------------------------------------------------------------------------------------------
+// Pair policies: A particle in registers, B particle = shared-memory record + travelling sums.
+// ------------------------------------------------------------------------------------------------
+struct SymNewton {
+    static constexpr int kRecs = 1, kPlanes = 3;
+    static constexpr bool kMin = false;
+    struct A { double x, y, z, nm, s[3]; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        const double4 r = p.a0[i];
+        a.x = r.x; a.y = r.y; a.z = r.z; a.nm = -r.w;
+        a.s[0] = a.s[1] = a.s[2] = 0.0;
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[3]) { b[0] = b[1] = b[2] = 0.0; }
+    // 20 FP64 instructions for both ordered pairs: 12 shared (x_ji, s^2, s^-3 by the series of
+    // NewtonPolicy::pair) + 2 x (mass weight + 3 accumulating FMAs).  a_i += m_j s^-3 x_ji,
+    // a_j -= m_i s^-3 x_ji (Eq. 24 both ways).  eps2 is floored by the launcher.
+    __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
+                                                const double4 &, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
+        const double y = rsqrt_seed(s2);
+        const double y2 = y * y;
+        const double e = fma(-s2, y2, 1.0);
+        const double w0 = y2 * y;
+        const double q = fma(1.875, e, 1.5);
+        const double qe = q * e;
+        const double w = fma(w0, qe, w0);
+        const double wa = w * j0.w;
+        const double wb = w * a.nm;
+        fma3_shared(a.s[0], a.s[1], a.s[2], wa, dx, dy, dz);
+        fma3_shared(b[0], b[1], b[2], wb, dx, dy, dz);
+    }
+};
+
+struct SymGradient {
+    static constexpr int kRecs = 2, kPlanes = 3;
+    static constexpr bool kMin = false;
+    struct A { double x, y, z, nm, ax, ay, az, s[3]; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        const double4 r = p.a0[i];
+        const double4 v = p.a1[i];
+        a.x = r.x; a.y = r.y; a.z = r.z; a.nm = -r.w; a.ax = v.x; a.ay = v.y; a.az = v.z;
+        a.s[0] = a.s[1] = a.s[2] = 0.0;
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[3]) { b[0] = b[1] = b[2] = 0.0; }
+    // 29 FP64 instructions for both ordered pairs: v = a_ji - 3 s^-2 (x_ji . a_ji) x_ji is odd
+    // under i <-> j, s^-3 is even: g_i += m_j s^-3 v, g_j -= m_i s^-3 v  (Eq. 27 both ways).
+    __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double ax = j1.x - a.ax, ay = j1.y - a.ay, az = j1.z - a.az;
+        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
+        const double ri = rsqrt_full_or_zero(s2);
+        const double dot = fma(dz, az, fma(dy, ay, dx * ax));
+        const double q = ri * ri;
+        const double w3 = ri * q;
+        const double t = q * dot;
+        const double u = t * -3.0;
+        double vx = ax, vy = ay, vz = az;
+        fma3_shared(vx, vy, vz, u, dx, dy, dz);
+        const double wa = w3 * j0.w;
+        const double wb = w3 * a.nm;
+        fma3_shared(a.s[0], a.s[1], a.s[2], wa, vx, vy, vz);
+        fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
+    }
+};
+
+struct SymTimestep {
+    static constexpr int kRecs = 2, kPlanes = 1;
+    static constexpr bool kMin = true;
+    struct A { double x, y, z, gm, vx, vy, vz, s[1]; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        const double4 r = p.a0[i];
+        const double4 v = p.a1[i];
+        a.x = r.x; a.y = r.y; a.z = r.z; a.gm = r.w; a.vx = v.x; a.vy = v.y; a.vz = v.z;
+        a.s[0] = __longlong_as_double(0x7ff0000000000000LL);
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[1]) {
+        b[0] = __longlong_as_double(0x7ff0000000000000LL);
+    }
+    // The symmetrised candidate of Eq. 49-54 is the same number for (i <- j) and (j <- i)
+    // (r.v, r^2, v^2 and m_i + m_j are even under the swap), so it is evaluated once
+    // -- exactly TimestepPolicy::pair -- and min-ed into both particles.
+    __device__ static __forceinline__ void pair(A &a, double (&b)[1], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double rx = j0.x - a.x, ry = j0.y - a.y, rz = j0.z - a.z;
+        const double vx = j1.x - a.vx, vy = j1.y - a.vy, vz = j1.z - a.vz;
+        const double r2 = fma(rz, rz, fma(ry, ry, rx * rx));
+        const double v2 = fma(vz, vz, fma(vy, vy, vx * vx));
+        const double rv = fma(rz, vz, fma(ry, vy, rx * vx));
+        const double mu = a.gm + j0.w;
+        const double ir = rsqrt_full(r2);
+        const double iv = rsqrt_full(v2);
+        const double ir2 = ir * ir;
+        const double mir = mu * ir;
+        const double t_ff = rsqrt_full(mir * ir2);
+        const double t_fb = (r2 * ir) * iv;
+        const double rvr2 = rv * ir2;
+        const double q_ff = (rvr2 * t_ff) * (1.5 * p.eta_ff);
+        const double f = rvr2 * t_fb;
+        const double q_fb = fma(f, mir * (iv * iv), f) * p.eta_fb;
+        const double c_ff = sym_factor(q_ff) * (t_ff * p.eta_ff);
+        const double c_fb = sym_factor(q_fb) * (t_fb * p.eta_fb);
+        const double c = fmin(c_ff, c_fb);
+        a.s[0] = fmin(a.s[0], c);
+        b[0] = fmin(b[0], c);
+    }
+};
+
+// ------------------------------------------------------------------------------------------------
+// The kernel.  grid = (A tiles, segments of the B list); block = NT threads; KA A particles/thread.
+// ------------------------------------------------------------------------------------------------
+template <class P, int KA, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
+    constexpr int kWarps = NT / 32;
+    constexpr int TA = NT * KA;
+    constexpr int PL = P::kPlanes;
+    constexpr uint32_t kStageBytes = P::kRecs * NT * kRecBytes;
+
+    const int I = blockIdx.x;
+    const int row_first_tile = prm.self ? I * KA : 0;          // first B tile this A tile visits
+    const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
+    const int tile0 = row_first_tile + blockIdx.y * prm.seg_tiles;
+    if (tile0 >= prm.nb_tiles) return;
+    const int ntiles = min(prm.seg_tiles, prm.nb_tiles - tile0);
+
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double4 *tiles = reinterpret_cast<double4 *>(smem_raw);                   // [kStages][kRecs][NT]
+    double *accB = reinterpret_cast<double *>(smem_raw + kStages * kStageBytes);   // [2][PL][NT]
+    uint64_t *full = reinterpret_cast<uint64_t *>(accB + 2 * PL * NT);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    if (tid == 0) {
+#pragma unroll
+        for (int s = 0; s < kStages; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    auto issue = [&](int t) {
+        const int s = t % kStages;
+        mbar_expect_tx(&full[s], kStageBytes);
+        double4 *dst = tiles + (size_t)s * P::kRecs * NT;
+        const size_t off = (size_t)(tile0 + t) * NT;
+        bulk_g2s(dst, prm.b0 + off, NT * kRecBytes, &full[s]);
+        if (P::kRecs == 2) bulk_g2s(dst + NT, prm.b1 + off, NT * kRecBytes, &full[s]);
+    };
+    if (tid == 0) {
+        const int pre = min(kStages, ntiles);
+        for (int t = 0; t < pre; ++t) issue(t);
+    }
+
+    typename P::A a[KA];
+    const int a_first = I * TA + tid;
+#pragma unroll
+    for (int k = 0; k < KA; ++k) P::load(a[k], prm, a_first + k * NT);
+
+    double *rowB = prm.partB + partB_row_offset(prm.self, PL, I, TA, prm.nb_pad);
+    const int row_len = partB_row_len(prm.self, I, TA, prm.nb_pad);
+    const int row_j0 = partB_row_first(prm.self, I, TA);
+    const int from = (lane + 31) & 31;          // travellers move to the next lane each step
+
+    for (int t = 0; t < ntiles; ++t) {
+        const int s = t % kStages;
+        mbar_wait(&full[s], (uint32_t)(t / kStages) & 1u);
+        const double4 *t0 = tiles + (size_t)s * P::kRecs * NT;
+        const bool two_sided = (tile0 + t) >= diag_end;
+        double *accT = accB + (size_t)(t & 1) * PL * NT;
+        for (int r = 0; r < kWarps; ++r) {
+            const int c = (warp + r) % kWarps;
+            const double4 *c0 = t0 + c * 32;
+            const double4 *c1 = c0 + (P::kRecs == 2 ? NT : 0);
+            double b[PL];
+            P::init_b(b);
+#pragma unroll 2
+            for (int step = 0; step < 32; ++step) {
+                const int src = (lane - step) & 31;
+                const double4 j0 = c0[src];
+                const double4 j1 = (P::kRecs == 2) ? c1[src] : j0;
+#pragma unroll
+                for (int k = 0; k < KA; ++k) P::pair(a[k], b, j0, j1, prm);
+#pragma unroll
+                for (int p = 0; p < PL; ++p) b[p] = __shfl_sync(0xffffffffu, b[p], from);
+            }
+            if (two_sided) {
+                double *dst = accT + c * 32 + lane;
+#pragma unroll
+                for (int p = 0; p < PL; ++p) {
+                    if (r == 0) dst[p * NT] = b[p];
+                    else dst[p * NT] = P::kMin ? fmin(dst[p * NT], b[p]) : dst[p * NT] + b[p];
+                }
+            }
+            __syncthreads();
+        }
+        // every warp is past the last round: the stage can be refilled, the B sums can leave
+        if (tid == 0 && t + kStages < ntiles) issue(t + kStages);
+        if (two_sided) {
+            const int j = (tile0 + t) * NT + tid - row_j0;
+#pragma unroll
+            for (int p = 0; p < PL; ++p) rowB[(size_t)p * row_len + j] = accT[p * NT + tid];
+        }
+    }
+
+    double *part = prm.partA + (size_t)blockIdx.y * PL * prm.na_pad;
+#pragma unroll
+    for (int k = 0; k < KA; ++k)
+#pragma unroll
+        for (int p = 0; p < PL; ++p) part[(size_t)p * prm.na_pad + a_first + k * NT] = a[k].s[p];
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fixed-order reduction of the partial sums of one side.
+//   total_i = sum over the segments of i's A tile of partA  (if i was on the A side)
+//           + sum over the A tiles that met i as a B particle of partB.
+// side 0: particles of the A list; side 1: particles of the B list (bipartite case only).
+// ------------------------------------------------------------------------------------------------
+template <int PL, bool MIN>
+__global__ void sym_reduce_kernel(const double *__restrict__ partA, const double *__restrict__ partB,
+                                  int self, int side, int TA, int NT, int na_pad, int nb_pad,
+                                  int nb_tiles, int seg_tiles, int n_out, double scale,
+                                  const int32_t *__restrict__ idx, int ld, double *__restrict__ out,
+                                  double4 *__restrict__ packed, double tau_pivot,
+                                  int32_t *__restrict__ out_bin) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_out) return;
+    double s[PL];
+#pragma unroll
+    for (int p = 0; p < PL; ++p) s[p] = MIN ? __longlong_as_double(0x7ff0000000000000LL) : 0.0;
+    auto add = [&](int p, double v) { s[p] = MIN ? fmin(s[p], v) : s[p] + v; };
+    if (side == 0) {
+        const int I = i / TA;
+        const int first = self ? I * (TA / NT) : 0;
+        const int nseg = (nb_tiles - first + seg_tiles - 1) / seg_tiles;
+        for (int g = 0; g < nseg; ++g)
+#pragma unroll
+            for (int p = 0; p < PL; ++p) add(p, partA[((size_t)g * PL + p) * na_pad + i]);
+    }
+    if (side == 1 || self) {
+        const int rows = self ? i / TA : na_pad / TA;        // A tiles that met i on their B side
+        for (int I = 0; I < rows; ++I) {
+            const double *row = partB + partB_row_offset(self, PL, I, TA, nb_pad);
+            const int len = partB_row_len(self, I, TA, nb_pad);
+            const int j = i - partB_row_first(self, I, TA);
+#pragma unroll
+            for (int p = 0; p < PL; ++p) add(p, row[(size_t)p * len + j]);
+        }
+    }
+    const int g = idx ? idx[i] : i;
+    if (MIN) {
+        out[g] = s[0];
+        if (out_bin) {
+            int k = 0;
+            if (!(s[0] > 0.0)) k = 2000;
+            else {
+                double pv = tau_pivot;
+                while (pv > s[0] && k < 2000) { pv *= 0.5; ++k; }
+            }
+            out_bin[g] = k;
+        }
+    } else {
+#pragma unroll
+        for (int p = 0; p < PL; ++p) { s[p] *= scale; out[(size_t)p * ld + g] = s[p]; }
+        if (packed) packed[i] = make_double4(s[0], PL > 1 ? s[1] : 0.0, PL > 2 ? s[2] : 0.0, 1.0);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Planning and launch
+// ------------------------------------------------------------------------------------------------
+struct SymPlan { int ta, nt, na_pad, nb_pad, a_tiles, nb_tiles, seg_tiles, segs; size_t partA, partB; };
+
+template <int KA, int NT>
+static SymPlan make_sym_plan(const frost_ctx *c, int planes, bool self, int nA, int nB, int resident) {
+    SymPlan pl;
+    pl.ta = KA * NT; pl.nt = NT;
+    pl.na_pad = round_up(nA > 0 ? nA : 1, pl.ta);
+    pl.nb_pad = self ? pl.na_pad : round_up(nB > 0 ? nB : 1, NT);
+    pl.a_tiles = pl.na_pad / pl.ta;
+    pl.nb_tiles = pl.nb_pad / NT;
+    // tile pairs in total; aim at >= 24 waves of work units, at least 4 tiles per unit
+    const long long pairs = self ? (long long)pl.a_tiles * pl.nb_tiles - (long long)KA * pl.a_tiles * (pl.a_tiles - 1) / 2
+                                 : (long long)pl.a_tiles * pl.nb_tiles;
+    long long seg = pairs / (24LL * resident);
+    if (seg < 4) seg = 4;
+    if (seg > pl.nb_tiles) seg = pl.nb_tiles;
+    if (c->tune_slices > 0) {
+        seg = (pl.nb_tiles + c->tune_slices - 1) / c->tune_slices;
+        if (seg < 1) seg = 1;
+    }
+    pl.seg_tiles = (int)seg;
+    pl.segs = (pl.nb_tiles + pl.seg_tiles - 1) / pl.seg_tiles;
+    pl.partA = (size_t)pl.segs * planes * pl.na_pad * sizeof(double);
+    pl.partB = partB_row_offset(self ? 1 : 0, planes, pl.a_tiles, pl.ta, pl.nb_pad) * sizeof(double);
+    return pl;
+}
+
+template <class P, int KA, int NT, int MINB>
+static int launch_sym(frost_ctx *c, const SymParams &prm, const SymPlan &pl) {
+    const size_t smem = (size_t)kStages * P::kRecs * NT * kRecBytes + 2 * P::kPlanes * NT * sizeof(double) +
+                        kStages * sizeof(uint64_t);
+    static bool attr_done = false;
+    if (!attr_done) {
+        FROST_CUDA(c, cudaFuncSetAttribute(sym_kernel<P, KA, NT, MINB>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    dim3 grid(pl.a_tiles, pl.segs);
+    sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
+    return check_launch(c);
+}
+
+constexpr int kSymNT = 256;
+constexpr int kSymKNewton = 4, kSymKGrad = 2, kSymKTau = 2;
+
+int sym_pad_a(int kind, int n) {
+    const int k = kind == 0 ? kSymKNewton : (kind == 1 ? kSymKGrad : kSymKTau);
+    return round_up(n > 0 ? n : 1, k * kSymNT);
+}
+
+// Newton sweep, both directions at once.  self: B == A (B arguments ignored).
+int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
+               const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
+               double *A_a_packed, double *B_a_packed) {
+    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
+    const SymPlan pl = make_sym_plan<kSymKNewton, kSymNT>(c, 3, self, nA, nB, c->num_sms * 2);
+    FROST_TRY(ensure(c, c->partial, pl.partA));
+    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
+    SymParams prm{};
+    prm.a0 = (const double4 *)A_xm; prm.b0 = (const double4 *)(self ? A_xm : B_xm);
+    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
+    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
+    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
+    prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
+    FROST_TRY((launch_sym<SymNewton, kSymKNewton, kSymNT, 2>(c, prm, pl)));
+    sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
+        prm.partA, prm.partB, prm.self, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+        pl.seg_tiles, nA, c->G, A_idx, ld, out_acc, (double4 *)A_a_packed, 0.0, nullptr);
+    FROST_TRY(check_launch(c));
+    if (!self) {
+        sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
+            prm.partA, prm.partB, 0, 1, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+            pl.seg_tiles, nB, c->G, B_idx, ld, out_acc, (double4 *)B_a_packed, 0.0, nullptr);
+        FROST_TRY(check_launch(c));
+    }
+    return FROST_OK;
+}
+
+int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
+                 const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
+                 int ld, double *out_grad) {
+    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
+    const SymPlan pl = make_sym_plan<kSymKGrad, kSymNT>(c, 3, self, nA, nB, c->num_sms * 2);
+    FROST_TRY(ensure(c, c->partial, pl.partA));
+    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
+    SymParams prm{};
+    prm.a0 = (const double4 *)A_xm; prm.a1 = (const double4 *)A_a;
+    prm.b0 = (const double4 *)(self ? A_xm : B_xm); prm.b1 = (const double4 *)(self ? A_a : B_a);
+    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
+    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
+    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
+    prm.eps2 = c->eps2;
+    FROST_TRY((launch_sym<SymGradient, kSymKGrad, kSymNT, 2>(c, prm, pl)));
+    sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
+        prm.partA, prm.partB, prm.self, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+        pl.seg_tiles, nA, 2.0 * c->G, A_idx, ld, out_grad, nullptr, 0.0, nullptr);
+    FROST_TRY(check_launch(c));
+    if (!self) {
+        sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
+            prm.partA, prm.partB, 0, 1, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+            pl.seg_tiles, nB, 2.0 * c->G, B_idx, ld, out_grad, nullptr, 0.0, nullptr);
+        FROST_TRY(check_launch(c));
+    }
+    return FROST_OK;
+}
+
+int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
+                 double tau_pivot, double *out_tau, int32_t *out_bin) {
+    if (n_set <= 0) return FROST_OK;
+    const SymPlan pl = make_sym_plan<kSymKTau, kSymNT>(c, 1, true, n_set, n_set, c->num_sms * 2);
+    FROST_TRY(ensure(c, c->partial, pl.partA));
+    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
+    SymParams prm{};
+    prm.a0 = (const double4 *)xm; prm.a1 = (const double4 *)v;
+    prm.b0 = prm.a0; prm.b1 = prm.a1;
+    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
+    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = 1;
+    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
+    prm.eps2 = 0.0; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+    FROST_TRY((launch_sym<SymTimestep, kSymKTau, kSymNT, 2>(c, prm, pl)));
+    sym_reduce_kernel<1, true><<<(n_set + 255) / 256, 256, 0, c->stream>>>(
+        prm.partA, prm.partB, 1, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles, pl.seg_tiles,
+        n_set, 1.0, idx, 0, out_tau, nullptr, tau_pivot, out_bin);
+    return check_launch(c);
+}
+
+}  // namespace frost
