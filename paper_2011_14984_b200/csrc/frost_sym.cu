@@ -362,20 +362,20 @@ static int launch_sym(frost_ctx *c, const SymParams &prm, const SymPlan &pl) {
     return check_launch(c);
 }
 
-constexpr int kSymNT = 256;
-constexpr int kSymKNewton = 4, kSymKGrad = 2, kSymKTau = 2;
+// Geometry chosen by measurement on B200 (N = 262144; ms for Newton / gradient / time step):
+//   256 threads x 2 CTAs/SM, KA = 4/2/2 (<=128 registers)   46.2 / 80.6 / 167.0
+//   256 threads x 1 CTA/SM,  KA = 8/4/4                      45.2 / 76.2 / 166.5
+//   128 threads x 2 CTAs/SM, KA = 8/4/4 (<=255 registers)    44.4 / 75.6 / 164.4   <- used
+// More A particles per thread amortise the per-step SHFL / LDS / address instructions; the A tile
+// is 1024 (Newton) or 512 (gradient, time step) particles, the B tile 128.
+constexpr int kSymNT = 128, kSymMinB = 2;
+constexpr int kSymKNewton = 8, kSymKGrad = 4, kSymKTau = 4;
 
-int sym_pad_a(int kind, int n) {
-    const int k = kind == 0 ? kSymKNewton : (kind == 1 ? kSymKGrad : kSymKTau);
-    return round_up(n > 0 ? n : 1, k * kSymNT);
-}
-
-// Newton sweep, both directions at once.  self: B == A (B arguments ignored).
-int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
+template <int KA, int NT, int MINB>
+static int sym_newton_t(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
                const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
                double *A_a_packed, double *B_a_packed) {
-    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
-    const SymPlan pl = make_sym_plan<kSymKNewton, kSymNT>(c, 3, self, nA, nB, c->num_sms * 2);
+    const SymPlan pl = make_sym_plan<KA, NT>(c, 3, self, nA, nB, c->num_sms * MINB);
     FROST_TRY(ensure(c, c->partial, pl.partA));
     FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
     SymParams prm{};
@@ -384,25 +384,34 @@ int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int
     prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
     prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
     prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
-    FROST_TRY((launch_sym<SymNewton, kSymKNewton, kSymNT, 2>(c, prm, pl)));
+    FROST_TRY((launch_sym<SymNewton, KA, NT, MINB>(c, prm, pl)));
     sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, prm.self, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+        prm.partA, prm.partB, prm.self, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
         pl.seg_tiles, nA, c->G, A_idx, ld, out_acc, (double4 *)A_a_packed, 0.0, nullptr);
     FROST_TRY(check_launch(c));
     if (!self) {
         sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
-            prm.partA, prm.partB, 0, 1, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+            prm.partA, prm.partB, 0, 1, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
             pl.seg_tiles, nB, c->G, B_idx, ld, out_acc, (double4 *)B_a_packed, 0.0, nullptr);
         FROST_TRY(check_launch(c));
     }
     return FROST_OK;
 }
 
-int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
+// Newton sweep, both directions at once.  self: B == A (B arguments ignored).
+int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
+               const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
+               double *A_a_packed, double *B_a_packed) {
+    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
+    return sym_newton_t<kSymKNewton, kSymNT, kSymMinB>(c, A_xm, nA, B_xm, nB, self, A_idx, B_idx, ld, out_acc,
+                                                        A_a_packed, B_a_packed);
+}
+
+template <int KA, int NT, int MINB>
+static int sym_gradient_t(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
                  const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
                  int ld, double *out_grad) {
-    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
-    const SymPlan pl = make_sym_plan<kSymKGrad, kSymNT>(c, 3, self, nA, nB, c->num_sms * 2);
+    const SymPlan pl = make_sym_plan<KA, NT>(c, 3, self, nA, nB, c->num_sms * MINB);
     FROST_TRY(ensure(c, c->partial, pl.partA));
     FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
     SymParams prm{};
@@ -412,24 +421,32 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
     prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
     prm.eps2 = c->eps2;
-    FROST_TRY((launch_sym<SymGradient, kSymKGrad, kSymNT, 2>(c, prm, pl)));
+    FROST_TRY((launch_sym<SymGradient, KA, NT, MINB>(c, prm, pl)));
     sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, prm.self, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+        prm.partA, prm.partB, prm.self, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
         pl.seg_tiles, nA, 2.0 * c->G, A_idx, ld, out_grad, nullptr, 0.0, nullptr);
     FROST_TRY(check_launch(c));
     if (!self) {
         sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
-            prm.partA, prm.partB, 0, 1, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
+            prm.partA, prm.partB, 0, 1, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
             pl.seg_tiles, nB, 2.0 * c->G, B_idx, ld, out_grad, nullptr, 0.0, nullptr);
         FROST_TRY(check_launch(c));
     }
     return FROST_OK;
 }
 
-int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
+int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
+                 const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
+                 int ld, double *out_grad) {
+    if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
+    return sym_gradient_t<kSymKGrad, kSymNT, kSymMinB>(c, A_xm, A_a, nA, B_xm, B_a, nB, self, A_idx, B_idx, ld,
+                                                        out_grad);
+}
+
+template <int KA, int NT, int MINB>
+static int sym_timestep_t(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
                  double tau_pivot, double *out_tau, int32_t *out_bin) {
-    if (n_set <= 0) return FROST_OK;
-    const SymPlan pl = make_sym_plan<kSymKTau, kSymNT>(c, 1, true, n_set, n_set, c->num_sms * 2);
+    const SymPlan pl = make_sym_plan<KA, NT>(c, 1, true, n_set, n_set, c->num_sms * MINB);
     FROST_TRY(ensure(c, c->partial, pl.partA));
     FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
     SymParams prm{};
@@ -439,11 +456,17 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
     prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = 1;
     prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
     prm.eps2 = 0.0; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-    FROST_TRY((launch_sym<SymTimestep, kSymKTau, kSymNT, 2>(c, prm, pl)));
+    FROST_TRY((launch_sym<SymTimestep, KA, NT, MINB>(c, prm, pl)));
     sym_reduce_kernel<1, true><<<(n_set + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, 1, 0, pl.ta, kSymNT, pl.na_pad, pl.nb_pad, pl.nb_tiles, pl.seg_tiles,
+        prm.partA, prm.partB, 1, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles, pl.seg_tiles,
         n_set, 1.0, idx, 0, out_tau, nullptr, tau_pivot, out_bin);
     return check_launch(c);
+}
+
+int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
+                 double tau_pivot, double *out_tau, int32_t *out_bin) {
+    if (n_set <= 0) return FROST_OK;
+    return sym_timestep_t<kSymKTau, kSymNT, kSymMinB>(c, xm, v, n_set, idx, tau_pivot, out_tau, out_bin);
 }
 
 }  // namespace frost
