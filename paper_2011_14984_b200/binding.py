@@ -64,7 +64,7 @@ def load_library():
     lib.frost_destroy.argtypes = [vp]
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
     lib.frost_set_tuning.argtypes = [vp, i32, i32, i32]
-    lib.frost_set_symmetric.argtypes = [vp, i32]
+    lib.frost_set_symmetric.argtypes = [vp, i32, i32]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_timesteps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, vp, vp]
@@ -149,9 +149,10 @@ class Frost:
                                               small_set_max),
                     "frost_set_tuning")
 
-    def set_symmetric(self, mode=0):
-        """0 = auto, 1 = one-sided sweeps only, 2 = pair-symmetric sweeps whenever applicable."""
-        self._check(self.lib.frost_set_symmetric(self.h, mode), "frost_set_symmetric")
+    def set_symmetric(self, mode=0, scratch_mib=0):
+        """0 = auto, 1 = one-sided sweeps only, 2 = pair-symmetric sweeps whenever applicable;
+        scratch_mib caps the B-side scratch (0 = default 4096 MiB)."""
+        self._check(self.lib.frost_set_symmetric(self.h, mode, scratch_mib), "frost_set_symmetric")
 
     def launch_count(self) -> int:
         return int(self.lib.frost_launch_count(self.h))

@@ -36,7 +36,7 @@ int frost_destroy(frost_ctx *c) {
     if (!c) return FROST_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->iota,
+    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->symtot, &c->iota,
                    &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
@@ -68,9 +68,10 @@ int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices, int 
     return FROST_OK;
 }
 
-int frost_set_symmetric(frost_ctx *c, int mode) {
-    if (!c || mode < 0 || mode > 2) return FROST_EINVAL;
+int frost_set_symmetric(frost_ctx *c, int mode, int scratch_mib) {
+    if (!c || mode < 0 || mode > 2 || scratch_mib < 0) return FROST_EINVAL;
     c->tune_sym = mode;
+    c->sym_scratch = (size_t)(scratch_mib > 0 ? scratch_mib : 4096) << 20;
     return FROST_OK;
 }
 

@@ -35,6 +35,8 @@ struct frost_ctx {
     frost::Buf recA_v, recB_v;     // packed {ax,ay,az,0} or {vx,vy,vz,0}
     frost::Buf partial;            // [slices][3][n_pad] partial sums / [slices][n_pad] partial minima
     frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
+    frost::Buf symtot;             // running totals across bands of a symmetric sweep
+    size_t sym_scratch = (size_t)4 << 30;   // cap of partialB: the B list is swept in bands
     frost::Buf iota;               // unused placeholder for identity lists
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
     frost::Buf blockcnt;           // partition scratch

@@ -4,7 +4,7 @@
 // symmetrised time-step candidate -- is either symmetric or antisymmetric under i <-> j
 // ("the force-gradient term ... obeys Newton's third law"), so one evaluation
 // can serve both ordered pairs (i <- j) and (j <- i): 20 instead of 2 x 16 FP64 instructions for
-// the Newton pair, 29 instead of 2 x 28 for the gradient pair, one candidate instead of two for
+// the Newton pair, 32 instead of 2 x 28 for the gradient pair, one candidate instead of two for
 // the time step.  The one-sided sweeps of frost_sweeps.cu cannot exploit this because their
 // sources are broadcast to all lanes; here both particles of a pair live in registers:
 //
@@ -33,23 +33,13 @@ struct SymParams {
     const double4 *a0, *a1;   // A records {x,y,z,m} and {ax,ay,az,.} / {vx,vy,vz,.}
     const double4 *b0, *b1;   // B records
     double *partA;            // [segments][planes][na_pad]
-    double *partB;            // per A tile: [planes][row length]   (see partB_row)
-    int na_pad, nb_pad;
+    double *partB;            // [A tile][planes][band_len]: B-side sums of the current band
+    int na_pad;
     int self;                 // A list == B list: visit only B tiles >= the A tile
-    int nb_tiles;             // B tiles of NT records
+    int bt0, bt1;             // the band: B tiles [bt0, bt1) of NT records (scratch is per band)
     int seg_tiles;            // B tiles per CTA
     double eps2, eta_ff, eta_fb;
 };
-
-// B-side partial sums of A tile I: self case rows are triangular (particles beyond the A tile).
-__host__ __device__ inline size_t partB_row_offset(int self, int planes, int I, int TA, int nb_pad) {
-    if (self) return (size_t)planes * ((size_t)I * nb_pad - (size_t)TA * ((size_t)I * (I + 1) / 2));
-    return (size_t)planes * (size_t)I * nb_pad;
-}
-__host__ __device__ inline int partB_row_len(int self, int I, int TA, int nb_pad) {
-    return self ? nb_pad - TA * (I + 1) : nb_pad;
-}
-__host__ __device__ inline int partB_row_first(int self, int I, int TA) { return self ? TA * (I + 1) : 0; }
 
 // ------------------------------------------------------------------------------------------------
 // Pair policies: A particle in registers, B particle = shared-memory record + travelling sums.
@@ -96,7 +86,7 @@ struct SymGradient {
         a.s[0] = a.s[1] = a.s[2] = 0.0;
     }
     __device__ static __forceinline__ void init_b(double (&b)[3]) { b[0] = b[1] = b[2] = 0.0; }
-    // 29 FP64 instructions for both ordered pairs: v = a_ji - 3 s^-2 (x_ji . a_ji) x_ji is odd
+    // 32 FP64 instructions for both ordered pairs: v = a_ji - 3 s^-2 (x_ji . a_ji) x_ji is odd
     // under i <-> j, s^-3 is even: g_i += m_j s^-3 v, g_j -= m_i s^-3 v  (Eq. 27 both ways).
     __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
                                                 const double4 &j1, const SymParams &p) {
@@ -171,11 +161,11 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     constexpr uint32_t kStageBytes = P::kRecs * NT * kRecBytes;
 
     const int I = blockIdx.x;
-    const int row_first_tile = prm.self ? I * KA : 0;          // first B tile this A tile visits
     const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
+    const int row_first_tile = max(prm.self ? I * KA : 0, prm.bt0);   // first B tile of this A tile in the band
     const int tile0 = row_first_tile + blockIdx.y * prm.seg_tiles;
-    if (tile0 >= prm.nb_tiles) return;
-    const int ntiles = min(prm.seg_tiles, prm.nb_tiles - tile0);
+    if (tile0 >= prm.bt1) return;
+    const int ntiles = min(prm.seg_tiles, prm.bt1 - tile0);
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double4 *tiles = reinterpret_cast<double4 *>(smem_raw);                   // [kStages][kRecs][NT]
@@ -208,9 +198,9 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
 #pragma unroll
     for (int k = 0; k < KA; ++k) P::load(a[k], prm, a_first + k * NT);
 
-    double *rowB = prm.partB + partB_row_offset(prm.self, PL, I, TA, prm.nb_pad);
-    const int row_len = partB_row_len(prm.self, I, TA, prm.nb_pad);
-    const int row_j0 = partB_row_first(prm.self, I, TA);
+    const int row_len = (prm.bt1 - prm.bt0) * NT;             // B particles of the band
+    double *rowB = prm.partB + (size_t)I * PL * row_len;
+    const int row_j0 = prm.bt0 * NT;
     const int from = (lane + 31) & 31;          // travellers move to the next lane each step
 
     for (int t = 0; t < ntiles; ++t) {
@@ -262,41 +252,49 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Fixed-order reduction of the partial sums of one side.
-//   total_i = sum over the segments of i's A tile of partA  (if i was on the A side)
-//           + sum over the A tiles that met i as a B particle of partB.
+// Fixed-order reduction of the partial sums of one band, carried in a running total.
+//   total_i (+)= sum over the segments of i's A tile of partA    (if i is on the A side)
+//              + sum over the A tiles that met i as a B particle of partB   (if i lies in the band)
 // side 0: particles of the A list; side 1: particles of the B list (bipartite case only).
+// first != 0: the total starts from zero (+inf for minima); last != 0: the scaled total is
+// scattered to the caller's planes (and the packed stream / the bins are written).
 // ------------------------------------------------------------------------------------------------
 template <int PL, bool MIN>
 __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double *__restrict__ partB,
-                                  int self, int side, int TA, int NT, int na_pad, int nb_pad,
-                                  int nb_tiles, int seg_tiles, int n_out, double scale,
+                                  double *__restrict__ total, int n_total, int self, int side,
+                                  int TA, int NT, int na_pad, int a_tiles, int bt0, int bt1,
+                                  int seg_tiles, int first, int last, int i0, int n_out, double scale,
                                   const int32_t *__restrict__ idx, int ld, double *__restrict__ out,
                                   double4 *__restrict__ packed, double tau_pivot,
                                   int32_t *__restrict__ out_bin) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = i0 + blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_out) return;
     double s[PL];
 #pragma unroll
-    for (int p = 0; p < PL; ++p) s[p] = MIN ? __longlong_as_double(0x7ff0000000000000LL) : 0.0;
+    for (int p = 0; p < PL; ++p)
+        s[p] = first ? (MIN ? __longlong_as_double(0x7ff0000000000000LL) : 0.0) : total[(size_t)p * n_total + i];
     auto add = [&](int p, double v) { s[p] = MIN ? fmin(s[p], v) : s[p] + v; };
     if (side == 0) {
         const int I = i / TA;
-        const int first = self ? I * (TA / NT) : 0;
-        const int nseg = (nb_tiles - first + seg_tiles - 1) / seg_tiles;
+        int t_first = self ? I * (TA / NT) : 0;
+        if (t_first < bt0) t_first = bt0;
+        const int nseg = t_first < bt1 ? (bt1 - t_first + seg_tiles - 1) / seg_tiles : 0;
         for (int g = 0; g < nseg; ++g)
 #pragma unroll
             for (int p = 0; p < PL; ++p) add(p, partA[((size_t)g * PL + p) * na_pad + i]);
     }
-    if (side == 1 || self) {
-        const int rows = self ? i / TA : na_pad / TA;        // A tiles that met i on their B side
-        for (int I = 0; I < rows; ++I) {
-            const double *row = partB + partB_row_offset(self, PL, I, TA, nb_pad);
-            const int len = partB_row_len(self, I, TA, nb_pad);
-            const int j = i - partB_row_first(self, I, TA);
+    if ((side == 1 || self) && i >= bt0 * NT && i < bt1 * NT) {
+        const int rows = self ? i / TA : a_tiles;            // A tiles that met i on their B side
+        const int len = (bt1 - bt0) * NT;
+        const double *col = partB + (i - bt0 * NT);
+        for (int I = 0; I < rows; ++I)
 #pragma unroll
-            for (int p = 0; p < PL; ++p) add(p, row[(size_t)p * len + j]);
-        }
+            for (int p = 0; p < PL; ++p) add(p, col[((size_t)I * PL + p) * len]);
+    }
+    if (!last) {
+#pragma unroll
+        for (int p = 0; p < PL; ++p) total[(size_t)p * n_total + i] = s[p];
+        return;
     }
     const int g = idx ? idx[i] : i;
     if (MIN) {
@@ -318,48 +316,100 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
 }
 
 // ------------------------------------------------------------------------------------------------
-// Planning and launch
+// Planning and launch.  The B list is processed in bands so that the B-side scratch
+// (A tiles x planes x band length) stays below frost_ctx::sym_scratch bytes whatever N is; one band
+// = one sweep launch + one reduction launch per side.
 // ------------------------------------------------------------------------------------------------
-struct SymPlan { int ta, nt, na_pad, nb_pad, a_tiles, nb_tiles, seg_tiles, segs; size_t partA, partB; };
-
-template <int KA, int NT>
-static SymPlan make_sym_plan(const frost_ctx *c, int planes, bool self, int nA, int nB, int resident) {
-    SymPlan pl;
-    pl.ta = KA * NT; pl.nt = NT;
-    pl.na_pad = round_up(nA > 0 ? nA : 1, pl.ta);
-    pl.nb_pad = self ? pl.na_pad : round_up(nB > 0 ? nB : 1, NT);
-    pl.a_tiles = pl.na_pad / pl.ta;
-    pl.nb_tiles = pl.nb_pad / NT;
-    // tile pairs in total; aim at >= 24 waves of work units, at least 4 tiles per unit
-    const long long pairs = self ? (long long)pl.a_tiles * pl.nb_tiles - (long long)KA * pl.a_tiles * (pl.a_tiles - 1) / 2
-                                 : (long long)pl.a_tiles * pl.nb_tiles;
-    long long seg = pairs / (24LL * resident);
-    if (seg < 4) seg = 4;
-    if (seg > pl.nb_tiles) seg = pl.nb_tiles;
-    if (c->tune_slices > 0) {
-        seg = (pl.nb_tiles + c->tune_slices - 1) / c->tune_slices;
-        if (seg < 1) seg = 1;
-    }
-    pl.seg_tiles = (int)seg;
-    pl.segs = (pl.nb_tiles + pl.seg_tiles - 1) / pl.seg_tiles;
-    pl.partA = (size_t)pl.segs * planes * pl.na_pad * sizeof(double);
-    pl.partB = partB_row_offset(self ? 1 : 0, planes, pl.a_tiles, pl.ta, pl.nb_pad) * sizeof(double);
-    return pl;
-}
+struct SymJob {
+    const double *A0, *A1, *B0, *B1;     // packed record streams (B* ignored when self)
+    int nA, nB;
+    bool self;
+    const int32_t *A_idx, *B_idx;
+    int ld;
+    double *out;                         // planes [3][ld] (sums) or tau[n] (minima)
+    double *A_packed, *B_packed;         // optional packed {s_x, s_y, s_z, 1} streams of the results
+    double scale, eps2, tau_pivot;
+    int32_t *out_bin;
+};
 
 template <class P, int KA, int NT, int MINB>
-static int launch_sym(frost_ctx *c, const SymParams &prm, const SymPlan &pl) {
-    const size_t smem = (size_t)kStages * P::kRecs * NT * kRecBytes + 2 * P::kPlanes * NT * sizeof(double) +
-                        kStages * sizeof(uint64_t);
+static int run_sym(frost_ctx *c, const SymJob &job) {
+    constexpr int PL = P::kPlanes, TA = KA * NT;
+    constexpr bool MIN = P::kMin;
+    const bool self = job.self;
+    const int na_pad = round_up(job.nA > 0 ? job.nA : 1, TA);
+    const int nb_pad = self ? na_pad : round_up(job.nB > 0 ? job.nB : 1, NT);
+    const int a_tiles = na_pad / TA, nb_tiles = nb_pad / NT;
+    const int nB = self ? job.nA : job.nB;
+    const int resident = c->num_sms * MINB;
+
+    // bands
+    const size_t row_bytes_per_tile = (size_t)a_tiles * PL * NT * sizeof(double);
+    long long band_tiles = (long long)(c->sym_scratch / row_bytes_per_tile);
+    if (band_tiles < 8) band_tiles = 8;
+    if (band_tiles > nb_tiles) band_tiles = nb_tiles;
+    const int nbands = (int)((nb_tiles + band_tiles - 1) / band_tiles);
+    band_tiles = (nb_tiles + nbands - 1) / nbands;
+    FROST_TRY(ensure(c, c->partialB, row_bytes_per_tile * (size_t)band_tiles + 256));
+    if (nbands > 1) FROST_TRY(ensure(c, c->symtot, (size_t)PL * na_pad * sizeof(double)));
+
     static bool attr_done = false;
+    const size_t smem = (size_t)kStages * P::kRecs * NT * kRecBytes + 2 * PL * NT * sizeof(double) +
+                        kStages * sizeof(uint64_t);
     if (!attr_done) {
         FROST_CUDA(c, cudaFuncSetAttribute(sym_kernel<P, KA, NT, MINB>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
     }
-    dim3 grid(pl.a_tiles, pl.segs);
-    sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
-    return check_launch(c);
+
+    for (int b = 0; b < nbands; ++b) {
+        const int bt0 = b * (int)band_tiles;
+        const int bt1 = bt0 + (int)band_tiles < nb_tiles ? bt0 + (int)band_tiles : nb_tiles;
+        const int a_rows = self ? (a_tiles < (bt1 + KA - 1) / KA ? a_tiles : (bt1 + KA - 1) / KA) : a_tiles;
+        long long pairs = 0;                                  // tile pairs of this band
+        for (int I = 0; I < a_rows; ++I) {
+            const int f = self && I * KA > bt0 ? I * KA : bt0;
+            if (f < bt1) pairs += bt1 - f;
+        }
+        long long seg = pairs / (24LL * resident);            // >= 24 waves of CTAs, >= 4 tiles each
+        if (seg < 4) seg = 4;
+        if (seg > bt1 - bt0) seg = bt1 - bt0;
+        if (c->tune_slices > 0) {
+            seg = (bt1 - bt0 + c->tune_slices - 1) / c->tune_slices;
+            if (seg < 1) seg = 1;
+        }
+        const int segs = (int)((bt1 - bt0 + seg - 1) / seg);
+        FROST_TRY(ensure(c, c->partial, (size_t)segs * PL * na_pad * sizeof(double)));
+
+        SymParams prm{};
+        prm.a0 = (const double4 *)job.A0; prm.a1 = (const double4 *)job.A1;
+        prm.b0 = (const double4 *)(self ? job.A0 : job.B0); prm.b1 = (const double4 *)(self ? job.A1 : job.B1);
+        prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
+        prm.na_pad = na_pad; prm.self = self ? 1 : 0; prm.bt0 = bt0; prm.bt1 = bt1;
+        prm.seg_tiles = (int)seg;
+        prm.eps2 = job.eps2; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+        dim3 grid(a_rows, segs);
+        sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
+        FROST_TRY(check_launch(c));
+
+        const int first = b == 0, last = b == nbands - 1;
+        sym_reduce_kernel<PL, MIN><<<(job.nA + 255) / 256, 256, 0, c->stream>>>(
+            prm.partA, prm.partB, (double *)c->symtot.p, na_pad, prm.self, 0, TA, NT, na_pad, a_tiles,
+            bt0, bt1, prm.seg_tiles, first, last, 0, job.nA, job.scale, job.A_idx, job.ld, job.out,
+            (double4 *)job.A_packed, job.tau_pivot, job.out_bin);
+        FROST_TRY(check_launch(c));
+        if (!self) {          // a B particle only collects in its own band: no running total
+            const int i0 = bt0 * NT, i1 = bt1 * NT < nB ? bt1 * NT : nB;
+            if (i1 > i0) {
+                sym_reduce_kernel<PL, MIN><<<(i1 - i0 + 255) / 256, 256, 0, c->stream>>>(
+                    prm.partA, prm.partB, nullptr, 0, 0, 1, TA, NT, na_pad, a_tiles, bt0, bt1,
+                    prm.seg_tiles, 1, 1, i0, i1, job.scale, job.B_idx, job.ld, job.out,
+                    (double4 *)job.B_packed, job.tau_pivot, job.out_bin);
+                FROST_TRY(check_launch(c));
+            }
+        }
+    }
+    return FROST_OK;
 }
 
 // Geometry chosen by measurement on B200 (N = 262144; ms for Newton / gradient / time step):
@@ -371,102 +421,39 @@ static int launch_sym(frost_ctx *c, const SymParams &prm, const SymPlan &pl) {
 constexpr int kSymNT = 128, kSymMinB = 2;
 constexpr int kSymKNewton = 8, kSymKGrad = 4, kSymKTau = 4;
 
-template <int KA, int NT, int MINB>
-static int sym_newton_t(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
-               const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
-               double *A_a_packed, double *B_a_packed) {
-    const SymPlan pl = make_sym_plan<KA, NT>(c, 3, self, nA, nB, c->num_sms * MINB);
-    FROST_TRY(ensure(c, c->partial, pl.partA));
-    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
-    SymParams prm{};
-    prm.a0 = (const double4 *)A_xm; prm.b0 = (const double4 *)(self ? A_xm : B_xm);
-    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
-    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
-    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
-    prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
-    FROST_TRY((launch_sym<SymNewton, KA, NT, MINB>(c, prm, pl)));
-    sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, prm.self, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
-        pl.seg_tiles, nA, c->G, A_idx, ld, out_acc, (double4 *)A_a_packed, 0.0, nullptr);
-    FROST_TRY(check_launch(c));
-    if (!self) {
-        sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
-            prm.partA, prm.partB, 0, 1, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
-            pl.seg_tiles, nB, c->G, B_idx, ld, out_acc, (double4 *)B_a_packed, 0.0, nullptr);
-        FROST_TRY(check_launch(c));
-    }
-    return FROST_OK;
-}
-
-// Newton sweep, both directions at once.  self: B == A (B arguments ignored).
+// Newton sweep, both directions at once (Eq. 24 / 42).  self: B == A (B arguments ignored).
 int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
                const int32_t *A_idx, const int32_t *B_idx, int ld, double *out_acc,
                double *A_a_packed, double *B_a_packed) {
     if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
-    return sym_newton_t<kSymKNewton, kSymNT, kSymMinB>(c, A_xm, nA, B_xm, nB, self, A_idx, B_idx, ld, out_acc,
-                                                        A_a_packed, B_a_packed);
+    SymJob j{};
+    j.A0 = A_xm; j.B0 = B_xm; j.nA = nA; j.nB = nB; j.self = self; j.A_idx = A_idx; j.B_idx = B_idx;
+    j.ld = ld; j.out = out_acc; j.A_packed = A_a_packed; j.B_packed = B_a_packed;
+    j.scale = c->G;
+    j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;      // see NewtonPolicy::pair
+    return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB>(c, j);
 }
 
-template <int KA, int NT, int MINB>
-static int sym_gradient_t(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
-                 const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
-                 int ld, double *out_grad) {
-    const SymPlan pl = make_sym_plan<KA, NT>(c, 3, self, nA, nB, c->num_sms * MINB);
-    FROST_TRY(ensure(c, c->partial, pl.partA));
-    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
-    SymParams prm{};
-    prm.a0 = (const double4 *)A_xm; prm.a1 = (const double4 *)A_a;
-    prm.b0 = (const double4 *)(self ? A_xm : B_xm); prm.b1 = (const double4 *)(self ? A_a : B_a);
-    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
-    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = self ? 1 : 0;
-    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
-    prm.eps2 = c->eps2;
-    FROST_TRY((launch_sym<SymGradient, KA, NT, MINB>(c, prm, pl)));
-    sym_reduce_kernel<3, false><<<(nA + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, prm.self, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
-        pl.seg_tiles, nA, 2.0 * c->G, A_idx, ld, out_grad, nullptr, 0.0, nullptr);
-    FROST_TRY(check_launch(c));
-    if (!self) {
-        sym_reduce_kernel<3, false><<<(nB + 255) / 256, 256, 0, c->stream>>>(
-            prm.partA, prm.partB, 0, 1, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles,
-            pl.seg_tiles, nB, 2.0 * c->G, B_idx, ld, out_grad, nullptr, 0.0, nullptr);
-        FROST_TRY(check_launch(c));
-    }
-    return FROST_OK;
-}
-
+// Gradient sweep, both directions at once (Eq. 27 / 43 / 44); *_a are the packed accelerations.
 int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, const double *B_xm,
                  const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
                  int ld, double *out_grad) {
     if (nA <= 0 || (!self && nB <= 0)) return FROST_OK;
-    return sym_gradient_t<kSymKGrad, kSymNT, kSymMinB>(c, A_xm, A_a, nA, B_xm, B_a, nB, self, A_idx, B_idx, ld,
-                                                        out_grad);
+    SymJob j{};
+    j.A0 = A_xm; j.A1 = A_a; j.B0 = B_xm; j.B1 = B_a; j.nA = nA; j.nB = nB; j.self = self;
+    j.A_idx = A_idx; j.B_idx = B_idx; j.ld = ld; j.out = out_grad;
+    j.scale = 2.0 * c->G; j.eps2 = c->eps2;
+    return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinB>(c, j);
 }
 
-template <int KA, int NT, int MINB>
-static int sym_timestep_t(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
-                 double tau_pivot, double *out_tau, int32_t *out_bin) {
-    const SymPlan pl = make_sym_plan<KA, NT>(c, 1, true, n_set, n_set, c->num_sms * MINB);
-    FROST_TRY(ensure(c, c->partial, pl.partA));
-    FROST_TRY(ensure(c, c->partialB, pl.partB + 256));
-    SymParams prm{};
-    prm.a0 = (const double4 *)xm; prm.a1 = (const double4 *)v;
-    prm.b0 = prm.a0; prm.b1 = prm.a1;
-    prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
-    prm.na_pad = pl.na_pad; prm.nb_pad = pl.nb_pad; prm.self = 1;
-    prm.nb_tiles = pl.nb_tiles; prm.seg_tiles = pl.seg_tiles;
-    prm.eps2 = 0.0; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-    FROST_TRY((launch_sym<SymTimestep, KA, NT, MINB>(c, prm, pl)));
-    sym_reduce_kernel<1, true><<<(n_set + 255) / 256, 256, 0, c->stream>>>(
-        prm.partA, prm.partB, 1, 0, pl.ta, NT, pl.na_pad, pl.nb_pad, pl.nb_tiles, pl.seg_tiles,
-        n_set, 1.0, idx, 0, out_tau, nullptr, tau_pivot, out_bin);
-    return check_launch(c);
-}
-
+// Time-step sweep over one level (Eq. 49-54); xm carries G*m in .w and NaN padding.
 int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
                  double tau_pivot, double *out_tau, int32_t *out_bin) {
     if (n_set <= 0) return FROST_OK;
-    return sym_timestep_t<kSymKTau, kSymNT, kSymMinB>(c, xm, v, n_set, idx, tau_pivot, out_tau, out_bin);
+    SymJob j{};
+    j.A0 = xm; j.A1 = v; j.nA = n_set; j.nB = n_set; j.self = true; j.A_idx = idx;
+    j.out = out_tau; j.out_bin = out_bin; j.tau_pivot = tau_pivot; j.scale = 1.0;
+    return run_sym<SymTimestep, kSymKTau, kSymNT, kSymMinB>(c, j);
 }
 
 }  // namespace frost
