@@ -1,0 +1,120 @@
+"""Parity of the pair-symmetric sweeps (csrc/frost_sym.cu; one evaluation of a pair updates both of
+its particles) against the CPU oracle, element by element, forced on at sizes the oracle finishes
+in seconds: ragged A tiles (1024 / 512 particles) and B tiles (128), several bands of the B list
+(scratch cap of 1-3 MiB), self, mutual (slow/fast) and time-step sweeps, softening, coincident
+particles, the central-mass-at-the-origin case that meets the zero padding, determinism.
+Tolerances as in test_gpu_parity.py (north_star; reading 19)."""
+import numpy as np
+import pytest
+import torch
+
+import frost_inputs as fi
+from test_gpu_parity import TOL_TAU, check_forces, dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture()
+def frs():
+    import paper_2011_14984_b200 as frost
+    f = frost.Frost()
+    f.set_symmetric(2, 0)
+    yield f
+    f.close()
+
+
+@pytest.mark.parametrize("n,mib", [(2, 0), (127, 0), (129, 0), (1025, 1), (3000, 1), (5000, 3), (9000, 1)])
+def test_self_forces_symmetric(frs, oracle, n, mib):
+    frs.set_symmetric(2, mib)
+    pos, vel, mass = fi.plummer(n, 11)
+    a, g, _, _ = check_forces(frs, oracle, pos, mass)
+    # Newton's third law holds pair by pair in these sweeps: momentum change at rounding level
+    assert np.abs((mass * a).sum(1)).max() <= 1e-14 * (mass * np.abs(a)).sum(1).max()
+    assert np.abs((mass * g).sum(1)).max() <= 1e-12 * (mass * np.abs(g)).sum(1).max()
+
+
+def test_self_forces_symmetric_unequal_masses_softened_scaled_G(frs, oracle):
+    # (binaries no harder than 1e-3: a distant particle's g sums the huge, nearly cancelling terms of
+    # both members of a hard binary, and plain fp64 summation -- one-sided or symmetric -- then loses
+    # 1e-16 x the condition number of that sum)
+    pos, vel, mass, _ = fi.star_cluster(4096, 4, a_lo=1e-3, a_hi=1e-2)
+    check_forces(frs, oracle, pos, mass)                       # central mass at the origin meets the padding
+    check_forces(frs, oracle, pos, mass, G=6.674e-3, eps2=1e-4)
+
+
+def test_gradient_only_on_given_accelerations(frs, oracle):
+    pos, vel, mass = fi.plummer(3000, 12)
+    rng = np.random.default_rng(3)
+    acc0 = np.ascontiguousarray(rng.normal(size=(3, 3000)))
+    check_forces(frs, oracle, pos, mass, flags=2, acc0=acc0)
+
+
+@pytest.mark.parametrize("nS,nF,mib", [(700, 1800, 0), (1800, 700, 0), (2500, 300, 1), (1, 2000, 0), (1500, 1, 0)])
+def test_mutual_sets_symmetric(frs, oracle, nS, nF, mib):
+    frs.set_symmetric(2, mib)
+    n = 3000
+    pos, vel, mass = fi.plummer(n, 5)
+    perm = np.random.default_rng(1).permutation(n).astype(np.int32)
+    S, F = np.sort(perm[:nS]), np.sort(perm[nS:nS + nF])
+    a, g, _, _ = check_forces(frs, oracle, pos, mass, I=S, J=F, flags=7)
+    out = np.sort(perm[nS + nF:])
+    assert (a[:, out] == 0).all() and (g[:, out] == 5.0).all()       # untouched outside S u F
+    both = np.concatenate([S, F])
+    assert np.abs((mass[both] * a[:, both]).sum(1)).max() <= 1e-14 * (mass[both] * np.abs(a[:, both])).sum(1).max()
+
+
+def test_coincident_particles_and_determinism(frs, oracle):
+    pos, vel, mass = fi.plummer(2500, 2)
+    pos[:, 5] = pos[:, 9]                # two coincident unsoftened particles: the pair is ignored
+    pos[:, 700] = pos[:, 2400]
+    check_forces(frs, oracle, pos, mass)
+    p, m = dev(pos), dev(mass)
+    a1, g1 = frs.forces(p, m)
+    a2, g2 = frs.forces(p, m)
+    torch.cuda.synchronize()
+    assert torch.equal(a1, a2) and torch.equal(g1, g2)
+
+
+@pytest.mark.parametrize("n,mib", [(2, 0), (100, 0), (513, 0), (4097, 1)])
+def test_timesteps_symmetric(frs, oracle, n, mib):
+    frs.set_symmetric(2, mib)
+    pos, vel, mass = fi.plummer(n, 4)
+    pivot = 1.0 / 64
+    tau_ref, bin_ref = oracle.timesteps(pos, vel, mass, tau_pivot=pivot)
+    tau, bins = frs.timesteps(dev(pos), dev(vel), dev(mass), tau_pivot=pivot)
+    np.testing.assert_allclose(tau.cpu().numpy(), tau_ref, rtol=TOL_TAU)
+    assert np.array_equal(bins.cpu().numpy(), bin_ref)
+
+
+def test_timesteps_symmetric_on_subset(frs, oracle):
+    n = 5000
+    pos, vel, mass, _ = fi.star_cluster(n, 6)
+    idx = fi.active_subset(n, 0.3, 6)
+    frs.set_params(eta_ff=0.1, eta_fb=0.3)
+    tau_ref, _ = oracle.timesteps(pos, vel, mass, idx=idx, eta_ff=0.1, eta_fb=0.3)
+    tau, _ = frs.timesteps(dev(pos), dev(vel), dev(mass), idx=dev(idx), want_bins=False)
+    t = tau.cpu().numpy()
+    np.testing.assert_allclose(t[idx], tau_ref[idx], rtol=TOL_TAU)
+    assert np.isinf(np.delete(t, idx)).all()
+    frs.set_params()
+
+
+@pytest.mark.parametrize("small", [0, 100])
+def test_hhs_step_symmetric_matches_oracle(frs, oracle, small):
+    """A whole HHS-FSI step (reduced-N replica of config 5) with every streamed sweep -- self,
+    mutual slow/fast and time step -- forced through the symmetric kernels."""
+    n = 3000
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    frs.set_params(eta_ff=0.2, eta_fb=0.2)
+    frs.set_tuning(0, 0, small)
+    pr, vr = pos.copy(), vel.copy()
+    st_ref = oracle.hhs_step(pr, vr, mass, 1.0 / 256)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = frs.hhs_step(p, v, dev(mass), 1.0 / 256)
+    finally:
+        frs.set_tuning(0, 0, -1)
+    assert st == st_ref
+    pg, vg = p.cpu().numpy(), v.cpu().numpy()
+    assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
+    assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
