@@ -29,7 +29,10 @@ if ROOT not in sys.path:
 import frost_inputs as fi  # noqa: E402
 
 FLOPS_NEWTON, FLOPS_GRAD = 18, 34          # per ordered pair (FMA = 2, add/mul = 1, rsqrt = 1)
-SLOTS_NEWTON, SLOTS_GRAD = 16, 28          # FP64-pipe instructions per ordered pair as compiled
+# FP64-pipe instructions per ORDERED pair as compiled: the pair-symmetric sweeps (frost_sym.cu) spend
+# 20 (Newton) and 32 (gradient) per unordered pair; the one-sided sweeps 16 and 28 per ordered pair
+SLOTS_NEWTON, SLOTS_GRAD = 10, 16
+SLOTS_NEWTON_1S, SLOTS_GRAD_1S = 16, 28
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM
 METRIC = "pair interactions/s (acc+gradient, fp64) at N=2^20"
 UNIT = "pair interactions/s"
@@ -163,6 +166,8 @@ def run_frost(args):
     acc = torch.zeros_like(pos); grad = torch.zeros_like(pos)
     fr = frost.Frost(local)
     fr.set_params(G=1.0, eps2=0.0)
+    if args.one_sided:
+        fr.set_symmetric(1)
     lo, hi = sharding.shard_range(n, rank, world)
     sink_idx = None if world == 1 else torch.arange(lo, hi, dtype=torch.int32, device=dev)
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # > 126 MB L2
@@ -259,19 +264,23 @@ def run_frost(args):
     g_ms = float(np.mean(t_grad)); n_ms = float(np.mean(t_newton))
     sinks_here = hi - lo
     pairs_rank = float(sinks_here) * n
-    roof = {"bound": "alu", "kernel": "sweep_kernel<GradientPolicy> (gradient sweep, Eq. 27)",
+    if world > 1 or args.one_sided:      # sink-sharded / forced: the one-sided sweeps run
+        slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
+    else:
+        slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradient> (pair-symmetric gradient sweep, Eq. 27)"
+    roof = {"bound": "alu", "kernel": kname,
             "achieved": pairs_rank * FLOPS_GRAD / (g_ms * 1e-3) / 1e12, "peak": peak_tflops,
             "unit": "TFLOP/s", "traffic": None,
             "peak_source": f"derived: {SM_COUNT} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                            f"{sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz); HBM peak n/a",
-            "flops_per_pair": FLOPS_GRAD, "fp64_slots_per_pair": SLOTS_GRAD,
+            "flops_per_pair": FLOPS_GRAD, "fp64_slots_per_pair": slots_g,
             "ms_per_launch": g_ms,
-            "fp64_pipe_frac_at_max_clock": pairs_rank * SLOTS_GRAD / (g_ms * 1e-3) / slot_peak,
+            "fp64_pipe_frac_at_max_clock": pairs_rank * slots_g / (g_ms * 1e-3) / slot_peak,
             "fp64_pipe_frac_at_sampled_clock":
-                pairs_rank * SLOTS_GRAD / (g_ms * 1e-3) / (slot_peak * sm_mhz / sm_max_mhz),
+                pairs_rank * slots_g / (g_ms * 1e-3) / (slot_peak * sm_mhz / sm_max_mhz),
             "newton": {"ms_per_launch": n_ms,
                        "achieved": pairs_rank * FLOPS_NEWTON / (n_ms * 1e-3) / 1e12,
-                       "fp64_pipe_frac_at_max_clock": pairs_rank * SLOTS_NEWTON / (n_ms * 1e-3) / slot_peak},
+                       "fp64_pipe_frac_at_max_clock": pairs_rank * slots_n / (n_ms * 1e-3) / slot_peak},
             "probe": probe,
             "probe_dfma_frac_of_nominal": probe.get("dfma_thread_inst_per_s", 0.0) / slot_peak}
     roof["frac"] = roof["achieved"] / roof["peak"]
@@ -324,7 +333,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--n", type=int, default=1 << 20)
     ap.add_argument("--impl", default="frost", choices=["frost", "reference"])
-    ap.add_argument("--cpu-sinks", type=int, default=2048)
+    ap.add_argument("--cpu-sinks", type=int, default=6144)
+    ap.add_argument("--one-sided", action="store_true", help="force the one-sided sweeps (no pair symmetry)")
     ap.add_argument("--ref-sinks", type=int, default=1024)
     ap.add_argument("--warmup-ref", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)

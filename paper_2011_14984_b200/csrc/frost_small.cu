@@ -52,10 +52,26 @@ struct SmallSmem {
     int st_depth;
 };
 
+// A "team" executes a subtree: the whole CTA, or -- for sets of <= 32 particles, where the cost is
+// the latency of the ~40 dependent phases per hierarchy entry, not arithmetic -- a single warp
+// that synchronises with __syncwarp while the other warps wait at one barrier.
+struct TeamCTA {
+    static constexpr int kThreads = kSmallThreads;
+    __device__ static __forceinline__ void sync() { __syncthreads(); }
+    __device__ static __forceinline__ int tid() { return threadIdx.x; }
+};
+struct TeamWarp {
+    static constexpr int kThreads = 32;
+    __device__ static __forceinline__ void sync() { __syncwarp(); }
+    __device__ static __forceinline__ int tid() { return threadIdx.x & 31; }
+};
+constexpr int kWarpTeamMax = 32;
+
 // lanes per sink: largest power of two <= 32 with nA * L <= blockDim
+template <class T>
 __device__ __forceinline__ int lanes_per_sink(int nA) {
     int L = 1;
-    while (L < 32 && nA * (L * 2) <= kSmallThreads) L *= 2;
+    while (L < 32 && nA * (L * 2) <= T::kThreads) L *= 2;
     return L;
 }
 
@@ -70,10 +86,11 @@ __device__ __forceinline__ double shfl_min(double v, int L) {
 
 // a_i = G sum_{j in B} ...  for i in segment A (Eq. 24 / 42).  Segments are [a0, a0+nA) and
 // [b0, b0+nB) of sm.perm.  All threads must call (uniform control flow, shuffles).
+template <class T>
 __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
-    const int L = lanes_per_sink(nA);
-    const int per = kSmallThreads / L;
-    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    const int L = lanes_per_sink<T>(nA);
+    const int per = T::kThreads / L;
+    const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = 0; base < nA; base += per) {
         const int a = base + slot;
         const bool live = a < nA;
@@ -89,14 +106,15 @@ __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA
         acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
         if (live && sub == 0) sm.aa[i] = make_double4(acc.x * prm.G, acc.y * prm.G, acc.z * prm.G, 1.0);
     }
-    __syncthreads();
+    T::sync();
 }
 
 // g_i = 2G sum_{j in B} ... using sm.aa of sinks and sources (Eq. 27 / 43 / 44).
+template <class T>
 __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
-    const int L = lanes_per_sink(nA);
-    const int per = kSmallThreads / L;
-    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    const int L = lanes_per_sink<T>(nA);
+    const int per = T::kThreads / L;
+    const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = 0; base < nA; base += per) {
         const int a = base + slot;
         const bool live = a < nA;
@@ -113,14 +131,15 @@ __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int 
         const double k2g = 2.0 * prm.G;
         if (live && sub == 0) sm.gg[i] = make_double4(acc.x * k2g, acc.y * k2g, acc.z * k2g, 0.0);
     }
-    __syncthreads();
+    T::sync();
 }
 
 // tau_i = min over the other members of the level (Eq. 49-54); a level of one particle: +inf.
+template <class T>
 __device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int nA) {
-    const int L = lanes_per_sink(nA);
-    const int per = kSmallThreads / L;
-    const int sub = threadIdx.x & (L - 1), slot = threadIdx.x / L;
+    const int L = lanes_per_sink<T>(nA);
+    const int per = T::kThreads / L;
+    const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = 0; base < nA; base += per) {
         const int a = base + slot;
         const bool live = a < nA;
@@ -138,12 +157,13 @@ __device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int
         acc.tau = shfl_min(acc.tau, L);
         if (live && sub == 0) sm.tau[i] = acc.tau;
     }
-    __syncthreads();
+    T::sync();
 }
 
 // v_i += c (a_i + kappa g_i) ; x_i += c v_i  on a segment (Eq. 6).
+template <class T>
 __device__ void cta_kick(SmallSmem &sm, int a0, int nA, double c, double kappa, bool with_g) {
-    for (int a = threadIdx.x; a < nA; a += kSmallThreads) {
+    for (int a = T::tid(); a < nA; a += T::kThreads) {
         const int i = sm.perm[a0 + a];
         double4 v = sm.vv[i];
         const double4 ac = sm.aa[i];
@@ -155,34 +175,46 @@ __device__ void cta_kick(SmallSmem &sm, int a0, int nA, double c, double kappa, 
         v.x = fma(c, ax, v.x); v.y = fma(c, ay, v.y); v.z = fma(c, az, v.z);
         sm.vv[i] = v;
     }
-    __syncthreads();
+    T::sync();
 }
 
+template <class T>
 __device__ void cta_drift(SmallSmem &sm, int a0, int nA, double c) {
-    for (int a = threadIdx.x; a < nA; a += kSmallThreads) {
+    for (int a = T::tid(); a < nA; a += T::kThreads) {
         const int i = sm.perm[a0 + a];
         double4 x = sm.xm[i];
         const double4 v = sm.vv[i];
         x.x = fma(c, v.x, x.x); x.y = fma(c, v.y, x.y); x.z = fma(c, v.z, x.z);
         sm.xm[i] = x;
     }
-    __syncthreads();
+    T::sync();
 }
 
 // Stable in-place partition of the segment [a0, a0+n) of sm.perm: slow (tau >= pivot) first.
 // Returns |S| (Eq. 29).
+template <class T>
 __device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    constexpr int kWarps = kSmallThreads / 32;
+    const int lane = T::tid() & 31, w = T::tid() >> 5;
+    constexpr int kWarps = T::kThreads / 32;
+    if (T::kThreads == 32) {     // one warp, n <= 32: ballot
+        const int i = (lane < n) ? sm.perm[a0 + lane] : 0;
+        const int f = (lane < n) ? (sm.tau[i] >= pivot) : 0;
+        const unsigned m = __ballot_sync(0xffffffffu, f);
+        const int nS = __popc(m), before = __popc(m & ((1u << lane) - 1u));
+        __syncwarp();
+        if (lane < n) sm.perm[a0 + (f ? before : nS + (lane - before))] = i;
+        __syncwarp();
+        return nS;
+    }
     int nS = 0;
-    for (int base = 0; base < n; base += kSmallThreads) {
-        const int k = base + threadIdx.x;
+    for (int base = 0; base < n; base += T::kThreads) {
+        const int k = base + T::tid();
         const int f = (k < n) ? (sm.tau[sm.perm[a0 + k]] >= pivot) : 0;
         nS += __syncthreads_count(f);
     }
     int carry = 0;
-    for (int base = 0; base < n; base += kSmallThreads) {
-        const int k = base + threadIdx.x;
+    for (int base = 0; base < n; base += T::kThreads) {
+        const int k = base + T::tid();
         const int i = (k < n) ? sm.perm[a0 + k] : 0;
         const int f = (k < n) ? (sm.tau[i] >= pivot) : 0;
         int inc = f;
@@ -192,7 +224,7 @@ __device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
             if (lane >= o) inc += t;
         }
         if (lane == 31) sm.scan[w] = inc;
-        __syncthreads();
+        T::sync();
         int wbase = 0, total = 0;
         for (int q = 0; q < kWarps; ++q) {
             const int v = sm.scan[q];
@@ -205,30 +237,117 @@ __device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
             else sm.tmp[nS + (k - slow_before)] = i;
         }
         carry += total;
-        __syncthreads();
+        T::sync();
     }
-    for (int k = threadIdx.x; k < n; k += kSmallThreads) sm.perm[a0 + k] = sm.tmp[k];
-    __syncthreads();
+    for (int k = T::tid(); k < n; k += T::kThreads) sm.perm[a0 + k] = sm.tmp[k];
+    T::sync();
     return nS;
 }
 
 // fsi(set, dt): Alg. 2 on the segment [a0, a0+nA).
+template <class T>
 __device__ void cta_fsi(SmallSmem &sm, const SweepParams &pN, const SweepParams &pG, int a0, int nA,
                         double dt) {
     if (nA <= 0) return;
-    cta_newton(sm, pN, a0, nA, a0, nA);
-    cta_kick(sm, a0, nA, dt / 6.0, 0.0, false);
-    cta_drift(sm, a0, nA, dt / 2.0);
-    cta_newton(sm, pN, a0, nA, a0, nA);
-    cta_gradient(sm, pG, a0, nA, a0, nA);
-    cta_kick(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true);
-    cta_drift(sm, a0, nA, dt / 2.0);
-    cta_newton(sm, pN, a0, nA, a0, nA);
-    cta_kick(sm, a0, nA, dt / 6.0, 0.0, false);
-    if (threadIdx.x == 0) {
+    cta_newton<T>(sm, pN, a0, nA, a0, nA);
+    cta_kick<T>(sm, a0, nA, dt / 6.0, 0.0, false);
+    cta_drift<T>(sm, a0, nA, dt / 2.0);
+    cta_newton<T>(sm, pN, a0, nA, a0, nA);
+    cta_gradient<T>(sm, pG, a0, nA, a0, nA);
+    cta_kick<T>(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true);
+    cta_drift<T>(sm, a0, nA, dt / 2.0);
+    cta_newton<T>(sm, pN, a0, nA, a0, nA);
+    cta_kick<T>(sm, a0, nA, dt / 6.0, 0.0, false);
+    if (T::tid() == 0) {
         const long long np = (long long)nA * nA;
         sm.st_pn += 3 * np;
         sm.st_pg += np;
+    }
+}
+
+// The hhs_fsi recursion of Alg. 3 as a state machine over the explicit frame stack; runs until the
+// frame at base_sp has been popped.
+template <class T>
+__device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams &pN, const SweepParams &pG,
+                         int base_sp) {
+    while (true) {
+        T::sync();
+        const int sp = sm.sp;
+        if (sp < base_sp || sm.err) break;
+        const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
+        const double tau = sm.f_tau[sp];
+        const int level = P.level0 + sp;
+        if (T::kThreads > 32 && stage == 0 && cnt > 0 && cnt <= kWarpTeamMax) {
+            // the whole subtree of this entry on warp 0 (latency-bound: see TeamWarp)
+            if (threadIdx.x < 32) hhs_loop<TeamWarp>(sm, P, pN, pG, sp);
+            continue;
+        }
+        if (stage == 0) {
+            if (cnt <= 0) {
+                T::sync();
+                if (T::tid() == 0) sm.sp = sp - 1;
+                continue;
+            }
+            if (level >= P.max_depth || sp >= FROST_MAX_LEVELS - 1) {
+                T::sync();
+                if (T::tid() == 0) sm.err = FROST_EDEPTH;
+                continue;
+            }
+            cta_timesteps<T>(sm, pG, start, cnt);
+            const int nS = cta_partition<T>(sm, start, cnt, tau);
+            const int nF = cnt - nS;
+            if (nS > 0 && nF > 0) {
+                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
+                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
+                cta_kick<T>(sm, start, cnt, tau / 6.0, 0.0, false);
+            }
+            cta_fsi<T>(sm, pN, pG, start, nS, 0.5 * tau);
+            T::sync();
+            if (T::tid() == 0) {
+                sm.f_ns[sp] = nS;
+                sm.st_entries[level] += 1; sm.st_slow[level] += nS; sm.st_fast[level] += nF;
+                sm.st_pt += (long long)cnt * cnt;
+                if (level > sm.st_depth) sm.st_depth = level;
+                sm.f_stage[sp] = 1;
+                if (nF > 0) {
+                    sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
+                    sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                    sm.sp = sp + 1;
+                }
+            }
+        } else if (stage == 1) {
+            const int nS = sm.f_ns[sp], nF = cnt - nS;
+            if (nS > 0 && nF > 0) {
+                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
+                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
+                cta_gradient<T>(sm, pG, start, nS, start + nS, nF);
+                cta_gradient<T>(sm, pG, start + nS, nF, start, nS);
+                cta_kick<T>(sm, start, cnt, 2.0 * tau / 3.0, tau * tau / 48.0, true);
+            }
+            T::sync();
+            if (T::tid() == 0) {
+                sm.f_stage[sp] = 2;
+                if (nF > 0) {
+                    sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
+                    sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                    sm.sp = sp + 1;
+                }
+            }
+        } else {
+            const int nS = sm.f_ns[sp], nF = cnt - nS;
+            cta_fsi<T>(sm, pN, pG, start, nS, 0.5 * tau);
+            if (nS > 0 && nF > 0) {
+                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
+                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
+                cta_kick<T>(sm, start, cnt, tau / 6.0, 0.0, false);
+            }
+            T::sync();
+            if (T::tid() == 0) {
+                const long long cr = 2LL * nS * nF;
+                sm.st_pn += 3 * cr; sm.st_pg += cr;
+                sm.sp = sp - 1;
+            }
+        }
     }
 }
 
@@ -256,82 +375,10 @@ __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const Small
     __syncthreads();
 
     if (P.mode == 1) {
-        cta_fsi(sm, pN, pG, 0, n, P.dt_fsi);
+        if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, pN, pG, 0, n, P.dt_fsi); }
+        else cta_fsi<TeamCTA>(sm, pN, pG, 0, n, P.dt_fsi);
     } else {
-        while (true) {
-            __syncthreads();
-            const int sp = sm.sp;
-            if (sp < 0 || sm.err) break;
-            const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
-            const double tau = sm.f_tau[sp];
-            const int level = P.level0 + sp;
-            if (stage == 0) {
-                if (cnt <= 0) {
-                    __syncthreads();
-                    if (threadIdx.x == 0) sm.sp = sp - 1;
-                    continue;
-                }
-                if (level >= P.max_depth || sp >= FROST_MAX_LEVELS - 1) {
-                    __syncthreads();
-                    if (threadIdx.x == 0) sm.err = FROST_EDEPTH;
-                    continue;
-                }
-                cta_timesteps(sm, pG, start, cnt);
-                const int nS = cta_partition(sm, start, cnt, tau);
-                const int nF = cnt - nS;
-                if (nS > 0 && nF > 0) {
-                    cta_newton(sm, pN, start, nS, start + nS, nF);
-                    cta_newton(sm, pN, start + nS, nF, start, nS);
-                    cta_kick(sm, start, cnt, tau / 6.0, 0.0, false);
-                }
-                cta_fsi(sm, pN, pG, start, nS, 0.5 * tau);
-                __syncthreads();
-                if (threadIdx.x == 0) {
-                    sm.f_ns[sp] = nS;
-                    sm.st_entries[level] += 1; sm.st_slow[level] += nS; sm.st_fast[level] += nF;
-                    sm.st_pt += (long long)cnt * cnt;
-                    if (level > sm.st_depth) sm.st_depth = level;
-                    sm.f_stage[sp] = 1;
-                    if (nF > 0) {
-                        sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
-                        sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
-                        sm.sp = sp + 1;
-                    }
-                }
-            } else if (stage == 1) {
-                const int nS = sm.f_ns[sp], nF = cnt - nS;
-                if (nS > 0 && nF > 0) {
-                    cta_newton(sm, pN, start, nS, start + nS, nF);
-                    cta_newton(sm, pN, start + nS, nF, start, nS);
-                    cta_gradient(sm, pG, start, nS, start + nS, nF);
-                    cta_gradient(sm, pG, start + nS, nF, start, nS);
-                    cta_kick(sm, start, cnt, 2.0 * tau / 3.0, tau * tau / 48.0, true);
-                }
-                __syncthreads();
-                if (threadIdx.x == 0) {
-                    sm.f_stage[sp] = 2;
-                    if (nF > 0) {
-                        sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
-                        sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
-                        sm.sp = sp + 1;
-                    }
-                }
-            } else {
-                const int nS = sm.f_ns[sp], nF = cnt - nS;
-                cta_fsi(sm, pN, pG, start, nS, 0.5 * tau);
-                if (nS > 0 && nF > 0) {
-                    cta_newton(sm, pN, start, nS, start + nS, nF);
-                    cta_newton(sm, pN, start + nS, nF, start, nS);
-                    cta_kick(sm, start, cnt, tau / 6.0, 0.0, false);
-                }
-                __syncthreads();
-                if (threadIdx.x == 0) {
-                    const long long cr = 2LL * nS * nF;
-                    sm.st_pn += 3 * cr; sm.st_pg += cr;
-                    sm.sp = sp - 1;
-                }
-            }
-        }
+        hhs_loop<TeamCTA>(sm, P, pN, pG, 0);
     }
     __syncthreads();
     for (int k = threadIdx.x; k < n; k += kSmallThreads) {
