@@ -142,6 +142,57 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+
+def measure_rows(fr, frost, torch, dev, flush, hbm_peak):
+    """Side measurements of the other SURVEY.md 8(a) rows (not part of `value`): the time-step sweep
+    on config 2 and the HBM-bound O(N) kernels at N = 2^20 (L2 flushed before every timed launch;
+    algorithmic bytes per particle as in DESIGN.md)."""
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def best(f, reps=5, do_flush=True):
+        f(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            if do_flush:
+                flush.fill_(1.0)
+            a, b = ev(), ev()
+            a.record(); f(); b.record(); torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+        return min(ts)
+
+    out = {}
+    n2 = 65536
+    pos, vel, mass = fi.plummer(n2, 1)
+    p, v, m = (torch.as_tensor(x).to(dev) for x in (pos, vel, mass))
+    tau = torch.empty(n2, dtype=torch.float64, device=dev)
+    bins = torch.empty(n2, dtype=torch.int32, device=dev)
+    ms = best(lambda: fr.timesteps(p, v, m, tau_pivot=1.0 / 128, out_tau=tau, out_bin=bins), 3, False)
+    out["timestep_sweep_config2"] = {"n": n2, "ms": ms, "pairs_per_s": float(n2) * n2 / (ms * 1e-3)}
+    n = 1 << 20
+    x = torch.randn((3, n), dtype=torch.float64, device=dev)
+    w = torch.randn((3, n), dtype=torch.float64, device=dev)
+    a = torch.randn((3, n), dtype=torch.float64, device=dev)
+    g = torch.randn((3, n), dtype=torch.float64, device=dev)
+    mm = torch.rand(n, dtype=torch.float64, device=dev)
+    rec = torch.empty((n, 4), dtype=torch.float64, device=dev)
+    lib, h = fr.lib, fr.h
+    import ctypes as C
+    P = lambda t: C.c_void_p(t.data_ptr())
+    cases = {
+        "kick_with_gradient": (96, lambda: fr.kick(w, a, g, c=1e-9, kappa=1e-9)),
+        "kick": (72, lambda: fr.kick(w, a, None, c=1e-9, kappa=0.0)),
+        "drift": (72, lambda: fr.drift(x, w, c=1e-12)),
+        "gather_pack": (64, lambda: lib.frost_gather_pack(h, n, n, P(x), P(mm), None, 0, n, P(rec))),
+    }
+    for name, (bpp, f) in cases.items():
+        ms = best(f)
+        gbs = n * bpp / (ms * 1e-3) / 1e9
+        out[name] = {"n": n, "us": ms * 1e3, "bytes_per_particle": bpp, "GB_per_s": gbs,
+                     "frac_of_hbm_peak": gbs / hbm_peak}
+    return out
+
+
 def run_frost(args):
     import torch
     import torch.distributed as dist
@@ -270,7 +321,12 @@ def run_frost(args):
         slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradient> (pair-symmetric gradient sweep, Eq. 27)"
     roof = {"bound": "alu", "kernel": kname,
             "achieved": pairs_rank * FLOPS_GRAD / (g_ms * 1e-3) / 1e12, "peak": peak_tflops,
-            "unit": "TFLOP/s", "traffic": None,
+            "unit": "TFLOP/s",
+            # dram__bytes_read+write of ONE band launch (gradient band 3 of 13) from the committed
+            # ncu --set full capture, profiles/sym_ncu_full_r1b.md; bands 1-3 measured 0.51 / 0.86 /
+            # 1.30 GB, a whole sweep ~26 GB (the B-side partial sums) = ~20 GB/s: ALU-bound
+            "traffic": None if (world > 1 or args.one_sided) else 1.3047e9,
+            "traffic_scope": "one band launch of 13 per sweep (profiles/sym_ncu_full_r1b.md)",
             "peak_source": f"derived: {SM_COUNT} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                            f"{sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz); HBM peak n/a",
             "flops_per_pair": FLOPS_GRAD, "fp64_slots_per_pair": slots_g,
@@ -321,6 +377,8 @@ def run_frost(args):
                             "kick+drift": float(np.mean(t_upd))},
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roof,
            "cpu_baseline": cpu, "e2e": e2e}
+    if world == 1 and not args.no_rows:
+        out["other_rows"] = measure_rows(fr, frost, torch, dev, flush, hbm_peak)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -339,6 +397,7 @@ def main():
     ap.add_argument("--warmup-ref", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-rows", action="store_true", help="skip the side measurements of the O(N) rows")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
