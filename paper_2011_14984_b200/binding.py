@@ -63,7 +63,7 @@ def load_library():
     lib.frost_create.argtypes = [C.POINTER(vp), i32, vp]
     lib.frost_destroy.argtypes = [vp]
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
-    lib.frost_set_tuning.argtypes = [vp, i32, i32, i32]
+    lib.frost_set_tuning.argtypes = [vp, i32, i32, i32, i32]
     lib.frost_set_symmetric.argtypes = [vp, i32, i32]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -144,9 +144,9 @@ class Frost:
         self._check(self.lib.frost_set_params(self.h, G, eps2, eta_ff, eta_fb, max_depth),
                     "frost_set_params")
 
-    def set_tuning(self, sinks_per_thread=0, source_slices=0, small_set_max=-1):
+    def set_tuning(self, sinks_per_thread=0, source_slices=0, small_set_max=-1, subtree_one_cta=0):
         self._check(self.lib.frost_set_tuning(self.h, sinks_per_thread, source_slices,
-                                              small_set_max),
+                                              small_set_max, subtree_one_cta),
                     "frost_set_tuning")
 
     def set_symmetric(self, mode=0, scratch_mib=0):

@@ -56,8 +56,10 @@ int frost_set_params(frost_ctx *c, double G, double eps2, double eta_ff, double 
     return FROST_OK;
 }
 
-int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices, int small_set_max) {
-    if (!c) return FROST_EINVAL;
+int frost_set_tuning(frost_ctx *c, int sinks_per_thread, int source_slices, int small_set_max,
+                     int subtree_one_cta) {
+    if (!c || subtree_one_cta < 0 || subtree_one_cta > 1) return FROST_EINVAL;
+    c->tune_cluster = subtree_one_cta;
     if (small_set_max < -1 || small_set_max > small_max()) return FROST_EINVAL;
     c->tune_small = small_set_max;
     if (!(sinks_per_thread == 0 || sinks_per_thread == 1 || sinks_per_thread == 2 || sinks_per_thread == 4))

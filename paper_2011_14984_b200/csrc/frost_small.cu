@@ -8,6 +8,8 @@
 // The arithmetic is the same pair code as the streaming sweeps (frost_pairs.cuh).  A sink is
 // served by L = 1..32 adjacent lanes that split the source list and combine with warp shuffles, so
 // small sink sets still use the whole CTA; the combination order is fixed (deterministic).
+#include <cooperative_groups.h>
+
 #include "frost_pairs.cuh"
 
 namespace frost {
@@ -56,16 +58,78 @@ struct SmallSmem {
 // the latency of the ~40 dependent phases per hierarchy entry, not arithmetic -- a single warp
 // that synchronises with __syncwarp while the other warps wait at one barrier.
 struct TeamCTA {
+    static constexpr bool kCluster = false;
     static constexpr int kThreads = kSmallThreads;
     __device__ static __forceinline__ void sync() { __syncthreads(); }
     __device__ static __forceinline__ int tid() { return threadIdx.x; }
 };
+// A cluster of CTAs, each holding a full replica of the set and of the recursion state: every CTA
+// executes the same state machine (kicks, drifts, partitions and tiny sub-sets redundantly --
+// bitwise identical), but a large sweep is shared out by sinks and its results are written into
+// every replica through distributed shared memory, so the pair arithmetic of a 256-1024 particle
+// set runs on kClusterSize SMs instead of one.
+struct TeamCluster {
+    static constexpr int kThreads = kSmallThreads;
+    static constexpr bool kCluster = true;
+    __device__ static __forceinline__ void sync() { __syncthreads(); }
+    __device__ static __forceinline__ int tid() { return threadIdx.x; }
+};
 struct TeamWarp {
+    static constexpr bool kCluster = false;
     static constexpr int kThreads = 32;
     __device__ static __forceinline__ void sync() { __syncwarp(); }
     __device__ static __forceinline__ int tid() { return threadIdx.x & 31; }
 };
 constexpr int kWarpTeamMax = 32;
+constexpr int kClusterSize = 8;            // portable maximum
+constexpr int kClusterMinSet = 192;        // smaller sets run on one CTA
+constexpr long long kSplitPairs = 32768;   // a sweep is shared out only if it has this many pairs
+
+// Sharing a sweep over nA sinks out among the CTAs of a cluster.  Protocol per shared sweep: arrive
+// on the cluster barrier at the start (peers may still be reading the replica fields this sweep
+// will overwrite), wait before the first remote store, cluster.sync() at the end.
+struct SinkShare { int lo, hi; bool split, waited; };
+
+template <class T>
+__device__ __forceinline__ SinkShare sweep_begin(int nA, int nB) {
+    SinkShare sh{0, nA, false, true};
+    if (T::kCluster) {
+        namespace cg = cooperative_groups;
+        cg::cluster_group cl = cg::this_cluster();
+        if ((long long)nA * nB >= kSplitPairs && cl.num_blocks() > 1) {
+            const int nr = (int)cl.num_blocks(), r = (int)cl.block_rank();
+            const int chunk = (nA + nr - 1) / nr;
+            sh.lo = min(nA, r * chunk); sh.hi = min(nA, sh.lo + chunk);
+            sh.split = true; sh.waited = false;
+            cl.barrier_arrive();
+        }
+    }
+    return sh;
+}
+template <class T>
+__device__ __forceinline__ void sweep_wait(SinkShare &sh) {
+    if (T::kCluster && !sh.waited) {
+        cooperative_groups::this_cluster().barrier_wait();
+        sh.waited = true;
+    }
+}
+// store one result into the replica(s)
+template <class T, class V>
+__device__ __forceinline__ void publish(const SinkShare &sh, V *slot, const V &val) {
+    if (T::kCluster && sh.split) {
+        namespace cg = cooperative_groups;
+        cg::cluster_group cl = cg::this_cluster();
+        const int nr = (int)cl.num_blocks();
+        for (int r = 0; r < nr; ++r) *cl.map_shared_rank(slot, r) = val;
+    } else {
+        *slot = val;
+    }
+}
+template <class T>
+__device__ __forceinline__ void sweep_end(const SinkShare &sh) {
+    if (T::kCluster && sh.split) cooperative_groups::this_cluster().sync();
+    else T::sync();
+}
 
 // lanes per sink: largest power of two <= 32 with nA * L <= blockDim
 template <class T>
@@ -88,76 +152,116 @@ __device__ __forceinline__ double shfl_min(double v, int L) {
 // [b0, b0+nB) of sm.perm.  All threads must call (uniform control flow, shuffles).
 template <class T>
 __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
-    const int L = lanes_per_sink<T>(nA);
+    SinkShare sh = sweep_begin<T>(nA, nB);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
-    for (int base = 0; base < nA; base += per) {
+    for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {
         const int a = base + slot;
-        const bool live = a < nA;
+        const bool live = a < sh.hi;
         const int i = sm.perm[a0 + (live ? a : 0)];
         NewtonPolicy::Sink s;
         const double4 r = sm.xm[i];
         s.x = r.x; s.y = r.y; s.z = r.z;
-        NewtonPolicy::Acc acc; NewtonPolicy::init(acc);
-        for (int b = sub; b < nB; b += L) {
-            const double4 j0 = sm.xm[sm.perm[b0 + b]];
-            NewtonPolicy::pair(s, acc, j0, j0, prm);
+        // kIlp independent partial sums per lane: the sweep of a small set is bound by the latency
+        // of the dependent FP64 chain of a pair, not by issue
+        constexpr int kIlp = 4;
+        NewtonPolicy::Acc accs[kIlp];
+#pragma unroll
+        for (int u = 0; u < kIlp; ++u) NewtonPolicy::init(accs[u]);
+        int b = sub;
+        for (; b + (kIlp - 1) * L < nB; b += kIlp * L) {
+#pragma unroll
+            for (int u = 0; u < kIlp; ++u) {
+                const double4 j0 = sm.xm[sm.perm[b0 + b + u * L]];
+                NewtonPolicy::pair(s, accs[u], j0, j0, prm);
+            }
         }
+        for (; b < nB; b += L) {
+            const double4 j0 = sm.xm[sm.perm[b0 + b]];
+            NewtonPolicy::pair(s, accs[0], j0, j0, prm);
+        }
+        NewtonPolicy::Acc acc;
+        acc.x = (accs[0].x + accs[1].x) + (accs[2].x + accs[3].x);
+        acc.y = (accs[0].y + accs[1].y) + (accs[2].y + accs[3].y);
+        acc.z = (accs[0].z + accs[1].z) + (accs[2].z + accs[3].z);
         acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
-        if (live && sub == 0) sm.aa[i] = make_double4(acc.x * prm.G, acc.y * prm.G, acc.z * prm.G, 1.0);
+        sweep_wait<T>(sh);
+        if (live && sub == 0)
+            publish<T>(sh, &sm.aa[i], make_double4(acc.x * prm.G, acc.y * prm.G, acc.z * prm.G, 1.0));
     }
-    T::sync();
+    sweep_end<T>(sh);
 }
 
 // g_i = 2G sum_{j in B} ... using sm.aa of sinks and sources (Eq. 27 / 43 / 44).
 template <class T>
 __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
-    const int L = lanes_per_sink<T>(nA);
+    SinkShare sh = sweep_begin<T>(nA, nB);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
-    for (int base = 0; base < nA; base += per) {
+    for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {
         const int a = base + slot;
-        const bool live = a < nA;
+        const bool live = a < sh.hi;
         const int i = sm.perm[a0 + (live ? a : 0)];
         GradientPolicy::Sink s;
         const double4 r = sm.xm[i], ai = sm.aa[i];
         s.x = r.x; s.y = r.y; s.z = r.z; s.ax = ai.x; s.ay = ai.y; s.az = ai.z;
-        GradientPolicy::Acc acc; GradientPolicy::init(acc);
-        for (int b = sub; b < nB; b += L) {
+        GradientPolicy::Acc acc, acc1; GradientPolicy::init(acc); GradientPolicy::init(acc1);
+        int b = sub;
+        for (; b + L < nB; b += 2 * L) {
+            const int j = sm.perm[b0 + b], j2 = sm.perm[b0 + b + L];
+            GradientPolicy::pair(s, acc, sm.xm[j], sm.aa[j], prm);
+            GradientPolicy::pair(s, acc1, sm.xm[j2], sm.aa[j2], prm);
+        }
+        if (b < nB) {
             const int j = sm.perm[b0 + b];
             GradientPolicy::pair(s, acc, sm.xm[j], sm.aa[j], prm);
         }
+        acc.x += acc1.x; acc.y += acc1.y; acc.z += acc1.z;
         acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
         const double k2g = 2.0 * prm.G;
-        if (live && sub == 0) sm.gg[i] = make_double4(acc.x * k2g, acc.y * k2g, acc.z * k2g, 0.0);
+        sweep_wait<T>(sh);
+        if (live && sub == 0) publish<T>(sh, &sm.gg[i], make_double4(acc.x * k2g, acc.y * k2g, acc.z * k2g, 0.0));
     }
-    T::sync();
+    sweep_end<T>(sh);
 }
 
 // tau_i = min over the other members of the level (Eq. 49-54); a level of one particle: +inf.
 template <class T>
 __device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int nA) {
-    const int L = lanes_per_sink<T>(nA);
+    SinkShare sh = sweep_begin<T>(nA, nA);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
-    for (int base = 0; base < nA; base += per) {
+    for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {
         const int a = base + slot;
-        const bool live = a < nA;
+        const bool live = a < sh.hi;
         const int i = sm.perm[a0 + (live ? a : 0)];
         TimestepPolicy::Sink s;
         const double4 r = sm.xm[i], v = sm.vv[i];
         s.x = r.x; s.y = r.y; s.z = r.z; s.gm = r.w * prm.G; s.vx = v.x; s.vy = v.y; s.vz = v.z;
-        TimestepPolicy::Acc acc; TimestepPolicy::init(acc);
-        for (int b = sub; b < nA; b += L) {
+        TimestepPolicy::Acc acc, acc1; TimestepPolicy::init(acc); TimestepPolicy::init(acc1);
+        int b = sub;
+        for (; b + L < nA; b += 2 * L) {
+            const int j = sm.perm[a0 + b], j2 = sm.perm[a0 + b + L];
+            double4 j0 = sm.xm[j], k0 = sm.xm[j2];
+            j0.w *= prm.G; k0.w *= prm.G;
+            TimestepPolicy::pair(s, acc, j0, sm.vv[j], prm);
+            TimestepPolicy::pair(s, acc1, k0, sm.vv[j2], prm);
+        }
+        if (b < nA) {
             const int j = sm.perm[a0 + b];
             double4 j0 = sm.xm[j];
             j0.w *= prm.G;
             TimestepPolicy::pair(s, acc, j0, sm.vv[j], prm);
         }
+        acc.tau = fmin(acc.tau, acc1.tau);
         acc.tau = shfl_min(acc.tau, L);
-        if (live && sub == 0) sm.tau[i] = acc.tau;
+        sweep_wait<T>(sh);
+        if (live && sub == 0) publish<T>(sh, &sm.tau[i], acc.tau);
     }
-    T::sync();
+    sweep_end<T>(sh);
 }
 
 // v_i += c (a_i + kappa g_i) ; x_i += c v_i  on a segment (Eq. 6).
@@ -351,6 +455,7 @@ __device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams 
     }
 }
 
+template <class T>
 __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const SmallParams P) {
     extern __shared__ __align__(16) unsigned char small_raw[];
     SmallSmem &sm = *reinterpret_cast<SmallSmem *>(small_raw);
@@ -376,11 +481,17 @@ __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const Small
 
     if (P.mode == 1) {
         if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, pN, pG, 0, n, P.dt_fsi); }
-        else cta_fsi<TeamCTA>(sm, pN, pG, 0, n, P.dt_fsi);
+        else cta_fsi<T>(sm, pN, pG, 0, n, P.dt_fsi);
     } else {
-        hhs_loop<TeamCTA>(sm, P, pN, pG, 0);
+        hhs_loop<T>(sm, P, pN, pG, 0);
     }
     __syncthreads();
+    if (T::kCluster) {      // replicas are identical: rank 0 writes back; nobody leaves while a peer
+        namespace cg = cooperative_groups;                       // could still store into its replica
+        cg::cluster_group cl = cg::this_cluster();
+        cl.sync();
+        if (cl.block_rank() != 0) return;
+    }
     for (int k = threadIdx.x; k < n; k += kSmallThreads) {
         const int i = P.idx ? P.idx[k] : k;
         const double4 x = sm.xm[k], v = sm.vv[k];
@@ -411,8 +522,10 @@ int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const
     if (n > kSmallMax) return FROST_EINVAL;
     static bool attr_done = false;
     if (!attr_done) {
-        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                            (int)sizeof(SmallSmem)));
+        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCluster>,
+                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem)));
         attr_done = true;
     }
     SmallParams P{};
@@ -420,7 +533,18 @@ int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const
     P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0;
     P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
     P.stats = (SmallStats *)dev_stats;
-    hhs_small_kernel<<<1, kSmallThreads, sizeof(SmallSmem), c->stream>>>(P);
+    if (n >= kClusterMinSet && c->tune_cluster != 1) {   // one cluster of kClusterSize replicas
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(kClusterSize); cfg.blockDim = dim3(kSmallThreads);
+        cfg.dynamicSmemBytes = sizeof(SmallSmem); cfg.stream = c->stream;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = kClusterSize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        FROST_CUDA(c, cudaLaunchKernelEx(&cfg, hhs_small_kernel<TeamCluster>, P));
+    } else {
+        hhs_small_kernel<TeamCTA><<<1, kSmallThreads, sizeof(SmallSmem), c->stream>>>(P);
+    }
     return check_launch(c);
 }
 
