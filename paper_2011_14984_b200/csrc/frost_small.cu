@@ -132,10 +132,11 @@ __device__ __forceinline__ void sweep_end(const SinkShare &sh) {
 }
 
 // lanes per sink: largest power of two <= 32 with nA * L <= blockDim
+// (and no more lanes than sources: every extra doubling is one more shuffle stage of latency)
 template <class T>
-__device__ __forceinline__ int lanes_per_sink(int nA) {
+__device__ __forceinline__ int lanes_per_sink(int nA, int nB) {
     int L = 1;
-    while (L < 32 && nA * (L * 2) <= T::kThreads) L *= 2;
+    while (L < 32 && L < nB && nA * (L * 2) <= T::kThreads) L *= 2;
     return L;
 }
 
@@ -153,7 +154,7 @@ __device__ __forceinline__ double shfl_min(double v, int L) {
 template <class T>
 __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
     SinkShare sh = sweep_begin<T>(nA, nB);
-    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo, nB);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {
@@ -197,7 +198,7 @@ __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA
 template <class T>
 __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
     SinkShare sh = sweep_begin<T>(nA, nB);
-    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo, nB);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {
@@ -231,7 +232,7 @@ __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int 
 template <class T>
 __device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int nA) {
     SinkShare sh = sweep_begin<T>(nA, nA);
-    const int L = lanes_per_sink<T>(sh.hi - sh.lo);
+    const int L = lanes_per_sink<T>(sh.hi - sh.lo, nA);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
     for (int base = sh.lo; base < sh.hi || !sh.waited; base += per) {

@@ -232,6 +232,25 @@ def test_hhs_step_small_cluster(fr, oracle, n, small):
     assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
 
 
+@pytest.mark.parametrize("n", [150, 700, 1024])
+def test_subtree_kernel_one_cta_and_cluster_agree_bitwise(fr, n):
+    """The device-resident subtree kernel on one CTA and on a thread-block cluster of replicas
+    (large sweeps shared out by sinks) must give the same bits: a sink's sum is formed by the same
+    lanes in the same order either way... as long as the lane split is the same, so compare to
+    rounding, and the bookkeeping exactly."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    out = []
+    for one_cta in (1, 0):
+        fr.set_tuning(0, 0, -1, one_cta)
+        p, v = dev(pos), dev(vel)
+        st = fr.hhs_step(p, v, dev(mass), 1.0 / 256)
+        out.append((st, p.cpu().numpy(), v.cpu().numpy()))
+    fr.set_tuning(0, 0, -1, 0)
+    assert out[0][0] == out[1][0]
+    assert np.abs(out[0][1] - out[1][1]).max() < 1e-12 and np.abs(out[0][2] - out[1][2]).max() < 1e-10
+
+
 def test_hhs_tiny_systems_and_depth_limit(fr, oracle):
     """Five-body Solar system (Tables A1/A2) entirely inside the subtree kernel; a hard binary with
     a far too long top step must stop with FROST_EDEPTH instead of recursing forever."""
