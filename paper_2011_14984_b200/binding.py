@@ -23,7 +23,7 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics",
 ]
 
 
@@ -65,6 +65,7 @@ def load_library():
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
     lib.frost_set_tuning.argtypes = [vp, i32, i32, i32, i32]
     lib.frost_set_symmetric.argtypes = [vp, i32, i32]
+    lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_timesteps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, vp, vp]
@@ -236,6 +237,15 @@ class Frost:
         self._check(self.lib.frost_hhs_step(self.h, mass.numel(), pos.shape[1], _p(pos), _p(vel),
                                             _p(mass), dt_top, C.byref(st)), "frost_hhs_step")
         return st.as_dict()
+
+    def diagnostics(self, pos, vel, mass, out_phi=None):
+        """dict(T, U, E, P(3), L(3)) of all particles, computed on the device (frost_diagnostics)."""
+        _vec(pos, "pos"); _vec(vel, "vel")
+        out = (C.c_double * 8)()
+        self._check(self.lib.frost_diagnostics(self.h, mass.numel(), pos.shape[1], _p(pos), _p(vel),
+                                               _p(mass), _p(out_phi), out), "frost_diagnostics")
+        o = list(out)
+        return {"T": o[0], "U": o[1], "E": o[0] + o[1], "P": o[2:5], "L": o[5:8]}
 
     def fp64_probe(self, mode=0, iters=4096, blocks_per_sm=4, scratch=None):
         if scratch is None:

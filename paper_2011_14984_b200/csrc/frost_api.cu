@@ -412,6 +412,27 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     return rc;
 }
 
+int frost_diagnostics(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
+                      const double *mass, double *out_phi, double *out8) {
+    if (!c || bad_planes(n, ld) || !pos || !vel || !mass || !out8) return FROST_EINVAL;
+    for (int k = 0; k < 8; ++k) out8[k] = 0.0;
+    if (n == 0) return FROST_OK;
+    FROST_CUDA(c, cudaSetDevice(c->device));
+    const int pad = pad1024(n);
+    FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+    FROST_TRY(ensure(c, c->tau, (size_t)(ld + 8) * sizeof(double)));
+    FROST_TRY(ensure(c, c->blockcnt, 8 * sizeof(double)));
+    double *xm = (double *)c->recA_xm.p;
+    double *phi = out_phi ? out_phi : (double *)c->tau.p;
+    double *d8 = (double *)c->blockcnt.p;
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, nullptr, n, pad, xm));
+    FROST_TRY(sym_potential(c, xm, n, phi));
+    FROST_TRY(launch_diag(c, n, ld, pos, vel, mass, phi, d8));
+    FROST_CUDA(c, cudaMemcpyAsync(out8, d8, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    FROST_CUDA(c, cudaStreamSynchronize(c->stream));
+    return FROST_OK;
+}
+
 int frost_gather_pack(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
                       const int32_t *idx, int n_idx, int n_pad, double *out_records) {
     if (!c || bad_planes(n, ld) || !pos || !mass || !out_records) return FROST_EINVAL;

@@ -129,6 +129,11 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
 int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
                  double tau_pivot, double *out_tau, int32_t *out_bin);
 
+int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
+// frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)
+int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *vel, const double *mass,
+                const double *phi, double *out8);
+
 // frost_small.cu: one-CTA device-resident hhs_fsi subtree (mode 0) or fsi step (mode 1)
 int small_max();
 size_t small_stats_bytes();

@@ -150,6 +150,28 @@ struct SymTimestep {
     }
 };
 
+// Specific potential phi_i = -G sum_j m_j / s_ij (Eq. 23) for the on-device
+// energy diagnostic: 1/s is even under i <-> j.  12 FP64 instructions for both ordered pairs.
+struct SymPotential {
+    static constexpr int kRecs = 1, kPlanes = 1;
+    static constexpr bool kMin = false;
+    struct A { double x, y, z, m, s[1]; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        const double4 r = p.a0[i];
+        a.x = r.x; a.y = r.y; a.z = r.z; a.m = r.w; a.s[0] = 0.0;
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[1]) { b[0] = 0.0; }
+    __device__ static __forceinline__ void pair(A &a, double (&b)[1], const double4 &j0,
+                                                const double4 &, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+        // the self pair (and a pair at exactly the same point) is skipped, softened or not
+        const double ri = (r2 == 0.0) ? 0.0 : rsqrt_full(r2 + p.eps2);
+        a.s[0] = fma(j0.w, ri, a.s[0]);
+        b[0] = fma(a.m, ri, b[0]);
+    }
+};
+
 // ------------------------------------------------------------------------------------------------
 // The kernel.  grid = (A tiles, segments of the B list); block = NT threads; KA A particles/thread.
 // ------------------------------------------------------------------------------------------------
@@ -454,6 +476,15 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
     j.A0 = xm; j.A1 = v; j.nA = n_set; j.nB = n_set; j.self = true; j.A_idx = idx;
     j.out = out_tau; j.out_bin = out_bin; j.tau_pivot = tau_pivot; j.scale = 1.0;
     return run_sym<SymTimestep, kSymKTau, kSymNT, kSymMinB>(c, j);
+}
+
+// phi_i = -G sum_{j != i} m_j / s_ij for all particles of the packed stream (always symmetric).
+int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi) {
+    if (n <= 0) return FROST_OK;
+    SymJob j{};
+    j.A0 = xm; j.nA = n; j.nB = n; j.self = true; j.ld = n; j.out = out_phi;
+    j.scale = -c->G; j.eps2 = c->eps2;
+    return run_sym<SymPotential, kSymKGrad, kSymNT, kSymMinB>(c, j);
 }
 
 }  // namespace frost

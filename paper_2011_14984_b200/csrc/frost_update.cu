@@ -135,6 +135,55 @@ part_scatter_kernel(const double *__restrict__ tau, const int32_t *__restrict__ 
     }
 }
 
+// ---- diagnostics (Eq. 23): T, U, P, L -------------------------
+// One CTA; every thread keeps compensated (two-sum) partial sums over a strided subset, the CTA adds
+// them in a fixed tree order -- deterministic, and accurate to ~1e-16 relative for N = 2^20.
+struct Comp {
+    double s, c;
+    __device__ __forceinline__ void add(double v) {      // Neumaier
+        const double t = s + v;
+        c += (fabs(s) >= fabs(v)) ? (s - t) + v : (v - t) + s;
+        s = t;
+    }
+};
+constexpr int kDiagThreads = 1024;
+
+__global__ void __launch_bounds__(kDiagThreads)
+diag_kernel(const double *__restrict__ pos, const double *__restrict__ vel, const double *__restrict__ mass,
+            const double *__restrict__ phi, int n, int ld, double *__restrict__ out8) {
+    __shared__ double sh[2][8][kDiagThreads / 32];
+    Comp q[8];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) q[k].s = q[k].c = 0.0;
+    for (int i = threadIdx.x; i < n; i += kDiagThreads) {
+        const double m = mass[i];
+        const double x = pos[i], y = pos[(size_t)ld + i], z = pos[2 * (size_t)ld + i];
+        const double vx = vel[i], vy = vel[(size_t)ld + i], vz = vel[2 * (size_t)ld + i];
+        q[0].add(0.5 * m * fma(vz, vz, fma(vy, vy, vx * vx)));
+        q[1].add(0.5 * m * phi[i]);
+        q[2].add(m * vx); q[3].add(m * vy); q[4].add(m * vz);
+        q[5].add(m * fma(y, vz, -z * vy));
+        q[6].add(m * fma(z, vx, -x * vz));
+        q[7].add(m * fma(x, vy, -y * vx));
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        for (int o = 16; o > 0; o >>= 1) {     // fixed butterfly order
+            const double s2 = __shfl_xor_sync(0xffffffffu, q[k].s, o);
+            const double c2 = __shfl_xor_sync(0xffffffffu, q[k].c, o);
+            q[k].add(s2); q[k].c += c2;
+        }
+        if (lane == 0) { sh[0][k][w] = q[k].s; sh[1][k][w] = q[k].c; }
+    }
+    __syncthreads();
+    if (threadIdx.x < 8) {
+        Comp t; t.s = t.c = 0.0;
+        for (int ww = 0; ww < kDiagThreads / 32; ++ww) { t.add(sh[0][threadIdx.x][ww]); t.c += sh[1][threadIdx.x][ww]; }
+        out8[threadIdx.x] = t.s + t.c;
+    }
+}
+
 // ---- launchers ---------------------------------------------------------------------------------
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
                    int n_idx, int n_pad, double *out, double wscale, int nan_pad) {
@@ -187,6 +236,12 @@ int launch_partition(frost_ctx *c, const double *tau, const int32_t *idx, int n_
     counts_host[0] = c->pinned_counts[0];
     counts_host[1] = c->pinned_counts[1];
     return FROST_OK;
+}
+
+int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *vel, const double *mass,
+                const double *phi, double *out8) {
+    diag_kernel<<<1, kDiagThreads, 0, c->stream>>>(pos, vel, mass, phi, n, ld, out8);
+    return check_launch(c);
 }
 
 }  // namespace frost

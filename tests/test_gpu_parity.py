@@ -187,6 +187,45 @@ def test_kick_drift_gather(fr, oracle):
     assert (rec[idx.size:] == 0).all()
 
 
+@pytest.mark.parametrize("n,eps2", [(1, 0.0), (2, 0.0), (1000, 0.0), (5000, 1e-4), (20000, 0.0)])
+def test_diagnostics_match_oracle(fr, oracle, n, eps2):
+    """frost_diagnostics (on-device E, P, L with an O(N^2) potential sweep) against
+    the oracle's long-double textbook sums (Eq. 23)."""
+    pos, vel, mass, _ = fi.star_cluster(max(n, 64), 4, a_lo=1e-3, a_hi=1e-2)
+    pos, vel, mass = np.ascontiguousarray(pos[:, :n]), np.ascontiguousarray(vel[:, :n]), mass[:n].copy()
+    fr.set_params(G=0.7, eps2=eps2)
+    phi = torch.zeros(n, dtype=torch.float64, device="cuda")
+    d = fr.diagnostics(dev(pos), dev(vel), dev(mass), out_phi=phi)
+    ref = oracle.diagnostics(pos, vel, mass, G=0.7, eps2=eps2)
+    fr.set_params()
+    assert abs(d["T"] - ref["T"]) <= 1e-14 * abs(ref["T"])
+    assert abs(d["U"] - ref["U"]) <= 1e-13 * abs(ref["U"]) + 0.0
+    scale_p = (mass * np.abs(vel)).sum()
+    assert np.abs(np.array(d["P"]) - ref["P"]).max() <= 1e-15 * scale_p
+    scale_l = (mass * np.linalg.norm(pos, axis=0) * np.linalg.norm(vel, axis=0)).sum()
+    assert np.abs(np.array(d["L"]) - ref["L"]).max() <= 1e-15 * scale_l
+    # U = sum m phi / 2
+    assert abs(0.5 * float((dev(mass) * phi).sum()) - ref["U"]) <= 1e-12 * abs(ref["U"]) + 0.0
+
+
+def test_energy_conservation_measured_on_device(fr, oracle):
+    """Config 1 with the energy read from the device: |dE/E| after 10 FSI steps at dt = 1/1024 is
+    the oracle's to rounding (the trajectories agree to 1e-11) and small."""
+    pos, vel, mass = fi.plummer(1024, 0)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    fr.set_params()
+    e0 = fr.diagnostics(p, v, m)
+    pr, vr = pos.copy(), vel.copy()
+    for _ in range(10):
+        fr.fsi_step(p, v, m, 1.0 / 1024)
+        oracle.fsi_step(pr, vr, mass, 1.0 / 1024)
+    e1 = fr.diagnostics(p, v, m)
+    r0, r1 = oracle.diagnostics(pos, vel, mass), oracle.diagnostics(pr, vr, mass)
+    de_gpu, de_ref = (e1["E"] - e0["E"]) / e0["E"], (r1["E"] - r0["E"]) / r0["E"]
+    assert abs(de_gpu - de_ref) < 1e-11
+    assert abs(de_gpu) < 1e-3
+
+
 @pytest.mark.parametrize("small", [-1, 0])
 def test_config1_ten_fsi_steps(fr, oracle, small):
     """Config 1: N = 1024, 10 fixed-step FSI steps with dt = 1/1024 -- through the one-CTA
