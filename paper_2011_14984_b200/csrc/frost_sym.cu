@@ -438,6 +438,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
 //   256 threads x 2 CTAs/SM, KA = 4/2/2 (<=128 registers)   46.2 / 80.6 / 167.0
 //   256 threads x 1 CTA/SM,  KA = 8/4/4                      45.2 / 76.2 / 166.5
 //   128 threads x 2 CTAs/SM, KA = 8/4/4 (<=255 registers)    44.4 / 75.6 / 164.4   <- used
+//   128 threads x 2 CTAs/SM, KA = 8/8/8 (255 registers)      44.3 / 79.8 / 175.9
 // More A particles per thread amortise the per-step SHFL / LDS / address instructions; the A tile
 // is 1024 (Newton) or 512 (gradient, time step) particles, the B tile 128.
 constexpr int kSymNT = 128, kSymMinB = 2;
