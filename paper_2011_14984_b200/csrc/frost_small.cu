@@ -83,7 +83,9 @@ struct TeamWarp {
 constexpr int kWarpTeamMax = 32;
 constexpr int kClusterSize = 8;            // portable maximum
 constexpr int kClusterMinSet = 192;        // smaller sets run on one CTA
-constexpr long long kSplitPairs = 32768;   // a sweep is shared out only if it has this many pairs
+// a sweep is shared out among the cluster from this many pairs (config-5 step on B200: 8192 and
+// below 14.2-14.3 s, 32768 14.8 s, 131072 16.2 s, never 17.5 s)
+constexpr long long kSplitPairs = 8192;
 
 // Sharing a sweep over nA sinks out among the CTAs of a cluster.  Protocol per shared sweep: arrive
 // on the cluster barrier at the start (peers may still be reading the replica fields this sweep
