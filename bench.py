@@ -219,8 +219,16 @@ def run_frost(args):
     fr.set_params(G=1.0, eps2=0.0)
     if args.one_sided:
         fr.set_symmetric(1)
-    lo, hi = sharding.shard_range(n, rank, world)
-    sink_idx = None if world == 1 else torch.arange(lo, hi, dtype=torch.int32, device=dev)
+    # N > 1: the PAIRS are sharded (frost_set_shard: every rank sweeps 1/world of the tile pairs of
+    # the symmetric kernels and holds partial sums for all particles; one all-reduce per sweep)
+    lo, hi = 0, n
+    sink_idx = None
+    pair_sharded = world > 1 and not args.one_sided
+    if pair_sharded:
+        fr.set_shard(rank, world)
+    elif world > 1:          # --one-sided: sinks sharded, all-gather of a between the sweeps
+        lo, hi = sharding.shard_range(n, rank, world)
+        sink_idx = torch.arange(lo, hi, dtype=torch.int32, device=dev)
     flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)   # > 126 MB L2
 
     def ev():
@@ -232,11 +240,15 @@ def run_frost(args):
         if e: e[0].record()
         fr.forces(pos, mass, sink_idx=sink_idx, source_idx=None, out_acc=acc, out_grad=grad,
                   flags=frost.ACC)
-        if world > 1:
+        if pair_sharded:
+            sharding.all_reduce_planes(acc, world)
+        elif world > 1:
             sharding.all_gather_planes(acc[:, lo:hi].contiguous(), n, rank, world, acc)
         if e: e[1].record()
         fr.forces(pos, mass, sink_idx=sink_idx, source_idx=None, out_acc=acc, out_grad=grad,
                   flags=frost.GRAD)
+        if pair_sharded:
+            sharding.all_reduce_planes(grad, world)
         if e: e[2].record()
         fr.kick(vel, acc, grad, idx=sink_idx, c=2.0 * dt / 3.0, kappa=dt * dt / 48.0)
         fr.drift(pos, vel, idx=sink_idx, c=dt / 2.0)
@@ -314,8 +326,8 @@ def run_frost(args):
     slot_peak = SM_COUNT * FP64_LANES_PER_SM * sm_max_mhz * 1e6          # thread-level FP64 inst / s
     g_ms = float(np.mean(t_grad)); n_ms = float(np.mean(t_newton))
     sinks_here = hi - lo
-    pairs_rank = float(sinks_here) * n
-    if world > 1 or args.one_sided:      # sink-sharded / forced: the one-sided sweeps run
+    pairs_rank = float(n) * n / world if pair_sharded else float(sinks_here) * n
+    if args.one_sided:      # forced: the one-sided sweeps run
         slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
     else:
         slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradient> (pair-symmetric gradient sweep, Eq. 27)"
@@ -325,7 +337,7 @@ def run_frost(args):
             # dram__bytes_read+write of ONE band launch (gradient band 3 of 13) from the committed
             # ncu --set full capture, profiles/sym_ncu_full_r1b.md; bands 1-3 measured 0.51 / 0.86 /
             # 1.30 GB, a whole sweep ~26 GB (the B-side partial sums) = ~20 GB/s: ALU-bound
-            "traffic": None if (world > 1 or args.one_sided) else 1.3047e9,
+            "traffic": None if args.one_sided else 1.3047e9,
             "traffic_scope": "one band launch of 13 per sweep (profiles/sym_ncu_full_r1b.md)",
             "peak_source": f"derived: {SM_COUNT} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                            f"{sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz); HBM peak n/a",
@@ -369,8 +381,10 @@ def run_frost(args):
            "config": {"workload": f"Plummer sphere N={n}, equal masses, G=1, seed 2 (config 3): full "
                                   "self acc+gradient pass + kick + drift per step",
                       "l2": "flushed between timed iterations (256 MB fill)",
-                      "parallelism": "1 GPU" if world == 1 else f"sinks sharded over {world} ranks, "
-                                     "all-gather of a between the sweeps"},
+                      "parallelism": "1 GPU" if world == 1 else (
+                          f"tile pairs of the symmetric sweeps sharded over {world} ranks, all-reduce of a "
+                          "and of g" if pair_sharded else
+                          f"sinks sharded over {world} ranks, all-gather of a between the sweeps")},
            "gflops": value * (FLOPS_NEWTON + FLOPS_GRAD) / 1e9,
            "flops_convention": "Newton 18 + gradient 34 = 52 flops per ordered pair (FMA=2, add/mul=1, rsqrt=1)",
            "breakdown_ms": {"newton+pack+reduce": n_ms, "gradient+pack+reduce": g_ms,

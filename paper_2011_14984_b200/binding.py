@@ -23,7 +23,7 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics", "frost_set_shard",
 ]
 
 
@@ -65,6 +65,7 @@ def load_library():
     lib.frost_set_params.argtypes = [vp, f64, f64, f64, f64, i32]
     lib.frost_set_tuning.argtypes = [vp, i32, i32, i32, i32]
     lib.frost_set_symmetric.argtypes = [vp, i32, i32]
+    lib.frost_set_shard.argtypes = [vp, i32, i32]
     lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -154,6 +155,10 @@ class Frost:
         """0 = auto, 1 = one-sided sweeps only, 2 = pair-symmetric sweeps whenever applicable;
         scratch_mib caps the B-side scratch (0 = default 4096 MiB)."""
         self._check(self.lib.frost_set_symmetric(self.h, mode, scratch_mib), "frost_set_symmetric")
+
+    def set_shard(self, rank=0, world=1):
+        """This context's share of the symmetric sweeps (partial sums; add them across ranks)."""
+        self._check(self.lib.frost_set_shard(self.h, rank, world), "frost_set_shard")
 
     def launch_count(self) -> int:
         return int(self.lib.frost_launch_count(self.h))

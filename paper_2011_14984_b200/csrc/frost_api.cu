@@ -77,6 +77,12 @@ int frost_set_symmetric(frost_ctx *c, int mode, int scratch_mib) {
     return FROST_OK;
 }
 
+int frost_set_shard(frost_ctx *c, int rank, int world) {
+    if (!c || world < 1 || rank < 0 || rank >= world) return FROST_EINVAL;
+    c->shard_rank = rank; c->shard_world = world;
+    return FROST_OK;
+}
+
 int64_t frost_launch_count(const frost_ctx *c) { return c ? c->launches : -1; }
 int frost_last_cuda_error(const frost_ctx *c) { return c ? c->last_cuda : 0; }
 const char *frost_version(void) { return "frost-b200 0.1 (sm_100a)"; }
@@ -136,6 +142,9 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
     const bool sym_self = self && use_sym(c, nI, nI);
     const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI);
     if (sym_self || sym_mut) {
+        // sharded: the outputs are partial sums the caller adds across ranks, so the gradient sweep
+        // cannot start from this call's own (partial) accelerations
+        if (c->shard_world > 1 && (flags & FROST_ACC) && (flags & FROST_GRAD)) return FROST_EINVAL;
         const bool swap = sym_mut && nJ > nI;            // A = the larger set
         const double *Pxm = swap ? Bxm : Axm, *Qxm = swap ? Axm : Bxm;
         double *Pv = swap ? Bv : Av, *Qv = swap ? Av : Bv;

@@ -38,6 +38,7 @@ struct SymParams {
     int self;                 // A list == B list: visit only B tiles >= the A tile
     int bt0, bt1;             // the band: B tiles [bt0, bt1) of NT records (scratch is per band)
     int seg_tiles;            // B tiles per CTA
+    int row0, row_stride;     // A tiles owned by this launch: row0, row0 + row_stride, ... (sharding)
     double eps2, eta_ff, eta_fb;
 };
 
@@ -182,7 +183,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     constexpr int PL = P::kPlanes;
     constexpr uint32_t kStageBytes = P::kRecs * NT * kRecBytes;
 
-    const int I = blockIdx.x;
+    const int I = prm.row0 + blockIdx.x * prm.row_stride;
     const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
     const int row_first_tile = max(prm.self ? I * KA : 0, prm.bt0);   // first B tile of this A tile in the band
     const int tile0 = row_first_tile + blockIdx.y * prm.seg_tiles;
@@ -221,7 +222,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     for (int k = 0; k < KA; ++k) P::load(a[k], prm, a_first + k * NT);
 
     const int row_len = (prm.bt1 - prm.bt0) * NT;             // B particles of the band
-    double *rowB = prm.partB + (size_t)I * PL * row_len;
+    double *rowB = prm.partB + (size_t)blockIdx.x * PL * row_len;     // indexed by owned row
     const int row_j0 = prm.bt0 * NT;
     const int from = (lane + 31) & 31;          // travellers move to the next lane each step
 
@@ -285,7 +286,8 @@ template <int PL, bool MIN>
 __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double *__restrict__ partB,
                                   double *__restrict__ total, int n_total, int self, int side,
                                   int TA, int NT, int na_pad, int a_tiles, int bt0, int bt1,
-                                  int seg_tiles, int first, int last, int i0, int n_out, double scale,
+                                  int seg_tiles, int row0, int row_stride, int first, int last, int i0,
+                                  int n_out, double scale,
                                   const int32_t *__restrict__ idx, int ld, double *__restrict__ out,
                                   double4 *__restrict__ packed, double tau_pivot,
                                   int32_t *__restrict__ out_bin) {
@@ -300,7 +302,8 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
         const int I = i / TA;
         int t_first = self ? I * (TA / NT) : 0;
         if (t_first < bt0) t_first = bt0;
-        const int nseg = t_first < bt1 ? (bt1 - t_first + seg_tiles - 1) / seg_tiles : 0;
+        const bool mine = I >= row0 && (I - row0) % row_stride == 0;      // this shard swept i's A tile
+        const int nseg = (mine && t_first < bt1) ? (bt1 - t_first + seg_tiles - 1) / seg_tiles : 0;
         for (int g = 0; g < nseg; ++g)
 #pragma unroll
             for (int p = 0; p < PL; ++p) add(p, partA[((size_t)g * PL + p) * na_pad + i]);
@@ -309,9 +312,9 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
         const int rows = self ? i / TA : a_tiles;            // A tiles that met i on their B side
         const int len = (bt1 - bt0) * NT;
         const double *col = partB + (i - bt0 * NT);
-        for (int I = 0; I < rows; ++I)
+        for (int I = row0, li = 0; I < rows; I += row_stride, ++li)      // owned rows, ascending
 #pragma unroll
-            for (int p = 0; p < PL; ++p) add(p, col[((size_t)I * PL + p) * len]);
+            for (int p = 0; p < PL; ++p) add(p, col[((size_t)li * PL + p) * len]);
     }
     if (!last) {
 #pragma unroll
@@ -352,6 +355,7 @@ struct SymJob {
     double *A_packed, *B_packed;         // optional packed {s_x, s_y, s_z, 1} streams of the results
     double scale, eps2, tau_pivot;
     int32_t *out_bin;
+    int shard_rank = 0, shard_world = 1;   // this launch sweeps A tiles rank, rank + world, ... only
 };
 
 template <class P, int KA, int NT, int MINB>
@@ -389,7 +393,9 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         const int bt1 = bt0 + (int)band_tiles < nb_tiles ? bt0 + (int)band_tiles : nb_tiles;
         const int a_rows = self ? (a_tiles < (bt1 + KA - 1) / KA ? a_tiles : (bt1 + KA - 1) / KA) : a_tiles;
         long long pairs = 0;                                  // tile pairs of this band
-        for (int I = 0; I < a_rows; ++I) {
+        const int row0 = job.shard_rank, row_stride = job.shard_world;
+        const int my_rows = a_rows > row0 ? (a_rows - row0 + row_stride - 1) / row_stride : 0;
+        for (int I = row0; I < a_rows; I += row_stride) {
             const int f = self && I * KA > bt0 ? I * KA : bt0;
             if (f < bt1) pairs += bt1 - f;
         }
@@ -408,16 +414,18 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         prm.b0 = (const double4 *)(self ? job.A0 : job.B0); prm.b1 = (const double4 *)(self ? job.A1 : job.B1);
         prm.partA = (double *)c->partial.p; prm.partB = (double *)c->partialB.p;
         prm.na_pad = na_pad; prm.self = self ? 1 : 0; prm.bt0 = bt0; prm.bt1 = bt1;
-        prm.seg_tiles = (int)seg;
+        prm.seg_tiles = (int)seg; prm.row0 = row0; prm.row_stride = row_stride;
         prm.eps2 = job.eps2; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-        dim3 grid(a_rows, segs);
-        sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
-        FROST_TRY(check_launch(c));
+        if (my_rows > 0) {
+            dim3 grid(my_rows, segs);
+            sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
+            FROST_TRY(check_launch(c));
+        }
 
         const int first = b == 0, last = b == nbands - 1;
         sym_reduce_kernel<PL, MIN><<<(job.nA + 255) / 256, 256, 0, c->stream>>>(
             prm.partA, prm.partB, (double *)c->symtot.p, na_pad, prm.self, 0, TA, NT, na_pad, a_tiles,
-            bt0, bt1, prm.seg_tiles, first, last, 0, job.nA, job.scale, job.A_idx, job.ld, job.out,
+            bt0, bt1, prm.seg_tiles, row0, row_stride, first, last, 0, job.nA, job.scale, job.A_idx, job.ld, job.out,
             (double4 *)job.A_packed, job.tau_pivot, job.out_bin);
         FROST_TRY(check_launch(c));
         if (!self) {          // a B particle only collects in its own band: no running total
@@ -425,7 +433,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
             if (i1 > i0) {
                 sym_reduce_kernel<PL, MIN><<<(i1 - i0 + 255) / 256, 256, 0, c->stream>>>(
                     prm.partA, prm.partB, nullptr, 0, 0, 1, TA, NT, na_pad, a_tiles, bt0, bt1,
-                    prm.seg_tiles, 1, 1, i0, i1, job.scale, job.B_idx, job.ld, job.out,
+                    prm.seg_tiles, row0, row_stride, 1, 1, i0, i1, job.scale, job.B_idx, job.ld, job.out,
                     (double4 *)job.B_packed, job.tau_pivot, job.out_bin);
                 FROST_TRY(check_launch(c));
             }
@@ -454,6 +462,7 @@ int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int
     j.ld = ld; j.out = out_acc; j.A_packed = A_a_packed; j.B_packed = B_a_packed;
     j.scale = c->G;
     j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;      // see NewtonPolicy::pair
+    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
     return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB>(c, j);
 }
 
@@ -466,6 +475,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.A0 = A_xm; j.A1 = A_a; j.B0 = B_xm; j.B1 = B_a; j.nA = nA; j.nB = nB; j.self = self;
     j.A_idx = A_idx; j.B_idx = B_idx; j.ld = ld; j.out = out_grad;
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
+    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
     return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinB>(c, j);
 }
 

@@ -4,6 +4,11 @@ source stream is replicated.  The one real exchange step of the path is the all-
 Newtonian accelerations between the Newton and the gradient sweep (Eq. 27 needs a_j of every
 source).  No reduction is involved, so results are bit-identical to one GPU.
 
+Pair sharding (`pair_sharded_acc_grad`) is the multi-GPU form of the pair-symmetric sweeps
+(csrc/frost_sym.cu, frost_set_shard): every rank evaluates 1/world of the TILE PAIRS and produces
+partial sums for all particles, which one all-reduce (sum) per sweep combines -- 24 B per particle
+against ~N^2/world pair evaluations.
+
 The compute is injected as callables so that the host logic can be exercised on CPU with gloo
 (tests/test_sharding_gloo.py); on GPUs the callables are Frost.forces.
 """
@@ -53,3 +58,23 @@ def sharded_acc_grad(n: int, rank: int, world: int, acc_fn: Callable, grad_fn: C
     all_gather_planes(acc[:, lo:hi].contiguous(), n, rank, world, acc)
     grad_fn(sink_idx, acc, grad)
     return lo, hi
+
+
+def all_reduce_planes(t: torch.Tensor, world: int) -> torch.Tensor:
+    """Sum the partial planes of all ranks in place (NCCL on GPUs, gloo in the CPU test)."""
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+    return t
+
+
+def pair_sharded_acc_grad(world: int, acc_fn: Callable, grad_fn: Callable, acc: torch.Tensor,
+                          grad: torch.Tensor):
+    """One full acc+gradient pass with the pairs sharded over ranks.
+
+    acc_fn(acc)        must write this rank's PARTIAL Eq. 24 sums for every particle into acc;
+    grad_fn(acc, grad) must write this rank's PARTIAL Eq. 27 sums into grad, reading the complete acc.
+    After the call acc and grad hold the complete sums on every rank."""
+    acc_fn(acc)
+    all_reduce_planes(acc, world)
+    grad_fn(acc, grad)
+    all_reduce_planes(grad, world)

@@ -118,3 +118,34 @@ def test_hhs_step_symmetric_matches_oracle(frs, oracle, small):
     pg, vg = p.cpu().numpy(), v.cpu().numpy()
     assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
     assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_pair_sharded_shares_add_up(frs, oracle, world):
+    """frost_set_shard: the partial sums of the `world` shares (computed one after the other on this
+    one GPU) add up to the unsharded result and match the oracle; FROST_ACC | FROST_GRAD in one
+    sharded call is refused."""
+    import paper_2011_14984_b200 as frost
+    n = 6000
+    pos, vel, mass = fi.plummer(n, 21)
+    p, m = dev(pos), dev(mass)
+    a_ref, g_ref = oracle.forces(pos, mass)
+    acc = torch.zeros_like(p)
+    for r in range(world):
+        frs.set_shard(r, world)
+        part = torch.zeros_like(p)
+        frs.forces(p, m, out_acc=part, flags=frost.ACC)
+        acc += part
+    a = acc.cpu().numpy()
+    assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+    grad = torch.zeros_like(p)
+    for r in range(world):
+        frs.set_shard(r, world)
+        part = torch.zeros_like(p)
+        frs.forces(p, m, out_acc=acc, out_grad=part, flags=frost.GRAD)
+        grad += part
+    g = grad.cpu().numpy()
+    assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+    with pytest.raises(frost.FrostError):
+        frs.forces(p, m, flags=frost.ACC | frost.GRAD)
+    frs.set_shard(0, 1)

@@ -62,3 +62,40 @@ def test_two_rank_sharded_pass_matches_unsharded(tmp_path, oracle):
     for r in range(world):
         assert np.array_equal(np.load(tmp_path / f"acc{r}.npy"), a_ref)
         assert np.array_equal(np.load(tmp_path / f"grad{r}.npy"), g_ref)
+
+
+def _pair_worker(rank, world, port, n, out_dir):
+    import oracle
+    from paper_2011_14984_b200 import sharding
+    os.environ["MASTER_ADDR"] = "127.0.0.1"; os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    oracle.set_num_threads(2)
+    pos, vel, mass = fi.plummer(n, 5)
+    mine = np.arange(rank, n, world).astype(np.int32)      # stands in for this rank's tile pairs
+    acc = torch.zeros((3, n), dtype=torch.float64); grad = torch.zeros((3, n), dtype=torch.float64)
+
+    def acc_fn(a):
+        a.zero_()
+        oracle.forces(pos, mass, sink_idx=mine, flags=oracle.ACC, acc=a.numpy(), grad=grad.numpy())
+
+    def grad_fn(a, g):
+        g.zero_()
+        oracle.forces(pos, mass, sink_idx=mine, flags=oracle.GRAD, acc=a.numpy().copy(), grad=g.numpy())
+
+    sharding.pair_sharded_acc_grad(world, acc_fn, grad_fn, acc, grad)
+    np.save(os.path.join(out_dir, f"pacc{rank}.npy"), acc.numpy())
+    np.save(os.path.join(out_dir, f"pgrad{rank}.npy"), grad.numpy())
+    dist.destroy_process_group()
+
+
+def test_two_rank_pair_sharded_pass_matches_unsharded(tmp_path, oracle):
+    """Host logic of the pair-sharded pass: partial sums, all-reduce of a, gradient on the complete
+    a, all-reduce of g (the partial sums here have disjoint support, so the result is exact)."""
+    n, world = 257, 2
+    port = _free_port()
+    mp.spawn(_pair_worker, args=(world, port, n, str(tmp_path)), nprocs=world, join=True)
+    pos, vel, mass = fi.plummer(n, 5)
+    a_ref, g_ref = oracle.forces(pos, mass)
+    for r in range(world):
+        assert np.array_equal(np.load(tmp_path / f"pacc{r}.npy"), a_ref)
+        assert np.array_equal(np.load(tmp_path / f"pgrad{r}.npy"), g_ref)
