@@ -152,12 +152,12 @@ static Plan make_plan(const frost_ctx *c, int n_snk, int n_src, int max_k) {
     const int sb = pl.nt * pl.k;
     pl.sink_blocks = (n_snk + sb - 1) / sb;
     const int resident = c->num_sms * ((sb >= 512) ? 2 : 4);
-    // slices: aim at >= 16 waves of work units, keep >= 4 tiles per slice
+    // slices: aim at >= 16 waves of work units
     int slices = 1;
     const long long want_units = 16LL * resident;
     if (pl.sink_blocks < want_units) slices = (int)((want_units + pl.sink_blocks - 1) / pl.sink_blocks);
-    int max_slices = pl.n_tiles / 4;
-    if (max_slices < 1) max_slices = 1;
+    int max_slices = pl.n_tiles;      // down to one tile per slice: a sweep of a few thousand particles
+    if (max_slices < 1) max_slices = 1;   // is bound by the serial work per thread, not by issue
     if (slices > max_slices) slices = max_slices;
     if (slices > 256) slices = 256;
     if (c->tune_slices > 0) slices = c->tune_slices < pl.n_tiles ? c->tune_slices : pl.n_tiles;
