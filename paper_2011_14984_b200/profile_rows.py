@@ -1,0 +1,39 @@
+"""Launches every kernel family of the path once or twice at a fixed size so that ncu can capture
+them (profiles/*.md name the exact command):  python -m paper_2011_14984_b200.profile_rows [N]
+
+The O(N) kernels (gather/pack, kick, drift, partition) run on N = 2^20 particles after an L2 flush;
+the time-step sweeps (symmetric and one-sided) on min(N, 65536) particles."""
+import sys
+
+import torch
+
+import frost_inputs as fi
+import paper_2011_14984_b200 as frost
+
+
+def main():
+    n = int(sys.argv[1]) if len(sys.argv) > 1 else 1 << 20
+    pos, vel, mass = fi.plummer(n, 2)
+    dev = torch.device("cuda", 0)
+    p, v, m = (torch.as_tensor(x).to(dev) for x in (pos, vel, mass))
+    a = torch.randn_like(p); g = torch.randn_like(p)
+    tau = torch.rand(n, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
+    fr = frost.Frost(0)
+    for _ in range(2):
+        flush.fill_(1.0); fr.gather_pack(p, m)
+        flush.fill_(1.0); fr.kick(v, a, g, c=1e-9, kappa=1e-9)
+        flush.fill_(1.0); fr.kick(v, a, None, c=1e-9, kappa=0.0)
+        flush.fill_(1.0); fr.drift(p, v, c=1e-12)
+        flush.fill_(1.0); fr.partition(tau, 0.5)
+    n2 = min(n, 65536)
+    p2, v2, m2 = p[:, :n2].contiguous(), v[:, :n2].contiguous(), m[:n2].contiguous()
+    for mode in (0, 1):
+        fr.set_symmetric(mode)
+        fr.timesteps(p2, v2, m2, tau_pivot=1.0 / 128)
+    torch.cuda.synchronize()
+    fr.close()
+
+
+if __name__ == "__main__":
+    main()
