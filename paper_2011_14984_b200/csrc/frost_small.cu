@@ -297,6 +297,29 @@ __device__ void cta_drift(SmallSmem &sm, int a0, int nA, double c) {
     T::sync();
 }
 
+// kick then drift of the same particles in one phase (both touch only the thread's own particle):
+// v_i += ck (a_i + kappa g_i) ; x_i += cd v_i.
+template <class T>
+__device__ void cta_kick_drift(SmallSmem &sm, int a0, int nA, double ck, double kappa, bool with_g,
+                               double cd) {
+    for (int a = T::tid(); a < nA; a += T::kThreads) {
+        const int i = sm.perm[a0 + a];
+        double4 v = sm.vv[i];
+        double4 x = sm.xm[i];
+        const double4 ac = sm.aa[i];
+        double ax = ac.x, ay = ac.y, az = ac.z;
+        if (with_g) {
+            const double4 g = sm.gg[i];
+            ax = fma(kappa, g.x, ax); ay = fma(kappa, g.y, ay); az = fma(kappa, g.z, az);
+        }
+        v.x = fma(ck, ax, v.x); v.y = fma(ck, ay, v.y); v.z = fma(ck, az, v.z);
+        x.x = fma(cd, v.x, x.x); x.y = fma(cd, v.y, x.y); x.z = fma(cd, v.z, x.z);
+        sm.vv[i] = v;
+        sm.xm[i] = x;
+    }
+    T::sync();
+}
+
 // Stable in-place partition of the segment [a0, a0+n) of sm.perm: slow (tau >= pivot) first.
 // Returns |S| (Eq. 29).
 template <class T>
@@ -357,12 +380,10 @@ __device__ void cta_fsi(SmallSmem &sm, const SweepParams &pN, const SweepParams 
                         double dt) {
     if (nA <= 0) return;
     cta_newton<T>(sm, pN, a0, nA, a0, nA);
-    cta_kick<T>(sm, a0, nA, dt / 6.0, 0.0, false);
-    cta_drift<T>(sm, a0, nA, dt / 2.0);
+    cta_kick_drift<T>(sm, a0, nA, dt / 6.0, 0.0, false, dt / 2.0);
     cta_newton<T>(sm, pN, a0, nA, a0, nA);
     cta_gradient<T>(sm, pG, a0, nA, a0, nA);
-    cta_kick<T>(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true);
-    cta_drift<T>(sm, a0, nA, dt / 2.0);
+    cta_kick_drift<T>(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true, dt / 2.0);
     cta_newton<T>(sm, pN, a0, nA, a0, nA);
     cta_kick<T>(sm, a0, nA, dt / 6.0, 0.0, false);
     if (T::tid() == 0) {
