@@ -29,6 +29,11 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters,
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
         for (int r = 0; r < 8; ++r) {
+            if (MODE == 10 || MODE == 11) {   // ONE dependent chain per thread: 8 x 8 instructions = latency
+#pragma unroll
+                for (int k = 0; k < 8; ++k) a[0] = (MODE == 10) ? fma(a[0], b[0], c[0]) : a[0] + b[0];
+                continue;
+            }
             if (MODE == 5) {            // triples sharing one multiplicand, adjacent (operand reuse)
 #pragma unroll
                 for (int k = 0; k < 2; ++k) {
@@ -81,7 +86,7 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters,
 extern "C" int frost_fp64_probe(frost_ctx *c, int mode, int iters, int blocks_per_sm, double *scratch,
                                 int64_t *out_instr) {
     using namespace frost;
-    if (!c || !scratch || iters < 1 || blocks_per_sm < 1 || mode < 0 || mode > 9) return FROST_EINVAL;
+    if (!c || !scratch || iters < 1 || blocks_per_sm < 1 || mode < 0 || mode > 11) return FROST_EINVAL;
     FROST_CUDA(c, cudaSetDevice(c->device));
     const int grid = c->num_sms * blocks_per_sm;
 #define FROST_PROBE_CASE(M) \
@@ -89,7 +94,7 @@ extern "C" int frost_fp64_probe(frost_ctx *c, int mode, int iters, int blocks_pe
     switch (mode) {
         FROST_PROBE_CASE(0) FROST_PROBE_CASE(1) FROST_PROBE_CASE(2) FROST_PROBE_CASE(3)
         FROST_PROBE_CASE(4) FROST_PROBE_CASE(5) FROST_PROBE_CASE(6) FROST_PROBE_CASE(7)
-        FROST_PROBE_CASE(8) FROST_PROBE_CASE(9)
+        FROST_PROBE_CASE(8) FROST_PROBE_CASE(9) FROST_PROBE_CASE(10) FROST_PROBE_CASE(11)
     }
 #undef FROST_PROBE_CASE
     if (out_instr) *out_instr = (int64_t)grid * 256 * (int64_t)iters * 64;   // thread-level FP64 instructions

@@ -50,6 +50,14 @@ def main():
             base = cyc
         extra = "" if not extras else f"{(cyc - base) * 16 / extras:6.2f}"
         print(f"  {name:78s} {cyc:6.3f}        {extra}")
+    # dependent-chain latency: 1 CTA of 8 warps per SM (2 warps per sub-partition), one chain per thread
+    for mode, name in ((10, "DFMA"), (11, "DADD")):
+        fr.fp64_probe(mode, 2000, 1, scratch); torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        iters = 40000
+        a.record(); fr.fp64_probe(mode, iters, 1, scratch); b.record(); torch.cuda.synchronize()
+        cyc = a.elapsed_time(b) * 1e-3 * mhz * 1e6 / (iters * 64)
+        print(f"  dependent {name} chain, 2 warps per sub-partition: {cyc:6.2f} cycles per instruction (latency)")
     fr.close()
 
 
