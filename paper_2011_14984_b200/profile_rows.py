@@ -1,5 +1,6 @@
 """Launches every kernel family of the path once or twice at a fixed size so that ncu can capture
 them (profiles/*.md name the exact command):  python -m paper_2011_14984_b200.profile_rows [N]
+                                               python -m paper_2011_14984_b200.profile_rows subtree 8
 
 The O(N) kernels (gather/pack, kick, drift, partition) run on N = 2^20 particles after an L2 flush;
 the time-step sweeps (symmetric and one-sided) on min(N, 65536) particles."""
@@ -11,7 +12,26 @@ import frost_inputs as fi
 import paper_2011_14984_b200 as frost
 
 
+def subtree(n):
+    """The device-resident subtree kernel on a set of n/2 hard binaries (a latency-bound case)."""
+    import numpy as np
+    pos, vel, mass, pairs = fi.star_cluster(4096, 4, binary_fraction=0.6)
+    sel = pairs[: n // 2].ravel()
+    dev = torch.device("cuda", 0)
+    p = torch.as_tensor(np.ascontiguousarray(pos[:, sel])).to(dev)
+    v = torch.as_tensor(np.ascontiguousarray(vel[:, sel])).to(dev)
+    m = torch.as_tensor(mass[sel].copy()).to(dev)
+    fr = frost.Frost(0)
+    for _ in range(2):
+        st = fr.hhs_step(p.clone(), v.clone(), m, 2.0 ** -12)
+    torch.cuda.synchronize()
+    print("hierarchy entries:", sum(st["entries"]), "depth:", st["depth"])
+    fr.close()
+
+
 def main():
+    if len(sys.argv) > 2 and sys.argv[1] == "subtree":
+        return subtree(int(sys.argv[2]))
     n = int(sys.argv[1]) if len(sys.argv) > 1 else 1 << 20
     pos, vel, mass = fi.plummer(n, 2)
     dev = torch.device("cuda", 0)
