@@ -81,7 +81,7 @@ struct TeamWarp {
     __device__ static __forceinline__ int tid() { return threadIdx.x & 31; }
 };
 constexpr int kWarpTeamMax = 32;
-constexpr int kClusterSize = 8;            // portable maximum
+constexpr int kClusterSize = 16;           // non-portable size (opt-in attribute), supported on sm_100
 constexpr int kClusterMinSet = 192;        // smaller sets run on one CTA
 // a sweep is shared out among the cluster from this many pairs (config-5 step on B200: 8192 and
 // below 14.2-14.3 s, 32768 14.8 s, 131072 16.2 s, never 17.5 s)
@@ -550,6 +550,8 @@ int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const
                                            (int)sizeof(SmallSmem)));
         FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCluster>,
                                            cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem)));
+        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCluster>,
+                                           cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
         attr_done = true;
     }
     SmallParams P{};
