@@ -108,13 +108,17 @@ static int zero_tail(frost_ctx *c, double *rec, int n, int n_pad) {
     return FROST_OK;
 }
 
-// Whether a sweep with nA register-resident particles against nB streamed ones goes through the
-// pair-symmetric kernels: they need enough tile pairs to fill the GPU (A tiles of 1024, B tiles of
-// 256 particles); below that the one-sided sweeps with source slices win.
-static bool use_sym(const frost_ctx *c, int nA, int nB) {
+// Whether a sweep goes through the pair-symmetric kernels (frost_sym.cu).  They need enough tile
+// pairs to fill the GPU (A tiles of 256 particles below 16384, B tiles of 128); measured crossovers
+// on B200 against the one-sided sweeps with source slices: self Newton ~6000, gradient ~5000, time
+// step ~4000 particles; mutual sweeps from ~1000 x 1000.  kind: 0 self force sweep, 1 mutual force
+// sweep (nA = the larger set), 2 time-step sweep.
+static bool use_sym(const frost_ctx *c, int nA, int nB, int kind) {
     if (c->tune_sym == 1) return false;
     if (c->tune_sym == 2) return nA > 0 && nB > 0;
-    return nA >= 16384 && nB >= 4096;
+    if (kind == 0) return nA >= 6144;
+    if (kind == 2) return nA >= 4096;
+    return nA >= 1024 && (long long)nA * nB >= 1000000LL;
 }
 
 static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
@@ -139,8 +143,8 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
     }
     // pair-symmetric sweeps (frost_sym.cu) serve both directions of every pair with one evaluation:
     // the self case, and the mutual case with the larger set as the register-resident A side
-    const bool sym_self = self && use_sym(c, nI, nI);
-    const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI);
+    const bool sym_self = self && use_sym(c, nI, nI, 0);
+    const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI, 1);
     if (sym_self || sym_mut) {
         // sharded: the outputs are partial sums the caller adds across ranks, so the gradient sweep
         // cannot start from this call's own (partial) accelerations
@@ -193,7 +197,7 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
     FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, c->G, 1));   // .w = G m, NaN padding
     FROST_TRY(launch_pack_vec(c, ld, vel, idx, n_idx, pad, v));
-    if (use_sym(c, n_idx, n_idx)) return sym_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
+    if (use_sym(c, n_idx, n_idx, 2)) return sym_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
     return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin);
 }
 

@@ -399,8 +399,8 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
             const int f = self && I * KA > bt0 ? I * KA : bt0;
             if (f < bt1) pairs += bt1 - f;
         }
-        long long seg = pairs / (24LL * resident);            // >= 24 waves of CTAs, >= 4 tiles each
-        if (seg < 4) seg = 4;
+        long long seg = pairs / (24LL * resident);            // >= 24 waves of CTAs
+        if (seg < 1) seg = 1;
         if (seg > bt1 - bt0) seg = bt1 - bt0;
         if (c->tune_slices > 0) {
             seg = (bt1 - bt0 + c->tune_slices - 1) / c->tune_slices;
@@ -451,6 +451,8 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
 // is 1024 (Newton) or 512 (gradient, time step) particles, the B tile 128.
 constexpr int kSymNT = 128, kSymMinB = 2;
 constexpr int kSymKNewton = 8, kSymKGrad = 4, kSymKTau = 4;
+// sets below kSymSmallN particles: A tiles of 256 so that there are enough tile pairs to fill the GPU
+constexpr int kSymSmallN = 16384, kSymKSmall = 2, kSymMinBSmall = 4;
 
 // Newton sweep, both directions at once (Eq. 24 / 42).  self: B == A (B arguments ignored).
 int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
@@ -463,6 +465,7 @@ int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int
     j.scale = c->G;
     j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;      // see NewtonPolicy::pair
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
+    if (nA < kSymSmallN) return run_sym<SymNewton, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB>(c, j);
 }
 
@@ -476,6 +479,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.A_idx = A_idx; j.B_idx = B_idx; j.ld = ld; j.out = out_grad;
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
+    if (nA < kSymSmallN) return run_sym<SymGradient, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinB>(c, j);
 }
 
@@ -486,6 +490,7 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
     SymJob j{};
     j.A0 = xm; j.A1 = v; j.nA = n_set; j.nB = n_set; j.self = true; j.A_idx = idx;
     j.out = out_tau; j.out_bin = out_bin; j.tau_pivot = tau_pivot; j.scale = 1.0;
+    if (n_set < kSymSmallN) return run_sym<SymTimestep, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymTimestep, kSymKTau, kSymNT, kSymMinB>(c, j);
 }
 
