@@ -309,3 +309,35 @@ def test_hhs_tiny_systems_and_depth_limit(fr, oracle):
     with pytest.raises(frost.FrostError, match="deeper"):
         fr.hhs_step(dev(b_pos), dev(b_vel), dev(b_mass), 1.0)
     fr.set_params()
+
+
+def test_solar_system_run_on_device(fr, oracle):
+    """the paper's only printed multi-level input (Sun + 4 giant planets, Tables
+    A1/A2) integrated for 40 top steps of 512 days by frost_hhs_step with the
+    conserved quantities read by frost_diagnostics -- nothing but the initial conditions crosses the
+    host.  |dE/E| falls steeply with eta (~eta^4), |dP| stays at roundoff
+    (PAPER.md:674), the hierarchy has several populated levels, and the end state equals the
+    oracle's."""
+    errs = []
+    for eta in (0.2, 0.05):
+        pos, vel, mass, G = fi.solar_system()
+        vel = np.ascontiguousarray(vel - (vel * mass).sum(1, keepdims=True) / mass.sum())
+        fr.set_params(G=G, eta_ff=eta, eta_fb=eta)
+        p, v, m = dev(pos), dev(vel), dev(mass)
+        pr, vr = pos.copy(), vel.copy()
+        d0 = fr.diagnostics(p, v, m)
+        depth = 0
+        for _ in range(40):
+            st = fr.hhs_step(p, v, m, 512.0)
+            oracle.hhs_step(pr, vr, mass, 512.0, G=G, eta_ff=eta, eta_fb=eta)
+            depth = max(depth, st["depth"])
+        d1 = fr.diagnostics(p, v, m)
+        ref = oracle.diagnostics(pr, vr, mass, G=G)
+        errs.append(abs(d1["E"] / d0["E"] - 1))
+        assert np.abs(np.array(d1["P"]) - np.array(d0["P"])).max() < 1e-17
+        assert np.linalg.norm(np.array(d1["L"]) - np.array(d0["L"])) < 1e-12 * np.linalg.norm(d0["L"])
+        assert depth >= 2
+        assert abs(d1["E"] - ref["E"]) < 1e-12 * abs(ref["E"])
+        assert np.abs(p.cpu().numpy() - pr).max() < 1e-9 * 30
+    fr.set_params()
+    assert errs[0] < 1e-6 and errs[1] < errs[0] / 20
