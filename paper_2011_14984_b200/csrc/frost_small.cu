@@ -74,6 +74,14 @@ struct TeamCluster {
     __device__ static __forceinline__ void sync() { __syncthreads(); }
     __device__ static __forceinline__ int tid() { return threadIdx.x; }
 };
+// Four warps of the CTA (named barrier 1): sets of 33-128 particles, where the 16-warp barrier of the
+// whole CTA costs more than the phases' arithmetic.
+struct TeamQuad {
+    static constexpr bool kCluster = false;
+    static constexpr int kThreads = 128;
+    __device__ static __forceinline__ void sync() { asm volatile("bar.sync 1, 128;" ::: "memory"); }
+    __device__ static __forceinline__ int tid() { return threadIdx.x; }
+};
 struct TeamWarp {
     static constexpr bool kCluster = false;
     static constexpr int kThreads = 32;
@@ -81,6 +89,7 @@ struct TeamWarp {
     __device__ static __forceinline__ int tid() { return threadIdx.x & 31; }
 };
 constexpr int kWarpTeamMax = 32;
+constexpr int kQuadTeamMax = 128;
 constexpr int kClusterSize = 16;           // non-portable size (opt-in attribute), supported on sm_100
 constexpr int kClusterMinSet = 192;        // smaller sets run on one CTA
 // a sweep is shared out among the cluster from this many pairs (config-5 step on B200: 8192 and
@@ -340,7 +349,11 @@ __device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
     for (int base = 0; base < n; base += T::kThreads) {
         const int k = base + T::tid();
         const int f = (k < n) ? (sm.tau[sm.perm[a0 + k]] >= pivot) : 0;
-        nS += __syncthreads_count(f);
+        const int cw = __popc(__ballot_sync(0xffffffffu, f));     // team-wide count of f
+        if (lane == 0) sm.scan[w] = cw;
+        T::sync();
+        for (int q = 0; q < kWarps; ++q) nS += sm.scan[q];
+        T::sync();
     }
     int carry = 0;
     for (int base = 0; base < n; base += T::kThreads) {
@@ -405,6 +418,11 @@ __device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams 
         const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
         const double tau = sm.f_tau[sp];
         const int level = P.level0 + sp;
+        if (T::kThreads > 128 && stage == 0 && cnt > kWarpTeamMax && cnt <= kQuadTeamMax) {
+            // the whole subtree of this entry on warps 0-3 (see TeamQuad)
+            if (threadIdx.x < 128) hhs_loop<TeamQuad>(sm, P, pN, pG, sp);
+            continue;
+        }
         if (T::kThreads > 32 && stage == 0 && cnt > 0 && cnt <= kWarpTeamMax) {
             // the whole subtree of this entry on warp 0 (latency-bound: see TeamWarp)
             if (threadIdx.x < 32) hhs_loop<TeamWarp>(sm, P, pN, pG, sp);
