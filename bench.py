@@ -143,7 +143,7 @@ def run_reference(args):
 
 
 
-def measure_rows(fr, frost, torch, dev, flush, hbm_peak):
+def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
     """Side measurements of the other SURVEY.md 8(a) rows (not part of `value`): the time-step sweep
     on config 2 and the HBM-bound O(N) kernels at N = 2^20 (L2 flushed before every timed launch;
     algorithmic bytes per particle as in DESIGN.md)."""
@@ -190,6 +190,22 @@ def measure_rows(fr, frost, torch, dev, flush, hbm_peak):
         gbs = n * bpp / (ms * 1e-3) / 1e9
         out[name] = {"n": n, "us": ms * 1e3, "bytes_per_particle": bpp, "GB_per_s": gbs,
                      "frac_of_hbm_peak": gbs / hbm_peak}
+    if hhs:
+        # config 5: one whole HHS-FSI step over all time-step levels (latency-bound: DESIGN.md 7)
+        n5 = 262144
+        pos5, vel5, mass5, _ = fi.star_cluster(n5, 4)
+        p5, v5, m5 = (torch.as_tensor(x).to(dev) for x in (pos5, vel5, mass5))
+        fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
+        l0 = fr.launch_count()
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
+        torch.cuda.synchronize(); t1 = time.perf_counter()
+        out["hhs_step_config5"] = {"n": n5, "dt_top": 2.0 ** -7, "seconds": t1 - t0, "depth": st["depth"],
+                                   "hierarchy_entries": int(sum(st["entries"])),
+                                   "launches": int(fr.launch_count() - l0),
+                                   "pairs_newton": int(st["pairs_newton"]),
+                                   "pairs_gradient": int(st["pairs_gradient"]),
+                                   "pairs_timestep": int(st["pairs_timestep"])}
     return out
 
 
@@ -392,7 +408,7 @@ def run_frost(args):
            "gpu_launches": int(launches), "clocks": clocks, "roofline": roof,
            "cpu_baseline": cpu, "e2e": e2e}
     if world == 1 and not args.no_rows:
-        out["other_rows"] = measure_rows(fr, frost, torch, dev, flush, hbm_peak)
+        out["other_rows"] = measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=not args.no_hhs)
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
@@ -412,6 +428,7 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-rows", action="store_true", help="skip the side measurements of the O(N) rows")
+    ap.add_argument("--no-hhs", action="store_true", help="skip the config-5 HHS-FSI step (about 15 s)")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)

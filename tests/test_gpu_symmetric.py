@@ -149,3 +149,49 @@ def test_pair_sharded_shares_add_up(frs, oracle, world):
     with pytest.raises(frost.FrostError):
         frs.forces(p, m, flags=frost.ACC | frost.GRAD)
     frs.set_shard(0, 1)
+
+
+def test_symmetric_and_one_sided_sweeps_agree_on_random_shapes(frs):
+    """Tile-edge fuzz (no oracle): 24 random set sizes, mutual splits, scratch caps (bands) and
+    shard counts; the symmetric and the one-sided kernels must agree to rounding everywhere and
+    leave everything outside the swept sets untouched."""
+    import paper_2011_14984_b200 as frost
+    rng = np.random.default_rng(2024)
+    for case in range(24):
+        n = int(rng.choice([rng.integers(1, 300), rng.integers(300, 5000), rng.integers(5000, 30000)]))
+        pos, vel, mass = fi.plummer(max(n, 2), 100 + case)
+        pos, vel, mass = np.ascontiguousarray(pos[:, :n]), np.ascontiguousarray(vel[:, :n]), mass[:n].copy()
+        mass *= rng.uniform(0.2, 5.0, size=n)
+        p, v, m = dev(pos), dev(vel), dev(mass)
+        mib = int(rng.choice([0, 1, 2, 7]))
+        mutual = n >= 4 and rng.random() < 0.5
+        if mutual:
+            perm = rng.permutation(n).astype(np.int32)
+            k1 = int(rng.integers(1, n - 1)); k2 = int(rng.integers(k1 + 1, n + 1))
+            I, J = dev(np.sort(perm[:k1])), dev(np.sort(perm[k1:k2]))
+            flags = frost.ACC | frost.GRAD | frost.MUTUAL
+        else:
+            I = J = None
+            flags = frost.ACC | frost.GRAD
+        res = []
+        for mode in (1, 2):
+            frs.set_symmetric(mode, mib)
+            a = torch.full_like(p, 3.0); g = torch.full_like(p, 5.0)
+            frs.forces(p, m, I, J, out_acc=a, out_grad=g, flags=flags)
+            t, b = frs.timesteps(p, v, m, tau_pivot=1.0 / 64)
+            res.append((a, g, t[:n], b[:n]))
+        (a1, g1, t1, b1), (a2, g2, t2, b2) = res
+        sel = torch.cat([I, J]).long() if mutual else torch.arange(n, device="cuda")
+        na, ng = a1[:, sel].norm(dim=0), g1[:, sel].norm(dim=0)
+        ok = na > 0
+        if ok.any():
+            assert (((a1 - a2)[:, sel].abs().max(0).values)[ok] / na[ok]).max() < 1e-12, (case, n)
+            assert (((g1 - g2)[:, sel].abs().max(0).values)[ok] / ng[ok]).max() < 1e-9, (case, n)
+        if mutual:
+            rest = torch.ones(n, dtype=torch.bool, device="cuda"); rest[sel] = False
+            assert (a2[:, rest] == 3.0).all() and (g2[:, rest] == 5.0).all(), (case, n)
+        fin = torch.isfinite(t1)
+        assert torch.equal(fin, torch.isfinite(t2)) and torch.equal(b1, b2), (case, n)
+        if fin.any():
+            assert ((t1 - t2)[fin].abs() / t1[fin]).max() < 1e-13, (case, n)
+    frs.set_symmetric(2, 0)
