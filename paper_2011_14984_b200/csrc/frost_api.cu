@@ -36,7 +36,7 @@ int frost_destroy(frost_ctx *c) {
     if (!c) return FROST_EINVAL;
     cudaSetDevice(c->device);
     cudaStreamSynchronize(c->stream);
-    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->symtot, &c->iota,
+    Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->symtot,
                    &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);

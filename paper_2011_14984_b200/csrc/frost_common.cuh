@@ -39,7 +39,6 @@ struct frost_ctx {
     frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
     frost::Buf symtot;             // running totals across bands of a symmetric sweep
     size_t sym_scratch = (size_t)4 << 30;   // cap of partialB: the B list is swept in bands
-    frost::Buf iota;               // unused placeholder for identity lists
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
     frost::Buf blockcnt;           // partition scratch
     frost::Buf dev_stats;          // SmallStats accumulated by the subtree kernel
