@@ -11,7 +11,7 @@ from typing import Optional
 
 import torch
 
-ACC, GRAD, MUTUAL = 1, 2, 4
+ACC, GRAD, MUTUAL, ACCUMULATE = 1, 2, 4, 8
 MAX_LEVELS = 64
 
 _HERE = os.path.dirname(os.path.abspath(__file__))

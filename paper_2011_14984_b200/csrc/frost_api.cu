@@ -121,7 +121,7 @@ static bool use_sym(const frost_ctx *c, int nA, int nB, int kind) {
     return nA >= 1024 && (long long)nA * nB >= 1000000LL;
 }
 
-static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
                        const int32_t *I, int nI, const int32_t *J, int nJ, double *acc, double *grad,
                        int flags) {
     if (!I) nI = n;
@@ -184,6 +184,18 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
         if (mutual && !self) FROST_TRY(sweep_gradient(c, Bxm, Bv, nJ, Axm, Av, nI, J, ld, grad));
     }
     return FROST_OK;
+}
+
+static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+                       const int32_t *I, int nI, const int32_t *J, int nJ, double *acc, double *grad,
+                       int flags) {
+    // FROST_ACCUMULATE: the gradient sweep of the same call would start from this call's own
+    // accelerations instead of the totals in out_acc
+    if ((flags & FROST_ACCUMULATE) && (flags & FROST_ACC) && (flags & FROST_GRAD)) return FROST_EINVAL;
+    c->accumulate = (flags & FROST_ACCUMULATE) ? 1 : 0;
+    const int rc = forces_impl_(c, n, ld, pos, mass, I, nI, J, nJ, acc, grad, flags);
+    c->accumulate = 0;
+    return rc;
 }
 
 static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
@@ -290,7 +302,7 @@ int frost_forces(frost_ctx *c, int n, int ld, const double *pos, const double *v
                  int flags) {
     (void)vel;
     if (!c || bad_planes(n, ld) || !pos || !mass || !out_acc) return FROST_EINVAL;
-    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~7)) return FROST_EINVAL;
+    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~15)) return FROST_EINVAL;
     if ((flags & FROST_GRAD) && !out_grad) return FROST_EINVAL;
     if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
     if ((sink_idx && n_sink < 0) || (source_idx && n_source < 0)) return FROST_EINVAL;
@@ -303,7 +315,7 @@ int frost_forces_host(frost_ctx *c, int n, int ld, const double *pos, const doub
                       const int32_t *sink_idx, int n_sink, const int32_t *source_idx,
                       int n_source, double *out_acc, double *out_grad, int flags) {
     if (!c || bad_planes(n, ld) || !pos || !mass || !out_acc) return FROST_EINVAL;
-    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~7)) return FROST_EINVAL;
+    if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~15)) return FROST_EINVAL;
     if ((flags & FROST_GRAD) && !out_grad) return FROST_EINVAL;
     if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
     if (n == 0) return FROST_OK;

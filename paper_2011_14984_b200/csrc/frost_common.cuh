@@ -26,6 +26,7 @@ struct frost_ctx {
     double G = 1.0, eps2 = 0.0, eta_ff = 0.2, eta_fb = 0.2;
     int max_depth = 64;
     int tune_k = 0, tune_slices = 0, tune_small = -1;   // -1: auto threshold for the subtree kernel
+    int accumulate = 0;            // FROST_ACCUMULATE of the current frost_forces call
     int shard_rank = 0, shard_world = 1;   // frost_set_shard: this context's share of a symmetric sweep
     int tune_cluster = 0;          // subtree kernel: 0 auto (cluster of CTAs for sets >= 192), 1 one CTA
     int tune_sym = 0;              // pair-symmetric sweeps: 0 auto, 1 never, 2 whenever applicable

@@ -95,7 +95,7 @@ sweep_kernel(const SweepParams prm) {
 // ------------------------------------------------------------------------------------------------
 __global__ void reduce_vec_kernel(const double *__restrict__ partial, int n_pad, int slices, int n_snk,
                                   double scale, const int32_t *__restrict__ idx, int ld,
-                                  double *__restrict__ out, double4 *__restrict__ packed) {
+                                  double *__restrict__ out, double4 *__restrict__ packed, int accumulate) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_snk) return;
     double sx = 0.0, sy = 0.0, sz = 0.0;
@@ -105,6 +105,7 @@ __global__ void reduce_vec_kernel(const double *__restrict__ partial, int n_pad,
     }
     sx *= scale; sy *= scale; sz *= scale;
     const int g = idx ? idx[i] : i;
+    if (accumulate) { sx += out[g]; sy += out[(size_t)ld + g]; sz += out[2 * (size_t)ld + g]; }
     out[g] = sx; out[(size_t)ld + g] = sy; out[2 * (size_t)ld + g] = sz;
     if (packed) packed[i] = make_double4(sx, sy, sz, 1.0);
 }
@@ -210,7 +211,7 @@ int sweep_newton(frost_ctx *c, const double *snk_xm, int n_snk, const double *sr
     FROST_TRY(launch_sweep<NewtonPolicy>(c, prm, pl));
     reduce_vec_kernel<<<(n_snk + 255) / 256, 256, 0, c->stream>>>(
         (const double *)c->partial.p, n_pad, pl.slices, n_snk, c->G, snk_idx, ld, out_acc,
-        (double4 *)snk_a_packed);
+        (double4 *)snk_a_packed, c->accumulate);
     return check_launch(c);
 }
 
@@ -231,7 +232,7 @@ int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int 
     FROST_TRY(launch_sweep<GradientPolicy>(c, prm, pl));
     reduce_vec_kernel<<<(n_snk + 255) / 256, 256, 0, c->stream>>>(
         (const double *)c->partial.p, n_pad, pl.slices, n_snk, 2.0 * c->G, snk_idx, ld, out_grad,
-        nullptr);
+        nullptr, c->accumulate);
     return check_launch(c);
 }
 

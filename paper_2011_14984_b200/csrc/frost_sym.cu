@@ -290,7 +290,7 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
                                   int n_out, double scale,
                                   const int32_t *__restrict__ idx, int ld, double *__restrict__ out,
                                   double4 *__restrict__ packed, double tau_pivot,
-                                  int32_t *__restrict__ out_bin) {
+                                  int32_t *__restrict__ out_bin, int accumulate) {
     const int i = i0 + blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_out) return;
     double s[PL];
@@ -335,7 +335,11 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
         }
     } else {
 #pragma unroll
-        for (int p = 0; p < PL; ++p) { s[p] *= scale; out[(size_t)p * ld + g] = s[p]; }
+        for (int p = 0; p < PL; ++p) {
+            s[p] *= scale;
+            if (accumulate) s[p] += out[(size_t)p * ld + g];
+            out[(size_t)p * ld + g] = s[p];
+        }
         if (packed) packed[i] = make_double4(s[0], PL > 1 ? s[1] : 0.0, PL > 2 ? s[2] : 0.0, 1.0);
     }
 }
@@ -356,6 +360,7 @@ struct SymJob {
     double scale, eps2, tau_pivot;
     int32_t *out_bin;
     int shard_rank = 0, shard_world = 1;   // this launch sweeps A tiles rank, rank + world, ... only
+    int accumulate = 0;                    // add the sums to `out` instead of overwriting it
 };
 
 template <class P, int KA, int NT, int MINB>
@@ -426,7 +431,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         sym_reduce_kernel<PL, MIN><<<(job.nA + 255) / 256, 256, 0, c->stream>>>(
             prm.partA, prm.partB, (double *)c->symtot.p, na_pad, prm.self, 0, TA, NT, na_pad, a_tiles,
             bt0, bt1, prm.seg_tiles, row0, row_stride, first, last, 0, job.nA, job.scale, job.A_idx, job.ld, job.out,
-            (double4 *)job.A_packed, job.tau_pivot, job.out_bin);
+            (double4 *)job.A_packed, job.tau_pivot, job.out_bin, job.accumulate);
         FROST_TRY(check_launch(c));
         if (!self) {          // a B particle only collects in its own band: no running total
             const int i0 = bt0 * NT, i1 = bt1 * NT < nB ? bt1 * NT : nB;
@@ -434,7 +439,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
                 sym_reduce_kernel<PL, MIN><<<(i1 - i0 + 255) / 256, 256, 0, c->stream>>>(
                     prm.partA, prm.partB, nullptr, 0, 0, 1, TA, NT, na_pad, a_tiles, bt0, bt1,
                     prm.seg_tiles, row0, row_stride, 1, 1, i0, i1, job.scale, job.B_idx, job.ld, job.out,
-                    (double4 *)job.B_packed, job.tau_pivot, job.out_bin);
+                    (double4 *)job.B_packed, job.tau_pivot, job.out_bin, job.accumulate);
                 FROST_TRY(check_launch(c));
             }
         }
@@ -464,7 +469,7 @@ int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int
     j.ld = ld; j.out = out_acc; j.A_packed = A_a_packed; j.B_packed = B_a_packed;
     j.scale = c->G;
     j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;      // see NewtonPolicy::pair
-    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
+    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymNewton, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB>(c, j);
 }
@@ -478,7 +483,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.A0 = A_xm; j.A1 = A_a; j.B0 = B_xm; j.B1 = B_a; j.nA = nA; j.nB = nB; j.self = self;
     j.A_idx = A_idx; j.B_idx = B_idx; j.ld = ld; j.out = out_grad;
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
-    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world;
+    j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymGradient, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinB>(c, j);
 }

@@ -195,3 +195,38 @@ def test_symmetric_and_one_sided_sweeps_agree_on_random_shapes(frs):
         if fin.any():
             assert ((t1 - t2)[fin].abs() / t1[fin]).max() < 1e-13, (case, n)
     frs.set_symmetric(2, 0)
+
+
+@pytest.mark.parametrize("mode", [0, 2])
+def test_active_subset_against_all_as_self_plus_mutual(frs, oracle, mode):
+    """Config 4's pair set {(i, j): i in A or j in A} swept in two pieces with FROST_ACCUMULATE --
+    self(A) + mutual(A, rest), both served by the pair-symmetric kernels -- equals the oracle's
+    A <- all and rest <- A sums, for a and (on the total a) for g; the resulting kick conserves
+    momentum to roundoff."""
+    import paper_2011_14984_b200 as frost
+    n = 20000
+    pos, vel, mass = fi.plummer(n, 3)
+    frs.set_symmetric(mode, 0)
+    p, m = dev(pos), dev(mass)
+    for frac in (0.01, 0.3):
+        A = fi.active_subset(n, frac, 3)
+        rest = np.setdiff1d(np.arange(n, dtype=np.int32), A).astype(np.int32)
+        a_ref = np.zeros((3, n)); g_ref = np.zeros((3, n))
+        oracle.forces(pos, mass, sink_idx=A, source_idx=None, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+        oracle.forces(pos, mass, sink_idx=rest, source_idx=A, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+        oracle.forces(pos, mass, sink_idx=A, source_idx=None, flags=oracle.GRAD, acc=a_ref, grad=g_ref)
+        oracle.forces(pos, mass, sink_idx=rest, source_idx=A, flags=oracle.GRAD, acc=a_ref, grad=g_ref)
+        dA, dR = dev(A), dev(rest)
+        acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+        frs.forces(p, m, dA, dA, out_acc=acc, out_grad=grad, flags=frost.ACC)
+        frs.forces(p, m, dA, dR, out_acc=acc, out_grad=grad, flags=frost.ACC | frost.MUTUAL | frost.ACCUMULATE)
+        frs.forces(p, m, dA, dA, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+        frs.forces(p, m, dA, dR, out_acc=acc, out_grad=grad, flags=frost.GRAD | frost.MUTUAL | frost.ACCUMULATE)
+        a, g = acc.cpu().numpy(), grad.cpu().numpy()
+        assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+        assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+        assert np.abs((mass * a).sum(1)).max() < 1e-14 * (mass * np.abs(a)).sum(1).max()
+        with pytest.raises(frost.FrostError):
+            frs.forces(p, m, dA, dR, out_acc=acc, out_grad=grad,
+                       flags=frost.ACC | frost.GRAD | frost.MUTUAL | frost.ACCUMULATE)
+    frs.set_symmetric(2, 0)
