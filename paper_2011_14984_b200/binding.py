@@ -23,7 +23,7 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics", "frost_set_shard",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics", "frost_set_shard", "frost_fsi_steps",
 ]
 
 
@@ -74,6 +74,7 @@ def load_library():
     lib.frost_kick.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, f64]
     lib.frost_drift.argtypes = [vp, i32, i32, vp, vp, vp, i32, f64]
     lib.frost_fsi_step.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64]
+    lib.frost_fsi_steps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, i32]
     lib.frost_hhs_step.argtypes = [vp, i32, i32, vp, vp, vp, f64, vp]
     lib.frost_gather_pack.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp]
     lib.frost_fp64_probe.argtypes = [vp, i32, i32, i32, vp, vp]
@@ -235,6 +236,12 @@ class Frost:
         ii, ni = _idx(idx, "idx")
         self._check(self.lib.frost_fsi_step(self.h, mass.numel(), pos.shape[1], _p(pos), _p(vel),
                                             _p(mass), _p(ii), ni, dt), "frost_fsi_step")
+
+    def fsi_steps(self, pos, vel, mass, dt, n_steps, idx=None):
+        _vec(pos, "pos"); _vec(vel, "vel")
+        ii, ni = _idx(idx, "idx")
+        self._check(self.lib.frost_fsi_steps(self.h, mass.numel(), pos.shape[1], _p(pos), _p(vel),
+                                             _p(mass), _p(ii), ni, dt, n_steps), "frost_fsi_steps")
 
     def hhs_step(self, pos, vel, mass, dt_top):
         _vec(pos, "pos"); _vec(vel, "vel")

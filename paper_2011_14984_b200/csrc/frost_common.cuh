@@ -139,7 +139,7 @@ int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *ve
 int small_max();
 size_t small_stats_bytes();
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
-                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats);
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps = 1);
 
 // ---- device-side PTX helpers ------------------------------------------------------------------
 #ifdef __CUDACC__

@@ -30,7 +30,8 @@ struct SmallParams {
     const double *mass;
     double tau_pivot;               // pivot step of the subtree's root
     double dt_fsi;                  // mode 1: plain fsi(set, dt_fsi) instead of hhs_fsi
-    int mode;                       // 0 = hhs_fsi subtree, 1 = fsi step
+    int mode;                       // 0 = hhs_fsi subtree, 1 = fsi step(s)
+    int n_steps;                    // mode 1: number of consecutive fsi steps
     int level0, max_depth;
     double G, eps2, eta_ff, eta_fb;
     SmallStats *stats;
@@ -522,8 +523,10 @@ __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const Small
     __syncthreads();
 
     if (P.mode == 1) {
-        if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, pN, pG, 0, n, P.dt_fsi); }
-        else cta_fsi<T>(sm, pN, pG, 0, n, P.dt_fsi);
+        for (int k = 0; k < P.n_steps; ++k) {
+            if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, pN, pG, 0, n, P.dt_fsi); }
+            else cta_fsi<T>(sm, pN, pG, 0, n, P.dt_fsi);
+        }
     } else {
         hhs_loop<T>(sm, P, pN, pG, 0);
     }
@@ -559,7 +562,7 @@ int small_max() { return kSmallMax; }
 
 // mode 0: hhs_fsi(set, tau) subtree rooted at hierarchy level `level0`; mode 1: fsi(set, dt).
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
-                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats) {
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps) {
     if (n <= 0) return FROST_OK;
     if (n > kSmallMax) return FROST_EINVAL;
     static bool attr_done = false;
@@ -574,7 +577,7 @@ int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const
     }
     SmallParams P{};
     P.idx = idx; P.n = n; P.ld = ld; P.pos = pos; P.vel = vel; P.mass = mass;
-    P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0;
+    P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0; P.n_steps = n_steps;
     P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
     P.stats = (SmallStats *)dev_stats;
     if (n >= kClusterMinSet && c->tune_cluster != 1) {   // one cluster of kClusterSize replicas

@@ -249,6 +249,21 @@ def test_config1_ten_fsi_steps(fr, oracle, small):
     assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-13
 
 
+@pytest.mark.parametrize("n", [700, 3000, 9000])
+def test_fsi_steps_equal_repeated_fsi_step_bitwise(fr, n):
+    """frost_fsi_steps reuses the trailing Newton sweep of a step as the leading one of the next:
+    same bits as repeated frost_fsi_step (device-resident kernel, one-sided and symmetric sweeps)."""
+    pos, vel, mass = fi.plummer(n, 13)
+    fr.set_params()
+    p1, v1, m = dev(pos), dev(vel), dev(mass)
+    p2, v2 = dev(pos), dev(vel)
+    for _ in range(4):
+        fr.fsi_step(p1, v1, m, 1.0 / 2048)
+    fr.fsi_steps(p2, v2, m, 1.0 / 2048, 4)
+    torch.cuda.synchronize()
+    assert torch.equal(p1, p2) and torch.equal(v1, v2)
+
+
 @pytest.mark.parametrize("n,small", [(1024, -1), (1024, 0), (1024, 48), (3000, -1), (3000, 100)])
 def test_hhs_step_small_cluster(fr, oracle, n, small):
     """Reduced-N replica of config 5: level sets, bookkeeping and the trajectory must match the
