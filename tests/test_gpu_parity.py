@@ -356,3 +356,23 @@ def test_solar_system_run_on_device(fr, oracle):
         assert np.abs(p.cpu().numpy() - pr).max() < 1e-9 * 30
     fr.set_params()
     assert errs[0] < 1e-6 and errs[1] < errs[0] / 20
+
+
+def test_hhs_multi_step_run_conserves_momentum_to_roundoff(fr):
+    """The paper's headline property on the device: eight HHS-FSI
+    steps of a 6000-star cluster with a central mass and binaries down to a = 1e-4 (depth >= 10);
+    linear momentum stays at rounding level, angular momentum at 1e-13 relative, energy at the
+    truncation level of eta = 0.2."""
+    n = 6000
+    pos, vel, mass, pairs = fi.star_cluster(n, 7, a_lo=1e-4, a_hi=1e-2)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    d0 = fr.diagnostics(p, v, m)
+    depth = 0
+    for _ in range(8):
+        depth = max(depth, fr.hhs_step(p, v, m, 2.0 ** -8)["depth"])
+    d1 = fr.diagnostics(p, v, m)
+    assert depth >= 10 and bool(torch.isfinite(p).all())
+    assert np.abs(np.array(d1["P"]) - np.array(d0["P"])).max() < 1e-15
+    assert np.linalg.norm(np.array(d1["L"]) - np.array(d0["L"])) < 1e-13 * np.linalg.norm(d0["L"])
+    assert abs(d1["E"] / d0["E"] - 1) < 1e-6
