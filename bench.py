@@ -378,6 +378,7 @@ def run_frost(args):
         cpu, sinks, acc_ref, grad_ref = cpu_oracle_rate(n, seed, args.cpu_sinks, acc_full=acc_np)
         # positions drifted after the last step: recompute the GPU result at the ORIGINAL positions
         a_chk = torch.zeros_like(pos0); g_chk = torch.zeros_like(pos0)
+        fr.set_shard(0, 1)                       # the check is a whole (unsharded) pass on rank 0
         fr.forces(pos0, mass, out_acc=a_chk, out_grad=g_chk)
         torch.cuda.synchronize()
         a_g = a_chk.cpu().numpy()
