@@ -101,13 +101,6 @@ const char *frost_strerror(int status) {
 
 }  // extern "C"
 
-// zero the padding records [n, n_pad) of a packed vector stream
-static int zero_tail(frost_ctx *c, double *rec, int n, int n_pad) {
-    if (n_pad > n)
-        FROST_CUDA(c, cudaMemsetAsync(rec + 4 * (size_t)n, 0, (size_t)(n_pad - n) * kRecBytes, c->stream));
-    return FROST_OK;
-}
-
 // Whether a sweep goes through the pair-symmetric kernels (frost_sym.cu).  They need enough tile
 // pairs to fill the GPU (A tiles of 256 particles below 16384, B tiles of 128); measured crossovers
 // on B200 against the one-sided sweeps with source slices: self Newton ~6000, gradient ~5000, time
@@ -134,12 +127,12 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
     FROST_TRY(ensure(c, c->recA_v, (size_t)padA * kRecBytes));
     double *Axm = (double *)c->recA_xm.p, *Av = (double *)c->recA_v.p;
     double *Bxm = Axm, *Bv = Av;
-    FROST_TRY(launch_pack_xm(c, ld, pos, mass, I, nI, padA, Axm));
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, I, nI, padA, Axm, 1.0, 0, (flags & FROST_ACC) ? Av : nullptr));
     if (!self) {
         FROST_TRY(ensure(c, c->recB_xm, (size_t)padB * kRecBytes));
         FROST_TRY(ensure(c, c->recB_v, (size_t)padB * kRecBytes));
         Bxm = (double *)c->recB_xm.p; Bv = (double *)c->recB_v.p;
-        FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm));
+        FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm, 1.0, 0, (flags & FROST_ACC) ? Bv : nullptr));
     }
     // pair-symmetric sweeps (frost_sym.cu) serve both directions of every pair with one evaluation:
     // the self case, and the mutual case with the larger set as the register-resident A side
@@ -155,8 +148,6 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
         const int32_t *Pi = swap ? J : I, *Qi = swap ? I : J;
         const int nP = swap ? nJ : nI, nQ = swap ? nI : nJ;
         if (flags & FROST_ACC) {
-            FROST_TRY(zero_tail(c, Av, nI, padA));
-            if (!self) FROST_TRY(zero_tail(c, Bv, nJ, padB));
             FROST_TRY(sym_newton(c, Pxm, nP, Qxm, nQ, self, Pi, Qi, ld, acc, Pv, self ? nullptr : Qv));
         }
         if (flags & FROST_GRAD) {
@@ -169,10 +160,8 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
         return FROST_OK;
     }
     if (flags & FROST_ACC) {
-        FROST_TRY(zero_tail(c, Av, nI, padA));
         FROST_TRY(sweep_newton(c, Axm, nI, Bxm, nJ, I, ld, acc, Av));
         if (mutual && !self) {
-            FROST_TRY(zero_tail(c, Bv, nJ, padB));
             FROST_TRY(sweep_newton(c, Bxm, nJ, Axm, nI, J, ld, acc, Bv));
         }
     }
@@ -272,8 +261,7 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     const double h = 0.5 * tau_pivot;
     if (cross) {
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, S, nS, tau_pivot / 6.0, 0.0));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, F, nF, tau_pivot / 6.0, 0.0));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
     }
     FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
     FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
@@ -281,15 +269,13 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad,
                               FROST_ACC | FROST_GRAD | FROST_MUTUAL));
         const double kap = tau_pivot * tau_pivot / 48.0;
-        FROST_TRY(launch_kick(c, ld, vel, acc, grad, S, nS, 2.0 * tau_pivot / 3.0, kap));
-        FROST_TRY(launch_kick(c, ld, vel, acc, grad, F, nF, 2.0 * tau_pivot / 3.0, kap));
+        FROST_TRY(launch_kick(c, ld, vel, acc, grad, set, n_set, 2.0 * tau_pivot / 3.0, kap));   // S u F
     }
     FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
     FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
     if (cross) {
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, S, nS, tau_pivot / 6.0, 0.0));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, F, nF, tau_pivot / 6.0, 0.0));
+        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
     }
     if (st) {
         const int64_t cr = 2 * (int64_t)nS * nF;

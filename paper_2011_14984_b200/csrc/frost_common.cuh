@@ -101,7 +101,8 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // frost_update.cu
 // wscale multiplies the mass written to .w; nan_pad != 0 pads with NaN positions instead of zeros
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
-                   int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0);
+                   int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0,
+                   double *zero_tail = nullptr);
 int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
                     int n_pad, double *out);
 int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,

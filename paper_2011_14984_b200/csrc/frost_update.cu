@@ -10,9 +10,13 @@ namespace frost {
 // is NULL or ascending-dense.
 __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__restrict__ mass, int ld,
                                const int32_t *__restrict__ idx, int n_idx, int n_pad,
-                               double4 *__restrict__ out, double wscale, int nan_pad) {
+                               double4 *__restrict__ out, double wscale, int nan_pad,
+                               double4 *__restrict__ zero_tail) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_pad) return;
+    // the padding of the companion vector stream (accelerations written later by a reduction) is
+    // zeroed here, so that no separate memset is needed
+    if (zero_tail && k >= n_idx) zero_tail[k] = make_double4(0.0, 0.0, 0.0, 0.0);
     const double fill = nan_pad ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
     double4 r = make_double4(fill, fill, fill, 0.0);
     if (k < n_idx) {
@@ -186,10 +190,11 @@ diag_kernel(const double *__restrict__ pos, const double *__restrict__ vel, cons
 
 // ---- launchers ---------------------------------------------------------------------------------
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
-                   int n_idx, int n_pad, double *out, double wscale, int nan_pad) {
+                   int n_idx, int n_pad, double *out, double wscale, int nan_pad, double *zero_tail) {
     if (n_pad <= 0) return FROST_OK;
     pack_xm_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(pos, mass, ld, idx, n_idx, n_pad,
-                                                             (double4 *)out, wscale, nan_pad);
+                                                             (double4 *)out, wscale, nan_pad,
+                                                             (double4 *)zero_tail);
     return check_launch(c);
 }
 
