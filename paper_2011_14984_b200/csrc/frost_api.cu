@@ -220,11 +220,10 @@ static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const
     for (int k = 0; k < n_steps; ++k) {
         if (k == 0)
             FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, nullptr, FROST_ACC));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0));
-        FROST_TRY(launch_drift(c, ld, pos, vel, idx, n_idx, dt / 2.0));
+        FROST_TRY(launch_kick_drift(c, ld, pos, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0, dt / 2.0));
         FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, grad, FROST_ACC | FROST_GRAD));
-        FROST_TRY(launch_kick(c, ld, vel, acc, grad, idx, n_idx, 2.0 * dt / 3.0, dt * dt / 48.0));
-        FROST_TRY(launch_drift(c, ld, pos, vel, idx, n_idx, dt / 2.0));
+        FROST_TRY(launch_kick_drift(c, ld, pos, vel, acc, grad, idx, n_idx, 2.0 * dt / 3.0, dt * dt / 48.0,
+                                    dt / 2.0));
         FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, nullptr, FROST_ACC));
         FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0));
     }

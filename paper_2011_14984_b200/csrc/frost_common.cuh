@@ -107,6 +107,8 @@ int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *i
                     int n_pad, double *out);
 int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
                 const int32_t *idx, int n_idx, double cc, double kappa);
+int launch_kick_drift(frost_ctx *c, int ld, double *pos, double *vel, const double *acc, const double *grad,
+                      const int32_t *idx, int n_idx, double ck, double kappa, double cd);
 int launch_drift(frost_ctx *c, int ld, double *pos, const double *vel, const int32_t *idx,
                  int n_idx, double cc);
 int launch_partition(frost_ctx *c, const double *tau, const int32_t *idx, int n_idx,

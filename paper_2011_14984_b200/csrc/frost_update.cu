@@ -56,6 +56,25 @@ __global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__
     }
 }
 
+// kick followed by drift of the same particles in one pass (the two middle operator pairs of Alg. 2)
+__global__ void kick_drift_kernel(double *__restrict__ pos, double *__restrict__ vel,
+                                  const double *__restrict__ acc, const double *__restrict__ grad, int ld,
+                                  const int32_t *__restrict__ idx, int n_idx, double ck, double kappa,
+                                  double cd) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_idx) return;
+    const int i = idx ? idx[k] : k;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+        const size_t o = (size_t)d * ld + i;
+        double a = acc[o];
+        if (grad) a = fma(kappa, grad[o], a);
+        const double v = fma(ck, a, vel[o]);
+        vel[o] = v;
+        pos[o] = fma(cd, v, pos[o]);
+    }
+}
+
 __global__ void drift_kernel(double *__restrict__ pos, const double *__restrict__ vel, int ld,
                              const int32_t *__restrict__ idx, int n_idx, double c) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -211,6 +230,14 @@ int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const doub
     if (n_idx <= 0) return FROST_OK;
     kick_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(vel, acc, kappa != 0.0 ? grad : nullptr,
                                                           ld, idx, n_idx, cc, kappa);
+    return check_launch(c);
+}
+
+int launch_kick_drift(frost_ctx *c, int ld, double *pos, double *vel, const double *acc, const double *grad,
+                      const int32_t *idx, int n_idx, double ck, double kappa, double cd) {
+    if (n_idx <= 0) return FROST_OK;
+    kick_drift_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(pos, vel, acc, kappa != 0.0 ? grad : nullptr,
+                                                                ld, idx, n_idx, ck, kappa, cd);
     return check_launch(c);
 }
 
