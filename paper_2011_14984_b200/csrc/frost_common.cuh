@@ -37,6 +37,7 @@ struct frost_ctx {
     frost::Buf recA_xm, recB_xm;   // packed {x,y,z,m} streams of set A (sinks) and set B (sources)
     frost::Buf recA_v, recB_v;     // packed {ax,ay,az,0} or {vx,vy,vz,0}
     frost::Buf partial;            // [slices][3][n_pad] partial sums / [slices][n_pad] partial minima
+    frost::Buf tau_scratch;        // Morton keys, sorted index list, bounding records, tau64 (frost_tau.cu)
     frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
     frost::Buf symtot;             // running totals across bands of a symmetric sweep
     size_t sym_scratch = (size_t)4 << 30;   // cap of partialB: the B list is swept in bands
@@ -137,6 +138,10 @@ int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
 // frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)
 int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *vel, const double *mass,
                 const double *phi, double *out8);
+
+// frost_tau.cu: time-step sweep in Morton order with exact block pruning (prune = 0: evaluate all)
+int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const double *mass,
+               const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune);
 
 // frost_small.cu: one-CTA device-resident hhs_fsi subtree (mode 0) or fsi step (mode 1)
 int small_max();

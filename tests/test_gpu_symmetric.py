@@ -230,3 +230,30 @@ def test_active_subset_against_all_as_self_plus_mutual(frs, oracle, mode):
             frs.forces(p, m, dA, dR, out_acc=acc, out_grad=grad,
                        flags=frost.ACC | frost.GRAD | frost.MUTUAL | frost.ACCUMULATE)
     frs.set_symmetric(2, 0)
+
+
+@pytest.mark.parametrize("kind,n", [("plummer", 1000), ("plummer", 60000), ("cluster", 50000)])
+def test_pruned_timestep_sweep_is_bitwise_the_unpruned_minimum(frs, oracle, kind, n):
+    """csrc/frost_tau.cu: Morton order + block-level discard of pairs that cannot lower a minimum.
+    The result must be bitwise that of the plain symmetric sweep and of the pruning machinery with
+    pruning off, and match the oracle on sampled particles (hard binaries, central mass included)."""
+    if kind == "plummer":
+        pos, vel, mass = fi.plummer(n, 31)
+        sample = fi.active_subset(n, min(1.0, 300 / n), 5)
+    else:
+        pos, vel, mass, pairs = fi.star_cluster(n, 4)
+        sample = np.concatenate([[0], pairs[:40].ravel(), fi.active_subset(n, 200 / n, 5)]).astype(np.int32)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    pivot = 2.0 ** -7
+    out = {}
+    for mode in (3, 4, 5):
+        frs.set_symmetric(mode, 0)
+        t, b = frs.timesteps(p, v, m, tau_pivot=pivot)
+        out[mode] = (t.clone(), b.clone())
+    frs.set_symmetric(2, 0)
+    assert torch.equal(out[3][0], out[4][0]) and torch.equal(out[3][0], out[5][0])
+    assert torch.equal(out[3][1], out[5][1])
+    tau_ref, bin_ref = oracle.timesteps_sampled(pos, vel, mass, sample, tau_pivot=pivot)
+    th, bh = out[5][0].cpu().numpy(), out[5][1].cpu().numpy()
+    np.testing.assert_allclose(th[sample], tau_ref[sample], rtol=TOL_TAU)
+    assert np.array_equal(bh[sample], bin_ref[sample])
