@@ -15,7 +15,9 @@
 //      (position box, velocity box, min / max of G m; outward-rounded fp32), tau64[] = +inf;
 //   3. pass 1: every A tile against its own (diagonal) block, one-sided -- after it every particle
 //      has met its nearest neighbours and tau64 is close to final;
-//   4. pass 2: the pair-symmetric rotation sweep of frost_sym.cu over the off-diagonal tile pairs,
+//   4. pass 2: the pair-symmetric rotation sweep of frost_sym.cu over the off-diagonal tile pairs
+//      (the warps of a CTA take the chunks of a tile in round-robin order but are synchronised only
+//      once per tile: the B-side minima go out by atomicMin, so nothing is combined in shared memory),
 //      where a warp first tests its 32*KA resident particles' box against the box of the 32-particle
 //      chunk it is about to meet and skips the chunk (32 rotation steps) if the bound allows;
 //   5. both sides publish their minima with 64-bit atomicMin on the bit pattern (tau >= 0): the minimum
@@ -228,10 +230,9 @@ __global__ void __launch_bounds__(kTauNT, 2) tau_sym_kernel(const TauParams prm)
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double4 *tiles = reinterpret_cast<double4 *>(smem_raw);                       // [kStages][2][NT]
-    double *accB = reinterpret_cast<double *>(smem_raw + kStages * kStageBytes);   // [2][NT]
-    TauBox *sbox = reinterpret_cast<TauBox *>(accB + 2 * NT);                      // [kTauWarps]
-    double *tbd = reinterpret_cast<double *>(sbox + kTauWarps);                    // [NT] current minima of the tile
-    uint64_t *full = reinterpret_cast<uint64_t *>(tbd + NT);
+    double *tbd2 = reinterpret_cast<double *>(smem_raw + kStages * kStageBytes);   // [2][NT] current minima of the tile
+    TauBox *sbox2 = reinterpret_cast<TauBox *>(tbd2 + 2 * NT);                     // [2][kTauWarps]
+    uint64_t *full = reinterpret_cast<uint64_t *>(sbox2 + 2 * kTauWarps);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     if (tid == 0) {
@@ -293,14 +294,18 @@ __global__ void __launch_bounds__(kTauNT, 2) tau_sym_kernel(const TauParams prm)
         const int s = t % kStages;
         const int tile = tile0 + t;
         const bool two_sided = !prm.diag_only;
-        // stage the tile's bounding records and the current bounds of its particles
+        // stage the tile's bounding records and the current bounds of its particles (double-buffered by
+        // tile parity: the warps are only synchronised once per tile and drift apart inside it)
+        TauBox *sbox = sbox2 + (t & 1) * kTauWarps;
+        double *tbd = tbd2 + (t & 1) * NT;
         if (tid < kTauWarps * 16)
             reinterpret_cast<float *>(sbox)[tid] = reinterpret_cast<const float *>(prm.box + (size_t)tile * kTauWarps)[tid];
         tbd[tid] = tau_from_bits(prm.tau64[(size_t)tile * NT + tid]);
         mbar_wait(&full[s], (uint32_t)(t / kStages) & 1u);
         __syncthreads();
+        // every warp is past tile t-1: its stage can be refilled
+        if (tid == 0 && t >= 1 && t - 1 + kStages < ntiles) issue(t - 1 + kStages);
         const double4 *t0 = tiles + (size_t)s * 2 * NT;
-        double *accT = accB + (size_t)(t & 1) * NT;
         for (int r = 0; r < kTauWarps; ++r) {
             const int c = (warp + r) % kTauWarps;
             double b = inf;
@@ -352,14 +357,9 @@ __global__ void __launch_bounds__(kTauNT, 2) tau_sym_kernel(const TauParams prm)
                     b = __shfl_sync(0xffffffffu, b, from);
                 }
             }
-            if (two_sided) {
-                double *dst = accT + c * 32 + lane;
-                *dst = (r == 0) ? b : fmin(*dst, b);
-            }
-            __syncthreads();
+            // the chunk's particles collect their minima by atomicMin (exact in any order)
+            if (two_sided && b < inf) atomic_min_tau(prm.tau64 + (size_t)tile * NT + c * 32 + lane, b);
         }
-        if (tid == 0 && t + kStages < ntiles) issue(t + kStages);
-        if (two_sided && accT[tid] < inf) atomic_min_tau(prm.tau64 + (size_t)tile * NT + tid, accT[tid]);
     }
 #pragma unroll
     for (int k = 0; k < KA; ++k) atomic_min_tau(prm.tau64 + a_first + k * NT, at[k]);
@@ -429,7 +429,7 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
 
     static bool attr_done = false;
     const size_t smem = (size_t)kStages * 2 * kTauNT * kRecBytes + 2 * kTauNT * sizeof(double) +
-                        kTauWarps * sizeof(TauBox) + kTauNT * sizeof(double) + kStages * sizeof(uint64_t);
+                        2 * kTauWarps * sizeof(TauBox) + kStages * sizeof(uint64_t);
     if (!attr_done) {
         FROST_CUDA(c, cudaFuncSetAttribute(tau_sym_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         attr_done = true;
