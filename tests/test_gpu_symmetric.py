@@ -257,3 +257,21 @@ def test_pruned_timestep_sweep_is_bitwise_the_unpruned_minimum(frs, oracle, kind
     th, bh = out[5][0].cpu().numpy(), out[5][1].cpu().numpy()
     np.testing.assert_allclose(th[sample], tau_ref[sample], rtol=TOL_TAU)
     assert np.array_equal(bh[sample], bin_ref[sample])
+
+
+def test_pruned_timestep_sweep_on_index_subset(frs):
+    """The pruned sweep on a level given as an index list (as frost_hhs_step passes it): bitwise the
+    plain symmetric sweep's result, everything outside the list untouched."""
+    n = 70000
+    pos, vel, mass, _ = fi.star_cluster(n, 9)
+    idx = fi.active_subset(n, 0.8, 9)
+    p, v, m, di = dev(pos), dev(vel), dev(mass), dev(idx)
+    res = []
+    for mode in (3, 5):
+        frs.set_symmetric(mode, 0)
+        t, b = frs.timesteps(p, v, m, idx=di, tau_pivot=2.0 ** -6)
+        res.append((t.clone(), b.clone()))
+    frs.set_symmetric(2, 0)
+    assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
+    out = np.setdiff1d(np.arange(n), idx)
+    assert torch.isinf(res[1][0][dev(out).long()]).all()
