@@ -34,7 +34,7 @@
 namespace frost {
 
 constexpr int kTauNT = 128;          // threads per CTA = records per B tile
-constexpr int kTauKA = 4;            // resident A particles per thread (A tile = 512)
+constexpr int kTauKA = 2;            // resident A particles per thread (A tile = 256); 4 / 2 / 1: 82 / 70 / 85 ms at N = 262144
 constexpr int kTauWarps = kTauNT / 32;
 
 struct __align__(16) TauBox {        // bounding record of 32 consecutive particles (64 bytes)
@@ -218,7 +218,7 @@ __device__ __forceinline__ double tau_candidate(double x, double y, double z, do
 // ---- 3./4. the sweep ------------------------------------------------------------------------------
 // grid = (A tiles, segments); pass 1 (diag_only): the kTauKA B tiles of the A tile itself, one-sided;
 // pass 2: the B tiles beyond the A tile, two-sided, with chunk-level pruning.
-__global__ void __launch_bounds__(kTauNT, 2) tau_sym_kernel(const TauParams prm) {
+__global__ void __launch_bounds__(kTauNT, 4) tau_sym_kernel(const TauParams prm) {
     constexpr int NT = kTauNT, KA = kTauKA, TA = NT * KA;
     constexpr uint32_t kStageBytes = 2 * NT * kRecBytes;
     const int I = blockIdx.x;
@@ -444,7 +444,7 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
     if (n_tiles > kTauKA) {
         // pass 2: ~16 waves of CTAs over the triangular tile-pair set
         const long long pairs = (long long)a_tiles * n_tiles - (long long)kTauKA * a_tiles * (a_tiles + 1) / 2;
-        long long seg = pairs / (16LL * c->num_sms * 2);
+        long long seg = pairs / (16LL * c->num_sms * 4);
         if (seg < 8) seg = 8;
         if (seg > n_tiles) seg = n_tiles;
         prm.diag_only = 0; prm.seg_tiles = (int)seg;
