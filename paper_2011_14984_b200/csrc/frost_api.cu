@@ -195,8 +195,8 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     // large levels: Morton order + exact block pruning (frost_tau.cu); tune_sym 3 = symmetric sweep
     // without pruning, 4 = the pruning machinery with pruning switched off, 5 = pruning at any size (tests)
     // (measured on B200 against the plain symmetric sweep: 1.3x at 65536, 2.4x at 262144, 2.8x at
-    // 2^20 particles; slower below ~50000, where the sort and the two passes dominate)
-    if (c->tune_sym == 4 || c->tune_sym == 5 || (c->tune_sym != 1 && c->tune_sym != 3 && n_idx >= 49152))
+    // 2^20 particles; break-even at ~30000, where the sort and the two passes start to dominate)
+    if (c->tune_sym == 4 || c->tune_sym == 5 || (c->tune_sym != 1 && c->tune_sym != 3 && n_idx >= 32768))
         return tau_pruned(c, ld, pos, vel, mass, idx, n_idx, tau_pivot, out_tau, out_bin, c->tune_sym != 4);
     const int pad = pad1024(n_idx);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));

@@ -48,7 +48,7 @@ def main():
         flush.fill_(1.0); fr.partition(tau, 0.5)
     n2 = min(n, 65536)
     p2, v2, m2 = p[:, :n2].contiguous(), v[:, :n2].contiguous(), m[:n2].contiguous()
-    for mode in (3, 1, 0):      # plain symmetric sweep, one-sided sweep, default (pruned from 49152 particles)
+    for mode in (3, 1, 0):      # plain symmetric sweep, one-sided sweep, default (pruned from 32768 particles)
         fr.set_symmetric(mode)
         fr.timesteps(p2, v2, m2, tau_pivot=1.0 / 128)
     torch.cuda.synchronize()
