@@ -10,7 +10,13 @@ One "pair interaction" = one ordered pair visited once by each of the two sweeps
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--n 1048576] [--impl reference]
 
-Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.  With --gpus N > 1 and
+no torchrun environment the script re-launches itself under torch.distributed.run with N ranks
+(one per GPU, NCCL).  Side modes used by the commands in profiles/*.md (no JSON line):
+    --probe          print the FP64 issue-model table of this GPU (frost_fp64_probe, CUDA events)
+    --rows-only      launch every O(N) kernel and the three time-step sweeps once or twice (for ncu)
+    --subtree K      the device-resident subtree kernel on K/2 hard binaries (for ncu)
+    --hhs-only       one HHS-FSI step of config 5 (N = 262144) with its validity numbers
 """
 import argparse
 import json
@@ -36,6 +42,19 @@ SLOTS_NEWTON_1S, SLOTS_GRAD_1S = 16, 28
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM
 METRIC = "pair interactions/s (acc+gradient, fp64) at N=2^20"
 UNIT = "pair interactions/s"
+
+
+def _sweep_traffic(one_sided, n):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one whole gradient sweep (all its band launches
+    and reductions) from the committed ncu --set full capture, if one exists for this configuration;
+    else None.  profiles/sym_gradient_traffic.csv: n,one_sided,dram_bytes,source."""
+    path = os.path.join(ROOT, "profiles", "sym_gradient_traffic.csv")
+    if os.path.exists(path):
+        for ln in open(path):
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 4 and f[0].isdigit() and int(f[0]) == n and int(f[1]) == int(bool(one_sided)):
+                return float(f[2]), f[3]
+    return None, "no ncu capture committed for this configuration (see profiles/)"
 
 
 def _peaks():
@@ -124,15 +143,15 @@ def run_reference(args):
     n, seed = args.n, 2
     sample = max(64, min(args.ref_sinks, n))
     vals = []
-    for s in range(args.warmup_ref + args.steps):
+    for s in range(args.warmup + args.steps):
         r, *_ = cpu_oracle_rate(n, seed, sample)
-        if s >= args.warmup_ref:
+        if s >= args.warmup:
             vals.append(r)
     val = float(np.mean([v["value"] for v in vals]))
     secs = float(np.mean([v["seconds"] for v in vals]))
     cb = dict(vals[-1]); cb["value"] = val
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
-           "steps": args.steps, "warmup": args.warmup_ref, "ms_per_step": secs * 1e3,
+           "steps": args.steps, "warmup": args.warmup, "ms_per_step": secs * 1e3,
            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic",
            "config": {"workload": f"Plummer sphere N={n}, equal masses, G=1, seed 2 (config 3); "
@@ -191,22 +210,133 @@ def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
         out[name] = {"n": n, "us": ms * 1e3, "bytes_per_particle": bpp, "GB_per_s": gbs,
                      "frac_of_hbm_peak": gbs / hbm_peak}
     if hhs:
-        # config 5: one whole HHS-FSI step over all time-step levels (latency-bound: DESIGN.md 7)
-        n5 = 262144
-        pos5, vel5, mass5, _ = fi.star_cluster(n5, 4)
-        p5, v5, m5 = (torch.as_tensor(x).to(dev) for x in (pos5, vel5, mass5))
-        fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
-        l0 = fr.launch_count()
-        torch.cuda.synchronize(); t0 = time.perf_counter()
-        st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
-        torch.cuda.synchronize(); t1 = time.perf_counter()
-        out["hhs_step_config5"] = {"n": n5, "dt_top": 2.0 ** -7, "seconds": t1 - t0, "depth": st["depth"],
-                                   "hierarchy_entries": int(sum(st["entries"])),
-                                   "launches": int(fr.launch_count() - l0),
-                                   "pairs_newton": int(st["pairs_newton"]),
-                                   "pairs_gradient": int(st["pairs_gradient"]),
-                                   "pairs_timestep": int(st["pairs_timestep"])}
+        out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
     return out
+
+
+def hhs_config5(fr, torch, dev, n5=262144):
+    """Config 5: one whole HHS-FSI step over all time-step levels (latency-bound: DESIGN.md 7), with
+    the numbers that make the timing valid: momentum, angular momentum and energy change read by
+    frost_diagnostics before and after (SURVEY 8(c) last pin row; expected floors PAPER.md:646-656,
+    696-698), and the level bookkeeping that tests/test_gpu_fullsize.py checks against the golden file."""
+    pos5, vel5, mass5, _ = fi.star_cluster(n5, 4)
+    p5, v5, m5 = (torch.as_tensor(x).to(dev) for x in (pos5, vel5, mass5))
+    fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
+    d0 = fr.diagnostics(p5, v5, m5)
+    l0 = fr.launch_count()
+    torch.cuda.synchronize(); t0 = time.perf_counter()
+    st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
+    torch.cuda.synchronize(); t1 = time.perf_counter()
+    launches = int(fr.launch_count() - l0)
+    d1 = fr.diagnostics(p5, v5, m5)
+    L0, L1 = np.array(d0["L"]), np.array(d1["L"])
+    return {"n": n5, "dt_top": 2.0 ** -7, "seconds": t1 - t0, "depth": st["depth"],
+            "hierarchy_entries": int(sum(st["entries"])), "launches": launches,
+            "pairs_newton": int(st["pairs_newton"]), "pairs_gradient": int(st["pairs_gradient"]),
+            "pairs_timestep": int(st["pairs_timestep"]),
+            "dP": float(np.abs(np.array(d1["P"]) - np.array(d0["P"])).max()),
+            "dL_rel": float(np.linalg.norm(L1 - L0) / np.linalg.norm(L0)),
+            "dE_rel": float(d1["E"] / d0["E"] - 1.0),
+            "level0": {"n_slow": int(st["n_slow"][0]), "n_fast": int(st["n_fast"][0])},
+            "entries_per_level": [int(x) for x in st["entries"]]}
+
+
+def run_probe():
+    """--probe: the FP64 issue-model table of this GPU: issue cycles per FP64 warp
+    instruction per SM sub-partition at the max SM clock (2.0 = the nominal rate of a 16-lane pipe)."""
+    import torch
+    import paper_2011_14984_b200 as frost
+    modes = [(1, "DADD, 2 distinct register pairs", 0),
+             (2, "DMUL, 2 distinct register pairs", 0),
+             (6, "DFMA, 2 register pairs + immediate", 0),
+             (0, "DFMA, 1 register pair + 2 loop-invariant pairs (.reuse)", 0),
+             (4, "DFMA, 3 distinct register pairs", 0),
+             (5, "DFMA triples sharing one operand, adjacent (.reuse) [48 of 64] + 16 DADD", 0),
+             (3, "mix: DFMA(2 pairs) / DADD / DMUL", 0),
+             (7, "DADD + 12 integer-ALU instr per 16 FP64 instr", 12),
+             (8, "DADD + 2 MUFU.RSQ64H per 16 FP64 instr", 2),
+             (9, "DADD + 4 LDS.128 per 16 FP64 instr", 4)]
+    _, mhz, _ = _peaks()
+    fr = frost.Frost(0)
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    scratch = torch.zeros(sms * 8 * 256, dtype=torch.float64, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    print(f"# {torch.cuda.get_device_name(0)}, {sms} SMs, cycles at {mhz:.0f} MHz; 4 CTAs x 256 threads per SM")
+    print(f"# {'probe':78s} cyc/FP64-inst  extra cyc per extra instr")
+    base = None
+    for mode, name, extras in modes:
+        fr.fp64_probe(mode, 2000, 4, scratch); torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record(); ninst = fr.fp64_probe(mode, 40000, 4, scratch); b.record(); torch.cuda.synchronize()
+        cyc = a.elapsed_time(b) * 1e-3 * mhz * 1e6 / (ninst / 32 / (sms * 4))
+        if mode == 1:
+            base = cyc
+        extra = "" if not extras else f"{(cyc - base) * 16 / extras:6.2f}"
+        print(f"  {name:78s} {cyc:6.3f}        {extra}")
+    for mode, name in ((10, "DFMA"), (11, "DADD")):      # latency: 1 CTA of 8 warps per SM, one chain per thread
+        fr.fp64_probe(mode, 2000, 1, scratch); torch.cuda.synchronize()
+        a, b = ev(), ev()
+        a.record(); fr.fp64_probe(mode, 40000, 1, scratch); b.record(); torch.cuda.synchronize()
+        cyc = a.elapsed_time(b) * 1e-3 * mhz * 1e6 / (40000 * 64)
+        print(f"  dependent {name} chain, 2 warps per sub-partition: {cyc:6.2f} cycles per instruction (latency)")
+    fr.close()
+
+
+def run_rows_only(n):
+    """--rows-only: every kernel family of the path once or twice at a fixed size, for ncu: the O(N)
+    kernels (gather/pack, kick, drift, partition) on n particles after an L2 flush, the time-step
+    sweeps (plain symmetric, one-sided, pruned) on min(n, 65536) particles."""
+    import torch
+    import paper_2011_14984_b200 as frost
+    pos, vel, mass = fi.plummer(n, 2)
+    dev = torch.device("cuda", 0)
+    p, v, m = (torch.as_tensor(x).to(dev) for x in (pos, vel, mass))
+    a = torch.randn_like(p); g = torch.randn_like(p)
+    tau = torch.rand(n, dtype=torch.float64, device=dev)
+    flush = torch.empty(256 * 1024 * 1024 // 8, dtype=torch.float64, device=dev)
+    fr = frost.Frost(0)
+    for _ in range(2):
+        flush.fill_(1.0); fr.gather_pack(p, m)
+        flush.fill_(1.0); fr.kick(v, a, g, c=1e-9, kappa=1e-9)
+        flush.fill_(1.0); fr.kick(v, a, None, c=1e-9, kappa=0.0)
+        flush.fill_(1.0); fr.drift(p, v, c=1e-12)
+        flush.fill_(1.0); fr.partition(tau, 0.5)
+    n2 = min(n, 65536)
+    p2, v2, m2 = p[:, :n2].contiguous(), v[:, :n2].contiguous(), m[:n2].contiguous()
+    for mode in (3, 1, 0):      # plain symmetric sweep, one-sided sweep, default (pruned from 32768 particles)
+        fr.set_symmetric(mode)
+        fr.timesteps(p2, v2, m2, tau_pivot=1.0 / 128)
+    torch.cuda.synchronize()
+    fr.close()
+
+
+def run_subtree(k):
+    """--subtree K: the device-resident subtree kernel on a set of K/2 hard binaries (latency-bound)."""
+    import torch
+    import paper_2011_14984_b200 as frost
+    pos, vel, mass, pairs = fi.star_cluster(4096, 4, binary_fraction=0.6)
+    sel = pairs[: k // 2].ravel()
+    dev = torch.device("cuda", 0)
+    p = torch.as_tensor(np.ascontiguousarray(pos[:, sel])).to(dev)
+    v = torch.as_tensor(np.ascontiguousarray(vel[:, sel])).to(dev)
+    m = torch.as_tensor(mass[sel].copy()).to(dev)
+    fr = frost.Frost(0)
+    for _ in range(2):
+        pp, vv = p.clone(), v.clone()
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        st = fr.hhs_step(pp, vv, m, 2.0 ** -12)
+        torch.cuda.synchronize(); t1 = time.perf_counter()
+    ent = sum(st["entries"])
+    print(f"hierarchy entries: {ent} depth: {st['depth']} seconds: {t1 - t0:.4f} us/entry: {(t1 - t0) / ent * 1e6:.2f}")
+    fr.close()
+
+
+def run_hhs_only():
+    import torch
+    import paper_2011_14984_b200 as frost
+    fr = frost.Frost(0)
+    print(json.dumps({"hhs_step_config5": hhs_config5(fr, torch, torch.device("cuda", 0))}))
+    fr.close()
 
 
 def run_frost(args):
@@ -319,7 +449,7 @@ def run_frost(args):
             fr.forces_host(hp, hm, out_acc=ha, out_grad=hg)        # synchronises internally
             ts.append(time.perf_counter() - t0)
         e2e = {"value": pairs_step / float(np.mean(ts)), "unit": UNIT,
-               "h2d_bytes_per_step": int(hp.numel() * 8 + hm.numel() * 8 + ha.numel() * 8 + hg.numel() * 8),
+               "h2d_bytes_per_step": int(hp.numel() * 8 + hm.numel() * 8),   # acc / grad are pure outputs here
                "d2h_bytes_per_step": int(ha.numel() * 8 + hg.numel() * 8),
                "steps": len(ts), "ms_per_step": float(np.mean(ts)) * 1e3}
 
@@ -330,7 +460,8 @@ def run_frost(args):
 
     # ---- FP64 issue-rate probe: measured sustained pipe rate (MEASURED_PEAKS.json has none) ------
     probe = {}
-    scratch = torch.zeros(148 * 8 * 256 * 2, dtype=torch.float64, device=dev)
+    scratch = torch.zeros(torch.cuda.get_device_properties(local).multi_processor_count * 8 * 256,
+                          dtype=torch.float64, device=dev)
     for mode, nm in ((0, "dfma"), (3, "mixed")):
         fr.fp64_probe(mode, 2000, 4, scratch); torch.cuda.synchronize()
         a, b = ev(), ev()
@@ -347,16 +478,18 @@ def run_frost(args):
         slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
     else:
         slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradient> (pair-symmetric gradient sweep, Eq. 27)"
+    traffic, traffic_src = _sweep_traffic(args.one_sided, n)
+    # measured FP64 rate of this run's probe (MEASURED_PEAKS.json carries no fp64 entry): a DFMA with two
+    # loop-invariant operands issues every 2 cycles, i.e. thread instructions/s x 2 flop
+    peak_measured = probe.get("dfma_thread_inst_per_s", 0.0) * 2 / 1e12
     roof = {"bound": "alu", "kernel": kname,
             "achieved": pairs_rank * FLOPS_GRAD / (g_ms * 1e-3) / 1e12, "peak": peak_tflops,
             "unit": "TFLOP/s",
-            # dram__bytes_read+write of ONE band launch (gradient band 3 of 13) from the committed
-            # ncu --set full capture, profiles/sym_ncu_full_r1b.md; bands 1-3 measured 0.51 / 0.86 /
-            # 1.30 GB, a whole sweep ~26 GB (the B-side partial sums) = ~20 GB/s: ALU-bound
-            "traffic": None if args.one_sided else 1.3047e9,
-            "traffic_scope": "one band launch of 13 per sweep (profiles/sym_ncu_full_r1b.md)",
+            "traffic": traffic, "traffic_scope": traffic_src,
             "peak_source": f"derived: {SM_COUNT} SMs x {FP64_LANES_PER_SM} FP64 lanes x 2 x "
                            f"{sm_max_mhz:.0f} MHz ({peak_src} sm_max_mhz); HBM peak n/a",
+            "peak_measured": peak_measured,
+            "peak_measured_source": "frost_fp64_probe mode 0 (DFMA, register-only chains) timed in this run",
             "flops_per_pair": FLOPS_GRAD, "fp64_slots_per_pair": slots_g,
             "ms_per_launch": g_ms,
             "fp64_pipe_frac_at_max_clock": pairs_rank * slots_g / (g_ms * 1e-3) / slot_peak,
@@ -367,6 +500,8 @@ def run_frost(args):
                        "fp64_pipe_frac_at_max_clock": pairs_rank * slots_n / (n_ms * 1e-3) / slot_peak},
             "probe": probe,
             "probe_dfma_frac_of_nominal": probe.get("dfma_thread_inst_per_s", 0.0) / slot_peak}
+    if peak_measured > 0:
+        roof["frac_of_peak_measured"] = roof["achieved"] / peak_measured
     roof["frac"] = roof["achieved"] / roof["peak"]
     roof["step_tflops"] = value * (FLOPS_NEWTON + FLOPS_GRAD) / 1e12
     roof["step_frac"] = roof["step_tflops"] / peak_tflops
@@ -425,15 +560,42 @@ def main():
     ap.add_argument("--cpu-sinks", type=int, default=6144)
     ap.add_argument("--one-sided", action="store_true", help="force the one-sided sweeps (no pair symmetry)")
     ap.add_argument("--ref-sinks", type=int, default=1024)
-    ap.add_argument("--warmup-ref", type=int, default=1)
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-rows", action="store_true", help="skip the side measurements of the O(N) rows")
     ap.add_argument("--no-hhs", action="store_true", help="skip the config-5 HHS-FSI step (about 15 s)")
+    ap.add_argument("--probe", action="store_true", help="print the FP64 issue-model table and exit")
+    ap.add_argument("--rows-only", action="store_true", help="launch the O(N) kernels and time-step sweeps (for ncu)")
+    ap.add_argument("--subtree", type=int, default=0, help="run the subtree kernel on K/2 hard binaries (for ncu)")
+    ap.add_argument("--hhs-only", action="store_true", help="one HHS-FSI step of config 5 with its validity numbers")
     args = ap.parse_args()
+    if args.probe:
+        return run_probe()
+    if args.rows_only:
+        return run_rows_only(args.n)
+    if args.subtree:
+        return run_subtree(args.subtree)
+    if args.hhs_only:
+        return run_hhs_only()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # not under torchrun: launch one rank per GPU ourselves (rank 0 prints the JSON line)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        env = dict(os.environ)
+        env.setdefault("NCCL_DEBUG", "INFO")              # the communicator log shows the N ranks ...
+        env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+        env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")  # ... and stays off stdout (one JSON line)
+        sys.exit(subprocess.call(cmd, env=env))
     if args.impl == "reference":
         run_reference(args)
     else:
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        if world != args.gpus:
+            sys.stderr.write(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE\n")
         run_frost(args)
 
 

@@ -136,14 +136,14 @@ def _orbit_relative(rng, mtot, a, e, G=1.0):
 
 
 def star_cluster(n: int, seed: int, binary_fraction: float = 0.05, central_mass: float = 0.01,
-                 a_lo: float = 1e-5, a_hi: float = 1e-3):
+                 a_lo: float = 1e-5, a_hi: float = 1e-3, e_max: float = 0.99):
     """Config 5 (stand-in for PAPER.md:680-684 with primordial binaries added as a stress test).
 
     Index 0 is a point mass ``central_mass`` at rest at the origin; the other n-1 stars share
     1-central_mass with Kroupa-like masses (0.08-100 before normalisation), Plummer x and v;
     floor(binary_fraction*n/2) disjoint random pairs become binaries with log-uniform semi-major
-    axis in [a_lo,a_hi], thermal eccentricities and random phase; the pair's centre of mass
-    takes the primary's Plummer phase-space point.  Returns pos(3,n), vel(3,n), mass(n),
+    axis in [a_lo,a_hi], thermal eccentricities (capped at e_max; config 5: 0.99) and random
+    phase; the pair's centre of mass takes the primary's Plummer phase-space point.  Returns pos(3,n), vel(3,n), mass(n),
     pairs(k,2) int32.
     """
     rng = _rng(seed)
@@ -158,7 +158,7 @@ def star_cluster(n: int, seed: int, binary_fraction: float = 0.05, central_mass:
         mt = m[i1] + m[i2]
         sma = np.exp(rng.uniform(math.log(a_lo), math.log(a_hi), nb))
         ecc = np.sqrt(rng.uniform(0.0, 1.0, nb))
-        ecc = np.minimum(ecc, 0.99)
+        ecc = np.minimum(ecc, e_max)
         xr, vr = _orbit_relative(rng, mt, sma, ecc)
         xc, vc = pos_s[:, i1].copy(), vel_s[:, i1].copy()
         pos_s[:, i1] = xc - xr * (m[i2] / mt)

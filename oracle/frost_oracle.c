@@ -166,6 +166,53 @@ static void gradient_one_direction(int ld, const double *pos, const double *mass
     }
 }
 
+/* ---------------------------------------------------------------------------------------------
+ * O2b.  Magnitude sum of the terms of Eq. (27) / (43)-(44), PAPER.md:234-239, 373-387:
+ *     T_i = 2 G * sum_{j in J, s>0} | m_j / s^5 * ( s^2 a_ji - 3 (x_ji . a_ji) x_ji ) |_2
+ * -- the same terms gradient_one_direction adds, with the Euclidean norm taken before the sum.
+ * T_i / |g_i| is the condition number of the gradient sum: any evaluation of Eq. (27) from fp64
+ * accelerations carries an error of order 2^-53 T_i (reading 22), which is what the
+ * parity tests gate on where hard binaries make T_i >> |g_i|.  Not a step of the method.
+ * Pins (tests/test_oracle_pins.py): equals |g_i| for two bodies (closed form of Eq. 25-26),
+ * collinear closed form, triangle inequality |g_i| <= T_i, homogeneity.
+ * ------------------------------------------------------------------------------------------- */
+int oracle_gradient_termsum(int n, int ld, const double *pos, const double *mass,
+                            const int32_t *I, int nI, const int32_t *J, int nJ, double G,
+                            double eps2, const double *acc, double *out_T) {
+    if (n < 0 || ld < n || !pos || !mass || !acc || !out_T) return ORACLE_EINVAL;
+    if (!I) nI = n;
+    if (!J) nJ = n;
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < nI; ++a) {
+        const int i = pick(I, a);
+        const ld_t xi = pos[i], yi = pos[ld + i], zi = pos[2 * ld + i];
+        const ld_t axi = acc[i], ayi = acc[ld + i], azi = acc[2 * ld + i];
+        ld_t T = 0;
+        for (int b = 0; b < nJ; ++b) {
+            const int j = pick(J, b);
+            const ld_t dx = (ld_t)pos[j] - xi;
+            const ld_t dy = (ld_t)pos[ld + j] - yi;
+            const ld_t dz = (ld_t)pos[2 * ld + j] - zi;
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) {
+                const ld_t dax = (ld_t)acc[j] - axi;
+                const ld_t day = (ld_t)acc[ld + j] - ayi;
+                const ld_t daz = (ld_t)acc[2 * ld + j] - azi;
+                const ld_t s = sqrtl(s2);
+                const ld_t s5 = s2 * s2 * s;
+                const ld_t xa = dx * dax + dy * day + dz * daz;
+                const ld_t w = (ld_t)mass[j] / s5;
+                const ld_t tx = w * (s2 * dax - 3 * xa * dx);
+                const ld_t ty = w * (s2 * day - 3 * xa * dy);
+                const ld_t tz = w * (s2 * daz - 3 * xa * dz);
+                T += sqrtl(tx * tx + ty * ty + tz * tz);
+            }
+        }
+        out_T[i] = (double)(2 * (ld_t)G * T);
+    }
+    return ORACLE_OK;
+}
+
 /* compute_acc_newton / compute_acc_gradient (Alg. 2) when I == J; one direction of
  * acc_sf_newton / acc_sf_gradient (Alg. 3) when I != J; both directions under
  * ORACLE_MUTUAL.  Entries of acc/grad outside I (and J under MUTUAL) are not touched. */

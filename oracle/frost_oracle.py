@@ -93,6 +93,21 @@ def forces(pos, mass, sink_idx=None, source_idx=None, G=1.0, eps2=0.0, flags=ACC
     return acc, grad
 
 
+def gradient_termsum(pos, mass, acc, sink_idx=None, source_idx=None, G=1.0, eps2=0.0):
+    """T_i = 2G sum_j |term_ij| of Eq. 27 for the sinks (shape (ld,), zero elsewhere): the
+    magnitude sum behind the forward-error gate of the gradient parity tests."""
+    ld = pos.shape[1]
+    n = mass.shape[0]
+    out = np.zeros(ld)
+    si, ns = _i(sink_idx)
+    so, nso = _i(source_idx)
+    rc = lib().oracle_gradient_termsum(C.c_int(n), C.c_int(ld), _d(pos), _d(mass), _ptr(si),
+                                       C.c_int(ns), _ptr(so), C.c_int(nso), C.c_double(G),
+                                       C.c_double(eps2), _d(acc), _d(out))
+    _check(rc, "oracle_gradient_termsum")
+    return out
+
+
 def timesteps(pos, vel, mass, idx=None, G=1.0, eta_ff=0.2, eta_fb=0.2, tau_pivot=1.0,
               eta_in_q=True, tau=None, bins=None):
     ld = pos.shape[1]

@@ -23,7 +23,8 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric", "frost_diagnostics", "frost_set_shard", "frost_fsi_steps",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
+    "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
 ]
 
 
@@ -66,6 +67,7 @@ def load_library():
     lib.frost_set_tuning.argtypes = [vp, i32, i32, i32, i32]
     lib.frost_set_symmetric.argtypes = [vp, i32, i32]
     lib.frost_set_shard.argtypes = [vp, i32, i32]
+    lib.frost_set_overlap.argtypes = [vp, i32]
     lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -160,6 +162,11 @@ class Frost:
     def set_shard(self, rank=0, world=1):
         """This context's share of the symmetric sweeps (partial sums; add them across ranks)."""
         self._check(self.lib.frost_set_shard(self.h, rank, world), "frost_set_shard")
+
+    def set_overlap(self, on=1):
+        """1 (default): fsi(S) of a host-driven hierarchy entry runs on a side stream concurrently
+        with the recursion into F; 0: back to back on the context's stream (same bits)."""
+        self._check(self.lib.frost_set_overlap(self.h, on), "frost_set_overlap")
 
     def launch_count(self) -> int:
         return int(self.lib.frost_launch_count(self.h))
@@ -261,7 +268,9 @@ class Frost:
 
     def fp64_probe(self, mode=0, iters=4096, blocks_per_sm=4, scratch=None):
         if scratch is None:
-            scratch = torch.zeros(148 * 8 * 256 * 2, dtype=torch.float64, device="cuda")
+            sms = torch.cuda.get_device_properties(self.device).multi_processor_count
+            scratch = torch.zeros(sms * max(blocks_per_sm, 1) * 256, dtype=torch.float64,
+                                  device=torch.device("cuda", self.device))
         n = C.c_int64()
         self._check(self.lib.frost_fp64_probe(self.h, mode, iters, blocks_per_sm, _p(scratch),
                                               C.byref(n)), "frost_fp64_probe")

@@ -16,10 +16,11 @@ int frost_create(frost_ctx **out, int device, void *stream) {
     *out = nullptr;
     int count = 0;
     if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return FROST_ECUDA;
-    if (cudaSetDevice(device) != cudaSuccess) return FROST_ECUDA;
     frost_ctx *c = new (std::nothrow) frost_ctx();
     if (!c) return FROST_ENOMEM;
     c->device = device;
+    DeviceGuard guard(c);
+    if (!guard.ok) { delete c; return FROST_ECUDA; }
     c->stream = (cudaStream_t)stream;
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) { delete c; return FROST_ECUDA; }
@@ -32,12 +33,9 @@ int frost_create(frost_ctx **out, int device, void *stream) {
     return FROST_OK;
 }
 
-int frost_destroy(frost_ctx *c) {
-    if (!c) return FROST_EINVAL;
-    cudaSetDevice(c->device);
-    cudaStreamSynchronize(c->stream);
+static void free_scratch(frost_ctx *c) {
     Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->tau_scratch, &c->symtot,
-                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats};
+                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats, &c->shard_idx};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
     for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
@@ -45,7 +43,46 @@ int frost_destroy(frost_ctx *c) {
         if (c->lvlF[k].p) cudaFree(c->lvlF[k].p);
     }
     if (c->pinned_counts) cudaFreeHost(c->pinned_counts);
+}
+
+int frost_destroy(frost_ctx *c) {
+    if (!c) return FROST_EINVAL;
+    DeviceGuard guard(c);
+    cudaStreamSynchronize(c->stream);
+    for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
+        if (frost_ctx *s = c->side[k]) {
+            cudaStreamSynchronize(s->stream);
+            free_scratch(s);
+            cudaStreamDestroy(s->stream);
+            delete s;
+        }
+        if (c->ev_fork[k]) cudaEventDestroy(c->ev_fork[k]);
+        if (c->ev_join[k]) cudaEventDestroy(c->ev_join[k]);
+    }
+    free_scratch(c);
     delete c;
+    return FROST_OK;
+}
+
+// The side context of hierarchy level k: its own stream and its own sweep scratch, the parent's
+// parameters.  fsi(S, tau/2) of an entry at level k runs there while hhs_fsi(F, tau/2) recurses on the
+// parent's stream (the two operators commute and touch disjoint particles).
+static int side_ctx(frost_ctx *c, int level, frost_ctx **out) {
+    frost_ctx *s = c->side[level];
+    if (!s) {
+        s = new (std::nothrow) frost_ctx();
+        if (!s) return FROST_ENOMEM;
+        s->device = c->device; s->num_sms = c->num_sms;
+        if (cudaStreamCreateWithFlags(&s->stream, cudaStreamNonBlocking) != cudaSuccess) { delete s; return FROST_ECUDA; }
+        FROST_CUDA(c, cudaEventCreateWithFlags(&c->ev_fork[level], cudaEventDisableTiming));
+        FROST_CUDA(c, cudaEventCreateWithFlags(&c->ev_join[level], cudaEventDisableTiming));
+        c->side[level] = s;
+    }
+    s->G = c->G; s->eps2 = c->eps2; s->eta_ff = c->eta_ff; s->eta_fb = c->eta_fb; s->max_depth = c->max_depth;
+    s->tune_k = c->tune_k; s->tune_slices = c->tune_slices; s->tune_small = c->tune_small;
+    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym;
+    s->sym_scratch = c->sym_scratch < ((size_t)1 << 30) ? c->sym_scratch : ((size_t)1 << 30);
+    *out = s;
     return FROST_OK;
 }
 
@@ -83,7 +120,18 @@ int frost_set_shard(frost_ctx *c, int rank, int world) {
     return FROST_OK;
 }
 
-int64_t frost_launch_count(const frost_ctx *c) { return c ? c->launches : -1; }
+int frost_set_overlap(frost_ctx *c, int on) {
+    if (!c || on < 0 || on > 1) return FROST_EINVAL;
+    c->overlap = on;
+    return FROST_OK;
+}
+
+int64_t frost_launch_count(const frost_ctx *c) {
+    if (!c) return -1;
+    int64_t t = c->launches;
+    for (int k = 0; k < FROST_MAX_LEVELS; ++k) if (c->side[k]) t += c->side[k]->launches;
+    return t;
+}
 int frost_last_cuda_error(const frost_ctx *c) { return c ? c->last_cuda : 0; }
 const char *frost_version(void) { return "frost-b200 0.1 (sm_100a)"; }
 
@@ -114,6 +162,13 @@ static bool use_sym(const frost_ctx *c, int nA, int nB, int kind) {
     return nA >= 1024 && (long long)nA * nB >= 1000000LL;
 }
 
+// This rank's contiguous block [lo, hi) of a list of k entries (frost_set_shard); larger blocks first.
+static void shard_block(const frost_ctx *c, int k, int *lo, int *hi) {
+    const int base = k / c->shard_world, rem = k % c->shard_world, r = c->shard_rank;
+    *lo = r * base + (r < rem ? r : rem);
+    *hi = *lo + base + (r < rem ? 1 : 0);
+}
+
 static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
                        const int32_t *I, int nI, const int32_t *J, int nJ, double *acc, double *grad,
                        int flags) {
@@ -121,8 +176,14 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
     if (!J) nJ = n;
     const bool mutual = (flags & FROST_MUTUAL) != 0;
     const bool self = (I == J) && (nI == nJ);
+    const bool sharded = c->shard_world > 1;
+    // sharded: the outputs are partial sums the caller adds across ranks, so the gradient sweep cannot
+    // start from this call's own (partial) accelerations, and adding into out_* would count the old
+    // content once per rank -- whichever kernels end up serving the sweep
+    if (sharded && (((flags & FROST_ACC) && (flags & FROST_GRAD)) || (flags & FROST_ACCUMULATE))) return FROST_EINVAL;
     if (nI <= 0 && !(mutual && nJ > 0)) return FROST_OK;
-    const int padA = pad1024(nI), padB = pad1024(nJ);
+    // (sharded one-sided sweeps read a block of the sink stream at an offset: one more tile of padding)
+    const int padA = pad1024(nI) + (sharded ? 1024 : 0), padB = pad1024(nJ) + (sharded ? 1024 : 0);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)padA * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)padA * kRecBytes));
     double *Axm = (double *)c->recA_xm.p, *Av = (double *)c->recA_v.p;
@@ -139,9 +200,6 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
     const bool sym_self = self && use_sym(c, nI, nI, 0);
     const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI, 1);
     if (sym_self || sym_mut) {
-        // sharded: the outputs are partial sums the caller adds across ranks, so the gradient sweep
-        // cannot start from this call's own (partial) accelerations
-        if (c->shard_world > 1 && (flags & FROST_ACC) && (flags & FROST_GRAD)) return FROST_EINVAL;
         const bool swap = sym_mut && nJ > nI;            // A = the larger set
         const double *Pxm = swap ? Bxm : Axm, *Qxm = swap ? Axm : Bxm;
         double *Pv = swap ? Bv : Av, *Qv = swap ? Av : Bv;
@@ -159,18 +217,40 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
         }
         return FROST_OK;
     }
+    // One-sided sweeps.  Sharded: each direction sweeps this rank's contiguous block of its sink list
+    // against all sources and zeroes the outputs of the other sinks, so that the caller's sum over the
+    // ranks is complete here too (each sink's sum then comes from one rank: bitwise the unsharded one).
+    int loA = 0, hiA = nI, loB = 0, hiB = nJ;
+    const int32_t *Ii = I, *Ji = J;
+    if (sharded) {
+        shard_block(c, nI, &loA, &hiA);
+        shard_block(c, nJ, &loB, &hiB);
+        if (!I || (!J && mutual)) {      // NULL = all particles: the block needs explicit indices
+            FROST_TRY(ensure(c, c->shard_idx, (size_t)n * sizeof(int32_t)));
+            FROST_TRY(launch_iota(c, (int32_t *)c->shard_idx.p, n, 0));
+            if (!I) Ii = (const int32_t *)c->shard_idx.p;
+            if (!J) Ji = (const int32_t *)c->shard_idx.p;
+        }
+    }
+    const size_t oA = (size_t)4 * loA, oB = (size_t)4 * loB;
     if (flags & FROST_ACC) {
-        FROST_TRY(sweep_newton(c, Axm, nI, Bxm, nJ, I, ld, acc, Av));
+        FROST_TRY(sweep_newton(c, Axm + oA, hiA - loA, Bxm, nJ, Ii ? Ii + loA : nullptr, ld, acc, Av + oA));
+        if (sharded) FROST_TRY(launch_zero_outside(c, ld, acc, I, nI, loA, hiA));
         if (mutual && !self) {
-            FROST_TRY(sweep_newton(c, Bxm, nJ, Axm, nI, J, ld, acc, Bv));
+            FROST_TRY(sweep_newton(c, Bxm + oB, hiB - loB, Axm, nI, Ji ? Ji + loB : nullptr, ld, acc, Bv + oB));
+            if (sharded) FROST_TRY(launch_zero_outside(c, ld, acc, J, nJ, loB, hiB));
         }
     }
     if (flags & FROST_GRAD) {
         if (!(flags & FROST_ACC)) FROST_TRY(launch_pack_vec(c, ld, acc, I, nI, padA, Av));
         if (!self && !((flags & FROST_ACC) && mutual))
             FROST_TRY(launch_pack_vec(c, ld, acc, J, nJ, padB, Bv));
-        FROST_TRY(sweep_gradient(c, Axm, Av, nI, Bxm, Bv, nJ, I, ld, grad));
-        if (mutual && !self) FROST_TRY(sweep_gradient(c, Bxm, Bv, nJ, Axm, Av, nI, J, ld, grad));
+        FROST_TRY(sweep_gradient(c, Axm + oA, Av + oA, hiA - loA, Bxm, Bv, nJ, Ii ? Ii + loA : nullptr, ld, grad));
+        if (sharded) FROST_TRY(launch_zero_outside(c, ld, grad, I, nI, loA, hiA));
+        if (mutual && !self) {
+            FROST_TRY(sweep_gradient(c, Bxm + oB, Bv + oB, hiB - loB, Axm, Av, nI, Ji ? Ji + loB : nullptr, ld, grad));
+            if (sharded) FROST_TRY(launch_zero_outside(c, ld, grad, J, nJ, loB, hiB));
+        }
     }
     return FROST_OK;
 }
@@ -214,12 +294,12 @@ static int small_threshold(const frost_ctx *c) { return c->tune_small < 0 ? smal
 // positions of the leading sweep of the next, so from the second step on the leading sweep is
 // skipped: 3 all-pairs sweeps per step instead of 4, bitwise the same result.
 static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
-                    const int32_t *idx, int n_idx, double dt, frost_hhs_stats *st, int n_steps = 1) {
+                    const int32_t *idx, int n_idx, double dt, frost_hhs_stats *st, void *dev_stats,
+                    int n_steps = 1) {
     if (!idx) n_idx = n;
     if (n_idx <= 0 || n_steps <= 0) return FROST_OK;
     if (n_idx <= small_threshold(c))     // device-resident, set in shared memory (row 11)
-        return launch_small(c, 1, ld, pos, vel, mass, idx, n_idx, dt, 0, st ? c->dev_stats.p : nullptr,
-                            n_steps);
+        return launch_small(c, 1, ld, pos, vel, mass, idx, n_idx, dt, 0, st ? dev_stats : nullptr, n_steps);
     FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
     double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
@@ -238,6 +318,31 @@ static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const
         st->pairs_newton += (2 * (int64_t)n_steps + 1) * np;
         st->pairs_gradient += (int64_t)n_steps * np;
     }
+    return FROST_OK;
+}
+
+// fsi(S, h) of an entry at `level`.  With overlap on it is enqueued on the level's side stream after
+// everything enqueued so far on the parent's stream (fork); join_side() makes the parent's stream
+// wait for it.  Same kernels, same inputs, disjoint particles: bitwise the serial result.
+static int fsi_side(frost_ctx *c, int level, int n, int ld, double *pos, double *vel, const double *mass,
+                    const int32_t *S, int nS, double h, frost_hhs_stats *st, bool *forked) {
+    *forked = false;
+    if (nS <= 0) return FROST_OK;
+    if (!c->overlap) return fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st, c->dev_stats.p);
+    frost_ctx *s = nullptr;
+    FROST_TRY(side_ctx(c, level, &s));
+    FROST_CUDA(c, cudaEventRecord(c->ev_fork[level], c->stream));
+    FROST_CUDA(c, cudaStreamWaitEvent(s->stream, c->ev_fork[level], 0));
+    const int rc = fsi_impl(s, n, ld, pos, vel, mass, S, nS, h, st, c->dev_stats.p);
+    if (rc != FROST_OK) { c->last_cuda = s->last_cuda; return rc; }
+    *forked = true;
+    return FROST_OK;
+}
+
+static int join_side(frost_ctx *c, int level, bool forked) {
+    if (!forked) return FROST_OK;
+    FROST_CUDA(c, cudaEventRecord(c->ev_join[level], c->side[level]->stream));
+    FROST_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_join[level], 0));
     return FROST_OK;
 }
 
@@ -264,20 +369,23 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     }
     const bool cross = nS > 0 && nF > 0;
     const double h = 0.5 * tau_pivot;
+    bool forked = false;
     if (cross) {
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
         FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
     }
-    FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
-    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
+    FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked));       // fsi(S, tau/2) ...
+    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));              // ... || hhs_fsi(F, tau/2)
+    FROST_TRY(join_side(c, level, forked));
     if (cross) {
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad,
                               FROST_ACC | FROST_GRAD | FROST_MUTUAL));
         const double kap = tau_pivot * tau_pivot / 48.0;
         FROST_TRY(launch_kick(c, ld, vel, acc, grad, set, n_set, 2.0 * tau_pivot / 3.0, kap));   // S u F
     }
+    FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked));
     FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
-    FROST_TRY(fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st));
+    FROST_TRY(join_side(c, level, forked));
     if (cross) {
         FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
         FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
@@ -305,7 +413,7 @@ int frost_forces(frost_ctx *c, int n, int ld, const double *pos, const double *v
     if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
     if ((sink_idx && n_sink < 0) || (source_idx && n_source < 0)) return FROST_EINVAL;
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return forces_impl(c, n, ld, pos, mass, sink_idx, n_sink, source_idx, n_source, out_acc, out_grad, flags);
 }
 
@@ -316,8 +424,9 @@ int frost_forces_host(frost_ctx *c, int n, int ld, const double *pos, const doub
     if (!(flags & (FROST_ACC | FROST_GRAD)) || (flags & ~15)) return FROST_EINVAL;
     if ((flags & FROST_GRAD) && !out_grad) return FROST_EINVAL;
     if ((flags & FROST_MUTUAL) && ((sink_idx == nullptr) != (source_idx == nullptr))) return FROST_EINVAL;
+    if ((sink_idx && n_sink < 0) || (source_idx && n_source < 0)) return FROST_EINVAL;
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     const size_t pb = (size_t)3 * ld * sizeof(double);
     FROST_TRY(ensure(c, c->host_stage[0], pb));
     FROST_TRY(ensure(c, c->host_stage[1], (size_t)n * sizeof(double)));
@@ -341,10 +450,14 @@ int frost_forces_host(frost_ctx *c, int n, int ld, const double *pos, const doub
     }
     FROST_CUDA(c, cudaMemcpyAsync(dpos, pos, pb, cudaMemcpyHostToDevice, c->stream));
     FROST_CUDA(c, cudaMemcpyAsync(dmass, mass, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, c->stream));
-    // out_acc is an input when the gradient is requested on caller-provided accelerations, and
-    // entries outside the swept sets must come back untouched
-    FROST_CUDA(c, cudaMemcpyAsync(dacc, out_acc, pb, cudaMemcpyHostToDevice, c->stream));
-    if (flags & FROST_GRAD)
+    // out_acc is an input when the gradient is requested on caller-provided accelerations or the sums
+    // are accumulated, and entries outside the swept sets must come back untouched; when every
+    // particle is a sink of an overwriting sweep the planes are pure outputs and are not uploaded
+    const bool all_sinks = !sink_idx && ld == n;
+    const bool accum = (flags & FROST_ACCUMULATE) != 0;
+    if (!(all_sinks && (flags & FROST_ACC) && !accum))
+        FROST_CUDA(c, cudaMemcpyAsync(dacc, out_acc, pb, cudaMemcpyHostToDevice, c->stream));
+    if ((flags & FROST_GRAD) && !(all_sinks && !accum))
         FROST_CUDA(c, cudaMemcpyAsync(dgrad, out_grad, pb, cudaMemcpyHostToDevice, c->stream));
     FROST_TRY(forces_impl(c, n, ld, dpos, dmass, dI, n_sink, dJ, n_source, dacc, dgrad, flags));
     if (flags & FROST_ACC)
@@ -362,7 +475,7 @@ int frost_timesteps(frost_ctx *c, int n, int ld, const double *pos, const double
     if (idx && n_idx < 0) return FROST_EINVAL;
     if (out_bin && !(tau_pivot > 0.0)) return FROST_EINVAL;
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return timesteps_impl(c, n, ld, pos, vel, mass, idx, n_idx, tau_pivot, out_tau, out_bin);
 }
 
@@ -371,7 +484,7 @@ int frost_partition(frost_ctx *c, int n, const double *tau, const int32_t *idx, 
     if (!c || n < 0 || !tau || !out_slow || !out_fast || !counts) return FROST_EINVAL;
     if (!idx) n_idx = n;
     if (n_idx < 0) return FROST_EINVAL;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return launch_partition(c, tau, idx, n_idx, tau_pivot, out_slow, out_fast, counts);
 }
 
@@ -381,7 +494,7 @@ int frost_kick(frost_ctx *c, int n, int ld, double *vel, const double *acc, cons
     if (kappa != 0.0 && !grad) return FROST_EINVAL;
     if (!idx) n_idx = n;
     if (n_idx < 0) return FROST_EINVAL;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return launch_kick(c, ld, vel, acc, grad, idx, n_idx, cc, kappa);
 }
 
@@ -390,7 +503,7 @@ int frost_drift(frost_ctx *c, int n, int ld, double *pos, const double *vel, con
     if (!c || bad_planes(n, ld) || !pos || !vel) return FROST_EINVAL;
     if (!idx) n_idx = n;
     if (n_idx < 0) return FROST_EINVAL;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return launch_drift(c, ld, pos, vel, idx, n_idx, cc);
 }
 
@@ -398,26 +511,35 @@ int frost_fsi_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
                    const int32_t *idx, int n_idx, double dt) {
     if (!c || bad_planes(n, ld) || !pos || !vel || !mass) return FROST_EINVAL;
     if (idx && n_idx < 0) return FROST_EINVAL;
+    if (c->shard_world > 1) return FROST_EINVAL;      // only frost_forces is shard-aware
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
-    return fsi_impl(c, n, ld, pos, vel, mass, idx, n_idx, dt, nullptr);
+    FROST_DEVICE(c);
+    return fsi_impl(c, n, ld, pos, vel, mass, idx, n_idx, dt, nullptr, nullptr);
 }
 
 int frost_fsi_steps(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                     const int32_t *idx, int n_idx, double dt, int n_steps) {
     if (!c || bad_planes(n, ld) || !pos || !vel || !mass || n_steps < 0) return FROST_EINVAL;
     if (idx && n_idx < 0) return FROST_EINVAL;
+    if (c->shard_world > 1) return FROST_EINVAL;      // only frost_forces is shard-aware
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
-    return fsi_impl(c, n, ld, pos, vel, mass, idx, n_idx, dt, nullptr, n_steps);
+    FROST_DEVICE(c);
+    return fsi_impl(c, n, ld, pos, vel, mass, idx, n_idx, dt, nullptr, nullptr, n_steps);
 }
 
 int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                    double dt_top, frost_hhs_stats *stats) {
     if (!c || bad_planes(n, ld) || !pos || !vel || !mass || !(dt_top > 0.0)) return FROST_EINVAL;
     if (stats) *stats = frost_hhs_stats{};
+    if (c->shard_world > 1) return FROST_EINVAL;      // only frost_forces is shard-aware
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
+    // every O(n) scratch buffer of the recursion is sized here, once, for the largest set it can
+    // meet (all n particles), so that ensure() never has to drain the stream to grow one mid-step
+    const size_t recb = (size_t)pad1024(n) * kRecBytes;
+    FROST_TRY(ensure(c, c->recA_xm, recb)); FROST_TRY(ensure(c, c->recA_v, recb));
+    FROST_TRY(ensure(c, c->recB_xm, recb)); FROST_TRY(ensure(c, c->recB_v, recb));
+    FROST_TRY(ensure(c, c->blockcnt, (size_t)(n / 1024 + 4) * sizeof(int)));
     FROST_TRY(ensure(c, c->acc, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
     FROST_TRY(ensure(c, c->tau, (size_t)ld * sizeof(double)));
@@ -426,6 +548,8 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     frost_hhs_stats local = frost_hhs_stats{};
     local.depth = -1;
     int rc = hhs_rec(c, n, ld, pos, vel, mass, nullptr, n, dt_top, 0, &local);
+    if (rc != FROST_OK)      // an aborted recursion may have left forked side streams unjoined
+        for (int k = 0; k < FROST_MAX_LEVELS; ++k) if (c->side[k]) cudaStreamSynchronize(c->side[k]->stream);
     // merge what the device-resident subtrees counted (also carries their status)
     struct { long long e[FROST_MAX_LEVELS], s[FROST_MAX_LEVELS], f[FROST_MAX_LEVELS], pn, pg, pt; int depth, status; } d;
     static_assert(sizeof(d) >= 1, "");
@@ -449,7 +573,7 @@ int frost_diagnostics(frost_ctx *c, int n, int ld, const double *pos, const doub
     if (!c || bad_planes(n, ld) || !pos || !vel || !mass || !out8) return FROST_EINVAL;
     for (int k = 0; k < 8; ++k) out8[k] = 0.0;
     if (n == 0) return FROST_OK;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     const int pad = pad1024(n);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
     FROST_TRY(ensure(c, c->tau, (size_t)(ld + 8) * sizeof(double)));
@@ -470,7 +594,7 @@ int frost_gather_pack(frost_ctx *c, int n, int ld, const double *pos, const doub
     if (!c || bad_planes(n, ld) || !pos || !mass || !out_records) return FROST_EINVAL;
     if (!idx) n_idx = n;
     if (n_idx < 0 || n_pad < n_idx) return FROST_EINVAL;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     return launch_pack_xm(c, ld, pos, mass, idx, n_idx, n_pad, out_records);
 }
 

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <unordered_set>
+
 #include "../../include/frost.h"
 
 namespace frost {
@@ -47,6 +49,14 @@ struct frost_ctx {
     frost::Buf host_stage[6];      // device staging for frost_forces_host
     frost::Buf lvlS[FROST_MAX_LEVELS], lvlF[FROST_MAX_LEVELS];
     int32_t *pinned_counts = nullptr;  // host pinned int32[4]
+    frost::Buf shard_idx;              // 0..n-1, for sharding the sinks of a NULL index list
+    // fsi(S) || hhs_fsi(F): one side context (own stream, own sweep scratch) per hierarchy level
+    int overlap = 1;
+    frost_ctx *side[FROST_MAX_LEVELS] = {};
+    cudaEvent_t ev_fork[FROST_MAX_LEVELS] = {}, ev_join[FROST_MAX_LEVELS] = {};
+    // function attributes (dynamic shared memory opt-in, cluster size) are per device, and a context
+    // is bound to one device: remembered per context, not per process
+    std::unordered_set<uint64_t> attr_done;
 };
 
 namespace frost {
@@ -85,6 +95,32 @@ inline int ensure(frost_ctx *c, Buf &b, size_t bytes) {
     b.cap = want;
     return FROST_OK;
 }
+
+// cudaFuncSetAttribute once per (context, kernel, attribute).
+template <class F>
+inline int set_func_attr(frost_ctx *c, F *func, cudaFuncAttribute attr, int value) {
+    const uint64_t key = (uint64_t)(uintptr_t)func * 8u + (uint64_t)attr;
+    if (c->attr_done.count(key)) return FROST_OK;
+    FROST_CUDA(c, cudaFuncSetAttribute(func, attr, value));
+    c->attr_done.insert(key);
+    return FROST_OK;
+}
+
+// Entry points make the context's device current for the duration of the call and restore the
+// caller's device on return.
+struct DeviceGuard {
+    int prev = -1;
+    bool ok;
+    explicit DeviceGuard(const frost_ctx *c) {
+        cudaGetDevice(&prev);
+        ok = (prev == c->device) || cudaSetDevice(c->device) == cudaSuccess;
+        if (prev == c->device) prev = -1;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define FROST_DEVICE(ctx)                                   \
+    frost::DeviceGuard guard_(ctx);                         \
+    if (!guard_.ok) { (ctx)->last_cuda = (int)cudaGetLastError(); return FROST_ECUDA; }
 
 inline int check_launch(frost_ctx *c) {
     c->launches++;
@@ -138,6 +174,9 @@ int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
 // frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)
 int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *vel, const double *mass,
                 const double *phi, double *out8);
+// out[k] = k0 + k ; zero the planes of the particles idx[k] (or k), k in [0, lo) and [hi, n_idx)
+int launch_iota(frost_ctx *c, int32_t *out, int n, int k0);
+int launch_zero_outside(frost_ctx *c, int ld, double *planes, const int32_t *idx, int n_idx, int lo, int hi);
 
 // frost_tau.cu: time-step sweep in Morton order with exact block pruning (prune = 0: evaluate all)
 int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const double *mass,

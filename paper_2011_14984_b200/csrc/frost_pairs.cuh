@@ -95,13 +95,17 @@ struct GradientPolicy {
 // Harmonic symmetrisation factor of Eq. (49) in the cancellation-free form 1 + q/(1+sqrt(1+q^2))
 // (reading 10), without IEEE sqrt/div sequences: with u = 1/sqrt(1+q^2) in (0,1],
 //   q/(1+sqrt(1+q^2)) = q u / (1 + u);  1/(1+u) by MUFU.RCP64H + one cubic step.  13 FP64 instr.
+// s(q) > 0 for every q, but for q < -1e15 the sum below cancels to within its rounding error and
+// can come out as -0 or a tiny negative number; the |.| (a free source modifier of the consuming
+// DMUL) keeps every candidate >= 0 in all three time-step routines alike, which the bit-pattern
+// atomicMin of frost_tau.cu relies on.  NaN (self pair, padding) stays NaN.
 __device__ __forceinline__ double sym_factor(double q) {
     const double h = fma(q, q, 1.0);
     const double u = rsqrt_full(h);
     const double qu = q * u;
     const double d = u + 1.0;
     const double rd = rcp_full(d);
-    return fma(qu, rd, 1.0);
+    return fabs(fma(qu, rd, 1.0));
 }
 
 struct TimestepPolicy {

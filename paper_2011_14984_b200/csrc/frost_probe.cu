@@ -2,7 +2,8 @@
 // MEASURED_PEAKS.json has no fp64 entry, and the FP64 pipe of sm_100a turned out not to be a
 // plain "one warp instruction per 2 cycles" unit: these probes measure what the sweep kernels
 // are bounded by.  bench.py times modes 0/3 next to the headline
-// number; `python -m paper_2011_14984_b200.probe_fp64` prints the whole table.
+// number; `python bench.py --probe` prints the whole table.
+#include "../../include/frost_probe.h"
 #include "frost_common.cuh"
 
 namespace frost {
@@ -87,7 +88,7 @@ extern "C" int frost_fp64_probe(frost_ctx *c, int mode, int iters, int blocks_pe
                                 int64_t *out_instr) {
     using namespace frost;
     if (!c || !scratch || iters < 1 || blocks_per_sm < 1 || mode < 0 || mode > 11) return FROST_EINVAL;
-    FROST_CUDA(c, cudaSetDevice(c->device));
+    FROST_DEVICE(c);
     const int grid = c->num_sms * blocks_per_sm;
 #define FROST_PROBE_CASE(M) \
     case M: fp64_probe_kernel<M><<<grid, 256, 0, c->stream>>>(scratch, iters, 0.5); break;

@@ -543,17 +543,21 @@ __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const Small
         P.pos[i] = x.x; P.pos[(size_t)ld + i] = x.y; P.pos[2 * (size_t)ld + i] = x.z;
         P.vel[i] = v.x; P.vel[(size_t)ld + i] = v.y; P.vel[2 * (size_t)ld + i] = v.z;
     }
-    if (P.stats) {
+    if (P.stats) {      // atomics: an fsi(S) launch on a side stream may run concurrently (frost_api.cu)
+        typedef unsigned long long ull;
         for (int k = threadIdx.x; k < FROST_MAX_LEVELS; k += kSmallThreads) {
-            P.stats->entries[k] += sm.st_entries[k];
-            P.stats->n_slow[k] += sm.st_slow[k];
-            P.stats->n_fast[k] += sm.st_fast[k];
+            if (sm.st_entries[k]) {
+                atomicAdd((ull *)&P.stats->entries[k], (ull)sm.st_entries[k]);
+                atomicAdd((ull *)&P.stats->n_slow[k], (ull)sm.st_slow[k]);
+                atomicAdd((ull *)&P.stats->n_fast[k], (ull)sm.st_fast[k]);
+            }
         }
         if (threadIdx.x == 0) {
-            P.stats->pairs_newton += sm.st_pn; P.stats->pairs_gradient += sm.st_pg;
-            P.stats->pairs_timestep += sm.st_pt;
-            if (sm.st_depth > P.stats->depth) P.stats->depth = sm.st_depth;
-            if (sm.err && !P.stats->status) P.stats->status = sm.err;
+            atomicAdd((ull *)&P.stats->pairs_newton, (ull)sm.st_pn);
+            atomicAdd((ull *)&P.stats->pairs_gradient, (ull)sm.st_pg);
+            atomicAdd((ull *)&P.stats->pairs_timestep, (ull)sm.st_pt);
+            atomicMax(&P.stats->depth, sm.st_depth);
+            if (sm.err) atomicCAS(&P.stats->status, 0, sm.err);
         }
     }
 }
@@ -565,16 +569,11 @@ int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const
                  const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps) {
     if (n <= 0) return FROST_OK;
     if (n > kSmallMax) return FROST_EINVAL;
-    static bool attr_done = false;
-    if (!attr_done) {
-        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                           (int)sizeof(SmallSmem)));
-        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCluster>,
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(SmallSmem)));
-        FROST_CUDA(c, cudaFuncSetAttribute(hhs_small_kernel<TeamCluster>,
-                                           cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        attr_done = true;
-    }
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)sizeof(SmallSmem)));
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)sizeof(SmallSmem)));
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     SmallParams P{};
     P.idx = idx; P.n = n; P.ld = ld; P.pos = pos; P.vel = vel; P.mass = mass;
     P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0; P.n_steps = n_steps;

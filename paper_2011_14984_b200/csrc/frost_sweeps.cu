@@ -170,12 +170,7 @@ static Plan make_plan(const frost_ctx *c, int n_snk, int n_src, int max_k) {
 template <class P, int K, int NT>
 static int launch_variant(frost_ctx *c, const SweepParams &prm, const Plan &pl) {
     const size_t smem = (size_t)kStages * P::kRecs * kTile * kRecBytes + 2 * kStages * sizeof(uint64_t);
-    static bool attr_done = false;
-    if (!attr_done) {
-        FROST_CUDA(c, cudaFuncSetAttribute(sweep_kernel<P, K, NT>,
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    FROST_TRY(set_func_attr(c, sweep_kernel<P, K, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     dim3 grid(pl.sink_blocks, pl.slices);
     sweep_kernel<P, K, NT><<<grid, NT, smem, c->stream>>>(prm);
     return check_launch(c);

@@ -384,14 +384,9 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
     FROST_TRY(ensure(c, c->partialB, row_bytes_per_tile * (size_t)band_tiles + 256));
     if (nbands > 1) FROST_TRY(ensure(c, c->symtot, (size_t)PL * na_pad * sizeof(double)));
 
-    static bool attr_done = false;
     const size_t smem = (size_t)kStages * P::kRecs * NT * kRecBytes + 2 * PL * NT * sizeof(double) +
                         kStages * sizeof(uint64_t);
-    if (!attr_done) {
-        FROST_CUDA(c, cudaFuncSetAttribute(sym_kernel<P, KA, NT, MINB>,
-                                           cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    FROST_TRY(set_func_attr(c, sym_kernel<P, KA, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
     for (int b = 0; b < nbands; ++b) {
         const int bt0 = b * (int)band_tiles;

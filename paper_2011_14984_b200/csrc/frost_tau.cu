@@ -427,13 +427,9 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
     tau_box_kernel<<<n_pad / 256, 256, 0, c->stream>>>((const double4 *)xm, (const double4 *)vv, n_pad, boxes, tau64);
     FROST_TRY(check_launch(c));
 
-    static bool attr_done = false;
     const size_t smem = (size_t)kStages * 2 * kTauNT * kRecBytes + 2 * kTauNT * sizeof(double) +
                         2 * kTauWarps * sizeof(TauBox) + kStages * sizeof(uint64_t);
-    if (!attr_done) {
-        FROST_CUDA(c, cudaFuncSetAttribute(tau_sym_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
+    FROST_TRY(set_func_attr(c, tau_sym_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     TauParams prm{};
     prm.xm = (const double4 *)xm; prm.vv = (const double4 *)vv; prm.box = boxes; prm.tau64 = tau64;
     prm.n_tiles = n_tiles; prm.prune = prune; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;

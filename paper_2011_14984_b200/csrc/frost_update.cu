@@ -87,6 +87,20 @@ __global__ void drift_kernel(double *__restrict__ pos, const double *__restrict_
     }
 }
 
+__global__ void iota_kernel(int32_t *__restrict__ out, int n, int k0) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) out[k] = k0 + k;
+}
+
+// planes[:, idx[k]] = 0 for the list positions k outside [lo, hi): the sinks another rank owns
+__global__ void zero_outside_kernel(double *__restrict__ planes, int ld, const int32_t *__restrict__ idx,
+                                    int n_idx, int lo, int hi) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_idx || (k >= lo && k < hi)) return;
+    const int i = idx ? idx[k] : k;
+    planes[i] = 0.0; planes[(size_t)ld + i] = 0.0; planes[2 * (size_t)ld + i] = 0.0;
+}
+
 // ---- stable partition: count per block -> scan of block counts -> scatter ----------------------
 constexpr int kPartBlock = 1024;
 
@@ -245,6 +259,18 @@ int launch_drift(frost_ctx *c, int ld, double *pos, const double *vel, const int
                  int n_idx, double cc) {
     if (n_idx <= 0) return FROST_OK;
     drift_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(pos, vel, ld, idx, n_idx, cc);
+    return check_launch(c);
+}
+
+int launch_iota(frost_ctx *c, int32_t *out, int n, int k0) {
+    if (n <= 0) return FROST_OK;
+    iota_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(out, n, k0);
+    return check_launch(c);
+}
+
+int launch_zero_outside(frost_ctx *c, int ld, double *planes, const int32_t *idx, int n_idx, int lo, int hi) {
+    if (n_idx <= 0 || (lo <= 0 && hi >= n_idx)) return FROST_OK;
+    zero_outside_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(planes, ld, idx, n_idx, lo, hi);
     return check_launch(c);
 }
 

@@ -1,7 +1,12 @@
 """Parity of the CUDA path (through the C-ABI binding) against the CPU oracle, element by element
 on the same seeded inputs.  Tolerances are north_star's, read per particle against the vector norm
 (reading 19): |da_k| <= 1e-12 |a_i|, |dg_k| <= 1e-10 |g_i|; bins identical; index work
-bit-exact."""
+bit-exact.  Inputs with config 5's hard binaries use the forward-error gate of DESIGN.md reading 22
+for g: |dg_k| <= 1e-10 |g_i| + C_FWD 2^-53 T_i, T_i = the oracle's magnitude sum of Eq. 27's terms
+(the definition itself moves by up to 2.4 x 2^-53 T_i > 1e-10 |g_i| under +-1 ulp of the fp64
+accelerations it is evaluated from: tests/test_oracle_pins.py)."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -11,6 +16,7 @@ import frost_inputs as fi
 pytestmark = pytest.mark.gpu
 
 TOL_A, TOL_G, TOL_TAU = 1e-12, 1e-10, 1e-13
+C_FWD = 8.0          # forward-error constant of reading 22 (<= 8; the definition's own floor is 2.4)
 
 
 @pytest.fixture(scope="module")
@@ -34,7 +40,22 @@ def vec_err(x, ref):
     return float((d[~ok0] / nrm[~ok0]).max()) if (~ok0).any() else 0.0
 
 
-def check_forces(fr, oracle, pos, mass, I=None, J=None, flags=3, G=1.0, eps2=0.0, acc0=None):
+def grad_gate_ratio(oracle, pos, mass, a_ref, g, g_ref, I=None, J=None, flags=3, G=1.0, eps2=0.0):
+    """max over the swept sinks of |dg_k| / (1e-10 |g_i| + C_FWD 2^-53 T_i)  (reading 22)."""
+    n = mass.size
+    T = oracle.gradient_termsum(pos, mass, a_ref, sink_idx=I, source_idx=J, G=G, eps2=eps2)
+    sel = np.arange(n) if I is None else np.asarray(I)
+    if flags & 4:
+        T += oracle.gradient_termsum(pos, mass, a_ref, sink_idx=J, source_idx=I, G=G, eps2=eps2)
+        sel = np.concatenate([sel, np.arange(n) if J is None else np.asarray(J)])
+    d = np.abs(g - g_ref).max(0)[sel]
+    bound = TOL_G * np.linalg.norm(g_ref, axis=0)[sel] + C_FWD * 2.0 ** -53 * T[sel]
+    assert (d[bound == 0] == 0).all()
+    return float((d[bound > 0] / bound[bound > 0]).max()) if (bound > 0).any() else 0.0
+
+
+def check_forces(fr, oracle, pos, mass, I=None, J=None, flags=3, G=1.0, eps2=0.0, acc0=None,
+                 forward_gate=False):
     fr.set_params(G=G, eps2=eps2)
     n = mass.size
     a0 = np.zeros((3, n)) if acc0 is None else acc0.copy()
@@ -47,9 +68,13 @@ def check_forces(fr, oracle, pos, mass, I=None, J=None, flags=3, G=1.0, eps2=0.0
     torch.cuda.synchronize()
     a, g = a_gpu.cpu().numpy(), g_gpu.cpu().numpy()
     ea = vec_err(a, a_ref)
-    eg = vec_err(g, g_ref) if flags & 2 else 0.0
     assert ea <= TOL_A, ea
-    assert eg <= TOL_G, eg
+    if (flags & 2) and forward_gate:
+        ratio = grad_gate_ratio(oracle, pos, mass, a_ref, g, g_ref, I, J, flags, G, eps2)
+        assert ratio <= 1.0, ratio
+    elif flags & 2:
+        eg = vec_err(g, g_ref)
+        assert eg <= TOL_G, eg
     return a, g, a_ref, g_ref
 
 
@@ -73,6 +98,29 @@ def test_every_kernel_variant_and_slice_count(fr, oracle, k, slices):
 def test_softened_and_scaled_G(fr, oracle):
     pos, vel, mass = fi.plummer(2048, 3)
     check_forces(fr, oracle, pos, mass, G=6.674e-3, eps2=1e-4)
+
+
+@pytest.mark.parametrize("sym", [1, 2])
+def test_self_forces_at_config5_hardness_forward_error_gate(fr, oracle, sym, capsys):
+    """Self sweep ACC|GRAD on config 5's recipe at its DEFAULT hardness (binaries a = 1e-5..1e-3),
+    one-sided (sym = 1) and pair-symmetric (sym = 2) kernels.  a holds 1e-12; g is gated by the
+    forward-error bound of reading 22.  Also the gradient alone from the ORACLE's accelerations
+    (identical fp64 inputs on both sides: what remains is the kernel's own arithmetic)."""
+    pos, vel, mass, _ = fi.star_cluster(4096, 4)
+    fr.set_symmetric(sym, 0)
+    try:
+        a, g, a_ref, g_ref = check_forces(fr, oracle, pos, mass, forward_gate=True)
+        r1 = grad_gate_ratio(oracle, pos, mass, a_ref, g, g_ref)
+        _, g2, _, g_ref2 = check_forces(fr, oracle, pos, mass, flags=2, acc0=a_ref, forward_gate=True)
+        r2 = grad_gate_ratio(oracle, pos, mass, a_ref, g2, g_ref2, flags=2)
+        check_forces(fr, oracle, pos, mass, G=6.674e-3, eps2=1e-12, forward_gate=True)
+    finally:
+        fr.set_symmetric(0, 0)
+    plain = vec_err(g, g_ref)
+    with capsys.disabled():
+        print(f"\n[g gate] sym={sym}: plain max |dg|/|g| = {plain:.2e}; gate ratio end-to-end {r1:.3f}, "
+              f"gradient-only on the oracle's a {r2:.3f} (C_FWD = {C_FWD})")
+    assert np.abs((mass * g).sum(1)).max() < 1e-12 * (mass * np.abs(g)).sum(1).max()
 
 
 def test_config1_plummer_1024_acc_grad(fr, oracle):
@@ -191,7 +239,7 @@ def test_kick_drift_gather(fr, oracle):
 def test_diagnostics_match_oracle(fr, oracle, n, eps2):
     """frost_diagnostics (on-device E, P, L with an O(N^2) potential sweep) against
     the oracle's long-double textbook sums (Eq. 23)."""
-    pos, vel, mass, _ = fi.star_cluster(max(n, 64), 4, a_lo=1e-3, a_hi=1e-2)
+    pos, vel, mass, _ = fi.star_cluster(max(n, 64), 4)
     pos, vel, mass = np.ascontiguousarray(pos[:, :n]), np.ascontiguousarray(vel[:, :n]), mass[:n].copy()
     fr.set_params(G=0.7, eps2=eps2)
     phi = torch.zeros(n, dtype=torch.float64, device="cuda")
@@ -264,35 +312,204 @@ def test_fsi_steps_equal_repeated_fsi_step_bitwise(fr, n):
     assert torch.equal(p1, p2) and torch.equal(v1, v2)
 
 
-@pytest.mark.parametrize("n,small", [(1024, -1), (1024, 0), (1024, 48), (3000, -1), (3000, 100)])
-def test_hhs_step_small_cluster(fr, oracle, n, small):
-    """Reduced-N replica of config 5: level sets, bookkeeping and the trajectory must match the
-    oracle whether the recursion runs on the host (small = 0), in the device-resident subtree
-    kernel (whole problem for n <= 1024) or in a mix of both."""
-    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+ENV_K = 8.0          # GPU-vs-oracle deviation allowed, in units of the oracle's own +-1-ulp envelope
+
+
+def oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, trials=3, seed=0, **kw):
+    """The oracle's HHS-FSI step plus its own sensitivity to the last bit of its inputs: the step is
+    repeated from positions and velocities moved by +-1 ulp per component (random signs, seeded).
+    Returns (pos_ref, vel_ref, stats_ref, env_pos[n], env_vel[n], stats_of_every_trial).
+
+    Why this is the yardstick (reading 23): a hard binary at |x| ~ 1 resolves its own
+    separation only to ulp(x)/a ~ 1e-11; any two correct fp64 evaluations of Alg. 3 (different
+    summation order, FMA contraction) part by an ulp of x or v somewhere along the 2^depth
+    sub-steps, after which they differ the way the oracle differs from itself under a 1-ulp input
+    change (the earliest, hence largest, such change).  Several independent partings add in
+    quadrature, so the GPU is held to ENV_K = 8 times the envelope, per particle."""
+    n = mass.size
+    if n <= 512:
+        oracle.set_num_threads(1)             # tiny level sets: OpenMP fork/join would dominate
+    try:
+        pr, vr = pos.copy(), vel.copy()
+        st = oracle.hhs_step(pr, vr, mass, dt, **kw)
+        rng = np.random.default_rng(seed)
+        env_p, env_v, sts = np.zeros(n), np.zeros(n), []
+        for _ in range(trials):
+            pp = np.ascontiguousarray(np.nextafter(pos, rng.choice([-1.0, 1.0], size=pos.shape) * np.inf))
+            vv = np.ascontiguousarray(np.nextafter(vel, rng.choice([-1.0, 1.0], size=vel.shape) * np.inf))
+            sts.append(oracle.hhs_step(pp, vv, mass, dt, **kw))
+            env_p = np.maximum(env_p, np.abs(pp - pr).max(0))
+            env_v = np.maximum(env_v, np.abs(vv - vr).max(0))
+    finally:
+        oracle.set_num_threads(os.cpu_count() or 1)
+    return pr, vr, st, env_p, env_v, sts
+
+
+def momentum_change(mass, v0, v1, v_ref=None):
+    """|sum m dv|_max of a step in units of what "roundoff" is for it: every kick is pairwise
+    antisymmetric but individually rounded, so the sum random-walks with the number of kicks (a hard
+    binary, |v| ~ 10-100, is kicked ~2^depth times per top step).  The unit is 4 x the oracle's own
+    |sum m dv| over the same step (v_ref) where given, and never less than 8 x 2^-53 x sum m |v|."""
+    unit = 8 * 2.0 ** -53 * (mass * np.linalg.norm(v1, axis=0)).sum()
+    if v_ref is not None:
+        unit = max(unit, 4 * np.abs((mass * (v_ref - v0)).sum(1)).max())
+    return float(np.abs((mass * (v1 - v0)).sum(1)).max() / unit)
+
+
+def envelope_ratio(pg, vg, pr, vr, env_p, env_v):
+    """max over particles of |dx| / (ENV_K env_x + 8 ulp) and the same for v."""
+    fl_p = 8 * np.spacing(np.abs(pr).max(0) + 1e-300)
+    fl_v = 8 * np.spacing(np.abs(vr).max(0) + 1e-300)
+    rp = np.abs(pg - pr).max(0) / (ENV_K * env_p + fl_p)
+    rv = np.abs(vg - vr).max(0) / (ENV_K * env_v + fl_v)
+    return float(rp.max()), float(rv.max())
+
+
+@pytest.mark.parametrize("n,small,log2dt", [(1024, -1, 8), (1024, 0, 11), (1024, 48, 8), (3000, -1, 8),
+                                            (3000, 100, 8)])
+def test_hhs_step_small_cluster(fr, oracle, n, small, log2dt):
+    """Reduced-N replica of config 5 at its full hardness (binaries a = 1e-5..1e-3; eccentricities
+    capped at 0.1 so that no time-step oscillates across a pivot and the level sets are a
+    reproducible function of the input -- the oracle's own +-1-ulp trials confirm it): level sets
+    and bookkeeping IDENTICAL to the oracle's and the trajectory inside the oracle's 1-ulp envelope,
+    whether the recursion runs on the host (small = 0; shorter top step, ~45 launches per entry), in
+    the device-resident subtree kernel (whole problem for n <= 1024) or in a mix of both."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
+    dt = 2.0 ** -log2dt
     fr.set_params(eta_ff=0.2, eta_fb=0.2)
     fr.set_tuning(0, 0, small)
-    pr, vr = pos.copy(), vel.copy()
-    st_ref = oracle.hhs_step(pr, vr, mass, 1.0 / 256)
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt)
+    assert all(s == st_ref for s in sts)
     p, v = dev(pos), dev(vel)
     try:
-        st = fr.hhs_step(p, v, dev(mass), 1.0 / 256)
+        st = fr.hhs_step(p, v, dev(mass), dt)
     finally:
         fr.set_tuning(0, 0, -1)
     assert st == st_ref
-    assert st["depth"] >= 3
+    assert st["depth"] >= (12 if small == 0 else 14)
+    rp, rv = envelope_ratio(p.cpu().numpy(), v.cpu().numpy(), pr, vr, env_p, env_v)
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, v.cpu().numpy(), vr) <= 1.0
+
+
+@pytest.mark.parametrize("small,one_cta,log2dt", [(-1, 0, 7), (-1, 1, 7), (48, 0, 7), (0, 0, 10)])
+def test_hhs_step_matches_oracle_at_config5_depth(fr, oracle, small, one_cta, log2dt, capsys):
+    """Alg. 3 at config 5's depth, element by element: 256 stars of config 5's
+    recipe (binaries down to a = 1e-5, e <= 0.1), dt_top = 2^-7 => depth 17 with every level
+    populated (2^18 - 1 hierarchy entries).  small = -1: one launch of the subtree kernel -- the
+    16-CTA cluster team (one_cta = 0) or the CTA team (one_cta = 1) at the top, the quad team for
+    sub-sets of 33-128 and the warp team for sub-sets of <= 32 at depth; small = 48: host recursion
+    down to sets of <= 48, then quad / warp teams; small = 0: host recursion only (2^-10: depth 14).
+    Bookkeeping identical to the oracle's; trajectory inside ENV_K x the oracle's 1-ulp envelope;
+    momentum change at rounding level."""
+    n = 256
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
+    dt = 2.0 ** -log2dt
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt)
+    assert all(s == st_ref for s in sts)
+    fr.set_tuning(0, 0, small, one_cta)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), dt)
+    finally:
+        fr.set_tuning(0, 0, -1, 0)
+    assert st == st_ref
+    assert st["depth"] >= (14 if small == 0 else 15)
     pg, vg = p.cpu().numpy(), v.cpu().numpy()
-    assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
-    assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
+    rp, rv = envelope_ratio(pg, vg, pr, vr, env_p, env_v)
+    with capsys.disabled():
+        print(f"\n[hhs depth {st['depth']}] small={small} one_cta={one_cta}: max |dx| {np.abs(pg - pr).max():.2e} "
+              f"(envelope {env_p.max():.2e}), max |dv| {np.abs(vg - vr).max():.2e} (envelope {env_v.max():.2e}); "
+              f"ratio to {ENV_K:.0f} x envelope: x {rp:.3f}, v {rv:.3f}")
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, vg, vr) <= 1.0
+
+
+@pytest.mark.parametrize("n,small", [(20000, -1), (6000, 200)])
+def test_hhs_overlap_of_fsi_S_with_hhs_F_is_bitwise_the_serial_step(fr, n, small):
+    """frost_set_overlap: fsi(S, tau/2) on a side stream concurrently with the recursion into F
+    (the two commute and touch disjoint particles) must give the bits of the serial
+    order, with the same bookkeeping, step after step."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-4, a_hi=1e-2)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    fr.set_tuning(0, 0, small)
+    out = []
+    try:
+        for on in (0, 1):
+            fr.set_overlap(on)
+            p, v, m = dev(pos), dev(vel), dev(mass)
+            sts = [fr.hhs_step(p, v, m, 2.0 ** -9) for _ in range(2)]
+            out.append((sts, p.clone(), v.clone()))
+    finally:
+        fr.set_overlap(1)
+        fr.set_tuning(0, 0, -1)
+    assert out[0][0] == out[1][0] and out[0][0][0]["depth"] >= 5
+    assert torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])
+
+
+def hhs_stats_invariants(st):
+    """What every correct execution of Alg. 3 satisfies whatever its rounding: a level is entered at
+    most twice per entry of its parent, and the members of level k+1 are the fast members of level k
+    entered twice."""
+    e, s, f = st["entries"], st["n_slow"], st["n_fast"]
+    assert e[0] == 1
+    for k in range(st["depth"]):
+        assert e[k + 1] <= 2 * e[k] and e[k + 1] % 2 == 0
+        assert s[k + 1] + f[k + 1] == 2 * f[k]
+    assert f[st["depth"]] == 0
+
+
+@pytest.mark.parametrize("n,small", [(256, -1), (1024, -1), (3000, -1)])
+def test_hhs_step_thermal_binaries_unique_part_and_validity(fr, oracle, n, small, capsys):
+    """Config 5's recipe unchanged (thermal eccentricities up to 0.99): an eccentric hard binary
+    sweeps its time-step across several pivots every orbit, thousands of times per top step, and the
+    oracle's own +-1-ulp trials then disagree with each other about the deepest levels' entry counts
+    (reading 23).  Compared here: what is unique -- the bookkeeping of every level down to the first
+    one on which the oracle's trials disagree must be IDENTICAL, and every particle must lie inside
+    ENV_K x the oracle's envelope (which is ~1e-16 for everything but the hard binaries) -- and that
+    the rest is valid: the structural invariants of Alg. 3's bookkeeping, momentum at rounding
+    level, energy error of the oracle's size."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4)
+    dt = 2.0 ** -8
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    fr.set_tuning(0, 0, small)
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), dt)
+    finally:
+        fr.set_tuning(0, 0, -1)
+    hhs_stats_invariants(st)
+    hhs_stats_invariants(st_ref)
+    agree = 0                                   # levels on which all oracle trials agree
+    keys = ("entries", "n_slow", "n_fast")
+    while agree <= min(s["depth"] for s in sts + [st_ref]) and all(
+            s[k][agree] == st_ref[k][agree] for s in sts for k in keys):
+        agree += 1
+    for k in keys:
+        assert st[k][:agree] == st_ref[k][:agree], (k, agree)
+    assert agree >= 6 and abs(st["depth"] - st_ref["depth"]) <= 2
+    pg, vg = p.cpu().numpy(), v.cpu().numpy()
+    rp, rv = envelope_ratio(pg, vg, pr, vr, env_p, env_v)
+    e0 = oracle.diagnostics(pos, vel, mass)["E"]
+    de_gpu = oracle.diagnostics(pg, vg, mass)["E"] / e0 - 1
+    de_ref = oracle.diagnostics(pr, vr, mass)["E"] / e0 - 1
+    with capsys.disabled():
+        print(f"\n[hhs thermal n={n}] levels identical down to {agree - 1} of {st_ref['depth']} "
+              f"(gpu depth {st['depth']}); envelope ratio x {rp:.3f}, v {rv:.3f}; dE/E gpu {de_gpu:.2e} oracle {de_ref:.2e}")
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, vg, vr) <= 1.0
+    assert abs(de_gpu) <= 2 * abs(de_ref) + 1e-12
 
 
 @pytest.mark.parametrize("n", [150, 700, 1024])
 def test_subtree_kernel_one_cta_and_cluster_agree_bitwise(fr, n):
     """The device-resident subtree kernel on one CTA and on a thread-block cluster of replicas
-    (large sweeps shared out by sinks) must give the same bits: a sink's sum is formed by the same
-    lanes in the same order either way... as long as the lane split is the same, so compare to
-    rounding, and the bookkeeping exactly."""
-    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    (large sweeps shared out by sinks) form a sink's sum with a different lane split, so the two
+    agree to rounding, not bitwise; the bookkeeping must be identical (config 5's hardness, e <= 0.1
+    so that the level sets do not depend on the last bit)."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
     fr.set_params(eta_ff=0.2, eta_fb=0.2)
     out = []
     for one_cta in (1, 0):
@@ -302,7 +519,8 @@ def test_subtree_kernel_one_cta_and_cluster_agree_bitwise(fr, n):
         out.append((st, p.cpu().numpy(), v.cpu().numpy()))
     fr.set_tuning(0, 0, -1, 0)
     assert out[0][0] == out[1][0]
-    assert np.abs(out[0][1] - out[1][1]).max() < 1e-12 and np.abs(out[0][2] - out[1][2]).max() < 1e-10
+    assert out[0][0]["depth"] >= 12
+    assert np.abs(out[0][1] - out[1][1]).max() < 1e-8 and np.abs(out[0][2] - out[1][2]).max() < 1e-3
 
 
 def test_hhs_tiny_systems_and_depth_limit(fr, oracle):

@@ -9,7 +9,8 @@ import pytest
 import torch
 
 import frost_inputs as fi
-from test_gpu_parity import TOL_TAU, check_forces, dev
+from test_gpu_parity import (TOL_TAU, check_forces, dev, envelope_ratio, momentum_change,
+                             oracle_hhs_with_envelope)
 
 pytestmark = pytest.mark.gpu
 
@@ -34,12 +35,10 @@ def test_self_forces_symmetric(frs, oracle, n, mib):
 
 
 def test_self_forces_symmetric_unequal_masses_softened_scaled_G(frs, oracle):
-    # (binaries no harder than 1e-3: a distant particle's g sums the huge, nearly cancelling terms of
-    # both members of a hard binary, and plain fp64 summation -- one-sided or symmetric -- then loses
-    # 1e-16 x the condition number of that sum)
-    pos, vel, mass, _ = fi.star_cluster(4096, 4, a_lo=1e-3, a_hi=1e-2)
-    check_forces(frs, oracle, pos, mass)                       # central mass at the origin meets the padding
-    check_forces(frs, oracle, pos, mass, G=6.674e-3, eps2=1e-4)
+    # config 5's recipe at its default hardness: g through the forward-error gate of reading 22
+    pos, vel, mass, _ = fi.star_cluster(4096, 4)
+    check_forces(frs, oracle, pos, mass, forward_gate=True)    # central mass at the origin meets the padding
+    check_forces(frs, oracle, pos, mass, G=6.674e-3, eps2=1e-4, forward_gate=True)
 
 
 def test_gradient_only_on_given_accelerations(frs, oracle):
@@ -101,23 +100,26 @@ def test_timesteps_symmetric_on_subset(frs, oracle):
 
 @pytest.mark.parametrize("small", [0, 100])
 def test_hhs_step_symmetric_matches_oracle(frs, oracle, small):
-    """A whole HHS-FSI step (reduced-N replica of config 5) with every streamed sweep -- self,
-    mutual slow/fast and time step -- forced through the symmetric kernels."""
+    """A whole HHS-FSI step (reduced-N replica of config 5 at full hardness, e <= 0.1; top step
+    2^-11 so that the host-driven recursion stays at ~1e4 entries) with every streamed sweep --
+    self, mutual slow/fast and time step -- forced through the symmetric kernels."""
     n = 3000
-    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
+    dt = 2.0 ** -11
     frs.set_params(eta_ff=0.2, eta_fb=0.2)
     frs.set_tuning(0, 0, small)
-    pr, vr = pos.copy(), vel.copy()
-    st_ref = oracle.hhs_step(pr, vr, mass, 1.0 / 256)
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt)
+    assert all(s == st_ref for s in sts)
     p, v = dev(pos), dev(vel)
     try:
-        st = frs.hhs_step(p, v, dev(mass), 1.0 / 256)
+        st = frs.hhs_step(p, v, dev(mass), dt)
     finally:
         frs.set_tuning(0, 0, -1)
-    assert st == st_ref
+    assert st == st_ref and st["depth"] >= 10
     pg, vg = p.cpu().numpy(), v.cpu().numpy()
-    assert np.abs(pg - pr).max() < 1e-10 and np.abs(vg - vr).max() < 1e-8 * np.abs(vr).max()
-    assert np.abs((mass * vg).sum(1) - (mass * vel).sum(1)).max() < 1e-16
+    rp, rv = envelope_ratio(pg, vg, pr, vr, env_p, env_v)
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, vg, vr) <= 1.0
 
 
 @pytest.mark.parametrize("world", [2, 3])
@@ -149,6 +151,66 @@ def test_pair_sharded_shares_add_up(frs, oracle, world):
     with pytest.raises(frost.FrostError):
         frs.forces(p, m, flags=frost.ACC | frost.GRAD)
     frs.set_shard(0, 1)
+
+
+@pytest.mark.parametrize("n,mode,world", [(3000, 0, 2), (3000, 1, 3), (9000, 1, 2), (9000, 0, 4)])
+def test_sharded_contract_is_path_independent(frs, oracle, n, mode, world):
+    """frost_set_shard on sweeps the ONE-SIDED kernels serve (n below the symmetric threshold in auto
+    mode 0, or mode 1 = never symmetric): every rank sweeps its block of the sink list and zeroes the
+    rest, so adding the ranks' outputs gives the complete sums exactly as on the symmetric path --
+    self, subset <- all, and mutual sweeps; ACC|GRAD in one call and ACCUMULATE are refused, and
+    frost_fsi_step / frost_hhs_step refuse to run on a sharded context before touching anything."""
+    import paper_2011_14984_b200 as frost
+    pos, vel, mass = fi.plummer(n, 21)
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    frs.set_symmetric(mode, 0)
+    rng = np.random.default_rng(5)
+    perm = rng.permutation(n).astype(np.int32)
+    A, B = np.sort(perm[: n // 5]), np.sort(perm[n // 5: n // 5 + 700])
+    cases = [(None, None, 0), (A, None, 0), (A, B, frost.MUTUAL)]
+    try:
+        for I, J, extra in cases:
+            dI = None if I is None else dev(I); dJ = None if J is None else dev(J)
+            frs.set_shard(0, 1)
+            a_one = torch.full_like(p, 3.0); g_one = torch.full_like(p, 5.0)
+            frs.forces(p, m, dI, dJ, out_acc=a_one, flags=frost.ACC | extra)
+            frs.forces(p, m, dI, dJ, out_acc=a_one, out_grad=g_one, flags=frost.GRAD | extra)
+            acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+            for r in range(world):
+                frs.set_shard(r, world)
+                part = torch.full_like(p, 3.0)
+                frs.forces(p, m, dI, dJ, out_acc=part, flags=frost.ACC | extra)
+                acc += part
+            swept = np.arange(n) if I is None else (I if not extra else np.concatenate([I, J]))
+            sw = dev(swept).long()
+            rest = torch.ones(n, dtype=torch.bool, device="cuda"); rest[sw] = False
+            assert (acc[:, rest] == 3.0 * world).all()                 # untouched outside the swept sets
+            full = a_one.clone(); full[:, sw] = acc[:, sw]
+            for r in range(world):
+                frs.set_shard(r, world)
+                part = torch.full_like(p, 5.0)
+                frs.forces(p, m, dI, dJ, out_acc=full, out_grad=part, flags=frost.GRAD | extra)
+                grad += part
+            na = a_one[:, sw].norm(dim=0); ng = g_one[:, sw].norm(dim=0)
+            assert ((acc - a_one)[:, sw].abs().max(0).values / na).max() < 1e-13
+            assert ((grad - g_one)[:, sw].abs().max(0).values / ng).max() < 1e-10
+            if mode == 1 or n < 6000:       # one-sided: each sink's sum comes from one rank, same bits
+                assert torch.equal(acc[:, sw], a_one[:, sw])
+        frs.set_shard(1, world)
+        with pytest.raises(frost.FrostError):
+            frs.forces(p, m, flags=frost.ACC | frost.GRAD)
+        with pytest.raises(frost.FrostError):
+            frs.forces(p, m, flags=frost.ACC | frost.ACCUMULATE)
+        p0, v0 = p.clone(), v.clone()
+        for call in (lambda: frs.fsi_step(p, v, m, 1e-3), lambda: frs.fsi_steps(p, v, m, 1e-3, 2),
+                     lambda: frs.hhs_step(p, v, m, 1e-3)):
+            with pytest.raises(frost.FrostError):
+                call()
+        torch.cuda.synchronize()
+        assert torch.equal(p, p0) and torch.equal(v, v0)
+    finally:
+        frs.set_shard(0, 1)
+        frs.set_symmetric(2, 0)
 
 
 def test_symmetric_and_one_sided_sweeps_agree_on_random_shapes(frs):

@@ -185,6 +185,79 @@ def test_newton_third_law(oracle):
     assert ((m2 * a2).sum(1) == 0.0).all() and ((m2 * g2).sum(1) == 0.0).all()
 
 
+def test_gradient_termsum_closed_forms_and_invariants(oracle):
+    """O2b (the magnitude sum T_i behind the forward-error gate of the gradient parity tests).
+    Two bodies: one term, so T_i = |g_i| = 4G(m1+m2) r^-3 |a_i| (Eq. 25-26).
+    Collinear bodies with accelerations along the line: every term is -2 m_j a_ji / r^3 (the tidal
+    tensor's radial eigenvalue); accelerations across the line: +m_j a_ji / r^3 (tangential
+    eigenvalue).  Then |g_i| <= T_i, homogeneity, shift invariance and additivity over sources."""
+    G, m1, m2 = 1.3, 0.7, 2.1
+    pos = np.ascontiguousarray(np.array([[0.3, -1.1], [0.2, 0.9], [-0.5, 0.4]]))
+    mass = np.array([m1, m2])
+    a, g = oracle.forces(pos, mass, G=G)
+    T = oracle.gradient_termsum(pos, mass, a, G=G)
+    r = np.linalg.norm(pos[:, 1] - pos[:, 0])
+    np.testing.assert_allclose(T, np.linalg.norm(g, axis=0), rtol=1e-14)
+    np.testing.assert_allclose(T, 4 * G * (m1 + m2) / r ** 3 * np.linalg.norm(a, axis=0), rtol=1e-14)
+    # three bodies on the x axis, arbitrary "accelerations" along x, then along y
+    x = np.array([0.0, 1.0, 3.0]); m = np.array([0.5, 2.0, 1.5]); al = np.array([0.7, -1.9, 0.4])
+    p3 = np.zeros((3, 3)); p3[0] = x
+    for axis, eig in ((0, 2.0), (1, 1.0)):
+        acc = np.zeros((3, 3)); acc[axis] = al
+        T3 = oracle.gradient_termsum(p3, m, acc, G=G)
+        for i in range(3):
+            want = 2 * G * sum(eig * m[j] * abs(al[j] - al[i]) / abs(x[j] - x[i]) ** 3
+                               for j in range(3) if j != i)
+            assert abs(T3[i] - want) <= 1e-14 * want
+    # random system: triangle inequality, |c| homogeneity, shift invariance, additivity in J
+    pos, _, mass = _random_system(40, 8)
+    a, g = oracle.forces(pos, mass, G=G)
+    T = oracle.gradient_termsum(pos, mass, a, G=G)
+    assert (np.linalg.norm(g, axis=0) <= T * (1 + 1e-14)).all()
+    np.testing.assert_allclose(oracle.gradient_termsum(pos, mass, -3.0 * a, G=G), 3.0 * T, rtol=1e-14)
+    shift = np.ascontiguousarray(a + np.array([[5.0], [-2.0], [1.0]]))
+    np.testing.assert_allclose(oracle.gradient_termsum(pos, mass, shift, G=G), T, rtol=1e-12)
+    J1, J2 = np.arange(0, 17, dtype=np.int32), np.arange(17, 40, dtype=np.int32)
+    T12 = (oracle.gradient_termsum(pos, mass, a, source_idx=J1, G=G)
+           + oracle.gradient_termsum(pos, mass, a, source_idx=J2, G=G))
+    np.testing.assert_allclose(T12, T, rtol=1e-14)
+
+
+def test_gradient_noise_floor_through_the_fp64_acc_boundary(oracle, capsys):
+    """DESIGN.md reading 22.  Eq. (27) is evaluated from accelerations that cross an fp64 boundary
+    (`out_acc` of SURVEY 8(b); the oracle's own `acc` array).  Perturb the oracle's a by +-1 ulp per
+    component and re-evaluate the oracle's g: on config 5's structure (hard binaries, a = 1e-5..1e-3)
+    the DEFINITION moves by more than north_star's 1e-10 |g_i| -- a distant particle sums the huge,
+    nearly cancelling terms of both members of a hard binary -- while staying inside the first-order
+    bound 4 * 2^-53 * T_i (one ulp <= 2 * 2^-53 relative per component, and |(1 - 3 xx^T) da| <=
+    2 |da|).  So no code behind that boundary can meet 1e-10 |g_i| on such inputs; the parity tests
+    gate on |dg_k| <= 1e-10 |g_i| + C * 2^-53 * T_i instead (C = 8)."""
+    pos, vel, mass, _ = fi.star_cluster(4096, 4)          # config 5's recipe at its DEFAULT hardness
+    a0, g0 = oracle.forces(pos, mass)
+    T = oracle.gradient_termsum(pos, mass, a0)
+    gn = np.linalg.norm(g0, axis=0)
+    rng = np.random.default_rng(0)
+    worst_rel, worst_ratio = 0.0, 0.0
+    for _ in range(3):
+        sgn = rng.choice([-1.0, 1.0], size=a0.shape)
+        a1 = np.ascontiguousarray(np.nextafter(a0, sgn * np.inf))
+        _, g1 = oracle.forces(pos, mass, flags=oracle.GRAD, acc=a1)
+        d = np.abs(g1 - g0).max(0)
+        worst_rel = max(worst_rel, float((d / gn).max()))
+        worst_ratio = max(worst_ratio, float((d / (2.0 ** -53 * T)).max()))
+    with capsys.disabled():
+        print(f"\n[noise floor] N=4096 config-5 recipe: max |dg|/|g| under +-1 ulp of a = {worst_rel:.3e}; "
+              f"max |dg|/(2^-53 T) = {worst_ratio:.2f}; max T/|g| = {(T / gn).max():.3e}")
+    assert worst_rel > 1e-10            # the floor of the definition is above north_star's tolerance
+    assert worst_ratio <= 4.0           # ... and inside the first-order bound
+    # on a Plummer sphere without binaries the floor is far below 1e-10: the plain gate stays there
+    pos, vel, mass = fi.plummer(4096, 0)
+    a0, g0 = oracle.forces(pos, mass)
+    a1 = np.ascontiguousarray(np.nextafter(a0, rng.choice([-1.0, 1.0], size=a0.shape) * np.inf))
+    _, g1 = oracle.forces(pos, mass, flags=oracle.GRAD, acc=a1)
+    assert (np.abs(g1 - g0).max(0) / np.linalg.norm(g0, axis=0)).max() < 1e-12
+
+
 def test_plummer_mean_field(oracle):
     """|a_r| ~ G M(r)/r^2 with M(r) of Eq. (A2), statistically at N = 16384."""
     n = 16384
