@@ -315,7 +315,7 @@ def test_fsi_steps_equal_repeated_fsi_step_bitwise(fr, n):
 ENV_K = 8.0          # GPU-vs-oracle deviation allowed, in units of the oracle's own +-1-ulp envelope
 
 
-def oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, trials=3, seed=0, **kw):
+def oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, trials=3, seed=0, keep_states=False, **kw):
     """The oracle's HHS-FSI step plus its own sensitivity to the last bit of its inputs: the step is
     repeated from positions and velocities moved by +-1 ulp per component (random signs, seeded).
     Returns (pos_ref, vel_ref, stats_ref, env_pos[n], env_vel[n], stats_of_every_trial).
@@ -333,15 +333,19 @@ def oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, trials=3, seed=0, **kw)
         pr, vr = pos.copy(), vel.copy()
         st = oracle.hhs_step(pr, vr, mass, dt, **kw)
         rng = np.random.default_rng(seed)
-        env_p, env_v, sts = np.zeros(n), np.zeros(n), []
+        env_p, env_v, sts, states = np.zeros(n), np.zeros(n), [], []
         for _ in range(trials):
             pp = np.ascontiguousarray(np.nextafter(pos, rng.choice([-1.0, 1.0], size=pos.shape) * np.inf))
             vv = np.ascontiguousarray(np.nextafter(vel, rng.choice([-1.0, 1.0], size=vel.shape) * np.inf))
             sts.append(oracle.hhs_step(pp, vv, mass, dt, **kw))
             env_p = np.maximum(env_p, np.abs(pp - pr).max(0))
             env_v = np.maximum(env_v, np.abs(vv - vr).max(0))
+            if keep_states:
+                states.append((pp, vv))
     finally:
         oracle.set_num_threads(os.cpu_count() or 1)
+    if keep_states:
+        return pr, vr, st, env_p, env_v, sts, states
     return pr, vr, st, env_p, env_v, sts
 
 
@@ -469,12 +473,16 @@ def test_hhs_step_thermal_binaries_unique_part_and_validity(fr, oracle, n, small
     one on which the oracle's trials disagree must be IDENTICAL, and every particle must lie inside
     ENV_K x the oracle's envelope (which is ~1e-16 for everything but the hard binaries) -- and that
     the rest is valid: the structural invariants of Alg. 3's bookkeeping, momentum at rounding
-    level, energy error of the oracle's size."""
+    level, energy error of the oracle's size -- the oracle's own dE/E moves by up to 10x between its
+    +-1-ulp trials here (2.3e-5 .. 2.1e-4 at n = 256: the truncation error of the e ~ 0.99 binaries
+    depends on where along the orbit a pivot is crossed), so "the oracle's size" is the largest
+    |dE/E| over the oracle's trials, and the GPU is held to twice that."""
     pos, vel, mass, pairs = fi.star_cluster(n, 4)
     dt = 2.0 ** -8
     fr.set_params(eta_ff=0.2, eta_fb=0.2)
     fr.set_tuning(0, 0, small)
-    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt)
+    pr, vr, st_ref, env_p, env_v, sts, states = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt,
+                                                                         keep_states=True)
     p, v = dev(pos), dev(vel)
     try:
         st = fr.hhs_step(p, v, dev(mass), dt)
@@ -495,12 +503,14 @@ def test_hhs_step_thermal_binaries_unique_part_and_validity(fr, oracle, n, small
     e0 = oracle.diagnostics(pos, vel, mass)["E"]
     de_gpu = oracle.diagnostics(pg, vg, mass)["E"] / e0 - 1
     de_ref = oracle.diagnostics(pr, vr, mass)["E"] / e0 - 1
+    de_size = max([abs(de_ref)] + [abs(oracle.diagnostics(pp, vv, mass)["E"] / e0 - 1) for pp, vv in states])
     with capsys.disabled():
         print(f"\n[hhs thermal n={n}] levels identical down to {agree - 1} of {st_ref['depth']} "
-              f"(gpu depth {st['depth']}); envelope ratio x {rp:.3f}, v {rv:.3f}; dE/E gpu {de_gpu:.2e} oracle {de_ref:.2e}")
+              f"(gpu depth {st['depth']}); envelope ratio x {rp:.3f}, v {rv:.3f}; dE/E gpu {de_gpu:.2e} oracle {de_ref:.2e} "
+              f"(largest over its +-1-ulp trials {de_size:.2e})")
     assert rp <= 1.0 and rv <= 1.0, (rp, rv)
     assert momentum_change(mass, vel, vg, vr) <= 1.0
-    assert abs(de_gpu) <= 2 * abs(de_ref) + 1e-12
+    assert abs(de_gpu) <= 2 * de_size + 1e-12
 
 
 @pytest.mark.parametrize("n", [150, 700, 1024])
