@@ -586,6 +586,79 @@ def test_solar_system_run_on_device(fr, oracle):
     assert errs[0] < 1e-6 and errs[1] < errs[0] / 20
 
 
+FIG5_ETAS = (0.032, 0.064, 0.128, 0.256, 0.512, 1.024)
+
+
+def test_solar_system_fig5_eta_sweep_order_four_and_fsi_gap(fr, oracle, capsys):
+    """SURVEY 8(f).2 / Fig. 5 (Tables A1/A2): Sun + 4 giant planets
+    for 45 top steps of 8192 days (1009 yr; the paper runs 1000 yr) at six accuracy parameters
+    eta = 0.032 ... 1.024 (the truncation-dominated range: the paper sees round-off below 0.004).
+      * HHS-FSI (frost_hhs_step, individual steps): max |dE/E| over the run follows eta^4
+        (PAPER.md:664, 672): every doubling of eta multiplies it by 10..50 (16 = fourth order; the
+        oracle gives 14.5-16.7 at both ends of the range and 30-38 between eta = 0.064 and 0.256,
+        whatever the top step: DESIGN.md section 10), least-squares slope 4 +- 0.5 (oracle: 4.4);
+      * the same span with all five bodies forced to the fastest level -- frost_fsi_steps at the
+        smallest sub-step the hierarchy reached -- has a smaller error at every eta (the paper:
+        "approximately an order of magnitude", PAPER.md:672);
+      * |dP| < 1e-15 and |dL/L| < 1e-13 in both arms (PAPER.md:674);
+      * the device run's final energy equals the oracle's run of the same steps to 1e-11 relative.
+    The energy is read by frost_diagnostics after every top step; nothing else crosses the host."""
+    dt_top, n_top = 8192.0, 45
+    rows = []
+    for eta in FIG5_ETAS:
+        pos, vel, mass, G = fi.solar_system()
+        vel = np.ascontiguousarray(vel - (vel * mass).sum(1, keepdims=True) / mass.sum())
+        fr.set_params(G=G, eta_ff=eta, eta_fb=eta)
+        p, v, m = dev(pos), dev(vel), dev(mass)
+        pr, vr = pos.copy(), vel.copy()
+        d0 = fr.diagnostics(p, v, m)
+        L0 = np.array(d0["L"])
+        de_hhs, depth = 0.0, 0
+        for _ in range(n_top):
+            st = fr.hhs_step(p, v, m, dt_top)
+            oracle.hhs_step(pr, vr, mass, dt_top, G=G, eta_ff=eta, eta_fb=eta)
+            depth = max(depth, st["depth"])
+            de_hhs = max(de_hhs, abs(fr.diagnostics(p, v, m)["E"] / d0["E"] - 1))
+        d1 = fr.diagnostics(p, v, m)
+        e_ref = oracle.diagnostics(pr, vr, mass, G=G)["E"]
+        assert abs(d1["E"] - e_ref) <= 1e-11 * abs(e_ref), (eta, d1["E"], e_ref)
+        dp_hhs = np.abs(np.array(d1["P"]) - np.array(d0["P"])).max()
+        dl_hhs = np.linalg.norm(np.array(d1["L"]) - L0) / np.linalg.norm(L0)
+        # all five bodies on the fastest level: fsi with the step of the deepest level's fsi(S, tau/2)
+        dt_min = dt_top * 2.0 ** -(depth + 1)
+        per_top = int(round(dt_top / dt_min))
+        p, v = dev(pos), dev(vel)
+        de_fsi = 0.0
+        for _ in range(n_top):
+            fr.fsi_steps(p, v, m, dt_min, per_top)
+            de_fsi = max(de_fsi, abs(fr.diagnostics(p, v, m)["E"] / d0["E"] - 1))
+        d2 = fr.diagnostics(p, v, m)
+        dp_fsi = np.abs(np.array(d2["P"]) - np.array(d0["P"])).max()
+        dl_fsi = np.linalg.norm(np.array(d2["L"]) - L0) / np.linalg.norm(L0)
+        rows.append((eta, depth, de_hhs, de_fsi, dp_hhs, dl_hhs, dp_fsi, dl_fsi))
+    fr.set_params()
+    slope = np.polyfit(np.log([r[0] for r in rows]), np.log([r[2] for r in rows]), 1)[0]
+    with capsys.disabled():
+        print("\n[Fig. 5] eta  depth  max|dE/E| HHS-FSI   FSI(fastest level)  ratio   |dP| HHS  |dL/L| HHS")
+        for r in rows:
+            print(f"[Fig. 5] {r[0]:5.3f} {r[1]:3d}   {r[2]:.3e}        {r[3]:.3e}         {r[2] / r[3]:6.1f}  "
+                  f"{r[4]:.1e}  {r[5]:.1e}")
+        print(f"[Fig. 5] log-log slope of the HHS-FSI energy error: {slope:.2f}")
+    slope_fsi = np.polyfit(np.log([r[0] for r in rows]), np.log([r[3] for r in rows]), 1)[0]
+    ratios = [rows[k + 1][2] / rows[k][2] for k in range(len(rows) - 1)]
+    with capsys.disabled():
+        print(f"[Fig. 5] error growth per doubling of eta: {' '.join(f'{x:.1f}' for x in ratios)}; "
+              f"slope of the FSI arm {slope_fsi:.2f}")
+    assert abs(slope - 4.0) <= 0.5, slope
+    assert abs(slope_fsi - 4.0) <= 0.1, slope_fsi
+    assert all(10.0 <= x <= 50.0 for x in ratios), ratios
+    for eta, depth, de_hhs, de_fsi, dp_hhs, dl_hhs, dp_fsi, dl_fsi in rows:
+        assert depth >= 2
+        assert de_fsi < de_hhs, (eta, de_fsi, de_hhs)
+        assert dp_hhs < 1e-15 and dp_fsi < 1e-15, (eta, dp_hhs, dp_fsi)
+        assert dl_hhs < 1e-13 and dl_fsi < 1e-13, (eta, dl_hhs, dl_fsi)
+
+
 def test_hhs_multi_step_run_conserves_momentum_to_roundoff(fr):
     """The paper's headline property on the device: eight HHS-FSI
     steps of a 6000-star cluster with a central mass and binaries down to a = 1e-4 (depth >= 10);

@@ -8,6 +8,7 @@ two-body flow; the operator sequences to their convergence order against the Kep
 Citations are PAPER.md line numbers.
 """
 import math
+import os
 
 import numpy as np
 import pytest
@@ -555,3 +556,42 @@ def test_small_plummer_run_conserves_as_the_paper_reports(oracle):
         assert np.abs(d1["P"] - d0["P"]).max() < 1e-16
         assert np.linalg.norm(d1["L"] - d0["L"]) < 1e-14
     assert res[1] < 1e-8 and res[1] < res[0] / 6
+
+
+def test_hhs_solar_system_fig5_energy_error_scales_as_eta4(oracle):
+    """Fig. 5 with the oracle alone: Sun + 4 giant planets (Tables A1/A2), 45 top
+    steps of 8192 days (1009 yr), eta = 0.064 ... 1.024.  max |dE/E| of HHS-FSI grows by a factor
+    10..50 per doubling of eta (16 = fourth order) with a least-squares slope of 4 +- 0.5; the same
+    span with all five bodies on the fastest level (plain FSI at the hierarchy's smallest sub-step)
+    is fourth order to +-0.1 and more accurate at every eta ("approximately an order
+    of magnitude"); |dP| < 1e-15."""
+    oracle.set_num_threads(1)
+    try:
+        dt_top, n_top, rows = 8192.0, 45, []
+        for eta in (0.064, 0.128, 0.256, 0.512, 1.024):
+            pos, vel, mass, G = fi.solar_system()
+            vel = np.ascontiguousarray(vel - (vel * mass).sum(1, keepdims=True) / mass.sum())
+            e0 = oracle.diagnostics(pos, vel, mass, G=G)["E"]
+            p0 = (mass * vel).sum(1)
+            pr, vr, de, depth = pos.copy(), vel.copy(), 0.0, 0
+            for _ in range(n_top):
+                st = oracle.hhs_step(pr, vr, mass, dt_top, G=G, eta_ff=eta, eta_fb=eta)
+                depth = max(depth, st["depth"])
+                de = max(de, abs(oracle.diagnostics(pr, vr, mass, G=G)["E"] / e0 - 1))
+            assert np.abs((mass * vr).sum(1) - p0).max() < 1e-15
+            dt_min = dt_top * 2.0 ** -(depth + 1)
+            pf, vf, de_f = pos.copy(), vel.copy(), 0.0
+            for _ in range(n_top):
+                for _ in range(int(round(dt_top / dt_min))):
+                    oracle.fsi_step(pf, vf, mass, dt_min, G=G)
+                de_f = max(de_f, abs(oracle.diagnostics(pf, vf, mass, G=G)["E"] / e0 - 1))
+            rows.append((eta, de, de_f))
+    finally:
+        oracle.set_num_threads(os.cpu_count() or 1)
+    le = np.log([r[0] for r in rows])
+    slope = np.polyfit(le, np.log([r[1] for r in rows]), 1)[0]
+    slope_f = np.polyfit(le, np.log([r[2] for r in rows]), 1)[0]
+    ratios = [rows[k + 1][1] / rows[k][1] for k in range(len(rows) - 1)]
+    assert abs(slope - 4.0) <= 0.5 and abs(slope_f - 4.0) <= 0.1, (slope, slope_f)
+    assert all(10.0 <= x <= 50.0 for x in ratios), ratios
+    assert all(r[2] < r[1] for r in rows), rows
