@@ -32,6 +32,11 @@
  *   O5 oracle_fsi_step     : 4th-order convergence against the Kepler closed form, time reversal.
  *   O6 oracle_hhs_step     : 4th-order convergence with a frozen partition on a star+planets
  *                            system, momentum at roundoff, five-body Solar system (Tables A1/A2).
+ *   O6s split fast levels  : (PAPER.md:759 names the idea only; the definition is DESIGN.md reading
+ *                            24) bit-for-bit Alg. 3 when F is one component; components against an
+ *                            independent graph routine; 4th-order convergence with a frozen
+ *                            partition into components; momentum at roundoff; energy error of the
+ *                            size of Alg. 3's on a cluster with binaries.
  *   O7 oracle_diagnostics  : textbook definitions (Eq. 23); used by the pins.
  *
  * Array convention (same as include/frost.h, restated independently): positions, velocities,
@@ -68,6 +73,8 @@ typedef struct {
     int64_t pairs_newton;                   /* ordered pairs swept by Eq. 24 / 42 */
     int64_t pairs_gradient;                 /* ordered pairs swept by Eq. 27 / 43 / 44 */
     int64_t pairs_timestep;                 /* ordered pairs swept by Eq. 49-54 */
+    int64_t n_comp[ORACLE_MAX_LEVELS];      /* sum over those entries of the number of fast components
+                                               recursed into (Alg. 3 itself: 1 per entry with |F| > 0) */
 } oracle_hhs_stats;
 
 int oracle_num_threads(void) {
@@ -427,6 +434,151 @@ int oracle_fsi_step(int n, int ld, double *pos, double *vel, const double *mass,
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * O6s.  Spatial splitting of a fast level.  The paper only names it: "the further
+ * spatial Hamiltonian splitting of the individual hierarchy levels into field stars, binaries and
+ * multiple star systems" (primordial binaries are left to future work).
+ * The definition used here (reading 24) applies the rule the paper already uses for
+ * particles -- "whatever evolves slower than tau_pivot is integrated with tau_pivot" (Eq. 29,
+ * PAPER.md:260-266) -- to PAIRS:
+ *   * the symmetrised pair step of Eq. (49)-(54) is c_ij = min(tau_ff_sym, tau_fb_sym), and
+ *     tau_i = min_j c_ij.  The pair (i, j) of one level's set is FAST iff
+ *     c_ij < tau_pivot.  Slow particles (tau_i >= tau_pivot) are exactly those without a fast pair;
+ *   * the fast pairs are the edges of a graph on F; its connected components C_1..C_m are mutually
+ *     coupled by slow pairs only, so H_F = sum_c H_{C_c} + sum_{c<c'} U_{cc'} and the second sum is
+ *     moved out of the recursion into the inter-level kick of Eq. (41): the kicked pair set becomes
+ *         P = { (i, j) in set^2 : not both slow, not in the same component }
+ *     (for m = 1 this is Alg. 3's S x F both ways), with the gradient force of Eq. (43)-(44)
+ *     evaluated on P with the accelerations of P ("the interaction potential");
+ *   * every component is then advanced on its own by hhs_fsi(C_c, tau/2), where the rule applies
+ *     again.
+ * ------------------------------------------------------------------------------------------- */
+
+/* Component label of every member of `set`: the smallest member index of its component in the
+ * graph whose edges are the fast pairs c_ij < tau_pivot; -1 for a member without a fast pair.
+ * Plain relabelling to a fixed point over the explicit edge list.  label is indexed globally. */
+int oracle_components(int n, int ld, const double *pos, const double *vel, const double *mass,
+                      const int32_t *set, int n_set, double G, double eta_ff, double eta_fb,
+                      int eta_in_q, double tau_pivot, int32_t *label) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !label) return ORACLE_EINVAL;
+    if (!set) n_set = n;
+    size_t cap = 1024, ne = 0;
+    int32_t *ei = (int32_t *)malloc(cap * sizeof(int32_t)), *ej = (int32_t *)malloc(cap * sizeof(int32_t));
+    if (!ei || !ej) { free(ei); free(ej); return ORACLE_ENOMEM; }
+    for (int a = 0; a < n_set; ++a) label[pick(set, a)] = -1;
+    for (int a = 0; a < n_set; ++a) {
+        const int i = pick(set, a);
+        const double xi[3] = {pos[i], pos[ld + i], pos[2 * ld + i]};
+        const double vi[3] = {vel[i], vel[ld + i], vel[2 * ld + i]};
+        for (int b = a + 1; b < n_set; ++b) {
+            const int j = pick(set, b);
+            const double xj[3] = {pos[j], pos[ld + j], pos[2 * ld + j]};
+            const double vj[3] = {vel[j], vel[ld + j], vel[2 * ld + j]};
+            double c[2];
+            oracle_pair_timestep(xi, vi, mass[i], xj, vj, mass[j], G, eta_ff, eta_fb, eta_in_q, c);
+            if (c[0] < tau_pivot || c[1] < tau_pivot) {
+                if (ne == cap) {
+                    cap *= 2;
+                    int32_t *ni = (int32_t *)realloc(ei, cap * sizeof(int32_t));
+                    int32_t *nj = ni ? (int32_t *)realloc(ej, cap * sizeof(int32_t)) : NULL;
+                    if (!ni || !nj) { free(ni ? ni : ei); free(nj ? nj : ej); return ORACLE_ENOMEM; }
+                    ei = ni; ej = nj;
+                }
+                ei[ne] = i; ej[ne] = j; ++ne;
+                if (label[i] < 0) label[i] = i;
+                if (label[j] < 0) label[j] = j;
+            }
+        }
+    }
+    for (int changed = 1; changed;) {
+        changed = 0;
+        for (size_t k = 0; k < ne; ++k) {
+            const int32_t li = label[ei[k]], lj = label[ej[k]];
+            if (li < lj) { label[ej[k]] = li; changed = 1; }
+            else if (lj < li) { label[ei[k]] = lj; changed = 1; }
+        }
+    }
+    free(ei); free(ej);
+    return ORACLE_OK;
+}
+
+/* Eq. (42) on the pair set P of O6s: a_i = G sum_{j in set, label_j != label_i} m_j x_ji / s^3.
+ * (label is -1 for every slow particle, so slow-slow pairs and i = j drop out with the same test.) */
+static void newton_masked(int ld, const double *pos, const double *mass, const int32_t *set,
+                          int n_set, const int32_t *label, double G, double eps2, double *acc) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < n_set; ++a) {
+        const int i = set[a];
+        const ld_t xi = pos[i], yi = pos[ld + i], zi = pos[2 * ld + i];
+        ld_t ax = 0, ay = 0, az = 0;
+        for (int b = 0; b < n_set; ++b) {
+            const int j = set[b];
+            if (label[j] == label[i]) continue;
+            const ld_t dx = (ld_t)pos[j] - xi;
+            const ld_t dy = (ld_t)pos[ld + j] - yi;
+            const ld_t dz = (ld_t)pos[2 * ld + j] - zi;
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) {
+                const ld_t s = sqrtl(s2);
+                const ld_t w = (ld_t)mass[j] / (s2 * s);
+                ax += w * dx;
+                ay += w * dy;
+                az += w * dz;
+            }
+        }
+        acc[i] = (double)((ld_t)G * ax);
+        acc[ld + i] = (double)((ld_t)G * ay);
+        acc[2 * ld + i] = (double)((ld_t)G * az);
+    }
+}
+
+/* Eq. (43)-(44) on the pair set P of O6s, with the accelerations of P. */
+static void gradient_masked(int ld, const double *pos, const double *mass, const int32_t *set,
+                            int n_set, const int32_t *label, double G, double eps2,
+                            const double *acc, double *grad) {
+#pragma omp parallel for schedule(dynamic, 16)
+    for (int a = 0; a < n_set; ++a) {
+        const int i = set[a];
+        const ld_t xi = pos[i], yi = pos[ld + i], zi = pos[2 * ld + i];
+        const ld_t axi = acc[i], ayi = acc[ld + i], azi = acc[2 * ld + i];
+        ld_t gx = 0, gy = 0, gz = 0;
+        for (int b = 0; b < n_set; ++b) {
+            const int j = set[b];
+            if (label[j] == label[i]) continue;
+            const ld_t dx = (ld_t)pos[j] - xi;
+            const ld_t dy = (ld_t)pos[ld + j] - yi;
+            const ld_t dz = (ld_t)pos[2 * ld + j] - zi;
+            const ld_t s2 = dx * dx + dy * dy + dz * dz + (ld_t)eps2;
+            if (s2 > 0) {
+                const ld_t dax = (ld_t)acc[j] - axi;
+                const ld_t day = (ld_t)acc[ld + j] - ayi;
+                const ld_t daz = (ld_t)acc[2 * ld + j] - azi;
+                const ld_t s = sqrtl(s2);
+                const ld_t s5 = s2 * s2 * s;
+                const ld_t xa = dx * dax + dy * day + dz * daz;
+                const ld_t w = (ld_t)mass[j] / s5;
+                gx += w * (s2 * dax - 3 * xa * dx);
+                gy += w * (s2 * day - 3 * xa * dy);
+                gz += w * (s2 * daz - 3 * xa * dz);
+            }
+        }
+        grad[i] = (double)(2 * (ld_t)G * gx);
+        grad[ld + i] = (double)(2 * (ld_t)G * gy);
+        grad[2 * ld + i] = (double)(2 * (ld_t)G * gz);
+    }
+}
+
+/* The masked sweeps as a callable (for the pins): label indexed globally, -1 = slow. */
+int oracle_forces_masked(int n, int ld, const double *pos, const double *mass, const int32_t *set,
+                         int n_set, const int32_t *label, double G, double eps2, double *acc,
+                         double *grad, int flags) {
+    if (n < 0 || ld < n || !pos || !mass || !acc || !label || !set) return ORACLE_EINVAL;
+    if ((flags & ORACLE_GRAD) && !grad) return ORACLE_EINVAL;
+    if (flags & ORACLE_ACC) newton_masked(ld, pos, mass, set, n_set, label, G, eps2, acc);
+    if (flags & ORACLE_GRAD) gradient_masked(ld, pos, mass, set, n_set, label, G, eps2, acc, grad);
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * O6.  HHS-FSI, Eq. (41); Alg. 3, line by line.
  * `frozen_level` (may be NULL): if given, particle i is slow at the first level k with
  * k >= frozen_level[i] instead of by its time-step -- the "frozen partition" used only by the
@@ -440,9 +592,18 @@ typedef struct {
     double G, eps2, eta_ff, eta_fb;
     int eta_in_q, max_depth;
     const int32_t *frozen_level;
+    int split_max;                     /* O6s: entries with |set| <= split_max split F into components */
+    const int32_t *frozen_comp;        /* with frozen_level: the component of particle i (any labels) */
     double *acc, *grad, *tau;
+    int32_t *label;
     oracle_hhs_stats *st;
 } hhs_env;
+
+static int cmp_label_then_index(const void *pa, const void *pb) {
+    const int32_t *a = (const int32_t *)pa, *b = (const int32_t *)pb;      /* {label, index} */
+    if (a[0] != b[0]) return a[0] < b[0] ? -1 : 1;
+    return a[1] < b[1] ? -1 : (a[1] > b[1] ? 1 : 0);
+}
 
 static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_pivot, int level) {
     if (n_set == 0) return ORACLE_OK;                          /* "if set != empty" */
@@ -454,9 +615,10 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
     /* partition (Eq. 29): slow iff tau_i >= tau_pivot; stable order */
     int32_t *S = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_set + 1));
     int32_t *F = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_set + 1));
-    if (!S || !F) {
-        free(S);
-        free(F);
+    int32_t *key = (int32_t *)malloc(sizeof(int32_t) * 2 * (size_t)(n_set + 1));
+    int32_t *cstart = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n_set + 2));
+    if (!S || !F || !key || !cstart) {
+        free(S); free(F); free(key); free(cstart);
         return ORACLE_ENOMEM;
     }
     int nS = 0, nF = 0;
@@ -468,39 +630,83 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
         if (slow) S[nS++] = i;
         else F[nF++] = i;
     }
+    /* O6s: the components of F (members ascending inside a component, components by their smallest
+     * member); one component = F itself when the entry is not split */
+    int m = nF > 0 ? 1 : 0;
+    cstart[0] = 0; cstart[1] = nF;
+    if (e->split_max > 0 && n_set <= e->split_max && nF > 0) {
+        if (e->frozen_level) {
+            for (int a = 0; a < nS; ++a) e->label[S[a]] = -1;
+            for (int a = 0; a < nF; ++a) e->label[F[a]] = e->frozen_comp ? e->frozen_comp[F[a]] : 0;
+        } else {
+            oracle_components(n, ld, e->pos, e->vel, e->mass, set, n_set, e->G, e->eta_ff, e->eta_fb,
+                              e->eta_in_q, tau_pivot, e->label);
+        }
+        for (int a = 0; a < nF; ++a) { key[2 * a] = e->label[F[a]]; key[2 * a + 1] = F[a]; }
+        qsort(key, (size_t)nF, 2 * sizeof(int32_t), cmp_label_then_index);
+        m = 0;
+        for (int a = 0; a < nF; ++a) {
+            F[a] = key[2 * a + 1];
+            if (a == 0 || key[2 * a] != key[2 * a - 2]) cstart[m++] = a;
+        }
+        cstart[m] = nF;
+    }
     oracle_hhs_stats *st = e->st;
     if (st) {
         if (level > st->depth) st->depth = level;
         st->entries[level] += 1;
         st->n_slow[level] += nS;
         st->n_fast[level] += nF;
+        st->n_comp[level] += m;
         st->pairs_timestep += (int64_t)n_set * n_set;
     }
-    const int64_t cross = 2 * (int64_t)nS * nF;
+    /* ordered pairs of P: everything but slow-slow and same-component pairs (m <= 1: 2 |S| |F|) */
+    int64_t cross = (int64_t)n_set * n_set - (int64_t)nS * nS;
+    for (int c = 0; c < m; ++c) cross -= (int64_t)(cstart[c + 1] - cstart[c]) * (cstart[c + 1] - cstart[c]);
     int rc = ORACLE_OK;
     const double h = 0.5 * tau_pivot;
-    /* acc_sf_newton (Eq. 42); kick_sf by tau/6 */
-    oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+    const double kap = tau_pivot * tau_pivot / 48.0;
+    /* acc_sf_newton (Eq. 42) on P; kick_sf by tau/6 */
+    if (m <= 1) oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+    else newton_masked(ld, e->pos, e->mass, set, n_set, e->label, e->G, e->eps2, e->acc);
     oracle_kick(n, ld, e->vel, e->acc, NULL, S, nS, tau_pivot / 6.0, 0.0);
     oracle_kick(n, ld, e->vel, e->acc, NULL, F, nF, tau_pivot / 6.0, 0.0);
-    /* fsi(S, tau/2); hhs_fsi(F, tau/2) */
+    /* fsi(S, tau/2); hhs_fsi(C_c, tau/2) for every component (Alg. 3: hhs_fsi(F, tau/2)) */
     rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
-    if (rc == ORACLE_OK) rc = hhs_recursive(e, F, nF, h, level + 1);
+    for (int c = 0; c < m && rc == ORACLE_OK; ++c)
+        rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
     if (rc == ORACLE_OK) {
         /* acc_sf_gradient (Eq. 43-44) with the inter-level a of Eq. 42; kick_sf by 2 tau/3 with
-         * a~ = a + tau_pivot^2 g / 48 (eps = this level's step, reading 7) */
-        oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, e->grad,
-                      ORACLE_ACC | ORACLE_GRAD | ORACLE_MUTUAL);
-        oracle_kick(n, ld, e->vel, e->acc, e->grad, S, nS, 2.0 * tau_pivot / 3.0, tau_pivot * tau_pivot / 48.0);
-        oracle_kick(n, ld, e->vel, e->acc, e->grad, F, nF, 2.0 * tau_pivot / 3.0, tau_pivot * tau_pivot / 48.0);
-        /* hhs_fsi(F, tau/2); fsi(S, tau/2) */
-        rc = hhs_recursive(e, F, nF, h, level + 1);
+         * a~ = a + tau_pivot^2 g / 48 (eps = this level's step, reading 7).  The recursion
+         * overwrote the labels of F's members: restore this entry's before the masked sweeps. */
+        if (m > 1) {
+            for (int c = 0; c < m; ++c)
+                for (int a = cstart[c]; a < cstart[c + 1]; ++a) e->label[F[a]] = c;
+            for (int a = 0; a < nS; ++a) e->label[S[a]] = -1;
+            newton_masked(ld, e->pos, e->mass, set, n_set, e->label, e->G, e->eps2, e->acc);
+            gradient_masked(ld, e->pos, e->mass, set, n_set, e->label, e->G, e->eps2, e->acc, e->grad);
+        } else {
+            oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, e->grad,
+                          ORACLE_ACC | ORACLE_GRAD | ORACLE_MUTUAL);
+        }
+        oracle_kick(n, ld, e->vel, e->acc, e->grad, S, nS, 2.0 * tau_pivot / 3.0, kap);
+        oracle_kick(n, ld, e->vel, e->acc, e->grad, F, nF, 2.0 * tau_pivot / 3.0, kap);
+        /* hhs_fsi(C_c, tau/2); fsi(S, tau/2) */
+        for (int c = 0; c < m && rc == ORACLE_OK; ++c)
+            rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
     }
     if (rc == ORACLE_OK)
         rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
     if (rc == ORACLE_OK) {
-        /* acc_sf_newton; kick_sf by tau/6 */
-        oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+        /* acc_sf_newton on P; kick_sf by tau/6 */
+        if (m > 1) {
+            for (int c = 0; c < m; ++c)
+                for (int a = cstart[c]; a < cstart[c + 1]; ++a) e->label[F[a]] = c;
+            for (int a = 0; a < nS; ++a) e->label[S[a]] = -1;
+            newton_masked(ld, e->pos, e->mass, set, n_set, e->label, e->G, e->eps2, e->acc);
+        } else {
+            oracle_forces(n, ld, e->pos, e->mass, S, nS, F, nF, e->G, e->eps2, e->acc, NULL, ORACLE_ACC | ORACLE_MUTUAL);
+        }
         oracle_kick(n, ld, e->vel, e->acc, NULL, S, nS, tau_pivot / 6.0, 0.0);
         oracle_kick(n, ld, e->vel, e->acc, NULL, F, nF, tau_pivot / 6.0, 0.0);
         if (st) {
@@ -508,32 +714,42 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
             st->pairs_gradient += cross;
         }
     }
-    free(S);
-    free(F);
+    free(S); free(F); free(key); free(cstart);
+    return rc;
+}
+
+/* split_max = 0: Alg. 3 as printed.  split_max > 0: O6s on every entry with |set| <= split_max. */
+int oracle_hhs_split_step(int n, int ld, double *pos, double *vel, const double *mass, double dt_top,
+                          double G, double eps2, double eta_ff, double eta_fb, int eta_in_q,
+                          int max_depth, const int32_t *frozen_level, int split_max,
+                          const int32_t *frozen_comp, oracle_hhs_stats *stats) {
+    if (n < 0 || ld < n || !pos || !vel || !mass || !(dt_top > 0.0) || split_max < 0) return ORACLE_EINVAL;
+    hhs_env e;
+    e.n = n; e.ld = ld; e.pos = pos; e.vel = vel; e.mass = mass;
+    e.G = G; e.eps2 = eps2; e.eta_ff = eta_ff; e.eta_fb = eta_fb;
+    e.eta_in_q = eta_in_q; e.max_depth = max_depth; e.frozen_level = frozen_level;
+    e.split_max = split_max; e.frozen_comp = frozen_comp;
+    e.acc = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    e.grad = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
+    e.tau = (double *)calloc((size_t)ld + 1, sizeof(double));
+    e.label = (int32_t *)calloc((size_t)ld + 1, sizeof(int32_t));
+    int32_t *all = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n + 1));
+    if (stats) memset(stats, 0, sizeof(*stats));
+    e.st = stats;
+    int rc = ORACLE_ENOMEM;
+    if (e.acc && e.grad && e.tau && e.label && all) {
+        for (int i = 0; i < n; ++i) all[i] = i;
+        rc = hhs_recursive(&e, all, n, dt_top, 0);
+    }
+    free(e.acc); free(e.grad); free(e.tau); free(e.label); free(all);
     return rc;
 }
 
 int oracle_hhs_step(int n, int ld, double *pos, double *vel, const double *mass, double dt_top,
                     double G, double eps2, double eta_ff, double eta_fb, int eta_in_q,
                     int max_depth, const int32_t *frozen_level, oracle_hhs_stats *stats) {
-    if (n < 0 || ld < n || !pos || !vel || !mass || !(dt_top > 0.0)) return ORACLE_EINVAL;
-    hhs_env e;
-    e.n = n; e.ld = ld; e.pos = pos; e.vel = vel; e.mass = mass;
-    e.G = G; e.eps2 = eps2; e.eta_ff = eta_ff; e.eta_fb = eta_fb;
-    e.eta_in_q = eta_in_q; e.max_depth = max_depth; e.frozen_level = frozen_level;
-    e.acc = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
-    e.grad = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
-    e.tau = (double *)calloc((size_t)ld + 1, sizeof(double));
-    int32_t *all = (int32_t *)malloc(sizeof(int32_t) * (size_t)(n + 1));
-    if (stats) memset(stats, 0, sizeof(*stats));
-    e.st = stats;
-    int rc = ORACLE_ENOMEM;
-    if (e.acc && e.grad && e.tau && all) {
-        for (int i = 0; i < n; ++i) all[i] = i;
-        rc = hhs_recursive(&e, all, n, dt_top, 0);
-    }
-    free(e.acc); free(e.grad); free(e.tau); free(all);
-    return rc;
+    return oracle_hhs_split_step(n, ld, pos, vel, mass, dt_top, G, eps2, eta_ff, eta_fb, eta_in_q,
+                                 max_depth, frozen_level, 0, NULL, stats);
 }
 
 /* ---------------------------------------------------------------------------------------------

@@ -22,14 +22,15 @@ class HHSStats(C.Structure):
     _fields_ = [("depth", C.c_int32), ("reserved", C.c_int32),
                 ("entries", C.c_int64 * MAX_LEVELS), ("n_slow", C.c_int64 * MAX_LEVELS),
                 ("n_fast", C.c_int64 * MAX_LEVELS), ("pairs_newton", C.c_int64),
-                ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64)]
+                ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64),
+                ("n_comp", C.c_int64 * MAX_LEVELS)]
 
     def as_dict(self):
         d = self.depth
         return {"depth": d, "entries": list(self.entries[: d + 1]),
                 "n_slow": list(self.n_slow[: d + 1]), "n_fast": list(self.n_fast[: d + 1]),
                 "pairs_newton": self.pairs_newton, "pairs_gradient": self.pairs_gradient,
-                "pairs_timestep": self.pairs_timestep}
+                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1])}
 
 
 def lib():
@@ -178,18 +179,52 @@ def fsi_step(pos, vel, mass, dt, idx=None, G=1.0, eps2=0.0):
 
 
 def hhs_step(pos, vel, mass, dt_top, G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2, eta_in_q=True,
-             max_depth=64, frozen_level=None):
+             max_depth=64, frozen_level=None, split_max=0, frozen_comp=None):
+    """One HHS-FSI step (Alg. 3).  split_max > 0: entries with at most split_max members split
+    their fast set into the connected components of the fast pairs (O6s in frost_oracle.c)."""
     ld = pos.shape[1]
     n = mass.shape[0]
     st = HHSStats()
     fl, _ = _i(frozen_level)
-    rc = lib().oracle_hhs_step(C.c_int(n), C.c_int(ld), _d(pos), _d(vel), _d(mass),
-                               C.c_double(dt_top), C.c_double(G), C.c_double(eps2),
-                               C.c_double(eta_ff), C.c_double(eta_fb),
-                               C.c_int(1 if eta_in_q else 0), C.c_int(max_depth), _ptr(fl),
-                               C.byref(st))
-    _check(rc, "oracle_hhs_step")
+    fc, _ = _i(frozen_comp)
+    rc = lib().oracle_hhs_split_step(C.c_int(n), C.c_int(ld), _d(pos), _d(vel), _d(mass),
+                                     C.c_double(dt_top), C.c_double(G), C.c_double(eps2),
+                                     C.c_double(eta_ff), C.c_double(eta_fb),
+                                     C.c_int(1 if eta_in_q else 0), C.c_int(max_depth), _ptr(fl),
+                                     C.c_int(split_max), _ptr(fc), C.byref(st))
+    _check(rc, "oracle_hhs_split_step")
     return st.as_dict()
+
+
+def components(pos, vel, mass, tau_pivot, idx=None, G=1.0, eta_ff=0.2, eta_fb=0.2, eta_in_q=True):
+    """Component label (smallest member index; -1 = no fast pair) of every member of the level `idx`,
+    shape (ld,), entries outside the level are -2."""
+    ld = pos.shape[1]
+    n = mass.shape[0]
+    label = np.full(ld, -2, dtype=np.int32)
+    ii, ni = _i(idx)
+    rc = lib().oracle_components(C.c_int(n), C.c_int(ld), _d(pos), _d(vel), _d(mass), _ptr(ii),
+                                 C.c_int(ni), C.c_double(G), C.c_double(eta_ff), C.c_double(eta_fb),
+                                 C.c_int(1 if eta_in_q else 0), C.c_double(tau_pivot), _ptr(label))
+    _check(rc, "oracle_components")
+    return label
+
+
+def forces_masked(pos, mass, idx, label, G=1.0, eps2=0.0, flags=ACC | GRAD, acc=None, grad=None):
+    """Eq. 42-44 on the pair set {(i, j) in idx^2 : label_i != label_j} (label indexed globally)."""
+    ld = pos.shape[1]
+    n = mass.shape[0]
+    if acc is None:
+        acc = np.zeros((3, ld))
+    if grad is None:
+        grad = np.zeros((3, ld))
+    ii, ni = _i(idx)
+    lab = np.ascontiguousarray(label, dtype=np.int32)
+    rc = lib().oracle_forces_masked(C.c_int(n), C.c_int(ld), _d(pos), _d(mass), _ptr(ii), C.c_int(ni),
+                                    _ptr(lab), C.c_double(G), C.c_double(eps2), _d(acc), _d(grad),
+                                    C.c_int(flags))
+    _check(rc, "oracle_forces_masked")
+    return acc, grad
 
 
 def diagnostics(pos, vel, mass, G=1.0, eps2=0.0):
