@@ -60,6 +60,8 @@ typedef struct {
     int64_t pairs_newton;               /* ordered pairs swept by the Newton kernel */
     int64_t pairs_gradient;             /* ordered pairs swept by the gradient kernel */
     int64_t pairs_timestep;             /* ordered pairs swept by the time-step kernel */
+    int64_t n_comp[FROST_MAX_LEVELS];   /* sum over those entries of the fast components recursed into
+                                           (Alg. 3 as printed: 1 per entry with |F| > 0; frost_set_split) */
 } frost_hhs_stats;
 
 /* allocate_memory / free_memory of Alg. 4: creates a context bound to CUDA
@@ -234,6 +236,34 @@ int frost_set_shard(frost_ctx *ctx, int rank, int world);
  * recursion into F, and joins it before the next inter-level sweep -- same kernels, same inputs:
  * bitwise the result of on = 0, where the two run back to back on the context's stream. */
 int frost_set_overlap(frost_ctx *ctx, int on);
+
+/* Spatial splitting of fast hierarchy levels -- the paper's own outlook ("the further spatial
+ * Hamiltonian splitting of the individual hierarchy levels into field stars, binaries and multiple
+ * star systems"; binaries are left to future work).  The paper gives no
+ * algorithm; the one built here applies Eq. 29's rule to pairs (reading 24):
+ *   - a pair of one entry's set is FAST iff its symmetrised step of Eq. 49-54 is below tau_pivot
+ *     (a particle is slow iff it has no fast pair -- Eq. 29 unchanged);
+ *   - the fast pairs are the edges of a graph on F; hhs_fsi(F, tau/2) of Alg. 3 becomes one
+ *     hhs_fsi(C, tau/2) per connected component C, and the pairs between different components join
+ *     the inter-level kicks of Eq. 41-44 (kicked set: every pair of the entry that is neither
+ *     slow-slow nor inside one component; for a single component this is Alg. 3 bit for bit).
+ * split_max > 0 applies this to every entry with at most split_max members (larger entries run Alg. 3
+ * as printed; a level that still percolates gains nothing from the component search); 0 (default)
+ * switches it off.  Components of at most 32 particles -- binaries, triples -- are advanced side by
+ * side, one warp each, by one batched launch per recursion pass; components of up to 1024 particles
+ * one CTA each; larger ones by the host recursion.  Result: deterministic; not the numbers of
+ * split_max = 0 (a different, equally fourth-order splitting of the same Hamiltonian). */
+int frost_set_split(frost_ctx *ctx, int split_max);
+
+/* The kick sweeps of a split entry on their own (Eq. 42-44 on the pair set "labels differ"):
+ *   out_acc[i]  <- G sum_{j in idx, label_j != label_i} m_j x_ji / s_ij^3,
+ *   out_grad[i] <- 2G sum over the same j of m_j s^-5 (s^2 a_ji - 3 (x_ji.a_ji) x_ji) with the a of this call
+ * for every i of the list idx (DEVICE int32[n_idx], NULL = all).  label (DEVICE int32[n_idx]) is
+ * indexed by LIST POSITION; equal labels = same component, so the pair is skipped (frost_hhs_step
+ * gives every slow particle -1).  out_grad nullable.  One-sided sweeps; asynchronous. */
+int frost_forces_masked(frost_ctx *ctx, int n, int ld, const double *pos, const double *mass,
+                        const int32_t *idx, int n_idx, const int32_t *label, double *out_acc,
+                        double *out_grad);
 
 #ifdef __cplusplus
 }

@@ -25,6 +25,7 @@ exported_symbols = [
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
     "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
     "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
+    "frost_set_split", "frost_forces_masked",
 ]
 
 
@@ -36,14 +37,15 @@ class HHSStats(C.Structure):
     _fields_ = [("depth", C.c_int32), ("reserved", C.c_int32),
                 ("entries", C.c_int64 * MAX_LEVELS), ("n_slow", C.c_int64 * MAX_LEVELS),
                 ("n_fast", C.c_int64 * MAX_LEVELS), ("pairs_newton", C.c_int64),
-                ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64)]
+                ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64),
+                ("n_comp", C.c_int64 * MAX_LEVELS)]
 
     def as_dict(self):
         d = self.depth
         return {"depth": d, "entries": list(self.entries[: d + 1]),
                 "n_slow": list(self.n_slow[: d + 1]), "n_fast": list(self.n_fast[: d + 1]),
                 "pairs_newton": self.pairs_newton, "pairs_gradient": self.pairs_gradient,
-                "pairs_timestep": self.pairs_timestep}
+                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1])}
 
 
 def library_path() -> str:
@@ -68,6 +70,8 @@ def load_library():
     lib.frost_set_symmetric.argtypes = [vp, i32, i32]
     lib.frost_set_shard.argtypes = [vp, i32, i32]
     lib.frost_set_overlap.argtypes = [vp, i32]
+    lib.frost_set_split.argtypes = [vp, i32]
+    lib.frost_forces_masked.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, vp, vp]
     lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
     lib.frost_forces_host.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -168,6 +172,11 @@ class Frost:
         with the recursion into F; 0: back to back on the context's stream (same bits)."""
         self._check(self.lib.frost_set_overlap(self.h, on), "frost_set_overlap")
 
+    def set_split(self, split_max=0):
+        """split_max > 0: hierarchy entries with at most split_max members recurse into the connected
+        components of their fast pairs one by one (frost.h: frost_set_split); 0 (default): Alg. 3."""
+        self._check(self.lib.frost_set_split(self.h, split_max), "frost_set_split")
+
     def launch_count(self) -> int:
         return int(self.lib.frost_launch_count(self.h))
 
@@ -185,6 +194,23 @@ class Frost:
         self._check(self.lib.frost_forces(self.h, n, ld, _p(pos), _p(vel), _p(mass), _p(si), ns,
                                           _p(so), nso, _p(_vec(out_acc, "out_acc")),
                                           _p(out_grad), flags), "frost_forces")
+        return out_acc, out_grad
+
+    def forces_masked(self, pos, mass, label, idx=None, out_acc=None, out_grad=None, grad=True):
+        """Eq. 42-44 over the pairs of the list whose labels (int32, by list position) differ."""
+        _vec(pos, "pos")
+        ld, n = pos.shape[1], mass.numel()
+        if out_acc is None:
+            out_acc = torch.zeros_like(pos)
+        if out_grad is None and grad:
+            out_grad = torch.zeros_like(pos)
+        ii, ni = _idx(idx, "idx")
+        lab, nl = _idx(label, "label")
+        if nl != (ni if idx is not None else n):
+            raise FrostError("label: one entry per list position expected")
+        self._check(self.lib.frost_forces_masked(self.h, n, ld, _p(pos), _p(mass), _p(ii), ni, _p(lab),
+                                                 _p(_vec(out_acc, "out_acc")), _p(out_grad if grad else None)),
+                    "frost_forces_masked")
         return out_acc, out_grad
 
     def forces_host(self, pos, mass, sink_idx=None, source_idx=None, out_acc=None, out_grad=None,

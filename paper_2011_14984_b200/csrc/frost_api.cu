@@ -35,12 +35,13 @@ int frost_create(frost_ctx **out, int device, void *stream) {
 
 static void free_scratch(frost_ctx *c) {
     Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->tau_scratch, &c->symtot,
-                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats, &c->shard_idx};
+                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats, &c->shard_idx, &c->uf, &c->comp};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
     for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
         if (c->lvlS[k].p) cudaFree(c->lvlS[k].p);
         if (c->lvlF[k].p) cudaFree(c->lvlF[k].p);
+        if (c->lvlC[k].p) cudaFree(c->lvlC[k].p);
     }
     if (c->pinned_counts) cudaFreeHost(c->pinned_counts);
 }
@@ -80,7 +81,7 @@ static int side_ctx(frost_ctx *c, int level, frost_ctx **out) {
     }
     s->G = c->G; s->eps2 = c->eps2; s->eta_ff = c->eta_ff; s->eta_fb = c->eta_fb; s->max_depth = c->max_depth;
     s->tune_k = c->tune_k; s->tune_slices = c->tune_slices; s->tune_small = c->tune_small;
-    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym;
+    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max;
     s->sym_scratch = c->sym_scratch < ((size_t)1 << 30) ? c->sym_scratch : ((size_t)1 << 30);
     *out = s;
     return FROST_OK;
@@ -123,6 +124,12 @@ int frost_set_shard(frost_ctx *c, int rank, int world) {
 int frost_set_overlap(frost_ctx *c, int on) {
     if (!c || on < 0 || on > 1) return FROST_EINVAL;
     c->overlap = on;
+    return FROST_OK;
+}
+
+int frost_set_split(frost_ctx *c, int split_max) {
+    if (!c || split_max < 0) return FROST_EINVAL;
+    c->split_max = split_max;
     return FROST_OK;
 }
 
@@ -267,11 +274,26 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
     return rc;
 }
 
+// forest != NULL (a split hierarchy entry): the sweep also unites the fast pairs -- candidate below
+// tau_pivot -- in the union-find forest over list positions; every pair must then be evaluated, so the
+// pruned sweep is not used.
 static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const double *vel,
                           const double *mass, const int32_t *idx, int n_idx, double tau_pivot,
-                          double *out_tau, int32_t *out_bin) {
+                          double *out_tau, int32_t *out_bin, int *forest = nullptr) {
     if (!idx) n_idx = n;
     if (n_idx <= 0) return FROST_OK;
+    if (forest) {
+        const int pad = pad1024(n_idx);
+        FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+        FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
+        double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
+        FROST_TRY(launch_iota(c, forest, n_idx, 0));
+        FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, c->G, 1));
+        FROST_TRY(launch_pack_vec(c, ld, vel, idx, n_idx, pad, v, 1));
+        if (c->tune_sym != 1 && n_idx >= 4096)
+            return sym_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin, forest);
+        return sweep_timestep(c, xm, v, n_idx, idx, tau_pivot, out_tau, out_bin, forest);
+    }
     // large levels: Morton order + exact block pruning (frost_tau.cu); tune_sym 3 = symmetric sweep
     // without pruning, 4 = the pruning machinery with pruning switched off, 5 = pruning at any size (tests)
     // (measured on B200 against the plain symmetric sweep: 1.3x at 65536, 2.4x at 262144, 2.8x at
@@ -346,52 +368,97 @@ static int join_side(frost_ctx *c, int level, bool forked) {
     return FROST_OK;
 }
 
+// The inter-level kick of one entry (Alg. 3's acc_sf_* + kick_sf; Eq. 41-44): masked = the entry was
+// split into several components and the kicked pair set is "labels differ" over the whole set.
+static int cross_kick(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                      const int32_t *set, int n_set, const int32_t *S, int nS, const int32_t *F, int nF,
+                      const SplitInfo &si, bool with_g, double cc, double kappa) {
+    double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
+    if (si.m > 1) {
+        const int pad = pad1024(n_set);
+        FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+        FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
+        double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
+        FROST_TRY(launch_pack_xm(c, ld, pos, mass, set, n_set, pad, xm, 1.0, 0, av));
+        FROST_TRY(launch_pack_label(c, si.labpos, n_set, pad, av));
+        FROST_TRY(sweep_masked(c, xm, av, n_set, set, ld, acc, with_g ? grad : nullptr));
+        return launch_kick(c, ld, vel, acc, with_g ? grad : nullptr, set, n_set, cc, kappa);
+    }
+    if (nS > 0 && nF > 0) {
+        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad,
+                              FROST_ACC | FROST_MUTUAL | (with_g ? FROST_GRAD : 0)));
+        return launch_kick(c, ld, vel, acc, with_g ? grad : nullptr, set, n_set, cc, kappa);   // S u F
+    }
+    return FROST_OK;
+}
+
+static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st);
+
+// hhs_fsi(C, tau/2) of every component of F (Alg. 3: hhs_fsi(F, tau/2))
+static int recurse_fast(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
+                        const int32_t *F, int nF, const SplitInfo &si, double h, int level,
+                        frost_hhs_stats *st) {
+    if (si.m <= 1) return hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st);
+    FROST_TRY(launch_comp_batch(c, 1, ld, pos, vel, mass, si.C, si.desc_small, si.n_small_dev, si.n_small, h,
+                                level + 1, c->dev_stats.p));
+    FROST_TRY(launch_comp_batch(c, 0, ld, pos, vel, mass, si.C, si.desc_med, si.n_med_dev, si.n_med, h,
+                                level + 1, c->dev_stats.p));
+    for (int b = 0; b < si.n_big; ++b)
+        FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, si.C + si.big_off[b], si.big_size[b], h, level + 1, st));
+    return FROST_OK;
+}
+
 static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                    const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st) {
     if (n_set <= 0) return FROST_OK;
     if (level >= c->max_depth || level >= FROST_MAX_LEVELS) return FROST_EDEPTH;
     if (n_set <= small_threshold(c))     // the whole subtree on the device, asynchronously (row 11)
         return launch_small(c, 0, ld, pos, vel, mass, set, n_set, tau_pivot, level, c->dev_stats.p);
-    double *tau = (double *)c->tau.p, *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
-    FROST_TRY(timesteps_impl(c, n, ld, pos, vel, mass, set, n_set, tau_pivot, tau, nullptr));
+    double *tau = (double *)c->tau.p;
+    const bool split = c->split_max > 0 && n_set <= c->split_max;
+    int *forest = nullptr;
+    if (split) {
+        FROST_TRY(ensure(c, c->uf, (size_t)pad1024(n_set) * sizeof(int)));
+        forest = (int *)c->uf.p;
+    }
+    FROST_TRY(timesteps_impl(c, n, ld, pos, vel, mass, set, n_set, tau_pivot, tau, nullptr, forest));
     FROST_TRY(ensure(c, c->lvlS[level], (size_t)n_set * sizeof(int32_t)));
     FROST_TRY(ensure(c, c->lvlF[level], (size_t)n_set * sizeof(int32_t)));
     int32_t *S = (int32_t *)c->lvlS[level].p, *F = (int32_t *)c->lvlF[level].p;
     int32_t cnt[2];
     FROST_TRY(launch_partition(c, tau, set, n_set, tau_pivot, S, F, cnt));
     const int nS = cnt[0], nF = cnt[1];
+    SplitInfo si;
+    si.m = nF > 0 ? 1 : 0;
+    si.sumsq = (long long)nF * nF;
+    if (split && nF > 0) {
+        FROST_TRY(split_components(c, level, ld, tau, set, n_set, tau_pivot, forest, F, nF, &si));
+        F = const_cast<int32_t *>(si.C);       // same members, components contiguous
+    }
     if (st) {
         if (level > st->depth) st->depth = level;
         st->entries[level] += 1;
         st->n_slow[level] += nS;
         st->n_fast[level] += nF;
+        st->n_comp[level] += si.m;
         st->pairs_timestep += (int64_t)n_set * n_set;
     }
-    const bool cross = nS > 0 && nF > 0;
     const double h = 0.5 * tau_pivot;
     bool forked = false;
-    if (cross) {
-        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
-    }
+    FROST_TRY(cross_kick(c, n, ld, pos, vel, mass, set, n_set, S, nS, F, nF, si, false, tau_pivot / 6.0, 0.0));
     FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked));       // fsi(S, tau/2) ...
-    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));              // ... || hhs_fsi(F, tau/2)
+    FROST_TRY(recurse_fast(c, n, ld, pos, vel, mass, F, nF, si, h, level, st));         // ... || hhs_fsi(F, tau/2)
     FROST_TRY(join_side(c, level, forked));
-    if (cross) {
-        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad,
-                              FROST_ACC | FROST_GRAD | FROST_MUTUAL));
-        const double kap = tau_pivot * tau_pivot / 48.0;
-        FROST_TRY(launch_kick(c, ld, vel, acc, grad, set, n_set, 2.0 * tau_pivot / 3.0, kap));   // S u F
-    }
+    FROST_TRY(cross_kick(c, n, ld, pos, vel, mass, set, n_set, S, nS, F, nF, si, true, 2.0 * tau_pivot / 3.0,
+                         tau_pivot * tau_pivot / 48.0));
     FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked));
-    FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st));
+    FROST_TRY(recurse_fast(c, n, ld, pos, vel, mass, F, nF, si, h, level, st));
     FROST_TRY(join_side(c, level, forked));
-    if (cross) {
-        FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, nullptr, FROST_ACC | FROST_MUTUAL));
-        FROST_TRY(launch_kick(c, ld, vel, acc, nullptr, set, n_set, tau_pivot / 6.0, 0.0));   // S u F
-    }
+    FROST_TRY(cross_kick(c, n, ld, pos, vel, mass, set, n_set, S, nS, F, nF, si, false, tau_pivot / 6.0, 0.0));
     if (st) {
-        const int64_t cr = 2 * (int64_t)nS * nF;
+        // ordered pairs of the kicked set: all but slow-slow and same-component pairs (2 |S| |F| unsplit)
+        const int64_t cr = (int64_t)n_set * n_set - (int64_t)nS * nS - si.sumsq;
         st->pairs_newton += 3 * cr;
         st->pairs_gradient += cr;
     }
@@ -551,7 +618,8 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     if (rc != FROST_OK)      // an aborted recursion may have left forked side streams unjoined
         for (int k = 0; k < FROST_MAX_LEVELS; ++k) if (c->side[k]) cudaStreamSynchronize(c->side[k]->stream);
     // merge what the device-resident subtrees counted (also carries their status)
-    struct { long long e[FROST_MAX_LEVELS], s[FROST_MAX_LEVELS], f[FROST_MAX_LEVELS], pn, pg, pt; int depth, status; } d;
+    struct { long long e[FROST_MAX_LEVELS], s[FROST_MAX_LEVELS], f[FROST_MAX_LEVELS], pn, pg, pt; int depth, status;
+             long long nc[FROST_MAX_LEVELS]; } d;
     static_assert(sizeof(d) >= 1, "");
     if (sizeof(d) != small_stats_bytes()) return FROST_EINVAL;
     FROST_CUDA(c, cudaMemcpyAsync(&d, c->dev_stats.p, sizeof(d), cudaMemcpyDeviceToHost, c->stream));
@@ -560,6 +628,7 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     // the device kernel records depth = -1 when it never entered a level
     for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
         local.entries[k] += d.e[k]; local.n_slow[k] += d.s[k]; local.n_fast[k] += d.f[k];
+        local.n_comp[k] += d.nc[k];
     }
     local.pairs_newton += d.pn; local.pairs_gradient += d.pg; local.pairs_timestep += d.pt;
     if (d.depth > local.depth) local.depth = d.depth;
@@ -587,6 +656,24 @@ int frost_diagnostics(frost_ctx *c, int n, int ld, const double *pos, const doub
     FROST_CUDA(c, cudaMemcpyAsync(out8, d8, 8 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     FROST_CUDA(c, cudaStreamSynchronize(c->stream));
     return FROST_OK;
+}
+
+int frost_forces_masked(frost_ctx *c, int n, int ld, const double *pos, const double *mass,
+                        const int32_t *idx, int n_idx, const int32_t *label, double *out_acc,
+                        double *out_grad) {
+    if (!c || bad_planes(n, ld) || !pos || !mass || !label || !out_acc) return FROST_EINVAL;
+    if (idx && n_idx < 0) return FROST_EINVAL;
+    if (c->shard_world > 1) return FROST_EINVAL;      // only frost_forces is shard-aware
+    if (!idx) n_idx = n;
+    if (n_idx == 0) return FROST_OK;
+    FROST_DEVICE(c);
+    const int pad = pad1024(n_idx);
+    FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+    FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
+    double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, 1.0, 0, av));
+    FROST_TRY(launch_pack_label(c, label, n_idx, pad, av));
+    return sweep_masked(c, xm, av, n_idx, idx, ld, out_acc, out_grad);
 }
 
 int frost_gather_pack(frost_ctx *c, int n, int ld, const double *pos, const double *mass,

@@ -50,6 +50,9 @@ struct frost_ctx {
     frost::Buf lvlS[FROST_MAX_LEVELS], lvlF[FROST_MAX_LEVELS];
     int32_t *pinned_counts = nullptr;  // host pinned int32[4]
     frost::Buf shard_idx;              // 0..n-1, for sharding the sinks of a NULL index list
+    int split_max = 0;             // frost_set_split: entries with <= split_max members split F into components
+    frost::Buf uf, comp;           // union-find forest / labels, sort and descriptor scratch of a split entry
+    frost::Buf lvlC[FROST_MAX_LEVELS];   // F of a split entry reordered by component
     // fsi(S) || hhs_fsi(F): one side context (own stream, own sweep scratch) per hierarchy level
     int overlap = 1;
     frost_ctx *side[FROST_MAX_LEVELS] = {};
@@ -140,8 +143,12 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
                    int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0,
                    double *zero_tail = nullptr);
+// w_index != 0: .w of record k carries the list position k in its low word (time-step sweeps that
+// enter their fast pairs into a union-find forest); otherwise 1.0
 int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
-                    int n_pad, double *out);
+                    int n_pad, double *out, int w_index = 0);
+// .w of record k <- component label lab[k] in its low word (records beyond n_idx: -2)
+int launch_pack_label(frost_ctx *c, const int *lab, int n_idx, int n_pad, double *vec);
 int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
                 const int32_t *idx, int n_idx, double cc, double kappa);
 int launch_kick_drift(frost_ctx *c, int ld, double *pos, double *vel, const double *acc, const double *grad,
@@ -157,8 +164,14 @@ int sweep_newton(frost_ctx *c, const double *snk_xm, int n_snk, const double *sr
 int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int n_snk,
                    const double *src_xm, const double *src_a, int n_src, const int32_t *snk_idx,
                    int ld, double *out_grad);
+// forest != NULL: pairs with a candidate below tau_pivot are united in the forest over list positions
 int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set,
-                   const int32_t *idx, double tau_pivot, double *out_tau, int32_t *out_bin);
+                   const int32_t *idx, double tau_pivot, double *out_tau, int32_t *out_bin,
+                   int *forest = nullptr);
+// Self sweep of one list over the pairs whose component labels differ (low word of a_lab[k].w; the
+// kicked pair set of a split hierarchy entry): accelerations, then (grad != NULL) gradient accelerations.
+int sweep_masked(frost_ctx *c, const double *xm, double *a_lab, int n_set, const int32_t *idx, int ld,
+                 double *out_acc, double *out_grad);
 
 // frost_sym.cu: pair-symmetric sweeps (one evaluation serves i<-j and j<-i).  self: B == A.
 int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
@@ -168,7 +181,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
                  const double *B_a, int nB, bool self, const int32_t *A_idx, const int32_t *B_idx,
                  int ld, double *out_grad);
 int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
-                 double tau_pivot, double *out_tau, int32_t *out_bin);
+                 double tau_pivot, double *out_tau, int32_t *out_bin, int *forest = nullptr);
 
 int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
 // frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)
@@ -182,11 +195,29 @@ int launch_zero_outside(frost_ctx *c, int ld, double *planes, const int32_t *idx
 int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const double *mass,
                const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune);
 
+// frost_split.cu: the components of the fast pairs of a split hierarchy entry (reading 24)
+struct SplitInfo {
+    int m = 0;                       // components of F
+    int n_small = 0, n_med = 0, n_big = 0;   // of <= comp_warp_max(), <= small_max(), more particles
+    long long sumsq = 0;             // sum of squared component sizes
+    const int32_t *C = nullptr;      // F reordered: components contiguous, by smallest member (device)
+    const int *labpos = nullptr;     // label of every list position of the entry's set, -1 = slow (device)
+    const void *desc_small = nullptr, *desc_med = nullptr;   // int2 {offset into C, size} (device)
+    const int *n_small_dev = nullptr, *n_med_dev = nullptr;
+    int big_off[64], big_size[64];   // the big components (host)
+};
+int split_components(frost_ctx *c, int level, int ld, const double *tau, const int32_t *set, int n_set,
+                     double pivot, const int *forest, const int32_t *F, int nF, SplitInfo *out);
+
 // frost_small.cu: one-CTA device-resident hhs_fsi subtree (mode 0) or fsi step (mode 1)
 int small_max();
 size_t small_stats_bytes();
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
                  const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps = 1);
+int comp_warp_max();
+int launch_comp_batch(frost_ctx *c, int warp_team, int ld, double *pos, double *vel, const double *mass,
+                      const int32_t *idx, const void *desc, const int *n_desc, int max_desc, double tau,
+                      int level0, void *dev_stats);
 
 // ---- device-side PTX helpers ------------------------------------------------------------------
 #ifdef __CUDACC__
@@ -228,6 +259,24 @@ __device__ __forceinline__ void bulk_g2s(void *dst_smem, const void *src_gmem, u
             "r"(smem_u32(dst_smem)),
         "l"(src_gmem), "r"(bytes), "r"(smem_u32(bar))
         : "memory");
+}
+
+// Lock-free union-find (global or shared memory): the root of a tree is its smallest member, so the
+// final forest does not depend on the order in which the pairs arrive.
+__device__ __forceinline__ int uf_find(const volatile int *par, int x) {
+    while (true) {
+        const int p = par[x];
+        if (p == x) return x;
+        x = p;
+    }
+}
+__device__ __forceinline__ void uf_union(int *par, int a, int b) {
+    while (true) {
+        a = uf_find(par, a); b = uf_find(par, b);
+        if (a == b) return;
+        if (a < b) { const int t = a; a = b; b = t; }       // hang the larger root under the smaller
+        if (atomicCAS(&par[a], a, b) == a) return;
+    }
 }
 
 // fp64 reciprocal square root seed: MUFU.RSQ64H on the high word (rel. error ~2^-22), low word 0.

@@ -21,6 +21,8 @@ struct SweepParams {
     int tiles_per_slice;
     double eps2;
     double G, eta_ff, eta_fb;
+    double pivot;          // TimestepEdgePolicy: pairs with a candidate below it are united in `forest`
+    int *forest;
 };
 
 struct NewtonPolicy {
@@ -124,8 +126,8 @@ struct TimestepPolicy {
     // padding record (NaN position) and a pair at rest (v2 = 0, fly-by only) turn into NaN through
     // MUFU(0) = +inf and 0*inf, and fmin() returns its non-NaN operand, so such candidates drop out
     // exactly as DESIGN.md reading 11 requires.  ~77 FP64 instructions + 7 MUFU per pair.
-    __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
-                                                const double4 &j1, const SweepParams &p) {
+    __device__ static __forceinline__ double candidate(const Sink &s, const double4 &j0, const double4 &j1,
+                                                       const SweepParams &p) {
         const double rx = j0.x - s.x, ry = j0.y - s.y, rz = j0.z - s.z;
         const double vx = j1.x - s.vx, vy = j1.y - s.vy, vz = j1.z - s.vz;
         const double r2 = fma(rz, rz, fma(ry, ry, rx * rx));
@@ -144,10 +146,82 @@ struct TimestepPolicy {
         const double q_fb = fma(f, mir * (iv * iv), f) * p.eta_fb;            // eta * Eq. 54
         const double c_ff = sym_factor(q_ff) * (t_ff * p.eta_ff);
         const double c_fb = sym_factor(q_fb) * (t_fb * p.eta_fb);
-        a.tau = fmin(a.tau, fmin(c_ff, c_fb));
+        return fmin(c_ff, c_fb);
+    }
+    __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
+                                                const double4 &j1, const SweepParams &p) {
+        a.tau = fmin(a.tau, candidate(s, j0, j1, p));
     }
     __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
         part[i] = a.tau;
+    }
+};
+
+// The time-step sweep of a split hierarchy entry (reading 24): as TimestepPolicy, and every
+// fast pair (candidate < pivot) is united in the union-find forest over list positions.  The list
+// position of a record travels in the low word of .w of its velocity record.
+struct TimestepEdgePolicy {
+    static constexpr int kRecs = 2;
+    static constexpr int kPlanes = 1;
+    struct Sink : TimestepPolicy::Sink { int id; };
+    using Acc = TimestepPolicy::Acc;
+    __device__ static __forceinline__ void load(Sink &s, const SweepParams &p, int i) {
+        TimestepPolicy::load(s, p, i);
+        s.id = __double2loint(p.snk1[i].w);
+    }
+    __device__ static __forceinline__ void init(Acc &a) { TimestepPolicy::init(a); }
+    __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
+                                                const double4 &j1, const SweepParams &p) {
+        const double c = TimestepPolicy::candidate(s, j0, j1, p);
+        a.tau = fmin(a.tau, c);
+        if (c < p.pivot) uf_union(p.forest, s.id, __double2loint(j1.w));
+    }
+    __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
+        part[i] = a.tau;
+    }
+};
+
+// Eq. 42 / 43-44 on the kicked pair set of a split entry: a source whose component label (low word of
+// .w of the second record) equals the sink's contributes nothing.  Slow particles all carry -1.
+struct MaskedNewtonPolicy {
+    static constexpr int kRecs = 2;
+    static constexpr int kPlanes = 3;
+    struct Sink : NewtonPolicy::Sink { int lab; };
+    using Acc = NewtonPolicy::Acc;
+    __device__ static __forceinline__ void load(Sink &s, const SweepParams &p, int i) {
+        NewtonPolicy::load(s, p, i);
+        s.lab = __double2loint(p.snk1[i].w);
+    }
+    __device__ static __forceinline__ void init(Acc &a) { NewtonPolicy::init(a); }
+    __device__ static __forceinline__ void pair(const Sink &s, Acc &a, const double4 &j0,
+                                                const double4 &j1, const SweepParams &p) {
+        double4 jm = j0;
+        if (__double2loint(j1.w) == s.lab) jm.w = 0.0;
+        NewtonPolicy::pair(s, a, jm, jm, p);
+    }
+    __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
+        NewtonPolicy::store(a, part, n_pad, i);
+    }
+};
+
+struct MaskedGradientPolicy {
+    static constexpr int kRecs = 2;
+    static constexpr int kPlanes = 3;
+    struct Sink : GradientPolicy::Sink { int lab; };
+    using Acc = GradientPolicy::Acc;
+    __device__ static __forceinline__ void load(Sink &s, const SweepParams &p, int i) {
+        GradientPolicy::load(s, p, i);
+        s.lab = __double2loint(p.snk1[i].w);
+    }
+    __device__ static __forceinline__ void init(Acc &a) { GradientPolicy::init(a); }
+    __device__ static __forceinline__ void pair(const Sink &s, Acc &g, const double4 &j0,
+                                                const double4 &j1, const SweepParams &p) {
+        double4 jm = j0;
+        if (__double2loint(j1.w) == s.lab) jm.w = 0.0;
+        GradientPolicy::pair(s, g, jm, j1, p);
+    }
+    __device__ static __forceinline__ void store(const Acc &a, double *part, int n_pad, int i) {
+        GradientPolicy::store(a, part, n_pad, i);
     }
 };
 

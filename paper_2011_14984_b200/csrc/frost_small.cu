@@ -16,11 +16,14 @@ namespace frost {
 
 constexpr int kSmallMax = 1024;     // particles the subtree kernel accepts
 constexpr int kSmallThreads = 512;
+constexpr int kCompWarpMax = 32;    // components up to this size: one warp each, kCompWarps per CTA
+constexpr int kCompWarps = 8;
 
 struct SmallStats {                 // device-side mirror of frost_hhs_stats (+ status)
     long long entries[FROST_MAX_LEVELS], n_slow[FROST_MAX_LEVELS], n_fast[FROST_MAX_LEVELS];
     long long pairs_newton, pairs_gradient, pairs_timestep;
     int depth, status;
+    long long n_comp[FROST_MAX_LEVELS];
 };
 
 struct SmallParams {
@@ -35,24 +38,43 @@ struct SmallParams {
     int level0, max_depth;
     double G, eps2, eta_ff, eta_fb;
     SmallStats *stats;
+    // spatial splitting of fast levels (reading 24): entries with at most split_max members
+    // recurse into the connected components of their fast pairs one by one
+    int split_max;
+    // batched launch: CTA (or warp) b takes the set idx[desc[b].x .. desc[b].x + desc[b].y)
+    const int2 *desc;
+    const int *n_desc;
 };
 
-struct SmallSmem {
-    double4 xm[kSmallMax];          // x, y, z, m
-    double4 vv[kSmallMax];          // vx, vy, vz, 1
-    double4 aa[kSmallMax];          // ax, ay, az, 1
-    double4 gg[kSmallMax];          // gx, gy, gz, -
-    double tau[kSmallMax];
-    int perm[kSmallMax];            // the level sets are contiguous segments of this list
-    int tmp[kSmallMax];
+template <int CAP>
+struct SmallSmemT {
+    static constexpr int kCap = CAP, kWords = (CAP + 31) / 32;
+    double4 xm[CAP];                // x, y, z, m
+    double4 vv[CAP];                // vx, vy, vz, 1
+    double4 aa[CAP];                // ax, ay, az, 1
+    double4 gg[CAP];                // gx, gy, gz, -
+    double tau[CAP];
+    int perm[CAP];                  // the level sets are contiguous segments of this list
+    int tmp[CAP];
+    int lab[CAP];                   // component of a particle in the entry being executed (-1 = slow)
+    int par[CAP];                   // union-find forest over the fast pairs of the entry's time-step sweep
     int scan[kSmallThreads / 32 + 1];
     // explicit recursion stack
     int f_start[FROST_MAX_LEVELS], f_n[FROST_MAX_LEVELS], f_ns[FROST_MAX_LEVELS], f_stage[FROST_MAX_LEVELS];
+    int f_cpos[FROST_MAX_LEVELS];   // next component of F to recurse into (offset inside F)
+    int f_m[FROST_MAX_LEVELS];      // number of components of F
+    long long f_sumsq[FROST_MAX_LEVELS];          // sum of squared component sizes
+    unsigned f_bnd[FROST_MAX_LEVELS][kWords];     // bit r: a component starts at position r of F
     double f_tau[FROST_MAX_LEVELS];
     int sp, err;
-    long long st_entries[FROST_MAX_LEVELS], st_slow[FROST_MAX_LEVELS], st_fast[FROST_MAX_LEVELS];
-    long long st_pn, st_pg, st_pt;
-    int st_depth;
+};
+using SmallSmem = SmallSmemT<kSmallMax>;
+
+struct SmStats {                    // per CTA, shared by its teams (atomics)
+    unsigned long long entries[FROST_MAX_LEVELS], slow[FROST_MAX_LEVELS], fast[FROST_MAX_LEVELS],
+        comps[FROST_MAX_LEVELS];
+    unsigned long long pn, pg, pt;
+    int depth;
 };
 
 // A "team" executes a subtree: the whole CTA, or -- for sets of <= 32 particles, where the cost is
@@ -103,9 +125,9 @@ constexpr long long kSplitPairs = 8192;
 struct SinkShare { int lo, hi; bool split, waited; };
 
 template <class T>
-__device__ __forceinline__ SinkShare sweep_begin(int nA, int nB) {
+__device__ __forceinline__ SinkShare sweep_begin(int nA, int nB, bool allow = true) {
     SinkShare sh{0, nA, false, true};
-    if (T::kCluster) {
+    if (T::kCluster && allow) {
         namespace cg = cooperative_groups;
         cg::cluster_group cl = cg::this_cluster();
         if ((long long)nA * nB >= kSplitPairs && cl.num_blocks() > 1) {
@@ -163,8 +185,10 @@ __device__ __forceinline__ double shfl_min(double v, int L) {
 
 // a_i = G sum_{j in B} ...  for i in segment A (Eq. 24 / 42).  Segments are [a0, a0+nA) and
 // [b0, b0+nB) of sm.perm.  All threads must call (uniform control flow, shuffles).
-template <class T>
-__device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
+// MASK: a source in the sink's own component (sm.lab equal; slow particles all carry -1) is skipped
+// -- the kicked pair set of a split entry (reading 24).
+template <class T, bool MASK, class SM>
+__device__ void cta_newton(SM &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
     SinkShare sh = sweep_begin<T>(nA, nB);
     const int L = lanes_per_sink<T>(sh.hi - sh.lo, nB);
     const int per = T::kThreads / L;
@@ -173,6 +197,7 @@ __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA
         const int a = base + slot;
         const bool live = a < sh.hi;
         const int i = sm.perm[a0 + (live ? a : 0)];
+        const int li = MASK ? sm.lab[i] : 0;
         NewtonPolicy::Sink s;
         const double4 r = sm.xm[i];
         s.x = r.x; s.y = r.y; s.z = r.z;
@@ -186,12 +211,16 @@ __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA
         for (; b + (kIlp - 1) * L < nB; b += kIlp * L) {
 #pragma unroll
             for (int u = 0; u < kIlp; ++u) {
-                const double4 j0 = sm.xm[sm.perm[b0 + b + u * L]];
+                const int j = sm.perm[b0 + b + u * L];
+                double4 j0 = sm.xm[j];
+                if (MASK && sm.lab[j] == li) j0.w = 0.0;
                 NewtonPolicy::pair(s, accs[u], j0, j0, prm);
             }
         }
         for (; b < nB; b += L) {
-            const double4 j0 = sm.xm[sm.perm[b0 + b]];
+            const int j = sm.perm[b0 + b];
+            double4 j0 = sm.xm[j];
+            if (MASK && sm.lab[j] == li) j0.w = 0.0;
             NewtonPolicy::pair(s, accs[0], j0, j0, prm);
         }
         NewtonPolicy::Acc acc;
@@ -207,8 +236,8 @@ __device__ void cta_newton(SmallSmem &sm, const SweepParams &prm, int a0, int nA
 }
 
 // g_i = 2G sum_{j in B} ... using sm.aa of sinks and sources (Eq. 27 / 43 / 44).
-template <class T>
-__device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
+template <class T, bool MASK, class SM>
+__device__ void cta_gradient(SM &sm, const SweepParams &prm, int a0, int nA, int b0, int nB) {
     SinkShare sh = sweep_begin<T>(nA, nB);
     const int L = lanes_per_sink<T>(sh.hi - sh.lo, nB);
     const int per = T::kThreads / L;
@@ -217,6 +246,7 @@ __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int 
         const int a = base + slot;
         const bool live = a < sh.hi;
         const int i = sm.perm[a0 + (live ? a : 0)];
+        const int li = MASK ? sm.lab[i] : 0;
         GradientPolicy::Sink s;
         const double4 r = sm.xm[i], ai = sm.aa[i];
         s.x = r.x; s.y = r.y; s.z = r.z; s.ax = ai.x; s.ay = ai.y; s.az = ai.z;
@@ -224,12 +254,17 @@ __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int 
         int b = sub;
         for (; b + L < nB; b += 2 * L) {
             const int j = sm.perm[b0 + b], j2 = sm.perm[b0 + b + L];
-            GradientPolicy::pair(s, acc, sm.xm[j], sm.aa[j], prm);
-            GradientPolicy::pair(s, acc1, sm.xm[j2], sm.aa[j2], prm);
+            double4 x0 = sm.xm[j], x1 = sm.xm[j2];
+            if (MASK && sm.lab[j] == li) x0.w = 0.0;
+            if (MASK && sm.lab[j2] == li) x1.w = 0.0;
+            GradientPolicy::pair(s, acc, x0, sm.aa[j], prm);
+            GradientPolicy::pair(s, acc1, x1, sm.aa[j2], prm);
         }
         if (b < nB) {
             const int j = sm.perm[b0 + b];
-            GradientPolicy::pair(s, acc, sm.xm[j], sm.aa[j], prm);
+            double4 x0 = sm.xm[j];
+            if (MASK && sm.lab[j] == li) x0.w = 0.0;
+            GradientPolicy::pair(s, acc, x0, sm.aa[j], prm);
         }
         acc.x += acc1.x; acc.y += acc1.y; acc.z += acc1.z;
         acc.x = shfl_sum(acc.x, L); acc.y = shfl_sum(acc.y, L); acc.z = shfl_sum(acc.z, L);
@@ -241,9 +276,17 @@ __device__ void cta_gradient(SmallSmem &sm, const SweepParams &prm, int a0, int 
 }
 
 // tau_i = min over the other members of the level (Eq. 49-54); a level of one particle: +inf.
-template <class T>
-__device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int nA) {
-    SinkShare sh = sweep_begin<T>(nA, nA);
+// pivot > 0: every fast pair (candidate < pivot) is also entered into the union-find forest sm.par
+// (the components of the level, reading 24).  Each pair is met from both sides, and in a
+// cluster every replica needs every pair, so the sweep is then not shared out.
+template <class T, class SM>
+__device__ void cta_timesteps(SM &sm, const SweepParams &prm, int a0, int nA, double pivot) {
+    const bool edges = pivot > 0.0;
+    if (edges) {
+        for (int a = T::tid(); a < nA; a += T::kThreads) { const int i = sm.perm[a0 + a]; sm.par[i] = i; }
+        T::sync();
+    }
+    SinkShare sh = sweep_begin<T>(nA, nA, !edges);
     const int L = lanes_per_sink<T>(sh.hi - sh.lo, nA);
     const int per = T::kThreads / L;
     const int sub = T::tid() & (L - 1), slot = T::tid() / L;
@@ -254,32 +297,39 @@ __device__ void cta_timesteps(SmallSmem &sm, const SweepParams &prm, int a0, int
         TimestepPolicy::Sink s;
         const double4 r = sm.xm[i], v = sm.vv[i];
         s.x = r.x; s.y = r.y; s.z = r.z; s.gm = r.w * prm.G; s.vx = v.x; s.vy = v.y; s.vz = v.z;
-        TimestepPolicy::Acc acc, acc1; TimestepPolicy::init(acc); TimestepPolicy::init(acc1);
+        double t0 = __longlong_as_double(0x7ff0000000000000LL), t1 = t0;
         int b = sub;
         for (; b + L < nA; b += 2 * L) {
             const int j = sm.perm[a0 + b], j2 = sm.perm[a0 + b + L];
             double4 j0 = sm.xm[j], k0 = sm.xm[j2];
             j0.w *= prm.G; k0.w *= prm.G;
-            TimestepPolicy::pair(s, acc, j0, sm.vv[j], prm);
-            TimestepPolicy::pair(s, acc1, k0, sm.vv[j2], prm);
+            const double c0 = TimestepPolicy::candidate(s, j0, sm.vv[j], prm);
+            const double c1 = TimestepPolicy::candidate(s, k0, sm.vv[j2], prm);
+            t0 = fmin(t0, c0); t1 = fmin(t1, c1);
+            if (edges && live) {
+                if (c0 < pivot) uf_union(sm.par, i, j);
+                if (c1 < pivot) uf_union(sm.par, i, j2);
+            }
         }
         if (b < nA) {
             const int j = sm.perm[a0 + b];
             double4 j0 = sm.xm[j];
             j0.w *= prm.G;
-            TimestepPolicy::pair(s, acc, j0, sm.vv[j], prm);
+            const double c0 = TimestepPolicy::candidate(s, j0, sm.vv[j], prm);
+            t0 = fmin(t0, c0);
+            if (edges && live && c0 < pivot) uf_union(sm.par, i, j);
         }
-        acc.tau = fmin(acc.tau, acc1.tau);
-        acc.tau = shfl_min(acc.tau, L);
+        t0 = fmin(t0, t1);
+        t0 = shfl_min(t0, L);
         sweep_wait<T>(sh);
-        if (live && sub == 0) publish<T>(sh, &sm.tau[i], acc.tau);
+        if (live && sub == 0) publish<T>(sh, &sm.tau[i], t0);
     }
     sweep_end<T>(sh);
 }
 
 // v_i += c (a_i + kappa g_i) ; x_i += c v_i  on a segment (Eq. 6).
-template <class T>
-__device__ void cta_kick(SmallSmem &sm, int a0, int nA, double c, double kappa, bool with_g) {
+template <class T, class SM>
+__device__ void cta_kick(SM &sm, int a0, int nA, double c, double kappa, bool with_g) {
     for (int a = T::tid(); a < nA; a += T::kThreads) {
         const int i = sm.perm[a0 + a];
         double4 v = sm.vv[i];
@@ -295,23 +345,10 @@ __device__ void cta_kick(SmallSmem &sm, int a0, int nA, double c, double kappa, 
     T::sync();
 }
 
-template <class T>
-__device__ void cta_drift(SmallSmem &sm, int a0, int nA, double c) {
-    for (int a = T::tid(); a < nA; a += T::kThreads) {
-        const int i = sm.perm[a0 + a];
-        double4 x = sm.xm[i];
-        const double4 v = sm.vv[i];
-        x.x = fma(c, v.x, x.x); x.y = fma(c, v.y, x.y); x.z = fma(c, v.z, x.z);
-        sm.xm[i] = x;
-    }
-    T::sync();
-}
-
 // kick then drift of the same particles in one phase (both touch only the thread's own particle):
 // v_i += ck (a_i + kappa g_i) ; x_i += cd v_i.
-template <class T>
-__device__ void cta_kick_drift(SmallSmem &sm, int a0, int nA, double ck, double kappa, bool with_g,
-                               double cd) {
+template <class T, class SM>
+__device__ void cta_kick_drift(SM &sm, int a0, int nA, double ck, double kappa, bool with_g, double cd) {
     for (int a = T::tid(); a < nA; a += T::kThreads) {
         const int i = sm.perm[a0 + a];
         double4 v = sm.vv[i];
@@ -332,8 +369,8 @@ __device__ void cta_kick_drift(SmallSmem &sm, int a0, int nA, double ck, double 
 
 // Stable in-place partition of the segment [a0, a0+n) of sm.perm: slow (tau >= pivot) first.
 // Returns |S| (Eq. 29).
-template <class T>
-__device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
+template <class T, class SM>
+__device__ int cta_partition(SM &sm, int a0, int n, double pivot) {
     const int lane = T::tid() & 31, w = T::tid() >> 5;
     constexpr int kWarps = T::kThreads / 32;
     if (T::kThreads == 32) {     // one warp, n <= 32: ballot
@@ -388,30 +425,125 @@ __device__ int cta_partition(SmallSmem &sm, int a0, int n, double pivot) {
     return nS;
 }
 
+// The connected components of the fast pairs of F = segment [f0, f0+nF) (forest sm.par built by
+// cta_timesteps): F is reordered so that every component is contiguous -- components by their
+// smallest member, members in their previous order -- and frame `sp` records where they start.
+// Returns the number of components; *sumsq = sum of their squared sizes.
+template <class T, class SM>
+__device__ int cta_components(SM &sm, int f0, int nF, int sp, long long *sumsq) {
+    for (int p = T::tid(); p < nF; p += T::kThreads) {
+        const int i = sm.perm[f0 + p];
+        sm.lab[i] = uf_find(sm.par, i);
+    }
+    for (int w = T::tid(); w < SM::kWords; w += T::kThreads) sm.f_bnd[sp][w] = 0u;
+    T::sync();
+    for (int p = T::tid(); p < nF; p += T::kThreads) {          // rank = position after a stable sort by label
+        const int i = sm.perm[f0 + p], li = sm.lab[i];
+        int rank = 0;
+        for (int q = 0; q < nF; ++q) {
+            const int lq = sm.lab[sm.perm[f0 + q]];
+            rank += (lq < li) || (lq == li && q < p);
+        }
+        sm.tmp[rank] = i;
+    }
+    T::sync();
+    for (int p = T::tid(); p < nF; p += T::kThreads) sm.perm[f0 + p] = sm.tmp[p];
+    T::sync();
+    for (int p = T::tid(); p < nF; p += T::kThreads)
+        if (p == 0 || sm.lab[sm.perm[f0 + p]] != sm.lab[sm.perm[f0 + p - 1]])
+            atomicOr(&sm.f_bnd[sp][p >> 5], 1u << (p & 31));
+    T::sync();
+    int m = 0, prev = -1;
+    long long ss = 0;
+    for (int w = 0; w < (nF + 31) / 32; ++w) {
+        unsigned bits = sm.f_bnd[sp][w];
+        while (bits) {
+            const int r = w * 32 + __ffs(bits) - 1;
+            bits &= bits - 1;
+            if (prev >= 0) ss += (long long)(r - prev) * (r - prev);
+            prev = r; ++m;
+        }
+    }
+    if (prev >= 0) ss += (long long)(nF - prev) * (nF - prev);
+    *sumsq = ss;
+    return m;
+}
+
+// sm.lab of the members of an entry from its recorded component boundaries: -1 for S, the component's
+// ordinal for F (the recursion below this entry reuses sm.lab for its own components).
+template <class T, class SM>
+__device__ void cta_labels(SM &sm, int start, int nS, int nF, int sp) {
+    for (int a = T::tid(); a < nS; a += T::kThreads) sm.lab[sm.perm[start + a]] = -1;
+    for (int p = T::tid(); p < nF; p += T::kThreads) {
+        int c = 0;
+        for (int w = 0; w < (p >> 5); ++w) c += __popc(sm.f_bnd[sp][w]);
+        c += __popc(sm.f_bnd[sp][p >> 5] & (0xffffffffu >> (31 - (p & 31))));
+        sm.lab[sm.perm[start + nS + p]] = c;
+    }
+    T::sync();
+}
+
+// size of the component of F that starts at position cpos (a set bit of the frame's boundary mask)
+template <class SM>
+__device__ __forceinline__ int comp_size(const SM &sm, int sp, int cpos, int nF) {
+    int w = (cpos + 1) >> 5;
+    if (cpos + 1 >= nF) return nF - cpos;
+    unsigned bits = sm.f_bnd[sp][w] & (0xffffffffu << ((cpos + 1) & 31));
+    const int words = (nF + 31) / 32;
+    while (!bits && ++w < words) bits = sm.f_bnd[sp][w];
+    const int next = bits ? w * 32 + __ffs(bits) - 1 : nF;
+    return (next < nF ? next : nF) - cpos;
+}
+
 // fsi(set, dt): Alg. 2 on the segment [a0, a0+nA).
-template <class T>
-__device__ void cta_fsi(SmallSmem &sm, const SweepParams &pN, const SweepParams &pG, int a0, int nA,
+template <class T, class SM>
+__device__ void cta_fsi(SM &sm, SmStats &st, const SweepParams &pN, const SweepParams &pG, int a0, int nA,
                         double dt) {
     if (nA <= 0) return;
-    cta_newton<T>(sm, pN, a0, nA, a0, nA);
+    cta_newton<T, false>(sm, pN, a0, nA, a0, nA);
     cta_kick_drift<T>(sm, a0, nA, dt / 6.0, 0.0, false, dt / 2.0);
-    cta_newton<T>(sm, pN, a0, nA, a0, nA);
-    cta_gradient<T>(sm, pG, a0, nA, a0, nA);
+    cta_newton<T, false>(sm, pN, a0, nA, a0, nA);
+    cta_gradient<T, false>(sm, pG, a0, nA, a0, nA);
     cta_kick_drift<T>(sm, a0, nA, 2.0 * dt / 3.0, dt * dt / 48.0, true, dt / 2.0);
-    cta_newton<T>(sm, pN, a0, nA, a0, nA);
+    cta_newton<T, false>(sm, pN, a0, nA, a0, nA);
     cta_kick<T>(sm, a0, nA, dt / 6.0, 0.0, false);
     if (T::tid() == 0) {
-        const long long np = (long long)nA * nA;
-        sm.st_pn += 3 * np;
-        sm.st_pg += np;
+        const unsigned long long np = (unsigned long long)nA * nA;
+        atomicAdd(&st.pn, 3 * np);
+        atomicAdd(&st.pg, np);
+    }
+}
+
+// The inter-level kick of an entry (Eq. 42-44 on its kicked pair set; Alg. 3's kick_sf): accelerations
+// (and gradient accelerations if with_g) of every member, then v += c (a + kappa g).  m <= 1: the pair
+// set is S x F both ways (Alg. 3 as printed); m > 1: every pair of the entry that is neither slow-slow
+// nor inside one component.
+template <class T, class SM>
+__device__ void cta_cross_kick(SM &sm, const SweepParams &pN, const SweepParams &pG, int start, int nS,
+                               int nF, int m, int sp, double c, double kappa, bool with_g) {
+    const int cnt = nS + nF;
+    if (m > 1) {
+        cta_labels<T>(sm, start, nS, nF, sp);
+        cta_newton<T, true>(sm, pN, start, cnt, start, cnt);
+        if (with_g) cta_gradient<T, true>(sm, pG, start, cnt, start, cnt);
+        cta_kick<T>(sm, start, cnt, c, kappa, with_g);
+    } else if (nS > 0 && nF > 0) {
+        cta_newton<T, false>(sm, pN, start, nS, start + nS, nF);
+        cta_newton<T, false>(sm, pN, start + nS, nF, start, nS);
+        if (with_g) {
+            cta_gradient<T, false>(sm, pG, start, nS, start + nS, nF);
+            cta_gradient<T, false>(sm, pG, start + nS, nF, start, nS);
+        }
+        cta_kick<T>(sm, start, cnt, c, kappa, with_g);
     }
 }
 
 // The hhs_fsi recursion of Alg. 3 as a state machine over the explicit frame stack; runs until the
-// frame at base_sp has been popped.
-template <class T>
-__device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams &pN, const SweepParams &pG,
-                         int base_sp) {
+// frame at base_sp has been popped.  Stages of a frame: 0 = entry (time steps, partition, components,
+// first kick, fsi(S)); 1 = first recursion pass over the components of F in progress; 2 = second pass.
+template <class T, class SM>
+__device__ void hhs_loop(SM &sm, SmStats &st, const SmallParams &P, const SweepParams &pN,
+                         const SweepParams &pG, int base_sp) {
     while (true) {
         T::sync();
         const int sp = sm.sp;
@@ -421,12 +553,12 @@ __device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams 
         const int level = P.level0 + sp;
         if (T::kThreads > 128 && stage == 0 && cnt > kWarpTeamMax && cnt <= kQuadTeamMax) {
             // the whole subtree of this entry on warps 0-3 (see TeamQuad)
-            if (threadIdx.x < 128) hhs_loop<TeamQuad>(sm, P, pN, pG, sp);
+            if (threadIdx.x < 128) hhs_loop<TeamQuad>(sm, st, P, pN, pG, sp);
             continue;
         }
         if (T::kThreads > 32 && stage == 0 && cnt > 0 && cnt <= kWarpTeamMax) {
             // the whole subtree of this entry on warp 0 (latency-bound: see TeamWarp)
-            if (threadIdx.x < 32) hhs_loop<TeamWarp>(sm, P, pN, pG, sp);
+            if (threadIdx.x < 32) hhs_loop<TeamWarp>(sm, st, P, pN, pG, sp);
             continue;
         }
         if (stage == 0) {
@@ -440,95 +572,145 @@ __device__ void hhs_loop(SmallSmem &sm, const SmallParams &P, const SweepParams 
                 if (T::tid() == 0) sm.err = FROST_EDEPTH;
                 continue;
             }
-            cta_timesteps<T>(sm, pG, start, cnt);
+            const bool split = P.split_max > 0 && cnt <= P.split_max;
+            cta_timesteps<T>(sm, pG, start, cnt, split ? tau : -1.0);
             const int nS = cta_partition<T>(sm, start, cnt, tau);
             const int nF = cnt - nS;
-            if (nS > 0 && nF > 0) {
-                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
-                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
-                cta_kick<T>(sm, start, cnt, tau / 6.0, 0.0, false);
-            }
-            cta_fsi<T>(sm, pN, pG, start, nS, 0.5 * tau);
+            int m = nF > 0 ? 1 : 0;
+            long long sumsq = (long long)nF * nF;
+            if (split && nF > 0) m = cta_components<T>(sm, start + nS, nF, sp, &sumsq);
+            else if (T::tid() == 0) sm.f_bnd[sp][0] = 1u;
+            cta_cross_kick<T>(sm, pN, pG, start, nS, nF, m, sp, tau / 6.0, 0.0, false);
+            cta_fsi<T>(sm, st, pN, pG, start, nS, 0.5 * tau);
             T::sync();
             if (T::tid() == 0) {
-                sm.f_ns[sp] = nS;
-                sm.st_entries[level] += 1; sm.st_slow[level] += nS; sm.st_fast[level] += nF;
-                sm.st_pt += (long long)cnt * cnt;
-                if (level > sm.st_depth) sm.st_depth = level;
+                sm.f_ns[sp] = nS; sm.f_m[sp] = m; sm.f_sumsq[sp] = sumsq; sm.f_cpos[sp] = 0;
+                atomicAdd(&st.entries[level], 1ull); atomicAdd(&st.slow[level], (unsigned long long)nS);
+                atomicAdd(&st.fast[level], (unsigned long long)nF); atomicAdd(&st.comps[level], (unsigned long long)m);
+                atomicAdd(&st.pt, (unsigned long long)cnt * cnt);
+                atomicMax(&st.depth, level);
                 sm.f_stage[sp] = 1;
-                if (nF > 0) {
-                    sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
-                    sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
-                    sm.sp = sp + 1;
-                }
-            }
-        } else if (stage == 1) {
-            const int nS = sm.f_ns[sp], nF = cnt - nS;
-            if (nS > 0 && nF > 0) {
-                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
-                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
-                cta_gradient<T>(sm, pG, start, nS, start + nS, nF);
-                cta_gradient<T>(sm, pG, start + nS, nF, start, nS);
-                cta_kick<T>(sm, start, cnt, 2.0 * tau / 3.0, tau * tau / 48.0, true);
-            }
-            T::sync();
-            if (T::tid() == 0) {
-                sm.f_stage[sp] = 2;
-                if (nF > 0) {
-                    sm.f_start[sp + 1] = start + nS; sm.f_n[sp + 1] = nF; sm.f_ns[sp + 1] = 0;
-                    sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
-                    sm.sp = sp + 1;
-                }
             }
         } else {
-            const int nS = sm.f_ns[sp], nF = cnt - nS;
-            cta_fsi<T>(sm, pN, pG, start, nS, 0.5 * tau);
-            if (nS > 0 && nF > 0) {
-                cta_newton<T>(sm, pN, start, nS, start + nS, nF);
-                cta_newton<T>(sm, pN, start + nS, nF, start, nS);
-                cta_kick<T>(sm, start, cnt, tau / 6.0, 0.0, false);
-            }
-            T::sync();
-            if (T::tid() == 0) {
-                const long long cr = 2LL * nS * nF;
-                sm.st_pn += 3 * cr; sm.st_pg += cr;
-                sm.sp = sp - 1;
+            const int nS = sm.f_ns[sp], nF = cnt - nS, m = sm.f_m[sp], cpos = sm.f_cpos[sp];
+            if (cpos < nF) {            // hhs_fsi(C_c, tau/2) of the next component
+                const int size = (m > 1) ? comp_size(sm, sp, cpos, nF) : nF;
+                T::sync();
+                if (T::tid() == 0) {
+                    sm.f_cpos[sp] = cpos + size;
+                    sm.f_start[sp + 1] = start + nS + cpos; sm.f_n[sp + 1] = size; sm.f_ns[sp + 1] = 0;
+                    sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                    sm.sp = sp + 1;
+                }
+            } else if (stage == 1) {
+                cta_cross_kick<T>(sm, pN, pG, start, nS, nF, m, sp, 2.0 * tau / 3.0, tau * tau / 48.0, true);
+                T::sync();
+                if (T::tid() == 0) { sm.f_stage[sp] = 2; sm.f_cpos[sp] = 0; }
+            } else {
+                cta_fsi<T>(sm, st, pN, pG, start, nS, 0.5 * tau);
+                cta_cross_kick<T>(sm, pN, pG, start, nS, nF, m, sp, tau / 6.0, 0.0, false);
+                T::sync();
+                if (T::tid() == 0) {
+                    // ordered pairs of the kicked set: all but slow-slow and same-component pairs
+                    const unsigned long long cr =
+                        (unsigned long long)((long long)cnt * cnt - (long long)nS * nS - sm.f_sumsq[sp]);
+                    atomicAdd(&st.pn, 3 * cr); atomicAdd(&st.pg, cr);
+                    sm.sp = sp - 1;
+                }
             }
         }
     }
 }
 
-template <class T>
-__global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const SmallParams P) {
-    extern __shared__ __align__(16) unsigned char small_raw[];
-    SmallSmem &sm = *reinterpret_cast<SmallSmem *>(small_raw);
-    const int n = P.n, ld = P.ld;
-    for (int k = threadIdx.x; k < n; k += kSmallThreads) {
-        const int i = P.idx ? P.idx[k] : k;
+__device__ __forceinline__ void stats_zero(SmStats &st, int tid, int nthreads) {
+    for (int k = tid; k < FROST_MAX_LEVELS; k += nthreads) {
+        st.entries[k] = 0; st.slow[k] = 0; st.fast[k] = 0; st.comps[k] = 0;
+    }
+    if (tid == 0) { st.pn = st.pg = st.pt = 0; st.depth = -1; }
+}
+
+// atomics: an fsi(S) launch on a side stream, or other CTAs of a batch, run concurrently
+__device__ __forceinline__ void stats_flush(const SmStats &st, SmallStats *out, int err, int tid, int nthreads) {
+    typedef unsigned long long ull;
+    for (int k = tid; k < FROST_MAX_LEVELS; k += nthreads) {
+        if (st.entries[k]) {
+            atomicAdd((ull *)&out->entries[k], st.entries[k]);
+            atomicAdd((ull *)&out->n_slow[k], st.slow[k]);
+            atomicAdd((ull *)&out->n_fast[k], st.fast[k]);
+            atomicAdd((ull *)&out->n_comp[k], st.comps[k]);
+        }
+    }
+    if (tid == 0) {
+        atomicAdd((ull *)&out->pairs_newton, st.pn);
+        atomicAdd((ull *)&out->pairs_gradient, st.pg);
+        atomicAdd((ull *)&out->pairs_timestep, st.pt);
+        atomicMax(&out->depth, st.depth);
+        if (err) atomicCAS(&out->status, 0, err);
+    }
+}
+
+template <class SM>
+__device__ __forceinline__ void set_load(SM &sm, const SmallParams &P, const int32_t *idx, int n, int tid,
+                                         int nthreads) {
+    const int ld = P.ld;
+    for (int k = tid; k < n; k += nthreads) {
+        const int i = idx ? idx[k] : k;
         sm.xm[k] = make_double4(P.pos[i], P.pos[(size_t)ld + i], P.pos[2 * (size_t)ld + i], P.mass[i]);
         sm.vv[k] = make_double4(P.vel[i], P.vel[(size_t)ld + i], P.vel[2 * (size_t)ld + i], 1.0);
         sm.perm[k] = k;
     }
-    for (int k = threadIdx.x; k < FROST_MAX_LEVELS; k += kSmallThreads) {
-        sm.st_entries[k] = 0; sm.st_slow[k] = 0; sm.st_fast[k] = 0;
-    }
-    if (threadIdx.x == 0) {
-        sm.sp = 0; sm.err = 0; sm.st_pn = sm.st_pg = sm.st_pt = 0; sm.st_depth = -1;
+    if (tid == 0) {
+        sm.sp = 0; sm.err = 0;
         sm.f_start[0] = 0; sm.f_n[0] = n; sm.f_ns[0] = 0; sm.f_stage[0] = 0; sm.f_tau[0] = P.tau_pivot;
     }
-    SweepParams pN{}, pG{};
+}
+
+template <class SM>
+__device__ __forceinline__ void set_store(const SM &sm, const SmallParams &P, const int32_t *idx, int n,
+                                          int tid, int nthreads) {
+    const int ld = P.ld;
+    for (int k = tid; k < n; k += nthreads) {
+        const int i = idx ? idx[k] : k;
+        const double4 x = sm.xm[k], v = sm.vv[k];
+        P.pos[i] = x.x; P.pos[(size_t)ld + i] = x.y; P.pos[2 * (size_t)ld + i] = x.z;
+        P.vel[i] = v.x; P.vel[(size_t)ld + i] = v.y; P.vel[2 * (size_t)ld + i] = v.z;
+    }
+}
+
+__device__ __forceinline__ void sweep_params(const SmallParams &P, SweepParams &pN, SweepParams &pG) {
+    pN = SweepParams{}; pG = SweepParams{};
     pN.G = pG.G = P.G; pN.eta_ff = pG.eta_ff = P.eta_ff; pN.eta_fb = pG.eta_fb = P.eta_fb;
     pG.eps2 = P.eps2;
     pN.eps2 = P.eps2 > 0x1p-400 ? P.eps2 : 0x1p-400;     // see NewtonPolicy::pair
+}
+
+// One set per CTA (or per cluster of replica CTAs).  With P.desc the launch is a batch: CTA b takes
+// the set described by desc[b] (components of 33-1024 particles of a split entry).
+template <class T>
+__global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const SmallParams P) {
+    extern __shared__ __align__(16) unsigned char small_raw[];
+    SmallSmem &sm = *reinterpret_cast<SmallSmem *>(small_raw);
+    SmStats &st = *reinterpret_cast<SmStats *>(small_raw + sizeof(SmallSmem));
+    const int32_t *idx = P.idx;
+    int n = P.n;
+    if (P.desc) {
+        if ((int)blockIdx.x >= *P.n_desc) return;
+        const int2 d = P.desc[blockIdx.x];
+        idx = P.idx + d.x; n = d.y;
+    }
+    set_load(sm, P, idx, n, threadIdx.x, kSmallThreads);
+    stats_zero(st, threadIdx.x, kSmallThreads);
+    SweepParams pN, pG;
+    sweep_params(P, pN, pG);
     __syncthreads();
 
     if (P.mode == 1) {
         for (int k = 0; k < P.n_steps; ++k) {
-            if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, pN, pG, 0, n, P.dt_fsi); }
-            else cta_fsi<T>(sm, pN, pG, 0, n, P.dt_fsi);
+            if (n <= kWarpTeamMax) { if (threadIdx.x < 32) cta_fsi<TeamWarp>(sm, st, pN, pG, 0, n, P.dt_fsi); }
+            else cta_fsi<T>(sm, st, pN, pG, 0, n, P.dt_fsi);
         }
     } else {
-        hhs_loop<T>(sm, P, pN, pG, 0);
+        hhs_loop<T>(sm, st, P, pN, pG, 0);
     }
     __syncthreads();
     if (T::kCluster) {      // replicas are identical: rank 0 writes back; nobody leaves while a peer
@@ -537,59 +719,105 @@ __global__ void __launch_bounds__(kSmallThreads, 1) hhs_small_kernel(const Small
         cl.sync();
         if (cl.block_rank() != 0) return;
     }
-    for (int k = threadIdx.x; k < n; k += kSmallThreads) {
-        const int i = P.idx ? P.idx[k] : k;
-        const double4 x = sm.xm[k], v = sm.vv[k];
-        P.pos[i] = x.x; P.pos[(size_t)ld + i] = x.y; P.pos[2 * (size_t)ld + i] = x.z;
-        P.vel[i] = v.x; P.vel[(size_t)ld + i] = v.y; P.vel[2 * (size_t)ld + i] = v.z;
+    set_store(sm, P, idx, n, threadIdx.x, kSmallThreads);
+    if (P.stats) stats_flush(st, P.stats, sm.err, threadIdx.x, kSmallThreads);
+}
+
+// Batch of small components (<= 32 particles each, in practice binaries and triples): one WARP per
+// component, kCompWarps per CTA, each with its own 8 KB of shared memory -- the deep hierarchy of a
+// hard binary is a chain of dependent phases on one warp, and all the unrelated
+// binaries of a split level run their chains side by side instead of one after the other.
+using CompSmem = SmallSmemT<kCompWarpMax>;
+
+__global__ void __launch_bounds__(kCompWarps * 32) hhs_comp_kernel(const SmallParams P) {
+    extern __shared__ __align__(16) unsigned char small_raw[];
+    CompSmem *sms = reinterpret_cast<CompSmem *>(small_raw);
+    SmStats &st = *reinterpret_cast<SmStats *>(small_raw + kCompWarps * sizeof(CompSmem));
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    stats_zero(st, threadIdx.x, kCompWarps * 32);
+    __syncthreads();
+    const int c = blockIdx.x * kCompWarps + warp;
+    int err = 0;
+    if (c < *P.n_desc) {
+        CompSmem &sm = sms[warp];
+        const int2 d = P.desc[c];
+        const int32_t *idx = P.idx + d.x;
+        set_load(sm, P, idx, d.y, lane, 32);
+        SweepParams pN, pG;
+        sweep_params(P, pN, pG);
+        __syncwarp();
+        hhs_loop<TeamWarp>(sm, st, P, pN, pG, 0);
+        __syncwarp();
+        set_store(sm, P, idx, d.y, lane, 32);
+        err = sm.err;
     }
-    if (P.stats) {      // atomics: an fsi(S) launch on a side stream may run concurrently (frost_api.cu)
-        typedef unsigned long long ull;
-        for (int k = threadIdx.x; k < FROST_MAX_LEVELS; k += kSmallThreads) {
-            if (sm.st_entries[k]) {
-                atomicAdd((ull *)&P.stats->entries[k], (ull)sm.st_entries[k]);
-                atomicAdd((ull *)&P.stats->n_slow[k], (ull)sm.st_slow[k]);
-                atomicAdd((ull *)&P.stats->n_fast[k], (ull)sm.st_fast[k]);
-            }
-        }
-        if (threadIdx.x == 0) {
-            atomicAdd((ull *)&P.stats->pairs_newton, (ull)sm.st_pn);
-            atomicAdd((ull *)&P.stats->pairs_gradient, (ull)sm.st_pg);
-            atomicAdd((ull *)&P.stats->pairs_timestep, (ull)sm.st_pt);
-            atomicMax(&P.stats->depth, sm.st_depth);
-            if (sm.err) atomicCAS(&P.stats->status, 0, sm.err);
-        }
-    }
+    err = __syncthreads_or(err);
+    if (P.stats) stats_flush(st, P.stats, err ? FROST_EDEPTH : 0, threadIdx.x, kCompWarps * 32);
 }
 
 int small_max() { return kSmallMax; }
+int comp_warp_max() { return kCompWarpMax; }
+
+static SmallParams small_params(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
+                                const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats,
+                                int n_steps) {
+    SmallParams P{};
+    P.idx = idx; P.n = n; P.ld = ld; P.pos = pos; P.vel = vel; P.mass = mass;
+    P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0; P.n_steps = n_steps;
+    P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
+    P.stats = (SmallStats *)dev_stats;
+    P.split_max = c->split_max;
+    return P;
+}
+
+static int small_attrs(frost_ctx *c) {
+    const int bytes = (int)(sizeof(SmallSmem) + sizeof(SmStats));
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    FROST_TRY(set_func_attr(c, hhs_comp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                            (int)(kCompWarps * sizeof(CompSmem) + sizeof(SmStats))));
+    return FROST_OK;
+}
 
 // mode 0: hhs_fsi(set, tau) subtree rooted at hierarchy level `level0`; mode 1: fsi(set, dt).
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
                  const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps) {
     if (n <= 0) return FROST_OK;
     if (n > kSmallMax) return FROST_EINVAL;
-    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCTA>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)sizeof(SmallSmem)));
-    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                            (int)sizeof(SmallSmem)));
-    FROST_TRY(set_func_attr(c, hhs_small_kernel<TeamCluster>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-    SmallParams P{};
-    P.idx = idx; P.n = n; P.ld = ld; P.pos = pos; P.vel = vel; P.mass = mass;
-    P.tau_pivot = tau_or_dt; P.dt_fsi = tau_or_dt; P.mode = mode; P.level0 = level0; P.n_steps = n_steps;
-    P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
-    P.stats = (SmallStats *)dev_stats;
+    FROST_TRY(small_attrs(c));
+    const SmallParams P = small_params(c, mode, ld, pos, vel, mass, idx, n, tau_or_dt, level0, dev_stats, n_steps);
+    const size_t bytes = sizeof(SmallSmem) + sizeof(SmStats);
     if (n >= kClusterMinSet && c->tune_cluster != 1) {   // one cluster of kClusterSize replicas
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(kClusterSize); cfg.blockDim = dim3(kSmallThreads);
-        cfg.dynamicSmemBytes = sizeof(SmallSmem); cfg.stream = c->stream;
+        cfg.dynamicSmemBytes = bytes; cfg.stream = c->stream;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
         at[0].val.clusterDim.x = kClusterSize; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         FROST_CUDA(c, cudaLaunchKernelEx(&cfg, hhs_small_kernel<TeamCluster>, P));
     } else {
-        hhs_small_kernel<TeamCTA><<<1, kSmallThreads, sizeof(SmallSmem), c->stream>>>(P);
+        hhs_small_kernel<TeamCTA><<<1, kSmallThreads, bytes, c->stream>>>(P);
+    }
+    return check_launch(c);
+}
+
+// hhs_fsi(C, tau) for a batch of components of one split entry (device-resident descriptors:
+// desc[b] = {offset into idx, size}, *n_desc of them, at most max_desc).  warp_team: components of at
+// most kCompWarpMax particles, one warp each; otherwise up to kSmallMax particles, one CTA each.
+int launch_comp_batch(frost_ctx *c, int warp_team, int ld, double *pos, double *vel, const double *mass,
+                      const int32_t *idx, const void *desc, const int *n_desc, int max_desc, double tau,
+                      int level0, void *dev_stats) {
+    if (max_desc <= 0) return FROST_OK;
+    FROST_TRY(small_attrs(c));
+    SmallParams P = small_params(c, 0, ld, pos, vel, mass, idx, 0, tau, level0, dev_stats, 1);
+    P.desc = (const int2 *)desc; P.n_desc = n_desc;
+    if (warp_team) {
+        const int grid = (max_desc + kCompWarps - 1) / kCompWarps;
+        hhs_comp_kernel<<<grid, kCompWarps * 32, kCompWarps * sizeof(CompSmem) + sizeof(SmStats), c->stream>>>(P);
+    } else {
+        hhs_small_kernel<TeamCTA><<<max_desc, kSmallThreads, sizeof(SmallSmem) + sizeof(SmStats), c->stream>>>(P);
     }
     return check_launch(c);
 }

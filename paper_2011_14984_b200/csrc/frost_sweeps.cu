@@ -95,7 +95,7 @@ sweep_kernel(const SweepParams prm) {
 // ------------------------------------------------------------------------------------------------
 __global__ void reduce_vec_kernel(const double *__restrict__ partial, int n_pad, int slices, int n_snk,
                                   double scale, const int32_t *__restrict__ idx, int ld,
-                                  double *__restrict__ out, double4 *__restrict__ packed, int accumulate) {
+                                  double *__restrict__ out, double4 *__restrict__ packed, int accumulate, int keep_w = 0) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_snk) return;
     double sx = 0.0, sy = 0.0, sz = 0.0;
@@ -107,7 +107,10 @@ __global__ void reduce_vec_kernel(const double *__restrict__ partial, int n_pad,
     const int g = idx ? idx[i] : i;
     if (accumulate) { sx += out[g]; sy += out[(size_t)ld + g]; sz += out[2 * (size_t)ld + g]; }
     out[g] = sx; out[(size_t)ld + g] = sy; out[2 * (size_t)ld + g] = sz;
-    if (packed) packed[i] = make_double4(sx, sy, sz, 1.0);
+    if (packed) {
+        if (keep_w) { double *q = (double *)(packed + i); q[0] = sx; q[1] = sy; q[2] = sz; }   // .w = label
+        else packed[i] = make_double4(sx, sy, sz, 1.0);
+    }
 }
 
 __global__ void reduce_tau_kernel(const double *__restrict__ partial, int n_pad, int slices, int n_set,
@@ -232,7 +235,7 @@ int sweep_gradient(frost_ctx *c, const double *snk_xm, const double *snk_a, int 
 }
 
 int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
-                   double tau_pivot, double *out_tau, int32_t *out_bin) {
+                   double tau_pivot, double *out_tau, int32_t *out_bin, int *forest) {
     if (n_set <= 0) return FROST_OK;
     const Plan pl = make_plan(c, n_set, n_set, 2);
     const int n_pad = pad1024(n_set);
@@ -243,10 +246,45 @@ int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, c
     prm.partial = (double *)c->partial.p; prm.n_pad = n_pad;
     prm.n_tiles = pl.n_tiles; prm.tiles_per_slice = pl.tiles_per_slice;
     prm.eps2 = 0.0; prm.G = c->G; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-    FROST_TRY(launch_sweep<TimestepPolicy>(c, prm, pl));
+    prm.pivot = tau_pivot; prm.forest = forest;
+    if (forest) FROST_TRY(launch_sweep<TimestepEdgePolicy>(c, prm, pl));
+    else FROST_TRY(launch_sweep<TimestepPolicy>(c, prm, pl));
     reduce_tau_kernel<<<(n_set + 255) / 256, 256, 0, c->stream>>>(
         (const double *)c->partial.p, n_pad, pl.slices, n_set, idx, tau_pivot, out_tau, out_bin);
     return check_launch(c);
+}
+
+// The inter-level kick of a split hierarchy entry needs a_i and g_i over the pairs of the entry's set
+// whose component labels differ (reading 24).  One-sided self sweep of the list; the label
+// stream shares the records of the packed accelerations.
+int sweep_masked(frost_ctx *c, const double *xm, double *a_lab, int n_set, const int32_t *idx, int ld,
+                 double *out_acc, double *out_grad) {
+    if (n_set <= 0) return FROST_OK;
+    const int n_pad = pad1024(n_set);
+    for (int pass = 0; pass < (out_grad ? 2 : 1); ++pass) {
+        const Plan pl = make_plan(c, n_set, n_set, pass == 0 ? 4 : 2);
+        FROST_TRY(ensure(c, c->partial, (size_t)pl.slices * 3 * n_pad * sizeof(double)));
+        SweepParams prm{};
+        prm.snk0 = prm.src0 = (const double4 *)xm; prm.snk1 = prm.src1 = (const double4 *)a_lab;
+        prm.partial = (double *)c->partial.p; prm.n_pad = n_pad;
+        prm.n_tiles = pl.n_tiles; prm.tiles_per_slice = pl.tiles_per_slice;
+        prm.G = c->G; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+        if (pass == 0) {
+            prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
+            FROST_TRY(launch_sweep<MaskedNewtonPolicy>(c, prm, pl));
+            reduce_vec_kernel<<<(n_set + 255) / 256, 256, 0, c->stream>>>(
+                (const double *)c->partial.p, n_pad, pl.slices, n_set, c->G, idx, ld, out_acc,
+                (double4 *)a_lab, 0, 1);
+        } else {
+            prm.eps2 = c->eps2;
+            FROST_TRY(launch_sweep<MaskedGradientPolicy>(c, prm, pl));
+            reduce_vec_kernel<<<(n_set + 255) / 256, 256, 0, c->stream>>>(
+                (const double *)c->partial.p, n_pad, pl.slices, n_set, 2.0 * c->G, idx, ld, out_grad,
+                nullptr, 0, 0);
+        }
+        FROST_TRY(check_launch(c));
+    }
+    return FROST_OK;
 }
 
 }  // namespace frost

@@ -40,6 +40,8 @@ struct SymParams {
     int seg_tiles;            // B tiles per CTA
     int row0, row_stride;     // A tiles owned by this launch: row0, row0 + row_stride, ... (sharding)
     double eps2, eta_ff, eta_fb;
+    double pivot;             // SymTimestepEdge: fast pairs (candidate < pivot) are united in `forest`
+    int *forest;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -125,8 +127,8 @@ struct SymTimestep {
     // The symmetrised candidate of Eq. 49-54 is the same number for (i <- j) and (j <- i)
     // (r.v, r^2, v^2 and m_i + m_j are even under the swap), so it is evaluated once
     // -- exactly TimestepPolicy::pair -- and min-ed into both particles.
-    __device__ static __forceinline__ void pair(A &a, double (&b)[1], const double4 &j0,
-                                                const double4 &j1, const SymParams &p) {
+    __device__ static __forceinline__ double candidate(const A &a, const double4 &j0, const double4 &j1,
+                                                       const SymParams &p) {
         const double rx = j0.x - a.x, ry = j0.y - a.y, rz = j0.z - a.z;
         const double vx = j1.x - a.vx, vy = j1.y - a.vy, vz = j1.z - a.vz;
         const double r2 = fma(rz, rz, fma(ry, ry, rx * rx));
@@ -145,9 +147,33 @@ struct SymTimestep {
         const double q_fb = fma(f, mir * (iv * iv), f) * p.eta_fb;
         const double c_ff = sym_factor(q_ff) * (t_ff * p.eta_ff);
         const double c_fb = sym_factor(q_fb) * (t_fb * p.eta_fb);
-        const double c = fmin(c_ff, c_fb);
+        return fmin(c_ff, c_fb);
+    }
+    __device__ static __forceinline__ void pair(A &a, double (&b)[1], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double c = candidate(a, j0, j1, p);
         a.s[0] = fmin(a.s[0], c);
         b[0] = fmin(b[0], c);
+    }
+};
+
+// SymTimestep for a split hierarchy entry (reading 24): every fast pair is also united in the
+// union-find forest over list positions (low word of .w of the velocity records).
+struct SymTimestepEdge {
+    static constexpr int kRecs = 2, kPlanes = 1;
+    static constexpr bool kMin = true;
+    struct A : SymTimestep::A { int id; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        SymTimestep::load(a, p, i);
+        a.id = __double2loint(p.a1[i].w);
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[1]) { SymTimestep::init_b(b); }
+    __device__ static __forceinline__ void pair(A &a, double (&b)[1], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double c = SymTimestep::candidate(a, j0, j1, p);
+        a.s[0] = fmin(a.s[0], c);
+        b[0] = fmin(b[0], c);
+        if (c < p.pivot) uf_union(p.forest, a.id, __double2loint(j1.w));
     }
 };
 
@@ -359,6 +385,7 @@ struct SymJob {
     double *A_packed, *B_packed;         // optional packed {s_x, s_y, s_z, 1} streams of the results
     double scale, eps2, tau_pivot;
     int32_t *out_bin;
+    int *forest = nullptr;                 // time-step sweep: union-find forest of the fast pairs
     int shard_rank = 0, shard_world = 1;   // this launch sweeps A tiles rank, rank + world, ... only
     int accumulate = 0;                    // add the sums to `out` instead of overwriting it
 };
@@ -416,6 +443,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         prm.na_pad = na_pad; prm.self = self ? 1 : 0; prm.bt0 = bt0; prm.bt1 = bt1;
         prm.seg_tiles = (int)seg; prm.row0 = row0; prm.row_stride = row_stride;
         prm.eps2 = job.eps2; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+        prm.pivot = job.tau_pivot; prm.forest = job.forest;
         if (my_rows > 0) {
             dim3 grid(my_rows, segs);
             sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
@@ -485,11 +513,15 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
 
 // Time-step sweep over one level (Eq. 49-54); xm carries G*m in .w and NaN padding.
 int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, const int32_t *idx,
-                 double tau_pivot, double *out_tau, int32_t *out_bin) {
+                 double tau_pivot, double *out_tau, int32_t *out_bin, int *forest) {
     if (n_set <= 0) return FROST_OK;
     SymJob j{};
     j.A0 = xm; j.A1 = v; j.nA = n_set; j.nB = n_set; j.self = true; j.A_idx = idx;
-    j.out = out_tau; j.out_bin = out_bin; j.tau_pivot = tau_pivot; j.scale = 1.0;
+    j.out = out_tau; j.out_bin = out_bin; j.tau_pivot = tau_pivot; j.scale = 1.0; j.forest = forest;
+    if (forest) {
+        if (n_set < kSymSmallN) return run_sym<SymTimestepEdge, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
+        return run_sym<SymTimestepEdge, kSymKTau, kSymNT, kSymMinB>(c, j);
+    }
     if (n_set < kSymSmallN) return run_sym<SymTimestep, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymTimestep, kSymKTau, kSymNT, kSymMinB>(c, j);
 }

@@ -30,15 +30,23 @@ __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__r
 // The 1 marks a real record (the time-step sweep skips records whose flag is 0).
 __global__ void pack_vec_kernel(const double *__restrict__ planes, int ld,
                                 const int32_t *__restrict__ idx, int n_idx, int n_pad,
-                                double4 *__restrict__ out) {
+                                double4 *__restrict__ out, int w_index) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_pad) return;
     double4 r = make_double4(0.0, 0.0, 0.0, 0.0);
     if (k < n_idx) {
         const int i = idx ? idx[k] : k;
-        r = make_double4(planes[i], planes[(size_t)ld + i], planes[2 * (size_t)ld + i], 1.0);
+        r = make_double4(planes[i], planes[(size_t)ld + i], planes[2 * (size_t)ld + i],
+                         w_index ? __hiloint2double(0, k) : 1.0);
     }
     out[k] = r;
+}
+
+// vec[k].w <- the component label of list position k in its low word (never read as a number)
+__global__ void pack_label_kernel(const int *__restrict__ lab, int n_idx, int n_pad, double4 *__restrict__ vec) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n_pad) return;
+    vec[k].w = __hiloint2double(0, k < n_idx ? lab[k] : -2);
 }
 
 __global__ void kick_kernel(double *__restrict__ vel, const double *__restrict__ acc,
@@ -232,10 +240,16 @@ int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, 
 }
 
 int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,
-                    int n_pad, double *out) {
+                    int n_pad, double *out, int w_index) {
     if (n_pad <= 0) return FROST_OK;
     pack_vec_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(planes, ld, idx, n_idx, n_pad,
-                                                              (double4 *)out);
+                                                              (double4 *)out, w_index);
+    return check_launch(c);
+}
+
+int launch_pack_label(frost_ctx *c, const int *lab, int n_idx, int n_pad, double *vec) {
+    if (n_pad <= 0) return FROST_OK;
+    pack_label_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(lab, n_idx, n_pad, (double4 *)vec);
     return check_launch(c);
 }
 

@@ -1,0 +1,125 @@
+"""Spatial splitting of fast hierarchy levels (frost_set_split) against the oracle's
+definition of it (oracle/frost_oracle.c O6s, reading 24): the masked kick sweeps element by
+element, the bookkeeping of a split step IDENTICAL (level sets, components per level, pair counts), the
+trajectory inside the oracle's own +-1-ulp envelope, momentum at rounding level -- on the host-driven
+levels, in the batched one-warp-per-component kernel and inside the device-resident subtree kernel."""
+import numpy as np
+import pytest
+import torch
+
+import frost_inputs as fi
+from test_gpu_parity import (TOL_A, TOL_G, dev, envelope_ratio, momentum_change, oracle_hhs_with_envelope,
+                             vec_err)
+
+pytestmark = pytest.mark.gpu
+BIG = 1 << 20
+
+
+@pytest.fixture(scope="module")
+def fr():
+    import paper_2011_14984_b200 as frost
+    f = frost.Frost()
+    yield f
+    f.close()
+
+
+@pytest.mark.parametrize("n,eps2", [(700, 0.0), (5000, 0.0), (5000, 1e-6)])
+def test_masked_kick_sweeps_match_oracle(fr, oracle, n, eps2):
+    """frost_forces_masked (the kick sweeps of a split entry, Eq. 42-44 on "labels differ") against
+    oracle_forces_masked on a sub-list with slow particles (-1), two-body and larger components."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    rng = np.random.default_rng(n)
+    idx = np.sort(rng.choice(n, size=n - n // 7, replace=False)).astype(np.int32)
+    lab_pos = rng.integers(0, idx.size // 3, size=idx.size).astype(np.int32)       # ~3 members per label
+    lab_pos[rng.random(idx.size) < 0.4] = -1
+    label_g = np.full(n, -7, dtype=np.int32)
+    label_g[idx] = lab_pos
+    fr.set_params(G=0.9, eps2=eps2)
+    a_ref, g_ref = oracle.forces_masked(pos, mass, idx, label_g, G=0.9, eps2=eps2)
+    a, g = fr.forces_masked(dev(pos), dev(mass), torch.as_tensor(lab_pos).cuda(), idx=torch.as_tensor(idx).cuda())
+    torch.cuda.synchronize()
+    fr.set_params()
+    a, g = a.cpu().numpy(), g.cpu().numpy()
+    out = np.setdiff1d(np.arange(n), idx)
+    assert (a[:, out] == 0).all() and (g[:, out] == 0).all()
+    assert vec_err(a[:, idx], a_ref[:, idx]) <= TOL_A
+    assert vec_err(g[:, idx], g_ref[:, idx]) <= TOL_G
+
+
+def _split_case(fr, oracle, pos, vel, mass, dt, small, one_cta=0, **kw):
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, split_max=BIG, **kw)
+    assert all(s == st_ref for s in sts)
+    fr.set_tuning(0, 0, small, one_cta)
+    fr.set_split(BIG)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), dt)
+    finally:
+        fr.set_split(0)
+        fr.set_tuning(0, 0, -1, 0)
+    return st, st_ref, p.cpu().numpy(), v.cpu().numpy(), pr, vr, env_p, env_v
+
+
+@pytest.mark.parametrize("n,small,one_cta,log2dt", [(256, -1, 0, 7), (256, -1, 1, 7), (256, 48, 0, 7), (256, 0, 0, 9),
+                                                    (1024, -1, 0, 8), (3000, -1, 0, 8), (3000, 100, 0, 8)])
+def test_split_step_matches_split_oracle(fr, oracle, n, small, one_cta, log2dt, capsys):
+    """One split HHS-FSI step of config 5's recipe (binaries a = 1e-5..1e-3, e <= 0.1 so that no pair
+    step oscillates across a pivot): n <= 1024 with small = -1 runs entirely inside the subtree kernel
+    (cluster or one CTA at the top, components handed to the quad / warp teams); small = 48 / 100 /
+    0 drive the top levels from the host, with the masked kick sweeps, and advance the components by
+    the batched one-warp-per-component launches."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    st, st_ref, pg, vg, pr, vr, env_p, env_v = _split_case(fr, oracle, pos, vel, mass, 2.0 ** -log2dt, small, one_cta)
+    assert st == st_ref
+    assert st["depth"] >= 12 and st["n_comp"][0] > 1
+    rp, rv = envelope_ratio(pg, vg, pr, vr, env_p, env_v)
+    with capsys.disabled():
+        print(f"\n[split n={n} small={small} one_cta={one_cta}] depth {st['depth']}, components per level "
+              f"{st['n_comp'][:6]}..., entries {sum(st['entries'])}; envelope ratio x {rp:.3f}, v {rv:.3f}")
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, vg, vr) <= 1.0
+
+
+def test_split_with_one_component_is_the_unsplit_step_bitwise(fr):
+    """A hard binary among distant slow stars: F is the binary (one component) at every level, so the
+    split step must be Alg. 3's bits -- from the host-driven levels (small = 0) and inside the subtree
+    kernel alike."""
+    b_pos, b_vel, b_mass, P = fi.kepler_binary(1.0, 0.7, 1e-3, 0.3)
+    rng = np.random.default_rng(3)
+    pos = np.ascontiguousarray(np.concatenate([b_pos, rng.normal(size=(3, 6)) * 3.0], axis=1))
+    vel = np.ascontiguousarray(np.concatenate([b_vel, rng.normal(size=(3, 6)) * 0.1], axis=1))
+    mass = np.concatenate([b_mass, np.full(6, 0.5)])
+    fr.set_params()
+    for small in (-1, 0):
+        out = []
+        for split in (0, BIG):
+            fr.set_tuning(0, 0, small)
+            fr.set_split(split)
+            p, v = dev(pos), dev(vel)
+            try:
+                st = fr.hhs_step(p, v, dev(mass), 2.0 ** -6)
+            finally:
+                fr.set_split(0)
+                fr.set_tuning(0, 0, -1)
+            out.append((st, p, v))
+        assert out[0][0] == out[1][0] and out[0][0]["depth"] >= 2
+        assert torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])
+
+
+def test_split_max_limits_the_split_to_small_entries(fr, oracle):
+    """split_max = 500 on a 2000-star cluster: the entries above 500 members run Alg. 3 as printed, the
+    ones below split -- bookkeeping identical to the oracle's with the same parameter."""
+    pos, vel, mass, pairs = fi.star_cluster(2000, 4, e_max=0.1)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    pr, vr = pos.copy(), vel.copy()
+    st_ref = oracle.hhs_step(pr, vr, mass, 2.0 ** -8, split_max=500)
+    fr.set_split(500)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), 2.0 ** -8)
+    finally:
+        fr.set_split(0)
+    assert st == st_ref
+    assert st["n_comp"][0] == 1 and any(c > e for c, e in zip(st["n_comp"], st["entries"]))
+    assert np.abs((mass * (v.cpu().numpy() - vel)).sum(1)).max() < 1e-15

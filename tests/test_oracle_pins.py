@@ -595,3 +595,138 @@ def test_hhs_solar_system_fig5_energy_error_scales_as_eta4(oracle):
     assert abs(slope - 4.0) <= 0.5 and abs(slope_f - 4.0) <= 0.1, (slope, slope_f)
     assert all(10.0 <= x <= 50.0 for x in ratios), ratios
     assert all(r[2] < r[1] for r in rows), rows
+
+
+# ----------------------------------------------- O6s: spatially split fast levels
+def _two_planet_moon_systems():
+    """Star + two planet-moon pairs far from each other (G = 1): indices 0 star, 1/2 planet A and
+    its moon, 3/4 planet B and its moon."""
+    mass = np.array([1.0, 1e-3, 1e-5, 8e-4, 2e-5])
+    pos = np.zeros((3, 5)); vel = np.zeros((3, 5))
+    for k, (a, ph, am, phm) in zip((1, 3), [(1.0, 0.3, 0.012, 1.0), (1.7, 2.6, 0.015, 4.0)]):
+        pos[0, k], pos[1, k] = a * math.cos(ph), a * math.sin(ph)
+        v = math.sqrt(1.0 / a)
+        vel[0, k], vel[1, k] = -v * math.sin(ph), v * math.cos(ph)
+        vm = math.sqrt(mass[k] / am)
+        pos[:, k + 1] = pos[:, k] + am * np.array([math.cos(phm), math.sin(phm), 0.1])
+        vel[:, k + 1] = vel[:, k] + vm * np.array([-math.sin(phm), math.cos(phm), 0.0])
+    pos -= (pos * mass).sum(1, keepdims=True) / mass.sum()
+    vel -= (vel * mass).sum(1, keepdims=True) / mass.sum()
+    return np.ascontiguousarray(pos), np.ascontiguousarray(vel), mass
+
+
+def test_components_match_an_independent_graph_routine(oracle):
+    """oracle_components against scipy's connected_components on the fast-pair matrix built pair by
+    pair from oracle_pair_timestep (itself pinned above): labels = smallest member, -1 = no fast
+    pair; the particles without a fast pair are exactly the slow ones of Eq. 29."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    pos, vel, mass, pairs = fi.star_cluster(96, 4, binary_fraction=0.3, a_lo=1e-3, a_hi=3e-2)
+    idx = np.arange(3, 96, dtype=np.int32)                       # a level that is not everything
+    for pivot in (2.0 ** -4, 2.0 ** -7, 2.0 ** -10):
+        lab = oracle.components(pos, vel, mass, pivot, idx=idx)
+        tau, _ = oracle.timesteps(pos, vel, mass, idx=idx, tau_pivot=pivot)
+        n = idx.size
+        A = np.zeros((n, n), dtype=bool)
+        for a in range(n):
+            for b in range(a + 1, n):
+                i, j = idx[a], idx[b]
+                c = oracle.pair_timestep(pos[:, i], vel[:, i], mass[i], pos[:, j], vel[:, j], mass[j])
+                A[a, b] = A[b, a] = min(c) < pivot
+        ncomp, cl = connected_components(csr_matrix(A), directed=False)
+        want = np.full(pos.shape[1], -2, dtype=np.int32)
+        for c in range(ncomp):
+            members = idx[cl == c]
+            want[members] = members.min() if members.size > 1 else -1
+        assert (lab == want).all()
+        assert ((lab[idx] == -1) == (tau[idx] >= pivot)).all()
+        assert (lab[:3] == -2).all()
+    assert len(set(lab[idx][lab[idx] >= 0])) >= 5                # several components at the last pivot
+
+
+def test_masked_forces_match_autograd_of_the_cross_component_potential(oracle):
+    """The kicked pair set of the split level, P = {label_i != label_j}: a = -(1/m) dU_P/dx and
+    g = -(1/m) dG_P/dx with G_P = -sum m |a^P|^2 (Eq. 39, 42-44), by autograd."""
+    n = 9
+    pos, vel, mass = _random_system(n, 5)
+    label = np.array([-1, 1, 1, -1, 4, 4, 4, -1, 8], dtype=np.int32)    # 3 slow, comps {1,2} {4,5,6} {8}
+    M = np.zeros((n, n), dtype=bool)
+    for i in range(n):
+        for j in range(i + 1, n):
+            M[i, j] = label[i] != label[j]
+    for eps2 in (0.0, 0.03):
+        a_ref, g_ref = _autograd_a_g(pos, mass, 0.8, eps2, M)
+        a, g = oracle.forces_masked(pos, mass, np.arange(n, dtype=np.int32), label, G=0.8, eps2=eps2)
+        assert np.abs(a - a_ref).max() < 1e-12 * np.abs(a_ref).max()
+        assert np.abs(g - g_ref).max() < 1e-11 * np.abs(g_ref).max()
+        assert np.abs((mass * a).sum(1)).max() < 1e-15 and np.abs((mass * g).sum(1)).max() < 1e-13
+
+
+def test_split_step_is_alg3_bit_for_bit_when_F_is_one_component(oracle):
+    """O6s with m = 1 must be Alg. 3 exactly: a hard binary among distant slow
+    stars (F = the binary at every level), and a star with planets (F connected through the star)."""
+    b_pos, b_vel, b_mass, P = fi.kepler_binary(1.0, 0.7, 1e-3, 0.3)
+    rng = np.random.default_rng(3)
+    pos = np.ascontiguousarray(np.concatenate([b_pos, rng.normal(size=(3, 6)) * 3.0], axis=1))
+    vel = np.ascontiguousarray(np.concatenate([b_vel, rng.normal(size=(3, 6)) * 0.1], axis=1))
+    mass = np.concatenate([b_mass, np.full(6, 0.5)])
+    for (p0, v0, m0, dt, kw) in ((pos, vel, mass, 2.0 ** -6, {}),
+                                 (*fi.solar_system()[:3], 512.0, {"G": fi.solar_system()[3], "eta_ff": 0.05, "eta_fb": 0.05})):
+        p1, v1, p2, v2 = p0.copy(), v0.copy(), p0.copy(), v0.copy()
+        st1 = oracle.hhs_step(p1, v1, m0, dt, **kw)
+        st2 = oracle.hhs_step(p2, v2, m0, dt, split_max=1 << 20, **kw)
+        assert st1 == st2 and st1["depth"] >= 2
+        assert all(c <= e for c, e in zip(st1["n_comp"], st1["entries"]))
+        assert (p1 == p2).all() and (v1 == v2).all()
+
+
+def _split_frozen_error(oracle, nsteps, ref, split):
+    pos, vel, mass = _two_planet_moon_systems()
+    frozen = np.array([0, 1, 2, 1, 2], dtype=np.int32)         # star slow; planets level 1; moons level 2
+    comp = np.array([0, 1, 1, 2, 2], dtype=np.int32)
+    T = 0.05
+    st = None
+    for _ in range(nsteps):
+        st = oracle.hhs_step(pos, vel, mass, T / nsteps, frozen_level=frozen,
+                             split_max=(8 if split else 0), frozen_comp=comp)
+    return np.abs(pos - ref).max(), pos, vel, mass, st
+
+
+def test_split_hhs_is_fourth_order_with_frozen_components(oracle):
+    """The split scheme keeps Eq. (41)'s order: with a frozen partition (star | planet A + moon |
+    planet B + moon; moons one level below their planets) the position error against a 2048-step
+    reference falls 16x per halving of the top step, for the split scheme and for Alg. 3 alike, and
+    the two converge to the same solution; momentum stays at roundoff."""
+    pos, vel, mass = _two_planet_moon_systems()
+    frozen = np.array([0, 1, 2, 1, 2], dtype=np.int32)
+    for _ in range(2048):
+        oracle.hhs_step(pos, vel, mass, 0.05 / 2048, frozen_level=frozen)
+    for split in (True, False):
+        e1, *_ = _split_frozen_error(oracle, 8, pos, split)
+        e2, *_ = _split_frozen_error(oracle, 16, pos, split)
+        e3, p3, v3, m3, st = _split_frozen_error(oracle, 32, pos, split)
+        assert 13.0 < e1 / e2 < 19.0 and 13.0 < e2 / e3 < 19.0, (split, e1, e2, e3)
+        assert np.abs((m3 * v3).sum(1)).max() < 1e-17
+        assert st["n_comp"][0] == (2 if split else 1) and st["depth"] == 2
+
+
+def test_split_step_on_a_cluster_with_binaries(oracle):
+    """A 300-star cluster with hard binaries: the split step recurses into many components per
+    entry, conserves momentum to roundoff, keeps the energy error at the size of Alg. 3's, and ends
+    within the truncation error of Alg. 3's end state (both are fourth-order approximations of the
+    same flow; the slow pairs between components are kicked with tau_pivot instead of inside the
+    recursion -- the same rule Eq. 29 applies to slow particles)."""
+    pos, vel, mass, pairs = fi.star_cluster(300, 4, binary_fraction=0.2, a_lo=1e-4, a_hi=1e-2, e_max=0.3)
+    e0 = oracle.diagnostics(pos, vel, mass)["E"]
+    out = []
+    for split in (0, 1 << 20):
+        p, v = pos.copy(), vel.copy()
+        st = oracle.hhs_step(p, v, mass, 2.0 ** -6, split_max=split)
+        out.append((st, p, v, oracle.diagnostics(p, v, mass)["E"] / e0 - 1))
+    (st0, p0, v0, de0), (st1, p1, v1, de1) = out
+    assert max(st1["n_comp"][k] / st1["entries"][k] for k in range(st1["depth"])) > 5
+    assert st1["pairs_timestep"] < 0.5 * st0["pairs_timestep"]
+    for (st, p, v, de) in out:
+        assert np.abs((mass * (v - vel)).sum(1)).max() < 1e-15
+    assert abs(de1) < 10 * abs(de0) + 1e-10, (de0, de1)
+    assert np.abs(p1 - p0).max() < 1e-5, np.abs(p1 - p0).max()
