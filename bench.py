@@ -40,6 +40,7 @@ FLOPS_NEWTON, FLOPS_GRAD = 18, 34          # per ordered pair (FMA = 2, add/mul 
 SLOTS_NEWTON, SLOTS_GRAD = 10, 16
 SLOTS_NEWTON_1S, SLOTS_GRAD_1S = 16, 28
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM
+SPLIT_MAX_CONFIG5 = 32768                  # frost_set_split for the split arm of the config-5 step
 METRIC = "pair interactions/s (acc+gradient, fp64) at N=2^20"
 UNIT = "pair interactions/s"
 
@@ -211,10 +212,11 @@ def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
                      "frac_of_hbm_peak": gbs / hbm_peak}
     if hhs:
         out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
+        out["hhs_step_config5_split"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)
     return out
 
 
-def hhs_config5(fr, torch, dev, n5=262144):
+def hhs_config5(fr, torch, dev, n5=262144, split_max=0):
     """Config 5: one whole HHS-FSI step over all time-step levels (latency-bound: DESIGN.md 7), with
     the numbers that make the timing valid: momentum, angular momentum and energy change read by
     frost_diagnostics before and after (SURVEY 8(c) last pin row; expected floors PAPER.md:646-656,
@@ -223,14 +225,18 @@ def hhs_config5(fr, torch, dev, n5=262144):
     p5, v5, m5 = (torch.as_tensor(x).to(dev) for x in (pos5, vel5, mass5))
     fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
     d0 = fr.diagnostics(p5, v5, m5)
+    fr.set_split(split_max)
     l0 = fr.launch_count()
     torch.cuda.synchronize(); t0 = time.perf_counter()
-    st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
+    try:
+        st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
+    finally:
+        fr.set_split(0)
     torch.cuda.synchronize(); t1 = time.perf_counter()
     launches = int(fr.launch_count() - l0)
     d1 = fr.diagnostics(p5, v5, m5)
     L0, L1 = np.array(d0["L"]), np.array(d1["L"])
-    return {"n": n5, "dt_top": 2.0 ** -7, "seconds": t1 - t0, "depth": st["depth"],
+    return {"n": n5, "dt_top": 2.0 ** -7, "split_max": split_max, "seconds": t1 - t0, "depth": st["depth"],
             "hierarchy_entries": int(sum(st["entries"])), "launches": launches,
             "pairs_newton": int(st["pairs_newton"]), "pairs_gradient": int(st["pairs_gradient"]),
             "pairs_timestep": int(st["pairs_timestep"]),
@@ -238,7 +244,8 @@ def hhs_config5(fr, torch, dev, n5=262144):
             "dL_rel": float(np.linalg.norm(L1 - L0) / np.linalg.norm(L0)),
             "dE_rel": float(d1["E"] / d0["E"] - 1.0),
             "level0": {"n_slow": int(st["n_slow"][0]), "n_fast": int(st["n_fast"][0])},
-            "entries_per_level": [int(x) for x in st["entries"]]}
+            "entries_per_level": [int(x) for x in st["entries"]],
+            "components_per_level": [int(x) for x in st["n_comp"]]}
 
 
 def run_probe():
@@ -335,7 +342,9 @@ def run_hhs_only():
     import torch
     import paper_2011_14984_b200 as frost
     fr = frost.Frost(0)
-    print(json.dumps({"hhs_step_config5": hhs_config5(fr, torch, torch.device("cuda", 0))}))
+    dev = torch.device("cuda", 0)
+    print(json.dumps({"hhs_step_config5": hhs_config5(fr, torch, dev),
+                      "hhs_step_config5_split": hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)}))
     fr.close()
 
 
