@@ -7,7 +7,10 @@
 
 using namespace frost;
 
-static int pad1024(int n) { return round_up(n > 0 ? n : 1, 1024); }
+// Packed record streams are zero-padded to a multiple of every tile size that reads them: 256-record
+// source tiles and <= 1024-sink blocks of the one-sided sweeps, A tiles of 128 x KA records (KA = 2, 4, 6,
+// 8) of the pair-symmetric sweeps.
+static int pad_rec(int n) { return round_up(n > 0 ? n : 1, 3072); }
 
 extern "C" {
 
@@ -190,7 +193,7 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
     if (sharded && (((flags & FROST_ACC) && (flags & FROST_GRAD)) || (flags & FROST_ACCUMULATE))) return FROST_EINVAL;
     if (nI <= 0 && !(mutual && nJ > 0)) return FROST_OK;
     // (sharded one-sided sweeps read a block of the sink stream at an offset: one more tile of padding)
-    const int padA = pad1024(nI) + (sharded ? 1024 : 0), padB = pad1024(nJ) + (sharded ? 1024 : 0);
+    const int padA = pad_rec(nI) + (sharded ? 1024 : 0), padB = pad_rec(nJ) + (sharded ? 1024 : 0);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)padA * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)padA * kRecBytes));
     double *Axm = (double *)c->recA_xm.p, *Av = (double *)c->recA_v.p;
@@ -283,7 +286,7 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     if (!idx) n_idx = n;
     if (n_idx <= 0) return FROST_OK;
     if (forest) {
-        const int pad = pad1024(n_idx);
+        const int pad = pad_rec(n_idx);
         FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
         FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
         double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
@@ -300,7 +303,7 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
     // 2^20 particles; break-even at ~30000, where the sort and the two passes start to dominate)
     if (c->tune_sym == 4 || c->tune_sym == 5 || (c->tune_sym != 1 && c->tune_sym != 3 && n_idx >= 32768))
         return tau_pruned(c, ld, pos, vel, mass, idx, n_idx, tau_pivot, out_tau, out_bin, c->tune_sym != 4);
-    const int pad = pad1024(n_idx);
+    const int pad = pad_rec(n_idx);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
     double *xm = (double *)c->recA_xm.p, *v = (double *)c->recA_v.p;
@@ -375,7 +378,7 @@ static int cross_kick(frost_ctx *c, int n, int ld, double *pos, double *vel, con
                       const SplitInfo &si, bool with_g, double cc, double kappa) {
     double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
     if (si.m > 1) {
-        const int pad = pad1024(n_set);
+        const int pad = pad_rec(n_set);
         FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
         FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
         double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
@@ -419,7 +422,7 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     const bool split = c->split_max > 0 && n_set <= c->split_max;
     int *forest = nullptr;
     if (split) {
-        FROST_TRY(ensure(c, c->uf, (size_t)pad1024(n_set) * sizeof(int)));
+        FROST_TRY(ensure(c, c->uf, (size_t)pad_rec(n_set) * sizeof(int)));
         forest = (int *)c->uf.p;
     }
     FROST_TRY(timesteps_impl(c, n, ld, pos, vel, mass, set, n_set, tau_pivot, tau, nullptr, forest));
@@ -603,7 +606,7 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     FROST_DEVICE(c);
     // every O(n) scratch buffer of the recursion is sized here, once, for the largest set it can
     // meet (all n particles), so that ensure() never has to drain the stream to grow one mid-step
-    const size_t recb = (size_t)pad1024(n) * kRecBytes;
+    const size_t recb = (size_t)pad_rec(n) * kRecBytes;
     FROST_TRY(ensure(c, c->recA_xm, recb)); FROST_TRY(ensure(c, c->recA_v, recb));
     FROST_TRY(ensure(c, c->recB_xm, recb)); FROST_TRY(ensure(c, c->recB_v, recb));
     FROST_TRY(ensure(c, c->blockcnt, (size_t)(n / 1024 + 4) * sizeof(int)));
@@ -643,7 +646,7 @@ int frost_diagnostics(frost_ctx *c, int n, int ld, const double *pos, const doub
     for (int k = 0; k < 8; ++k) out8[k] = 0.0;
     if (n == 0) return FROST_OK;
     FROST_DEVICE(c);
-    const int pad = pad1024(n);
+    const int pad = pad_rec(n);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
     FROST_TRY(ensure(c, c->tau, (size_t)(ld + 8) * sizeof(double)));
     FROST_TRY(ensure(c, c->blockcnt, 8 * sizeof(double)));
@@ -667,7 +670,7 @@ int frost_forces_masked(frost_ctx *c, int n, int ld, const double *pos, const do
     if (!idx) n_idx = n;
     if (n_idx == 0) return FROST_OK;
     FROST_DEVICE(c);
-    const int pad = pad1024(n_idx);
+    const int pad = pad_rec(n_idx);
     FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
     double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;

@@ -207,7 +207,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     constexpr int kWarps = NT / 32;
     constexpr int TA = NT * KA;
     constexpr int PL = P::kPlanes;
-    constexpr uint32_t kStageBytes = P::kRecs * NT * kRecBytes;
+    constexpr uint32_t kStageBytes = P::kRecs * 2 * NT * kRecBytes;      // chunks stored twice
 
     const int I = prm.row0 + blockIdx.x * prm.row_stride;
     const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
@@ -217,7 +217,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     const int ntiles = min(prm.seg_tiles, prm.bt1 - tile0);
 
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    double4 *tiles = reinterpret_cast<double4 *>(smem_raw);                   // [kStages][kRecs][NT]
+    double4 *tiles = reinterpret_cast<double4 *>(smem_raw);                   // [kStages][kRecs][2 NT]
     double *accB = reinterpret_cast<double *>(smem_raw + kStages * kStageBytes);   // [2][PL][NT]
     uint64_t *full = reinterpret_cast<uint64_t *>(accB + 2 * PL * NT);
 
@@ -229,13 +229,22 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     }
     __syncthreads();
 
+    // Every 32-record chunk of a B tile is stored TWICE back to back, so that the rotated read of step
+    // s -- record (lane - s) mod 32 -- is the plain address (chunk + 32 + lane) - s: an immediate offset
+    // in the unrolled loop instead of three address instructions per step.
     auto issue = [&](int t) {
         const int s = t % kStages;
         mbar_expect_tx(&full[s], kStageBytes);
-        double4 *dst = tiles + (size_t)s * P::kRecs * NT;
+        double4 *dst = tiles + (size_t)s * P::kRecs * 2 * NT;
         const size_t off = (size_t)(tile0 + t) * NT;
-        bulk_g2s(dst, prm.b0 + off, NT * kRecBytes, &full[s]);
-        if (P::kRecs == 2) bulk_g2s(dst + NT, prm.b1 + off, NT * kRecBytes, &full[s]);
+#pragma unroll
+        for (int c = 0; c < kWarps; ++c)
+#pragma unroll
+            for (int d = 0; d < 2; ++d) {
+                bulk_g2s(dst + (c * 2 + d) * 32, prm.b0 + off + c * 32, 32 * kRecBytes, &full[s]);
+                if (P::kRecs == 2)
+                    bulk_g2s(dst + 2 * NT + (c * 2 + d) * 32, prm.b1 + off + c * 32, 32 * kRecBytes, &full[s]);
+            }
     };
     if (tid == 0) {
         const int pre = min(kStages, ntiles);
@@ -255,20 +264,19 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     for (int t = 0; t < ntiles; ++t) {
         const int s = t % kStages;
         mbar_wait(&full[s], (uint32_t)(t / kStages) & 1u);
-        const double4 *t0 = tiles + (size_t)s * P::kRecs * NT;
+        const double4 *t0 = tiles + (size_t)s * P::kRecs * 2 * NT;
         const bool two_sided = (tile0 + t) >= diag_end;
         double *accT = accB + (size_t)(t & 1) * PL * NT;
         for (int r = 0; r < kWarps; ++r) {
             const int c = (warp + r) % kWarps;
-            const double4 *c0 = t0 + c * 32;
-            const double4 *c1 = c0 + (P::kRecs == 2 ? NT : 0);
+            const double4 *c0 = t0 + c * 64 + 32 + lane;
+            const double4 *c1 = c0 + (P::kRecs == 2 ? 2 * NT : 0);
             double b[PL];
             P::init_b(b);
 #pragma unroll 2
             for (int step = 0; step < 32; ++step) {
-                const int src = (lane - step) & 31;
-                const double4 j0 = c0[src];
-                const double4 j1 = (P::kRecs == 2) ? c1[src] : j0;
+                const double4 j0 = c0[-step];
+                const double4 j1 = (P::kRecs == 2) ? c1[-step] : j0;
 #pragma unroll
                 for (int k = 0; k < KA; ++k) P::pair(a[k], b, j0, j1, prm);
 #pragma unroll
@@ -411,7 +419,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
     FROST_TRY(ensure(c, c->partialB, row_bytes_per_tile * (size_t)band_tiles + 256));
     if (nbands > 1) FROST_TRY(ensure(c, c->symtot, (size_t)PL * na_pad * sizeof(double)));
 
-    const size_t smem = (size_t)kStages * P::kRecs * NT * kRecBytes + 2 * PL * NT * sizeof(double) +
+    const size_t smem = (size_t)kStages * P::kRecs * 2 * NT * kRecBytes + 2 * PL * NT * sizeof(double) +
                         kStages * sizeof(uint64_t);
     FROST_TRY(set_func_attr(c, sym_kernel<P, KA, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
@@ -475,10 +483,24 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
 //   256 threads x 1 CTA/SM,  KA = 8/4/4                      45.2 / 76.2 / 166.5
 //   128 threads x 2 CTAs/SM, KA = 8/4/4 (<=255 registers)    44.4 / 75.6 / 164.4   <- used
 //   128 threads x 2 CTAs/SM, KA = 8/8/8 (255 registers)      44.3 / 79.8 / 175.9
+// Round 2, N = 2^20 gradient sweep (ms): KA = 4: 1184.8; 4 with 3 CTAs/SM (166 registers): 1194.5; 3 with
+// 3 CTAs/SM: 1206.5; 5: 1160.2; 6 (242 registers): 1150.4 <- used; 7 (246): 1169.8.  More warps do not help
+// (the loop is not latency-bound); amortising the per-step SHFL / LDS / address instructions does: they
+// cost ~27 issue cycles per rotation step.  Newton KA = 8 / 9 / 10: 702.8 / 700.6 / 699.0 (kept at 8).
 // More A particles per thread amortise the per-step SHFL / LDS / address instructions; the A tile
 // is 1024 (Newton) or 512 (gradient, time step) particles, the B tile 128.
 constexpr int kSymNT = 128, kSymMinB = 2;
-constexpr int kSymKNewton = 8, kSymKGrad = 4, kSymKTau = 4;
+#ifndef FROST_GRAD_KA
+#define FROST_GRAD_KA 6
+#endif
+#ifndef FROST_GRAD_MINB
+#define FROST_GRAD_MINB 2
+#endif
+#ifndef FROST_NEWTON_KA
+#define FROST_NEWTON_KA 8
+#endif
+constexpr int kSymKNewton = FROST_NEWTON_KA, kSymKGrad = FROST_GRAD_KA, kSymKTau = 4;
+constexpr int kSymMinBGrad = FROST_GRAD_MINB;
 // sets below kSymSmallN particles: A tiles of 256 so that there are enough tile pairs to fill the GPU
 constexpr int kSymSmallN = 16384, kSymKSmall = 2, kSymMinBSmall = 4;
 
@@ -508,7 +530,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymGradient, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
-    return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinB>(c, j);
+    return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinBGrad>(c, j);
 }
 
 // Time-step sweep over one level (Eq. 49-54); xm carries G*m in .w and NaN padding.
