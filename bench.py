@@ -338,13 +338,17 @@ def run_subtree(k):
     fr.close()
 
 
-def run_hhs_only():
+def run_hhs_only(arm):
     import torch
     import paper_2011_14984_b200 as frost
     fr = frost.Frost(0)
     dev = torch.device("cuda", 0)
-    print(json.dumps({"hhs_step_config5": hhs_config5(fr, torch, dev),
-                      "hhs_step_config5_split": hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)}))
+    out = {}
+    if arm in ("both", "alg3"):
+        out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
+    if arm in ("both", "split"):
+        out["hhs_step_config5_split"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)
+    print(json.dumps(out))
     fr.close()
 
 
@@ -577,6 +581,8 @@ def main():
     ap.add_argument("--rows-only", action="store_true", help="launch the O(N) kernels and time-step sweeps (for ncu)")
     ap.add_argument("--subtree", type=int, default=0, help="run the subtree kernel on K/2 hard binaries (for ncu)")
     ap.add_argument("--hhs-only", action="store_true", help="one HHS-FSI step of config 5 with its validity numbers")
+    ap.add_argument("--hhs-arm", default="both", choices=["both", "alg3", "split"],
+                    help="--hhs-only: Alg. 3 as printed, the split fast levels (frost_set_split), or both")
     args = ap.parse_args()
     if args.probe:
         return run_probe()
@@ -585,7 +591,7 @@ def main():
     if args.subtree:
         return run_subtree(args.subtree)
     if args.hhs_only:
-        return run_hhs_only()
+        return run_hhs_only(args.hhs_arm)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not under torchrun: launch one rank per GPU ourselves (rank 0 prints the JSON line)
         import socket

@@ -84,7 +84,7 @@ static int side_ctx(frost_ctx *c, int level, frost_ctx **out) {
     }
     s->G = c->G; s->eps2 = c->eps2; s->eta_ff = c->eta_ff; s->eta_fb = c->eta_fb; s->max_depth = c->max_depth;
     s->tune_k = c->tune_k; s->tune_slices = c->tune_slices; s->tune_small = c->tune_small;
-    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max;
+    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max; s->tune_pair = c->tune_pair;
     s->sym_scratch = c->sym_scratch < ((size_t)1 << 30) ? c->sym_scratch : ((size_t)1 << 30);
     *out = s;
     return FROST_OK;
@@ -133,6 +133,12 @@ int frost_set_overlap(frost_ctx *c, int on) {
 int frost_set_split(frost_ctx *c, int split_max) {
     if (!c || split_max < 0) return FROST_EINVAL;
     c->split_max = split_max;
+    return FROST_OK;
+}
+
+int frost_set_pair_path(frost_ctx *c, int on) {
+    if (!c || on < 0 || on > 1) return FROST_EINVAL;
+    c->tune_pair = on;
     return FROST_OK;
 }
 

@@ -50,6 +50,7 @@ struct frost_ctx {
     frost::Buf lvlS[FROST_MAX_LEVELS], lvlF[FROST_MAX_LEVELS];
     int32_t *pinned_counts = nullptr;  // host pinned int32[4]
     frost::Buf shard_idx;              // 0..n-1, for sharding the sinks of a NULL index list
+    int tune_pair = 1;             // two-body frames of the subtree kernels on one thread (frost_set_pair_path)
     int split_max = 0;             // frost_set_split: entries with <= split_max members split F into components
     frost::Buf uf, comp;           // union-find forest / labels, sort and descriptor scratch of a split entry
     frost::Buf lvlC[FROST_MAX_LEVELS];   // F of a split entry reordered by component

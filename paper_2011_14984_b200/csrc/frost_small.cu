@@ -44,6 +44,7 @@ struct SmallParams {
     // batched launch: CTA (or warp) b takes the set idx[desc[b].x .. desc[b].x + desc[b].y)
     const int2 *desc;
     const int *n_desc;
+    int pair_path;                  // two-body frames on one thread (binary_subtree); 0: team path (tests)
 };
 
 template <int CAP>
@@ -538,6 +539,116 @@ __device__ void cta_cross_kick(SM &sm, const SweepParams &pN, const SweepParams 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// A frame of exactly two particles, executed by ONE thread with both particles in registers.
+// In a two-body set both members have the same time step (the one pair candidate, symmetric), so
+// every entry of Alg. 3 is either a leaf -- both slow: fsi(pair, tau/2) twice, every inter-level term
+// empty -- or an inner node -- both fast: hhs_fsi(pair, tau/2) twice.  The subtree is therefore a
+// binary tree over the interval [0, tau0), walked here with a time index instead of a frame stack:
+// a node of relative depth d spans 2^(62-d) units; after a leaf that ends at index t the next node
+// starts at t with depth 62 - ctz(t) (the second child of the deepest unfinished ancestor).  Same
+// pair arithmetic (frost_pairs.cuh), same operator order and same bookkeeping as the team path --
+// the results are bitwise those of hhs_loop on the same frame; what changes is the latency: no
+// barriers, no shuffles, no shared-memory round trips between the ~20 dependent phases of an entry.
+// This is the critical path of a split level: the hardest binary's chain.
+// ------------------------------------------------------------------------------------------------
+struct Body { double x, y, z, vx, vy, vz, m; };
+
+__device__ __forceinline__ void pair_newton(const Body &p, const Body &q, const SweepParams &pN, double &ax,
+                                            double &ay, double &az) {
+    NewtonPolicy::Sink s; s.x = p.x; s.y = p.y; s.z = p.z;
+    NewtonPolicy::Acc a; NewtonPolicy::init(a);
+    const double4 j0 = make_double4(q.x, q.y, q.z, q.m);
+    NewtonPolicy::pair(s, a, j0, j0, pN);
+    ax = a.x * pN.G; ay = a.y * pN.G; az = a.z * pN.G;
+}
+
+__device__ __forceinline__ void pair_gradient(const Body &p, const double (&ap)[3], const Body &q,
+                                              const double (&aq)[3], const SweepParams &pG, double &gx,
+                                              double &gy, double &gz) {
+    GradientPolicy::Sink s; s.x = p.x; s.y = p.y; s.z = p.z; s.ax = ap[0]; s.ay = ap[1]; s.az = ap[2];
+    GradientPolicy::Acc g; GradientPolicy::init(g);
+    GradientPolicy::pair(s, g, make_double4(q.x, q.y, q.z, q.m), make_double4(aq[0], aq[1], aq[2], 1.0), pG);
+    const double k2g = 2.0 * pG.G;
+    gx = g.x * k2g; gy = g.y * k2g; gz = g.z * k2g;
+}
+
+__device__ __forceinline__ void body_kick(Body &p, const double (&a)[3], double c) {
+    p.vx = fma(c, a[0], p.vx); p.vy = fma(c, a[1], p.vy); p.vz = fma(c, a[2], p.vz);
+}
+__device__ __forceinline__ void body_kick_g(Body &p, const double (&a)[3], const double (&g)[3], double c,
+                                            double kappa) {
+    p.vx = fma(c, fma(kappa, g[0], a[0]), p.vx);
+    p.vy = fma(c, fma(kappa, g[1], a[1]), p.vy);
+    p.vz = fma(c, fma(kappa, g[2], a[2]), p.vz);
+}
+__device__ __forceinline__ void body_drift(Body &p, double c) {
+    p.x = fma(c, p.vx, p.x); p.y = fma(c, p.vy, p.y); p.z = fma(c, p.vz, p.z);
+}
+
+// fsi(pair, dt): Alg. 2 on two bodies.
+__device__ __forceinline__ void pair_fsi(Body &p, Body &q, const SweepParams &pN, const SweepParams &pG,
+                                         double dt) {
+    double ap[3], aq[3], gp[3], gq[3];
+    pair_newton(p, q, pN, ap[0], ap[1], ap[2]); pair_newton(q, p, pN, aq[0], aq[1], aq[2]);
+    body_kick(p, ap, dt / 6.0); body_kick(q, aq, dt / 6.0);
+    body_drift(p, dt / 2.0); body_drift(q, dt / 2.0);
+    pair_newton(p, q, pN, ap[0], ap[1], ap[2]); pair_newton(q, p, pN, aq[0], aq[1], aq[2]);
+    pair_gradient(p, ap, q, aq, pG, gp[0], gp[1], gp[2]); pair_gradient(q, aq, p, ap, pG, gq[0], gq[1], gq[2]);
+    body_kick_g(p, ap, gp, 2.0 * dt / 3.0, dt * dt / 48.0); body_kick_g(q, aq, gq, 2.0 * dt / 3.0, dt * dt / 48.0);
+    body_drift(p, dt / 2.0); body_drift(q, dt / 2.0);
+    pair_newton(p, q, pN, ap[0], ap[1], ap[2]); pair_newton(q, p, pN, aq[0], aq[1], aq[2]);
+    body_kick(p, ap, dt / 6.0); body_kick(q, aq, dt / 6.0);
+}
+
+template <class SM>
+__device__ void binary_subtree(SM &sm, SmStats &st, const SmallParams &P, const SweepParams &pN,
+                               const SweepParams &pG, int sp) {
+    const int start = sm.f_start[sp];
+    const int i1 = sm.perm[start], i2 = sm.perm[start + 1];
+    const double tau0 = sm.f_tau[sp];
+    const int level0 = P.level0 + sp;
+    Body p, q;
+    { const double4 x = sm.xm[i1], v = sm.vv[i1]; p.x = x.x; p.y = x.y; p.z = x.z; p.m = x.w; p.vx = v.x; p.vy = v.y; p.vz = v.z; }
+    { const double4 x = sm.xm[i2], v = sm.vv[i2]; q.x = x.x; q.y = x.y; q.z = x.z; q.m = x.w; q.vx = v.x; q.vy = v.y; q.vz = v.z; }
+    const double inf = __longlong_as_double(0x7ff0000000000000LL);
+    unsigned long long t = 0, leaves = 0, nodes = 0;
+    int d = 0, dmax = 0, err = 0;
+    while (true) {
+        if (level0 + d >= P.max_depth || sp + d >= FROST_MAX_LEVELS - 1 || d > 61) { err = FROST_EDEPTH; break; }
+        TimestepPolicy::Sink s;
+        s.x = p.x; s.y = p.y; s.z = p.z; s.gm = p.m * pG.G; s.vx = p.vx; s.vy = p.vy; s.vz = p.vz;
+        const double c = fmin(inf, TimestepPolicy::candidate(s, make_double4(q.x, q.y, q.z, q.m * pG.G),
+                                                              make_double4(q.vx, q.vy, q.vz, 1.0), pG));
+        const double tau = ldexp(tau0, -d);
+        const int level = level0 + d;
+        ++nodes;
+        atomicAdd(&st.entries[level], 1ull);
+        if (d > dmax) dmax = d;
+        if (c >= tau) {                       // both slow: a leaf
+            atomicAdd(&st.slow[level], 2ull);
+            pair_fsi(p, q, pN, pG, 0.5 * tau);
+            pair_fsi(p, q, pN, pG, 0.5 * tau);
+            ++leaves;
+            t += 1ull << (62 - d);
+            if (t >> 62) break;               // the root's interval is done
+            d = 62 - (__ffsll((long long)t) - 1);
+        } else {                              // both fast: one component, recursed into twice
+            atomicAdd(&st.fast[level], 2ull);
+            atomicAdd(&st.comps[level], 1ull);
+            ++d;
+        }
+    }
+    atomicAdd(&st.pt, 4ull * nodes);
+    atomicAdd(&st.pn, 24ull * leaves);        // two fsi per leaf, three sweeps of 4 ordered pairs each
+    atomicAdd(&st.pg, 8ull * leaves);
+    atomicMax(&st.depth, level0 + dmax);
+    sm.xm[i1] = make_double4(p.x, p.y, p.z, p.m); sm.vv[i1] = make_double4(p.vx, p.vy, p.vz, 1.0);
+    sm.xm[i2] = make_double4(q.x, q.y, q.z, q.m); sm.vv[i2] = make_double4(q.vx, q.vy, q.vz, 1.0);
+    if (err) sm.err = err;
+    sm.sp = sp - 1;
+}
+
 // The hhs_fsi recursion of Alg. 3 as a state machine over the explicit frame stack; runs until the
 // frame at base_sp has been popped.  Stages of a frame: 0 = entry (time steps, partition, components,
 // first kick, fsi(S)); 1 = first recursion pass over the components of F in progress; 2 = second pass.
@@ -551,6 +662,10 @@ __device__ void hhs_loop(SM &sm, SmStats &st, const SmallParams &P, const SweepP
         const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
         const double tau = sm.f_tau[sp];
         const int level = P.level0 + sp;
+        if (stage == 0 && cnt == 2 && P.pair_path) {      // a binary: one thread, both bodies in registers
+            if (T::tid() == 0) binary_subtree(sm, st, P, pN, pG, sp);
+            continue;
+        }
         if (T::kThreads > 128 && stage == 0 && cnt > kWarpTeamMax && cnt <= kQuadTeamMax) {
             // the whole subtree of this entry on warps 0-3 (see TeamQuad)
             if (threadIdx.x < 128) hhs_loop<TeamQuad>(sm, st, P, pN, pG, sp);
@@ -767,6 +882,7 @@ static SmallParams small_params(frost_ctx *c, int mode, int ld, double *pos, dou
     P.max_depth = c->max_depth; P.G = c->G; P.eps2 = c->eps2; P.eta_ff = c->eta_ff; P.eta_fb = c->eta_fb;
     P.stats = (SmallStats *)dev_stats;
     P.split_max = c->split_max;
+    P.pair_path = c->tune_pair;
     return P;
 }
 

@@ -123,3 +123,26 @@ def test_split_max_limits_the_split_to_small_entries(fr, oracle):
     assert st == st_ref
     assert st["n_comp"][0] == 1 and any(c > e for c, e in zip(st["n_comp"], st["entries"]))
     assert np.abs((mass * (v.cpu().numpy() - vel)).sum(1)).max() < 1e-15
+
+
+@pytest.mark.parametrize("n,split", [(256, 0), (256, BIG), (3000, BIG)])
+def test_pair_path_is_bitwise_the_team_path(fr, n, split):
+    """frost_set_pair_path: two-body hierarchy entries on one thread (both bodies in registers, the
+    subtree walked as a binary tree over the step interval) against the same entries on the warp
+    team -- same pair arithmetic, operator order and bookkeeping, so the same bits: with Alg. 3 as
+    printed (binaries that end up alone at depth) and with split levels (every binary its own tree)."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    out = []
+    try:
+        for on in (0, 1):
+            fr.set_pair_path(on)
+            fr.set_split(split)
+            p, v = dev(pos), dev(vel)
+            st = fr.hhs_step(p, v, dev(mass), 2.0 ** -8)
+            out.append((st, p, v))
+    finally:
+        fr.set_pair_path(1)
+        fr.set_split(0)
+    assert out[0][0] == out[1][0] and out[0][0]["depth"] >= 14
+    assert torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])

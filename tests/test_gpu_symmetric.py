@@ -337,3 +337,63 @@ def test_pruned_timestep_sweep_on_index_subset(frs):
     assert torch.equal(res[0][0], res[1][0]) and torch.equal(res[0][1], res[1][1])
     out = np.setdiff1d(np.arange(n), idx)
     assert torch.isinf(res[1][0][dev(out).long()]).all()
+
+
+@pytest.mark.skipif(torch.cuda.device_count() < 2, reason="needs two CUDA devices")
+def test_two_devices_pair_sharded_and_sink_sharded(oracle):
+    """SURVEY 8(f).3 on real peers (skipped on a one-GPU box): rank r = a context on device r with the
+    state replicated.  Pair sharding (the default N > 1 arm of bench.py): the two ranks' partial sums,
+    added the way the all-reduce adds them, equal the unsharded result to 1e-12 / 1e-10 and the oracle.
+    Sink sharding (bench.py --one-sided, the paper's scatter-compute-gather): each rank's
+    block of sinks is bitwise the one-GPU result."""
+    import paper_2011_14984_b200 as frost
+    from paper_2011_14984_b200 import sharding
+    n = 20000
+    pos, vel, mass = fi.plummer(n, 23)
+    a_ref, g_ref = oracle.forces(pos, mass)
+    ctx = [frost.Frost(d) for d in (0, 1)]
+    P = [torch.as_tensor(pos).to(f"cuda:{d}") for d in (0, 1)]
+    M = [torch.as_tensor(mass).to(f"cuda:{d}") for d in (0, 1)]
+    try:
+        one_a, one_g = ctx[0].forces(P[0], M[0])
+        # pair sharding
+        parts = []
+        for r in (0, 1):
+            ctx[r].set_shard(r, 2)
+            part = torch.zeros_like(P[r])
+            ctx[r].forces(P[r], M[r], out_acc=part, flags=frost.ACC)
+            parts.append(part)
+        acc = parts[0] + parts[1].to("cuda:0")
+        gparts = []
+        for r in (0, 1):
+            part = torch.zeros_like(P[r])
+            ctx[r].forces(P[r], M[r], out_acc=acc.to(f"cuda:{r}"), out_grad=part, flags=frost.GRAD)
+            gparts.append(part)
+        grad = gparts[0] + gparts[1].to("cuda:0")
+        a, g = acc.cpu().numpy(), grad.cpu().numpy()
+        assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+        assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+        assert (np.abs(a - one_a.cpu().numpy()).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+        # sink sharding with the one-sided kernels: bitwise per block
+        for r in (0, 1):
+            ctx[r].set_shard(0, 1)
+            ctx[r].set_symmetric(1)
+        ref_a = torch.zeros_like(P[0]); ref_g = torch.zeros_like(P[0])
+        ctx[0].forces(P[0], M[0], out_acc=ref_a, out_grad=ref_g)
+        full_a = torch.zeros_like(P[0])
+        blocks = []
+        for r in (0, 1):
+            lo, hi = sharding.shard_range(n, r, 2)
+            idx = torch.arange(lo, hi, dtype=torch.int32, device=f"cuda:{r}")
+            part = torch.zeros_like(P[r])
+            ctx[r].forces(P[r], M[r], sink_idx=idx, out_acc=part, flags=frost.ACC)
+            full_a[:, lo:hi] = part[:, lo:hi].to("cuda:0")
+            blocks.append((lo, hi, idx))
+        assert torch.equal(full_a, ref_a)
+        for r, (lo, hi, idx) in enumerate(blocks):
+            part = torch.zeros_like(P[r])
+            ctx[r].forces(P[r], M[r], sink_idx=idx, out_acc=full_a.to(f"cuda:{r}"), out_grad=part, flags=frost.GRAD)
+            assert torch.equal(part[:, lo:hi].to("cuda:0"), ref_g[:, lo:hi])
+    finally:
+        for f in ctx:
+            f.close()
