@@ -501,6 +501,10 @@ constexpr int kSymNT = 128, kSymMinB = 2;
 #endif
 constexpr int kSymKNewton = FROST_NEWTON_KA, kSymKGrad = FROST_GRAD_KA, kSymKTau = 4;
 constexpr int kSymMinBGrad = FROST_GRAD_MINB;
+#ifndef FROST_GRAD_NT
+#define FROST_GRAD_NT 128
+#endif
+constexpr int kSymNTGrad = FROST_GRAD_NT;
 // sets below kSymSmallN particles: A tiles of 256 so that there are enough tile pairs to fill the GPU
 constexpr int kSymSmallN = 16384, kSymKSmall = 2, kSymMinBSmall = 4;
 
@@ -530,7 +534,7 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymGradient, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
-    return run_sym<SymGradient, kSymKGrad, kSymNT, kSymMinBGrad>(c, j);
+    return run_sym<SymGradient, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j);
 }
 
 // Time-step sweep over one level (Eq. 49-54); xm carries G*m in .w and NaN padding.

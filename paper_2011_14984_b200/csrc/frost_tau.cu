@@ -57,12 +57,22 @@ __device__ __forceinline__ void atomic_min_tau(unsigned long long *p, double v) 
     if (v == v) atomicMin(p, (unsigned long long)__double_as_longlong(v));    // v >= 0: bit order = value order
 }
 
-// ---- 1. bounding box of the level (one CTA) ------------------------------------------------------
+// ---- 1. bounding box of the level: one partial box per CTA, then one CTA over the partial boxes ---
+// (pos = NULL: second stage, `idx`-less reduction of the n partial boxes stored as box6[b*6 + 0..5])
 __global__ void __launch_bounds__(1024)
-tau_bbox_kernel(const double *__restrict__ pos, int ld, const int32_t *__restrict__ idx, int n, double *box6) {
+tau_bbox_kernel(const double *__restrict__ pos, int ld, const int32_t *__restrict__ idx, int n,
+                const double *__restrict__ part_in, double *box6) {
     __shared__ double sh[6][32];
     double lo[3] = {1e300, 1e300, 1e300}, hi[3] = {-1e300, -1e300, -1e300};
-    for (int k = threadIdx.x; k < n; k += 1024) {
+    if (!pos) {
+        for (int b = threadIdx.x; b < n; b += 1024) {
+#pragma unroll
+            for (int d = 0; d < 3; ++d) {
+                lo[d] = fmin(lo[d], part_in[b * 6 + d]); hi[d] = fmax(hi[d], part_in[b * 6 + 3 + d]);
+            }
+        }
+    }
+    for (int k = blockIdx.x * 1024 + threadIdx.x; pos && k < n; k += gridDim.x * 1024) {
         const int i = idx ? idx[k] : k;
 #pragma unroll
         for (int d = 0; d < 3; ++d) {
@@ -82,7 +92,7 @@ tau_bbox_kernel(const double *__restrict__ pos, int ld, const int32_t *__restric
     if (threadIdx.x < 6) {
         double v = sh[threadIdx.x][0];
         for (int w = 1; w < 32; ++w) v = threadIdx.x < 3 ? fmin(v, sh[threadIdx.x][w]) : fmax(v, sh[threadIdx.x][w]);
-        box6[threadIdx.x] = v;
+        box6[blockIdx.x * 6 + threadIdx.x] = v;
     }
 }
 
@@ -409,11 +419,19 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
     int32_t *vals = (int32_t *)(base + o_vals), *vals2 = (int32_t *)(base + o_vals2);
     int32_t *sidx = (int32_t *)(base + o_sidx);
     double *box6 = (double *)(base + o_box6);
+    double *box_part = (double *)keys2;      // <= 256 partial boxes; keys2 is first written by the sort
     TauBox *boxes = (TauBox *)(base + o_boxes);
     unsigned long long *tau64 = (unsigned long long *)(base + o_tau);
     double *xm = (double *)c->recA_xm.p, *vv = (double *)c->recA_v.p;
 
-    tau_bbox_kernel<<<1, 1024, 0, c->stream>>>(pos, ld, idx, n, box6);
+    const int bb = (n + 8191) / 8192 < 256 ? (n + 8191) / 8192 : 256;       // 8 particles per thread
+    if (bb > 1) {
+        tau_bbox_kernel<<<bb, 1024, 0, c->stream>>>(pos, ld, idx, n, nullptr, box_part);
+        FROST_TRY(check_launch(c));
+        tau_bbox_kernel<<<1, 1024, 0, c->stream>>>(nullptr, 0, nullptr, bb, box_part, box6);
+    } else {
+        tau_bbox_kernel<<<1, 1024, 0, c->stream>>>(pos, ld, idx, n, nullptr, box6);
+    }
     FROST_TRY(check_launch(c));
     tau_morton_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(pos, ld, idx, n, box6, keys, vals);
     FROST_TRY(check_launch(c));

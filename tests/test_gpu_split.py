@@ -146,3 +146,44 @@ def test_pair_path_is_bitwise_the_team_path(fr, n, split):
         fr.set_split(0)
     assert out[0][0] == out[1][0] and out[0][0]["depth"] >= 14
     assert torch.equal(out[0][1], out[1][1]) and torch.equal(out[0][2], out[1][2])
+
+
+def test_split_tiny_and_degenerate_systems(fr, oracle):
+    """Edge cases of the split step against the oracle: one, two, three and five bodies (no fast pair,
+    one fast pair, a chain), softening, the five-body Solar system (F = {Sun, Jupiter}: one component,
+    several levels), an empty fast set at the top (everything slow)."""
+    rng = np.random.default_rng(11)
+    cases = []
+    for n in (1, 2, 3, 5):
+        pos = np.ascontiguousarray(rng.normal(size=(3, n)))
+        vel = np.ascontiguousarray(rng.normal(size=(3, n)) * 0.3)
+        mass = rng.uniform(0.5, 2.0, n)
+        if n >= 3:                                  # a close pair on a circular orbit inside
+            r = np.array([1e-3, 2e-3, 0.0])
+            pos[:, 1] = pos[:, 0] + r
+            vc = np.sqrt((mass[0] + mass[1]) / np.linalg.norm(r))
+            vel[:, 1] = vel[:, 0] + vc * np.array([-r[1], r[0], 0.0]) / np.linalg.norm(r)
+        cases.append((pos, vel, mass, 2.0 ** -5, dict(G=1.0, eps2=0.0)))
+        cases.append((pos, vel, mass, 2.0 ** -5, dict(G=1.0, eps2=1e-6)))
+        cases.append((pos, vel, mass, 2.0 ** -20, dict(G=1.0, eps2=0.0)))       # all slow at the top
+    sp, sv, sm, sG = fi.solar_system()
+    cases.append((sp, sv, sm, 512.0, dict(G=sG, eps2=0.0)))
+    for pos, vel, mass, dt, kw in cases:
+        for small in (-1, 0):
+            fr.set_params(G=kw["G"], eps2=kw["eps2"], eta_ff=0.1, eta_fb=0.1)
+            fr.set_tuning(0, 0, small)
+            fr.set_split(BIG)
+            pr, vr = pos.copy(), vel.copy()
+            st_ref = oracle.hhs_step(pr, vr, mass, dt, eta_ff=0.1, eta_fb=0.1, split_max=BIG, **kw)
+            p, v = dev(pos), dev(vel)
+            try:
+                st = fr.hhs_step(p, v, dev(mass), dt)
+            finally:
+                fr.set_split(0)
+                fr.set_tuning(0, 0, -1)
+                fr.set_params()
+            assert st == st_ref, (mass.size, dt, small)
+            scale = max(1.0, np.abs(pr).max())
+            # (a tight pair turns a rounding difference into an orbital phase difference: |dv| ~ v dphi)
+            assert np.abs(p.cpu().numpy() - pr).max() < 1e-10 * scale
+            assert np.abs(v.cpu().numpy() - vr).max() < 1e-7 * max(1.0, np.abs(vr).max())
