@@ -263,6 +263,15 @@ int frost_set_split(frost_ctx *ctx, int split_max);
  * such entries on the warp team (tests). */
 int frost_set_pair_path(frost_ctx *ctx, int on);
 
+/* Pair-symmetric gradient sweeps of 16384 particles or more run WITHOUT the per-pair test for
+ * coincident particles (|x_j - x_i|^2 + eps2 == 0, which the contract above ignores): such a pair then
+ * yields NaN, the reduction that scatters the result notices any non-finite sum, and a gated second
+ * pass with the guarded kernel recomputes the sweep -- a handful of empty launches for every input
+ * without distinct coincident particles, a sweep at 2.5 x the cost for one that has them; the result
+ * honours the contract either way.  on = 1 keeps the guard in the loop instead (one pass, 2.6 % slower
+ * at N = 2^20).  Default 0. */
+int frost_set_gradient_guard(frost_ctx *ctx, int on);
+
 /* The kick sweeps of a split entry on their own (Eq. 42-44 on the pair set "labels differ"):
  *   out_acc[i]  <- G sum_{j in idx, label_j != label_i} m_j x_ji / s_ij^3,
  *   out_grad[i] <- 2G sum over the same j of m_j s^-5 (s^2 a_ji - 3 (x_ji.a_ji) x_ji) with the a of this call

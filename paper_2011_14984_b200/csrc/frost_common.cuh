@@ -42,6 +42,8 @@ struct frost_ctx {
     frost::Buf tau_scratch;        // Morton keys, sorted index list, bounding records, tau64 (frost_tau.cu)
     frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
     frost::Buf symtot;             // running totals across bands of a symmetric sweep
+    frost::Buf symflag;            // "a sum came out non-finite" flag of the unguarded gradient pass
+    int tune_guard = 0;            // 1: large symmetric gradient sweeps keep the per-pair coincidence guard
     size_t sym_scratch = (size_t)4 << 30;   // cap of partialB: the B list is swept in bands
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
     frost::Buf blockcnt;           // partition scratch
@@ -140,7 +142,8 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 
 // ---- launchers implemented in the other translation units ------------------------------------
 // frost_update.cu
-// wscale multiplies the mass written to .w; nan_pad != 0 pads with NaN positions instead of zeros
+// wscale multiplies the mass written to .w; nan_pad = 1 pads with NaN positions instead of zeros,
+// 2 with positions (1e150, 1e150, 1e150) -- mass 0 either way
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
                    int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0,
                    double *zero_tail = nullptr);

@@ -25,6 +25,8 @@
 // diagonal block is evaluated one-sided (its B-side sums are dropped), everything beyond it
 // two-sided.  For the bipartite case (slow/fast sets of Alg. 3) every tile pair
 // is two-sided and one sweep yields both directions of acc_sf_*.
+#include <type_traits>
+
 #include "frost_pairs.cuh"
 
 namespace frost {
@@ -42,6 +44,7 @@ struct SymParams {
     double eps2, eta_ff, eta_fb;
     double pivot;             // SymTimestepEdge: fast pairs (candidate < pivot) are united in `forest`
     int *forest;
+    const int *gate;          // non-NULL: the launch does nothing unless *gate != 0 (repair pass, below)
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -110,6 +113,43 @@ struct SymGradient {
         fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
     }
 };
+
+// The gradient pair without the coincident-pair guard (ISETP + SEL per pair, 2.6 % of the loop).  A pair
+// with s^2 = 0 -- two distinct coincident unsoftened particles; the self pair only occurs in the
+// diagonal blocks, which keep the guarded routine -- then yields NaN instead of being ignored: MUFU(0)
+// = +inf, 0 * inf = NaN, and NaN sticks to every sum it enters.  The reduction that scatters the
+// result flags any non-finite output, and a gated second pass with the guarded kernel (a few empty
+// launches when the flag is clear) recomputes the sweep: the contract of DESIGN.md reading 11 holds
+// for every input, and inputs without coincident particles never pay for the guard.  Padding records
+// sit at (1e150, 1e150, 1e150) with mass 0 (frost_api.cu), so that they coincide with no particle.
+struct SymGradientFast : SymGradient {
+    static constexpr bool kDiagGuard = true;
+    __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double ax = j1.x - a.ax, ay = j1.y - a.ay, az = j1.z - a.az;
+        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
+        const double ri = rsqrt_full(s2);
+        const double dot = fma(dz, az, fma(dy, ay, dx * ax));
+        const double q = ri * ri;
+        const double w3 = ri * q;
+        const double t = q * dot;
+        const double u = t * -3.0;
+        double vx = ax, vy = ay, vz = az;
+        fma3_shared(vx, vy, vz, u, dx, dy, dz);
+        const double wa = w3 * j0.w;
+        const double wb = w3 * a.nm;
+        fma3_shared(a.s[0], a.s[1], a.s[2], wa, vx, vy, vz);
+        fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
+    }
+    __device__ static __forceinline__ void pair_diag(A &a, double (&b)[3], const double4 &j0,
+                                                     const double4 &j1, const SymParams &p) {
+        SymGradient::pair(a, b, j0, j1, p);
+    }
+};
+
+template <class P, class = void> struct DiagGuard { static constexpr bool value = false; };
+template <class P> struct DiagGuard<P, std::enable_if_t<P::kDiagGuard>> { static constexpr bool value = true; };
 
 struct SymTimestep {
     static constexpr int kRecs = 2, kPlanes = 1;
@@ -209,6 +249,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     constexpr int PL = P::kPlanes;
     constexpr uint32_t kStageBytes = P::kRecs * 2 * NT * kRecBytes;      // chunks stored twice
 
+    if (prm.gate && *prm.gate == 0) return;
     const int I = prm.row0 + blockIdx.x * prm.row_stride;
     const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
     const int row_first_tile = max(prm.self ? I * KA : 0, prm.bt0);   // first B tile of this A tile in the band
@@ -273,14 +314,28 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
             const double4 *c1 = c0 + (P::kRecs == 2 ? 2 * NT : 0);
             double b[PL];
             P::init_b(b);
+            if (DiagGuard<P>::value && !two_sided) {      // diagonal block: the self pairs live here
 #pragma unroll 2
-            for (int step = 0; step < 32; ++step) {
-                const double4 j0 = c0[-step];
-                const double4 j1 = (P::kRecs == 2) ? c1[-step] : j0;
+                for (int step = 0; step < 32; ++step) {
+                    const double4 j0 = c0[-step];
+                    const double4 j1 = (P::kRecs == 2) ? c1[-step] : j0;
+                    if constexpr (DiagGuard<P>::value) {
 #pragma unroll
-                for (int k = 0; k < KA; ++k) P::pair(a[k], b, j0, j1, prm);
+                        for (int k = 0; k < KA; ++k) P::pair_diag(a[k], b, j0, j1, prm);
+                    }
 #pragma unroll
-                for (int p = 0; p < PL; ++p) b[p] = __shfl_sync(0xffffffffu, b[p], from);
+                    for (int p = 0; p < PL; ++p) b[p] = __shfl_sync(0xffffffffu, b[p], from);
+                }
+            } else {
+#pragma unroll 2
+                for (int step = 0; step < 32; ++step) {
+                    const double4 j0 = c0[-step];
+                    const double4 j1 = (P::kRecs == 2) ? c1[-step] : j0;
+#pragma unroll
+                    for (int k = 0; k < KA; ++k) P::pair(a[k], b, j0, j1, prm);
+#pragma unroll
+                    for (int p = 0; p < PL; ++p) b[p] = __shfl_sync(0xffffffffu, b[p], from);
+                }
             }
             if (two_sided) {
                 double *dst = accT + c * 32 + lane;
@@ -324,7 +379,9 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
                                   int n_out, double scale,
                                   const int32_t *__restrict__ idx, int ld, double *__restrict__ out,
                                   double4 *__restrict__ packed, double tau_pivot,
-                                  int32_t *__restrict__ out_bin, int accumulate) {
+                                  int32_t *__restrict__ out_bin, int accumulate,
+                                  const int *__restrict__ gate, int *__restrict__ flag) {
+    if (gate && *gate == 0) return;          // repair pass of a sweep that needed none
     const int i = i0 + blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n_out) return;
     double s[PL];
@@ -373,6 +430,8 @@ __global__ void sym_reduce_kernel(const double *__restrict__ partA, const double
             s[p] *= scale;
             if (accumulate) s[p] += out[(size_t)p * ld + g];
             out[(size_t)p * ld + g] = s[p];
+            // (SymGradientFast: a coincident pair leaves NaN here and asks for the guarded pass)
+            if (flag && !(fabs(s[p]) <= 1.7976931348623157e308)) *flag = 1;
         }
         if (packed) packed[i] = make_double4(s[0], PL > 1 ? s[1] : 0.0, PL > 2 ? s[2] : 0.0, 1.0);
     }
@@ -394,6 +453,8 @@ struct SymJob {
     double scale, eps2, tau_pivot;
     int32_t *out_bin;
     int *forest = nullptr;                 // time-step sweep: union-find forest of the fast pairs
+    const int *gate = nullptr;             // the whole sweep runs only if *gate != 0
+    int *flag = nullptr;                   // set to 1 if any scattered sum is not finite
     int shard_rank = 0, shard_world = 1;   // this launch sweeps A tiles rank, rank + world, ... only
     int accumulate = 0;                    // add the sums to `out` instead of overwriting it
 };
@@ -451,7 +512,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         prm.na_pad = na_pad; prm.self = self ? 1 : 0; prm.bt0 = bt0; prm.bt1 = bt1;
         prm.seg_tiles = (int)seg; prm.row0 = row0; prm.row_stride = row_stride;
         prm.eps2 = job.eps2; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-        prm.pivot = job.tau_pivot; prm.forest = job.forest;
+        prm.pivot = job.tau_pivot; prm.forest = job.forest; prm.gate = job.gate;
         if (my_rows > 0) {
             dim3 grid(my_rows, segs);
             sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
@@ -462,7 +523,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         sym_reduce_kernel<PL, MIN><<<(job.nA + 255) / 256, 256, 0, c->stream>>>(
             prm.partA, prm.partB, (double *)c->symtot.p, na_pad, prm.self, 0, TA, NT, na_pad, a_tiles,
             bt0, bt1, prm.seg_tiles, row0, row_stride, first, last, 0, job.nA, job.scale, job.A_idx, job.ld, job.out,
-            (double4 *)job.A_packed, job.tau_pivot, job.out_bin, job.accumulate);
+            (double4 *)job.A_packed, job.tau_pivot, job.out_bin, job.accumulate, job.gate, job.flag);
         FROST_TRY(check_launch(c));
         if (!self) {          // a B particle only collects in its own band: no running total
             const int i0 = bt0 * NT, i1 = bt1 * NT < nB ? bt1 * NT : nB;
@@ -470,7 +531,7 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
                 sym_reduce_kernel<PL, MIN><<<(i1 - i0 + 255) / 256, 256, 0, c->stream>>>(
                     prm.partA, prm.partB, nullptr, 0, 0, 1, TA, NT, na_pad, a_tiles, bt0, bt1,
                     prm.seg_tiles, row0, row_stride, 1, 1, i0, i1, job.scale, job.B_idx, job.ld, job.out,
-                    (double4 *)job.B_packed, job.tau_pivot, job.out_bin, job.accumulate);
+                    (double4 *)job.B_packed, job.tau_pivot, job.out_bin, job.accumulate, job.gate, job.flag);
                 FROST_TRY(check_launch(c));
             }
         }
@@ -534,6 +595,16 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
     j.scale = 2.0 * c->G; j.eps2 = c->eps2;
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymGradient, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
+    if (c->tune_guard == 0 && !c->accumulate) {
+        // unguarded pass (SymGradientFast), then the guarded pass behind a gate that only opens if a
+        // scattered sum came out non-finite, i.e. if the input has distinct coincident particles
+        FROST_TRY(ensure(c, c->symflag, 256));
+        int *flag = (int *)c->symflag.p;
+        FROST_CUDA(c, cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
+        j.flag = flag;
+        FROST_TRY((run_sym<SymGradientFast, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j)));
+        j.flag = nullptr; j.gate = flag;
+    }
     return run_sym<SymGradient, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j);
 }
 

@@ -17,7 +17,9 @@ __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__r
     // the padding of the companion vector stream (accelerations written later by a reduction) is
     // zeroed here, so that no separate memset is needed
     if (zero_tail && k >= n_idx) zero_tail[k] = make_double4(0.0, 0.0, 0.0, 0.0);
-    const double fill = nan_pad ? __longlong_as_double(0x7ff8000000000000LL) : 0.0;
+    // 1: NaN (time-step streams: the candidate of a padding record drops out of every fmin); 2: far away
+    // (force streams: a padding record must coincide with no particle, see SymGradientFast); 0: zeros
+    const double fill = nan_pad == 1 ? __longlong_as_double(0x7ff8000000000000LL) : (nan_pad == 2 ? 1e150 : 0.0);
     double4 r = make_double4(fill, fill, fill, 0.0);
     if (k < n_idx) {
         const int i = idx ? idx[k] : k;

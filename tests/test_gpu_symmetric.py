@@ -397,3 +397,38 @@ def test_two_devices_pair_sharded_and_sink_sharded(oracle):
     finally:
         for f in ctx:
             f.close()
+
+
+@pytest.mark.parametrize("guard", [0, 1])
+def test_unguarded_gradient_pass_and_its_repair(frs, oracle, guard):
+    """frost_set_gradient_guard: pair-symmetric gradient sweeps of >= 16384 particles run without the
+    per-pair coincidence test; an input with two DISTINCT coincident unsoftened particles (ignored
+    pairwise, reading 11) then turns up as NaN in the first pass and is recomputed by the
+    gated guarded pass -- same contract, same tolerances, self and mutual sweeps; a particle at the
+    exact origin must not meet the padding records; guard = 1 keeps the test in the loop."""
+    import paper_2011_14984_b200 as frost
+    n = 20000
+    pos, vel, mass = fi.plummer(n, 31)
+    frs.set_gradient_guard(guard)
+    try:
+        for coincident in (False, True):
+            x = pos.copy()
+            x[:, 7] = 0.0                                  # exactly at the origin
+            if coincident:
+                x[:, 5] = x[:, 9]                          # inside one set
+                x[:, 17000] = x[:, 100]                    # across the two sets of the mutual sweep
+            a_ref, g_ref = oracle.forces(x, mass)
+            a, g = frs.forces(dev(x), dev(mass))
+            a, g = a.cpu().numpy(), g.cpu().numpy()
+            assert np.isfinite(g).all()
+            assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+            assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+            I = np.arange(0, 16500, dtype=np.int32); J = np.arange(16500, n, dtype=np.int32)
+            a_ref, g_ref = oracle.forces(x, mass, sink_idx=I, source_idx=J, flags=oracle.ACC | oracle.GRAD | oracle.MUTUAL)
+            am, gm = frs.forces(dev(x), dev(mass), dev(I), dev(J), flags=frost.ACC | frost.GRAD | frost.MUTUAL)
+            am, gm = am.cpu().numpy(), gm.cpu().numpy()
+            assert np.isfinite(gm).all()
+            assert (np.abs(am - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+            assert (np.abs(gm - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+    finally:
+        frs.set_gradient_guard(0)
