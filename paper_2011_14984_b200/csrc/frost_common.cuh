@@ -299,6 +299,24 @@ __device__ __forceinline__ double rsqrt_seed(double x) {
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     return y;
 }
+// The same seed with its LOW word taken from `junk` -- any value the caller no longer needs -- instead of
+// zero: ptxas then lets MUFU.RSQ64H write into the high half of junk's register pair and the MOV that
+// zeroes the low word (one issue slot per pair) disappears.  The seed's relative
+// error grows from 2^-22 to below 2^-19.7 (32 arbitrary low mantissa bits); one cubic step still
+// lands below 2^-57, the three-term series of the Newton weight below 2^-55.  Deterministic.
+__device__ __forceinline__ double rsqrt_seed_lo(double x, double junk) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return __hiloint2double(__double2hiint(y), __double2loint(junk));
+}
+__device__ __forceinline__ double rsqrt_full_lo(double x, double junk) {
+    const double y = rsqrt_seed_lo(x, junk);
+    const double t = x * y;
+    const double e = fma(-t, y, 1.0);
+    const double p = fma(0.375, e, 0.5);
+    const double ep = e * p;
+    return fma(y, ep, y);
+}
 // x += w*dx; y += w*dy; z += w*dz as three adjacent DFMAs with w in the same operand slot.
 __device__ __forceinline__ void fma3_shared(double &x, double &y, double &z, double w, double dx,
                                             double dy, double dz) {

@@ -67,7 +67,7 @@ struct SymNewton {
                                                 const double4 &, const SymParams &p) {
         const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
         const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
-        const double y = rsqrt_seed(s2);
+        const double y = rsqrt_seed(s2);      // (rsqrt_seed_lo measured 0.6 % slower here: 698.2 vs 694.2 ms)
         const double y2 = y * y;
         const double e = fma(-s2, y2, 1.0);
         const double w0 = y2 * y;
@@ -128,8 +128,9 @@ struct SymGradientFast : SymGradient {
                                                 const double4 &j1, const SymParams &p) {
         const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
         const double ax = j1.x - a.ax, ay = j1.y - a.ay, az = j1.z - a.az;
-        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
-        const double ri = rsqrt_full(s2);
+        const double part = fma(dy, dy, fma(dx, dx, p.eps2));
+        const double s2 = fma(dz, dz, part);
+        const double ri = rsqrt_full_lo(s2, part);        // (low word of the seed: see rsqrt_seed_lo)
         const double dot = fma(dz, az, fma(dy, ay, dx * ax));
         const double q = ri * ri;
         const double w3 = ri * q;
