@@ -38,6 +38,8 @@ FLOPS_NEWTON, FLOPS_GRAD = 18, 34          # per ordered pair (FMA = 2, add/mul 
 # FP64-pipe instructions per ORDERED pair as compiled: the pair-symmetric sweeps (frost_sym.cu) spend
 # 20 (Newton) and 32 (gradient) per unordered pair; the one-sided sweeps 16 and 28 per ordered pair
 SLOTS_NEWTON, SLOTS_GRAD = 10, 16
+# ... and one DMUL less per unordered pair in their equal-mass variant (frost_set_equal_mass_path; config 3)
+SLOTS_NEWTON_EQ, SLOTS_GRAD_EQ = 9.5, 15.5
 SLOTS_NEWTON_1S, SLOTS_GRAD_1S = 16, 28
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM
 SPLIT_MAX_CONFIG5 = 32768                  # frost_set_split for the split arm of the config-5 step
@@ -489,8 +491,11 @@ def run_frost(args):
     pairs_rank = float(n) * n / world if pair_sharded else float(sinks_here) * n
     if args.one_sided:      # forced: the one-sided sweeps run
         slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
+    elif bool((mass_h == mass_h[0]).all()):
+        slots_n, slots_g = SLOTS_NEWTON_EQ, SLOTS_GRAD_EQ
+        kname = "sym_kernel<SymGradientFastT<true>> (pair-symmetric gradient sweep, Eq. 27; equal-mass variant, no coincidence guard)"
     else:
-        slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradient> (pair-symmetric gradient sweep, Eq. 27)"
+        slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradientFastT<false>> (pair-symmetric gradient sweep, Eq. 27)"
     traffic, traffic_src = _sweep_traffic(args.one_sided, n)
     # measured FP64 rate of this run's probe (MEASURED_PEAKS.json carries no fp64 entry): a DFMA with two
     # loop-invariant operands issues every 2 cycles, i.e. thread instructions/s x 2 flop

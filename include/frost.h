@@ -272,6 +272,14 @@ int frost_set_pair_path(frost_ctx *ctx, int on);
  * at N = 2^20).  Default 0. */
 int frost_set_gradient_guard(frost_ctx *ctx, int on);
 
+/* Pair-symmetric force sweeps of 16384 particles or more have an equal-mass variant: if every particle
+ * of the sink and source lists has bitwise the same mass -- checked on the device while the streams
+ * are packed; Plummer models, configs 1-4 -- the weight of the reverse direction is the forward weight
+ * negated, one FP64 multiplication less per pair and bitwise the same sums.  Both variants of a sweep
+ * are enqueued behind complementary device-side gates, so no host decision or read-back is involved.
+ * on = 1 (default); 0 always runs the general kernels. */
+int frost_set_equal_mass_path(frost_ctx *ctx, int on);
+
 /* The kick sweeps of a split entry on their own (Eq. 42-44 on the pair set "labels differ"):
  *   out_acc[i]  <- G sum_{j in idx, label_j != label_i} m_j x_ji / s_ij^3,
  *   out_grad[i] <- 2G sum over the same j of m_j s^-5 (s^2 a_ji - 3 (x_ji.a_ji) x_ji) with the a of this call

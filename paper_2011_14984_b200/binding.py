@@ -26,7 +26,7 @@ exported_symbols = [
     "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
     "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
     "frost_set_split", "frost_forces_masked", "frost_set_pair_path",
-    "frost_set_gradient_guard",
+    "frost_set_gradient_guard", "frost_set_equal_mass_path",
 ]
 
 
@@ -74,6 +74,7 @@ def load_library():
     lib.frost_set_split.argtypes = [vp, i32]
     lib.frost_set_pair_path.argtypes = [vp, i32]
     lib.frost_set_gradient_guard.argtypes = [vp, i32]
+    lib.frost_set_equal_mass_path.argtypes = [vp, i32]
     lib.frost_forces_masked.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, vp, vp]
     lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -179,6 +180,11 @@ class Frost:
         """split_max > 0: hierarchy entries with at most split_max members recurse into the connected
         components of their fast pairs one by one (frost.h: frost_set_split); 0 (default): Alg. 3."""
         self._check(self.lib.frost_set_split(self.h, split_max), "frost_set_split")
+
+    def set_equal_mass_path(self, on=1):
+        """1 (default): large pair-symmetric force sweeps take their equal-mass variant when every mass
+        of the swept lists is the same (decided on the device; bitwise the same sums); 0: never."""
+        self._check(self.lib.frost_set_equal_mass_path(self.h, on), "frost_set_equal_mass_path")
 
     def set_gradient_guard(self, on=0):
         """0 (default): large pair-symmetric gradient sweeps run unguarded with a gated guarded repair

@@ -38,7 +38,7 @@ int frost_create(frost_ctx **out, int device, void *stream) {
 
 static void free_scratch(frost_ctx *c) {
     Buf *bufs[] = {&c->recA_xm, &c->recB_xm, &c->recA_v, &c->recB_v, &c->partial, &c->partialB, &c->tau_scratch, &c->symtot,
-                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats, &c->shard_idx, &c->uf, &c->comp, &c->symflag};
+                   &c->acc, &c->grad, &c->tau, &c->blockcnt, &c->dev_stats, &c->shard_idx, &c->uf, &c->comp, &c->symflag, &c->eqflag};
     for (Buf *b : bufs) if (b->p) cudaFree(b->p);
     for (Buf &b : c->host_stage) if (b.p) cudaFree(b.p);
     for (int k = 0; k < FROST_MAX_LEVELS; ++k) {
@@ -84,7 +84,7 @@ static int side_ctx(frost_ctx *c, int level, frost_ctx **out) {
     }
     s->G = c->G; s->eps2 = c->eps2; s->eta_ff = c->eta_ff; s->eta_fb = c->eta_fb; s->max_depth = c->max_depth;
     s->tune_k = c->tune_k; s->tune_slices = c->tune_slices; s->tune_small = c->tune_small;
-    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max; s->tune_pair = c->tune_pair; s->tune_guard = c->tune_guard;
+    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max; s->tune_pair = c->tune_pair; s->tune_guard = c->tune_guard; s->tune_eqmass = c->tune_eqmass;
     s->sym_scratch = c->sym_scratch < ((size_t)1 << 30) ? c->sym_scratch : ((size_t)1 << 30);
     *out = s;
     return FROST_OK;
@@ -133,6 +133,12 @@ int frost_set_overlap(frost_ctx *c, int on) {
 int frost_set_split(frost_ctx *c, int split_max) {
     if (!c || split_max < 0) return FROST_EINVAL;
     c->split_max = split_max;
+    return FROST_OK;
+}
+
+int frost_set_equal_mass_path(frost_ctx *c, int on) {
+    if (!c || on < 0 || on > 1) return FROST_EINVAL;
+    c->tune_eqmass = on;
     return FROST_OK;
 }
 
@@ -210,17 +216,26 @@ static int forces_impl_(frost_ctx *c, int n, int ld, const double *pos, const do
     FROST_TRY(ensure(c, c->recA_v, (size_t)padA * kRecBytes));
     double *Axm = (double *)c->recA_xm.p, *Av = (double *)c->recA_v.p;
     double *Bxm = Axm, *Bv = Av;
-    FROST_TRY(launch_pack_xm(c, ld, pos, mass, I, nI, padA, Axm, 1.0, 2, (flags & FROST_ACC) ? Av : nullptr));
-    if (!self) {
-        FROST_TRY(ensure(c, c->recB_xm, (size_t)padB * kRecBytes));
-        FROST_TRY(ensure(c, c->recB_v, (size_t)padB * kRecBytes));
-        Bxm = (double *)c->recB_xm.p; Bv = (double *)c->recB_v.p;
-        FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm, 1.0, 2, (flags & FROST_ACC) ? Bv : nullptr));
-    }
     // pair-symmetric sweeps (frost_sym.cu) serve both directions of every pair with one evaluation:
     // the self case, and the mutual case with the larger set as the register-resident A side
     const bool sym_self = self && use_sym(c, nI, nI, 0);
     const bool sym_mut = mutual && !self && use_sym(c, nI > nJ ? nI : nJ, nI > nJ ? nJ : nI, 1);
+    // ... and have an equal-mass variant (one DMUL less per pair): the pack kernels clear the flag if any
+    // mass of either list differs from the first one's
+    int *eq = nullptr;
+    if ((sym_self || sym_mut) && c->tune_eqmass) {
+        FROST_TRY(ensure(c, c->eqflag, 256));
+        eq = (int *)c->eqflag.p;
+        FROST_CUDA(c, cudaMemsetAsync(eq, 1, sizeof(int), c->stream));
+    }
+    FROST_TRY(launch_pack_xm(c, ld, pos, mass, I, nI, padA, Axm, 1.0, 2, (flags & FROST_ACC) ? Av : nullptr, eq, I));
+    if (!self) {
+        FROST_TRY(ensure(c, c->recB_xm, (size_t)padB * kRecBytes));
+        FROST_TRY(ensure(c, c->recB_v, (size_t)padB * kRecBytes));
+        Bxm = (double *)c->recB_xm.p; Bv = (double *)c->recB_v.p;
+        FROST_TRY(launch_pack_xm(c, ld, pos, mass, J, nJ, padB, Bxm, 1.0, 2, (flags & FROST_ACC) ? Bv : nullptr, eq, I));
+    }
+    c->eq_flag_cur = eq;
     if (sym_self || sym_mut) {
         const bool swap = sym_mut && nJ > nI;            // A = the larger set
         const double *Pxm = swap ? Bxm : Axm, *Qxm = swap ? Axm : Bxm;
@@ -286,6 +301,7 @@ static int forces_impl(frost_ctx *c, int n, int ld, const double *pos, const dou
     c->accumulate = (flags & FROST_ACCUMULATE) ? 1 : 0;
     const int rc = forces_impl_(c, n, ld, pos, mass, I, nI, J, nJ, acc, grad, flags);
     c->accumulate = 0;
+    c->eq_flag_cur = nullptr;
     return rc;
 }
 

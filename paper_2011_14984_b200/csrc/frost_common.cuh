@@ -43,6 +43,9 @@ struct frost_ctx {
     frost::Buf partialB;           // B-side partial sums of the pair-symmetric sweeps (frost_sym.cu)
     frost::Buf symtot;             // running totals across bands of a symmetric sweep
     frost::Buf symflag;            // "a sum came out non-finite" flag of the unguarded gradient pass
+    frost::Buf eqflag;             // "all masses of the packed lists are equal" flag (frost_update.cu)
+    const int *eq_flag_cur = nullptr;   // valid for the duration of one frost_forces call, else NULL
+    int tune_eqmass = 1;           // 1: equal-mass variants of the large symmetric sweeps where the flag allows
     int tune_guard = 0;            // 1: large symmetric gradient sweeps keep the per-pair coincidence guard
     size_t sym_scratch = (size_t)4 << 30;   // cap of partialB: the B list is swept in bands
     frost::Buf acc, grad, tau;     // internal planes for fsi / hhs
@@ -144,9 +147,11 @@ inline int round_up(int v, int m) { return (v + m - 1) / m * m; }
 // frost_update.cu
 // wscale multiplies the mass written to .w; nan_pad = 1 pads with NaN positions instead of zeros,
 // 2 with positions (1e150, 1e150, 1e150) -- mass 0 either way
+// eq_flag != NULL: *eq_flag is cleared if any packed mass differs (bitwise) from the mass of the first
+// particle of the list eq_ref (NULL = particle 0)
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
                    int n_idx, int n_pad, double *out, double wscale = 1.0, int nan_pad = 0,
-                   double *zero_tail = nullptr);
+                   double *zero_tail = nullptr, int *eq_flag = nullptr, const int32_t *eq_ref = nullptr);
 // w_index != 0: .w of record k carries the list position k in its low word (time-step sweeps that
 // enter their fast pairs into a union-find forest); otherwise 1.0
 int launch_pack_vec(frost_ctx *c, int ld, const double *planes, const int32_t *idx, int n_idx,

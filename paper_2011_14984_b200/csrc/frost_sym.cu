@@ -44,13 +44,19 @@ struct SymParams {
     double eps2, eta_ff, eta_fb;
     double pivot;             // SymTimestepEdge: fast pairs (candidate < pivot) are united in `forest`
     int *forest;
-    const int *gate;          // non-NULL: the launch does nothing unless *gate != 0 (repair pass, below)
+    const int *gate;          // non-NULL: the launch does nothing unless (*gate != 0) == (gate_want != 0)
+    int gate_want;            // (repair pass of the gradient sweep; equal-mass / general variants)
 };
 
 // ------------------------------------------------------------------------------------------------
 // Pair policies: A particle in registers, B particle = shared-memory record + travelling sums.
 // ------------------------------------------------------------------------------------------------
-struct SymNewton {
+// EQ: every particle of both lists has the same mass (checked on the device while the streams are
+// packed, frost_update.cu): then m_i s^-3 = m_j s^-3 and the second mass weight is the first one negated
+// -- one DMUL less per pair, bitwise the same sums.  The two variants of a sweep are launched behind
+// complementary gates on that flag.
+template <bool EQ>
+struct SymNewtonT {
     static constexpr int kRecs = 1, kPlanes = 3;
     static constexpr bool kMin = false;
     struct A { double x, y, z, nm, s[3]; };
@@ -75,11 +81,16 @@ struct SymNewton {
         const double qe = q * e;
         const double w = fma(w0, qe, w0);
         const double wa = w * j0.w;
-        const double wb = w * a.nm;
         fma3_shared(a.s[0], a.s[1], a.s[2], wa, dx, dy, dz);
-        fma3_shared(b[0], b[1], b[2], wb, dx, dy, dz);
+        if (EQ) {
+            b[0] = fma(-wa, dx, b[0]); b[1] = fma(-wa, dy, b[1]); b[2] = fma(-wa, dz, b[2]);
+        } else {
+            const double wb = w * a.nm;
+            fma3_shared(b[0], b[1], b[2], wb, dx, dy, dz);
+        }
     }
 };
+using SymNewton = SymNewtonT<false>;
 
 struct SymGradient {
     static constexpr int kRecs = 2, kPlanes = 3;
@@ -122,7 +133,8 @@ struct SymGradient {
 // launches when the flag is clear) recomputes the sweep: the contract of DESIGN.md reading 11 holds
 // for every input, and inputs without coincident particles never pay for the guard.  Padding records
 // sit at (1e150, 1e150, 1e150) with mass 0 (frost_api.cu), so that they coincide with no particle.
-struct SymGradientFast : SymGradient {
+template <bool EQ>
+struct SymGradientFastT : SymGradient {
     static constexpr bool kDiagGuard = true;
     __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
                                                 const double4 &j1, const SymParams &p) {
@@ -139,15 +151,21 @@ struct SymGradientFast : SymGradient {
         double vx = ax, vy = ay, vz = az;
         fma3_shared(vx, vy, vz, u, dx, dy, dz);
         const double wa = w3 * j0.w;
-        const double wb = w3 * a.nm;
         fma3_shared(a.s[0], a.s[1], a.s[2], wa, vx, vy, vz);
-        fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
+        if (EQ) {                          // equal masses: see SymNewtonT
+            b[0] = fma(-wa, vx, b[0]); b[1] = fma(-wa, vy, b[1]); b[2] = fma(-wa, vz, b[2]);
+        } else {
+            const double wb = w3 * a.nm;
+            fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
+        }
     }
     __device__ static __forceinline__ void pair_diag(A &a, double (&b)[3], const double4 &j0,
                                                      const double4 &j1, const SymParams &p) {
         SymGradient::pair(a, b, j0, j1, p);
     }
 };
+
+using SymGradientFast = SymGradientFastT<false>;
 
 template <class P, class = void> struct DiagGuard { static constexpr bool value = false; };
 template <class P> struct DiagGuard<P, std::enable_if_t<P::kDiagGuard>> { static constexpr bool value = true; };
@@ -250,7 +268,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
     constexpr int PL = P::kPlanes;
     constexpr uint32_t kStageBytes = P::kRecs * 2 * NT * kRecBytes;      // chunks stored twice
 
-    if (prm.gate && *prm.gate == 0) return;
+    if (prm.gate && ((*prm.gate != 0) != (prm.gate_want != 0))) return;
     const int I = prm.row0 + blockIdx.x * prm.row_stride;
     const int diag_end = prm.self ? (I + 1) * KA : 0;          // tiles below this are the diagonal block
     const int row_first_tile = max(prm.self ? I * KA : 0, prm.bt0);   // first B tile of this A tile in the band
@@ -455,12 +473,13 @@ struct SymJob {
     int32_t *out_bin;
     int *forest = nullptr;                 // time-step sweep: union-find forest of the fast pairs
     const int *gate = nullptr;             // the whole sweep runs only if *gate != 0
+    const int *eq_flag = nullptr;          // run_sym<P, ..., PEQ>: *eq_flag != 0 selects the PEQ kernel
     int *flag = nullptr;                   // set to 1 if any scattered sum is not finite
     int shard_rank = 0, shard_world = 1;   // this launch sweeps A tiles rank, rank + world, ... only
     int accumulate = 0;                    // add the sums to `out` instead of overwriting it
 };
 
-template <class P, int KA, int NT, int MINB>
+template <class P, int KA, int NT, int MINB, class PEQ = P>
 static int run_sym(frost_ctx *c, const SymJob &job) {
     constexpr int PL = P::kPlanes, TA = KA * NT;
     constexpr bool MIN = P::kMin;
@@ -484,6 +503,9 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
     const size_t smem = (size_t)kStages * P::kRecs * 2 * NT * kRecBytes + 2 * PL * NT * sizeof(double) +
                         kStages * sizeof(uint64_t);
     FROST_TRY(set_func_attr(c, sym_kernel<P, KA, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    constexpr bool kHasEq = !std::is_same<P, PEQ>::value;
+    if (kHasEq)
+        FROST_TRY(set_func_attr(c, sym_kernel<PEQ, KA, NT, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
 
     for (int b = 0; b < nbands; ++b) {
         const int bt0 = b * (int)band_tiles;
@@ -513,11 +535,18 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
         prm.na_pad = na_pad; prm.self = self ? 1 : 0; prm.bt0 = bt0; prm.bt1 = bt1;
         prm.seg_tiles = (int)seg; prm.row0 = row0; prm.row_stride = row_stride;
         prm.eps2 = job.eps2; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
-        prm.pivot = job.tau_pivot; prm.forest = job.forest; prm.gate = job.gate;
+        prm.pivot = job.tau_pivot; prm.forest = job.forest; prm.gate = job.gate; prm.gate_want = 1;
         if (my_rows > 0) {
             dim3 grid(my_rows, segs);
+            if (kHasEq && job.eq_flag && !job.gate) {       // equal-mass variant | general variant
+                prm.gate = job.eq_flag; prm.gate_want = 1;
+                sym_kernel<PEQ, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
+                FROST_TRY(check_launch(c));
+                prm.gate_want = 0;
+            }
             sym_kernel<P, KA, NT, MINB><<<grid, NT, smem, c->stream>>>(prm);
             FROST_TRY(check_launch(c));
+            prm.gate = job.gate; prm.gate_want = 1;
         }
 
         const int first = b == 0, last = b == nbands - 1;
@@ -582,7 +611,8 @@ int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int
     j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;      // see NewtonPolicy::pair
     j.shard_rank = c->shard_rank; j.shard_world = c->shard_world; j.accumulate = c->accumulate;
     if (nA < kSymSmallN) return run_sym<SymNewton, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
-    return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB>(c, j);
+    j.eq_flag = c->eq_flag_cur;
+    return run_sym<SymNewton, kSymKNewton, kSymNT, kSymMinB, SymNewtonT<true>>(c, j);
 }
 
 // Gradient sweep, both directions at once (Eq. 27 / 43 / 44); *_a are the packed accelerations.
@@ -602,9 +632,9 @@ int sym_gradient(frost_ctx *c, const double *A_xm, const double *A_a, int nA, co
         FROST_TRY(ensure(c, c->symflag, 256));
         int *flag = (int *)c->symflag.p;
         FROST_CUDA(c, cudaMemsetAsync(flag, 0, sizeof(int), c->stream));
-        j.flag = flag;
-        FROST_TRY((run_sym<SymGradientFast, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j)));
-        j.flag = nullptr; j.gate = flag;
+        j.flag = flag; j.eq_flag = c->eq_flag_cur;
+        FROST_TRY((run_sym<SymGradientFast, kSymKGrad, kSymNTGrad, kSymMinBGrad, SymGradientFastT<true>>(c, j)));
+        j.flag = nullptr; j.eq_flag = nullptr; j.gate = flag;
     }
     return run_sym<SymGradient, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j);
 }

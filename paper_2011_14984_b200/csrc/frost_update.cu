@@ -11,7 +11,8 @@ namespace frost {
 __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__restrict__ mass, int ld,
                                const int32_t *__restrict__ idx, int n_idx, int n_pad,
                                double4 *__restrict__ out, double wscale, int nan_pad,
-                               double4 *__restrict__ zero_tail) {
+                               double4 *__restrict__ zero_tail, int *__restrict__ eq_flag,
+                               const int32_t *__restrict__ eq_ref) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n_pad) return;
     // the padding of the companion vector stream (accelerations written later by a reduction) is
@@ -24,6 +25,10 @@ __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__r
     if (k < n_idx) {
         const int i = idx ? idx[k] : k;
         r = make_double4(pos[i], pos[(size_t)ld + i], pos[2 * (size_t)ld + i], mass[i] * wscale);
+        // equal-mass detection for the pair-symmetric sweeps (SymNewtonT<true>): bitwise comparison
+        // against the first particle of the list eq_ref (NULL = particle 0)
+        if (eq_flag && __double_as_longlong(mass[i]) != __double_as_longlong(mass[eq_ref ? eq_ref[0] : 0]))
+            *eq_flag = 0;
     }
     out[k] = r;
 }
@@ -233,11 +238,12 @@ diag_kernel(const double *__restrict__ pos, const double *__restrict__ vel, cons
 
 // ---- launchers ---------------------------------------------------------------------------------
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
-                   int n_idx, int n_pad, double *out, double wscale, int nan_pad, double *zero_tail) {
+                   int n_idx, int n_pad, double *out, double wscale, int nan_pad, double *zero_tail,
+                   int *eq_flag, const int32_t *eq_ref) {
     if (n_pad <= 0) return FROST_OK;
     pack_xm_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(pos, mass, ld, idx, n_idx, n_pad,
                                                              (double4 *)out, wscale, nan_pad,
-                                                             (double4 *)zero_tail);
+                                                             (double4 *)zero_tail, eq_flag, eq_ref);
     return check_launch(c);
 }
 

@@ -432,3 +432,32 @@ def test_unguarded_gradient_pass_and_its_repair(frs, oracle, guard):
             assert (np.abs(gm - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
     finally:
         frs.set_gradient_guard(0)
+
+
+def test_equal_mass_variant_is_bitwise_the_general_kernels(frs, oracle):
+    """frost_set_equal_mass_path: on an equal-mass Plummer sphere the large pair-symmetric sweeps take
+    the variant with one multiplication less per pair (flag computed on the device by the pack kernels,
+    both variants enqueued behind complementary gates) -- bitwise the general kernels' sums, self and
+    mutual; one different mass anywhere in the swept lists switches the sweep back to the general
+    kernels (parity with the oracle either way)."""
+    import paper_2011_14984_b200 as frost
+    n = 20000
+    pos, vel, mass = fi.plummer(n, 33)
+    I = np.arange(0, 16500, dtype=np.int32); J = np.arange(16500, n, dtype=np.int32)
+    for tweak in (False, True):
+        m = mass.copy()
+        if tweak:
+            m[17777] *= 1.5
+        res = []
+        for on in (1, 0):
+            frs.set_equal_mass_path(on)
+            a, g = frs.forces(dev(pos), dev(m))
+            am, gm = frs.forces(dev(pos), dev(m), dev(I), dev(J), flags=frost.ACC | frost.GRAD | frost.MUTUAL)
+            res.append((a, g, am, gm))
+        frs.set_equal_mass_path(1)
+        for x, y in zip(res[0], res[1]):
+            assert torch.equal(x, y)
+        a_ref, g_ref = oracle.forces(pos, m)
+        a, g = res[0][0].cpu().numpy(), res[0][1].cpu().numpy()
+        assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
+        assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
