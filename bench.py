@@ -380,6 +380,8 @@ def run_frost(args):
     fr.set_params(G=1.0, eps2=0.0)
     if args.one_sided:
         fr.set_symmetric(1)
+    if args.no_eqmass:
+        fr.set_equal_mass_path(0)
     # N > 1: the PAIRS are sharded (frost_set_shard: every rank sweeps 1/world of the tile pairs of
     # the symmetric kernels and holds partial sums for all particles; one all-reduce per sweep)
     lo, hi = 0, n
@@ -491,7 +493,7 @@ def run_frost(args):
     pairs_rank = float(n) * n / world if pair_sharded else float(sinks_here) * n
     if args.one_sided:      # forced: the one-sided sweeps run
         slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
-    elif bool((mass_h == mass_h[0]).all()):
+    elif bool((mass_h == mass_h[0]).all()) and not args.no_eqmass:
         slots_n, slots_g = SLOTS_NEWTON_EQ, SLOTS_GRAD_EQ
         kname = "sym_kernel<SymGradientFastT<true>> (pair-symmetric gradient sweep, Eq. 27; equal-mass variant, no coincidence guard)"
     else:
@@ -586,6 +588,7 @@ def main():
     ap.add_argument("--rows-only", action="store_true", help="launch the O(N) kernels and time-step sweeps (for ncu)")
     ap.add_argument("--subtree", type=int, default=0, help="run the subtree kernel on K/2 hard binaries (for ncu)")
     ap.add_argument("--hhs-only", action="store_true", help="one HHS-FSI step of config 5 with its validity numbers")
+    ap.add_argument("--no-eqmass", action="store_true", help="general kernels even on equal masses (frost_set_equal_mass_path(0))")
     ap.add_argument("--hhs-arm", default="both", choices=["both", "alg3", "split"],
                     help="--hhs-only: Alg. 3 as printed, the split fast levels (frost_set_split), or both")
     args = ap.parse_args()

@@ -27,6 +27,15 @@
 // is two-sided and one sweep yields both directions of acc_sf_*.
 #include <type_traits>
 
+// Rotation steps per iteration of the main loop of sym_kernel, and whether the Newton seed takes its low
+// word from a dying value (rsqrt_seed_lo).  ptxas' schedule of this loop moves the sweep time by +-1.5 %
+// with such details; chosen by measurement at N = 2^20 (ms per sweep, B200):
+//   Newton, equal masses:   unroll 1 / 2 / 4 = 668.5 / 670.6 / 655.6; 4 with the seed trick 665.2; 8 with it 662.4
+//   Newton, general:        unroll 2 = 694.8; 4 = 692.5; 4 with the seed trick 688.2; 1 = 697.4
+//                           (the seed trick is not used: both variants keep the same seed => same bits)
+//   gradient, equal masses: unroll 1 / 2 / 4 = 1080.2 / 1094.8 / 1087.5
+//   gradient, general:      unroll 1 / 2 / 4 = 1117.7 / 1110.3 / 1102.4
+
 #include "frost_pairs.cuh"
 
 namespace frost {
@@ -57,7 +66,7 @@ struct SymParams {
 // complementary gates on that flag.
 template <bool EQ>
 struct SymNewtonT {
-    static constexpr int kRecs = 1, kPlanes = 3;
+    static constexpr int kRecs = 1, kPlanes = 3, kUnroll = 4;
     static constexpr bool kMin = false;
     struct A { double x, y, z, nm, s[3]; };
     __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
@@ -73,7 +82,8 @@ struct SymNewtonT {
                                                 const double4 &, const SymParams &p) {
         const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
         const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
-        const double y = rsqrt_seed(s2);      // (rsqrt_seed_lo measured 0.6 % slower here: 698.2 vs 694.2 ms)
+        const double y = rsqrt_seed(s2);      // (rsqrt_seed_lo: table at the top of the file; the two variants
+                                              //  must use the same seed to stay bitwise equal)
         const double y2 = y * y;
         const double e = fma(-s2, y2, 1.0);
         const double w0 = y2 * y;
@@ -136,6 +146,7 @@ struct SymGradient {
 template <bool EQ>
 struct SymGradientFastT : SymGradient {
     static constexpr bool kDiagGuard = true;
+    static constexpr int kUnroll = EQ ? 1 : 4;
     __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
                                                 const double4 &j1, const SymParams &p) {
         const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
@@ -167,6 +178,8 @@ struct SymGradientFastT : SymGradient {
 
 using SymGradientFast = SymGradientFastT<false>;
 
+template <class P, class = void> struct UnrollOf { static constexpr int value = 2; };
+template <class P> struct UnrollOf<P, std::enable_if_t<(P::kUnroll > 0)>> { static constexpr int value = P::kUnroll; };
 template <class P, class = void> struct DiagGuard { static constexpr bool value = false; };
 template <class P> struct DiagGuard<P, std::enable_if_t<P::kDiagGuard>> { static constexpr bool value = true; };
 
@@ -346,7 +359,7 @@ __global__ void __launch_bounds__(NT, MINB) sym_kernel(const SymParams prm) {
                     for (int p = 0; p < PL; ++p) b[p] = __shfl_sync(0xffffffffu, b[p], from);
                 }
             } else {
-#pragma unroll 2
+#pragma unroll (UnrollOf<P>::value)
                 for (int step = 0; step < 32; ++step) {
                     const double4 j0 = c0[-step];
                     const double4 j1 = (P::kRecs == 2) ? c1[-step] : j0;
