@@ -75,6 +75,7 @@ typedef struct {
     int64_t pairs_timestep;                 /* ordered pairs swept by Eq. 49-54 */
     int64_t n_comp[ORACLE_MAX_LEVELS];      /* sum over those entries of the number of fast components
                                                recursed into (Alg. 3 itself: 1 per entry with |F| > 0) */
+    int64_t n_kepler;                       /* two-body components advanced by the Kepler propagator (O6k) */
 } oracle_hhs_stats;
 
 int oracle_num_threads(void) {
@@ -579,6 +580,106 @@ int oracle_forces_masked(int n, int ld, const double *pos, const double *mass, c
 }
 
 /* ---------------------------------------------------------------------------------------------
+ * O6k.  Two-body propagator for a component of exactly two particles (second half: the
+ * paper lists "regularised integrators ..., Wisdom-Holman integrators and Kepler solvers" as the
+ * modules a spatially split level can hand its few-body systems to; it defines none.
+ * DESIGN.md reading 25).  A two-body component's Hamiltonian H_C is integrable: the centre of mass
+ * moves uniformly and the relative vector r = x_2 - x_1, v = v_2 - v_1 follows the Kepler flow with
+ * mu = G (m_1 + m_2), advanced here over dt by the universal-variable form of Kepler's equation
+ * (valid for ellipses, parabolas and hyperbolas alike), with the Stumpff functions
+ *     c_k(z) = sum_{n>=0} (-z)^n / (2n + k)!,   z = alpha s^2,   alpha = 2 mu / r_0 - v_0^2 :
+ *     r_0 s c_1 + (r_0.v_0) s^2 c_2 + mu s^3 c_3 = dt                       (solved for s)
+ *     f = 1 - (mu/r_0) s^2 c_2,   g = dt - mu s^3 c_3,
+ *     r = r_0 c_0 + (r_0.v_0) s c_1 + mu s^2 c_2,
+ *     f' = -(mu / (r r_0)) s c_1,   g' = 1 - (mu / r) s^2 c_2,
+ *     r(dt) = f r_0 + g v_0,   v(dt) = f' r_0 + g' v_0.
+ * The left-hand side is increasing in s (its derivative is the separation r > 0): the root is found
+ * by Newton's method kept inside a bracket.  For a bound orbit whole periods are removed from dt first.
+ * long double throughout (the oracle's accuracy margin); unsoftened only.
+ * ------------------------------------------------------------------------------------------- */
+static void stumpff(ld_t z, ld_t c[4]) {
+    /* quarter the argument until the series converges fast, then the duplication formulas
+     * c_0(4z) = 2 c_0(z)^2 - 1, c_1(4z) = c_0 c_1, c_2(4z) = c_1^2 / 2, c_3(4z) = (c_2 + c_0 c_3) / 4 */
+    int k = 0;
+    while (fabsl(z) > 0.1L) { z *= 0.25L; ++k; }
+    ld_t c2 = 0, c3 = 0, t2 = 0.5L, t3 = 1.0L / 6.0L;
+    for (int n = 0; n < 16; ++n) {            /* (-z)^n / (2n+2)!  and  (-z)^n / (2n+3)! */
+        c2 += t2; c3 += t3;
+        t2 *= -z / (ld_t)((2 * n + 3) * (2 * n + 4));
+        t3 *= -z / (ld_t)((2 * n + 4) * (2 * n + 5));
+    }
+    ld_t c1 = 1.0L - z * c3, c0 = 1.0L - z * c2;
+    for (; k > 0; --k) {
+        c3 = 0.25L * (c2 + c0 * c3);
+        c2 = 0.5L * c1 * c1;
+        c1 = c0 * c1;
+        c0 = 2.0L * c0 * c0 - 1.0L;
+    }
+    c[0] = c0; c[1] = c1; c[2] = c2; c[3] = c3;
+}
+
+/* relative position r and velocity v (in place) advanced by dt > 0 along the Kepler flow of mu */
+int oracle_kepler_relative(double mu, double dt, double r[3], double v[3]) {
+    if (!(mu > 0.0) || !(dt >= 0.0)) return ORACLE_EINVAL;
+    const ld_t rx = r[0], ry = r[1], rz = r[2], vx = v[0], vy = v[1], vz = v[2];
+    const ld_t r0 = sqrtl(rx * rx + ry * ry + rz * rz);
+    if (!(r0 > 0)) return ORACLE_EINVAL;
+    const ld_t v2 = vx * vx + vy * vy + vz * vz, u = rx * vx + ry * vy + rz * vz;
+    const ld_t M = mu, alpha = 2 * M / r0 - v2;
+    ld_t t = dt;
+    if (alpha > 0) {                                   /* bound: remove whole periods */
+        const ld_t P = 2 * 3.14159265358979323846264338327950288L * M / (alpha * sqrtl(alpha));
+        t -= floorl(t / P) * P;
+    }
+    ld_t c[4], lo = 0, hi = t / r0, s;
+    for (;;) {                                         /* bracket the root: F(lo) <= 0 < F(hi) */
+        stumpff(alpha * hi * hi, c);
+        if (r0 * hi * c[1] + u * hi * hi * c[2] + M * hi * hi * hi * c[3] - t > 0) break;
+        lo = hi; hi = 2 * hi + 1e-300L;
+    }
+    s = 0.5L * (lo + hi);
+    for (int it = 0; it < 200; ++it) {
+        stumpff(alpha * s * s, c);
+        const ld_t F = r0 * s * c[1] + u * s * s * c[2] + M * s * s * s * c[3] - t;
+        const ld_t dF = r0 * c[0] + u * s * c[1] + M * s * s * c[2];
+        if (F == 0) break;
+        if (F > 0) hi = s; else lo = s;
+        ld_t sn = s - F / dF;
+        if (!(sn >= lo && sn <= hi)) sn = 0.5L * (lo + hi);
+        if (fabsl(sn - s) <= 1e-19L * fabsl(s)) { s = sn; break; }
+        s = sn;
+    }
+    stumpff(alpha * s * s, c);
+    const ld_t rr = r0 * c[0] + u * s * c[1] + M * s * s * c[2];
+    const ld_t f = 1 - (M / r0) * s * s * c[2], g = t - M * s * s * s * c[3];
+    const ld_t fd = -(M / (rr * r0)) * s * c[1], gd = 1 - (M / rr) * s * s * c[2];
+    r[0] = (double)(f * rx + g * vx); r[1] = (double)(f * ry + g * vy); r[2] = (double)(f * rz + g * vz);
+    v[0] = (double)(fd * rx + gd * vx); v[1] = (double)(fd * ry + gd * vy); v[2] = (double)(fd * rz + gd * vz);
+    return ORACLE_OK;
+}
+
+/* particles i and j advanced by dt along their exact two-body motion (centre of mass uniform) */
+static int kepler_pair(int ld, double *pos, double *vel, const double *mass, int i, int j, double G, double dt) {
+    const ld_t mi = mass[i], mj = mass[j], mt = mi + mj;
+    ld_t X[3], V[3];
+    double r[3], v[3];
+    for (int k = 0; k < 3; ++k) {
+        X[k] = (mi * pos[k * ld + i] + mj * pos[k * ld + j]) / mt;
+        V[k] = (mi * vel[k * ld + i] + mj * vel[k * ld + j]) / mt;
+        r[k] = pos[k * ld + j] - pos[k * ld + i];
+        v[k] = vel[k * ld + j] - vel[k * ld + i];
+    }
+    const int rc = oracle_kepler_relative(G * (mass[i] + mass[j]), dt, r, v);
+    if (rc != ORACLE_OK) return rc;
+    for (int k = 0; k < 3; ++k) {
+        const ld_t Xk = X[k] + V[k] * (ld_t)dt;
+        pos[k * ld + i] = (double)(Xk - (mj / mt) * r[k]); pos[k * ld + j] = (double)(Xk + (mi / mt) * r[k]);
+        vel[k * ld + i] = (double)(V[k] - (mj / mt) * v[k]); vel[k * ld + j] = (double)(V[k] + (mi / mt) * v[k]);
+    }
+    return ORACLE_OK;
+}
+
+/* ---------------------------------------------------------------------------------------------
  * O6.  HHS-FSI, Eq. (41); Alg. 3, line by line.
  * `frozen_level` (may be NULL): if given, particle i is slow at the first level k with
  * k >= frozen_level[i] instead of by its time-step -- the "frozen partition" used only by the
@@ -593,6 +694,7 @@ typedef struct {
     int eta_in_q, max_depth;
     const int32_t *frozen_level;
     int split_max;                     /* O6s: entries with |set| <= split_max split F into components */
+    int kepler;                        /* O6k: two-body components of a split entry follow their Kepler orbit */
     const int32_t *frozen_comp;        /* with frozen_level: the component of particle i (any labels) */
     double *acc, *grad, *tau;
     int32_t *label;
@@ -673,8 +775,13 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
     oracle_kick(n, ld, e->vel, e->acc, NULL, F, nF, tau_pivot / 6.0, 0.0);
     /* fsi(S, tau/2); hhs_fsi(C_c, tau/2) for every component (Alg. 3: hhs_fsi(F, tau/2)) */
     rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
-    for (int c = 0; c < m && rc == ORACLE_OK; ++c)
-        rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
+    const int kep = e->kepler && e->split_max > 0 && n_set <= e->split_max && e->eps2 == 0.0;
+    for (int c = 0; c < m && rc == ORACLE_OK; ++c) {
+        if (kep && cstart[c + 1] - cstart[c] == 2) {
+            rc = kepler_pair(ld, e->pos, e->vel, e->mass, F[cstart[c]], F[cstart[c] + 1], e->G, h);
+            if (st) st->n_kepler += 1;
+        } else rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
+    }
     if (rc == ORACLE_OK) {
         /* acc_sf_gradient (Eq. 43-44) with the inter-level a of Eq. 42; kick_sf by 2 tau/3 with
          * a~ = a + tau_pivot^2 g / 48 (eps = this level's step, reading 7).  The recursion
@@ -692,8 +799,12 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
         oracle_kick(n, ld, e->vel, e->acc, e->grad, S, nS, 2.0 * tau_pivot / 3.0, kap);
         oracle_kick(n, ld, e->vel, e->acc, e->grad, F, nF, 2.0 * tau_pivot / 3.0, kap);
         /* hhs_fsi(C_c, tau/2); fsi(S, tau/2) */
-        for (int c = 0; c < m && rc == ORACLE_OK; ++c)
-            rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
+        for (int c = 0; c < m && rc == ORACLE_OK; ++c) {
+            if (kep && cstart[c + 1] - cstart[c] == 2) {
+                rc = kepler_pair(ld, e->pos, e->vel, e->mass, F[cstart[c]], F[cstart[c] + 1], e->G, h);
+                if (st) st->n_kepler += 1;
+            } else rc = hhs_recursive(e, F + cstart[c], cstart[c + 1] - cstart[c], h, level + 1);
+        }
     }
     if (rc == ORACLE_OK)
         rc = fsi_on_set(n, ld, e->pos, e->vel, e->mass, S, nS, h, e->G, e->eps2, e->acc, e->grad, st);
@@ -722,13 +833,13 @@ static int hhs_recursive(hhs_env *e, const int32_t *set, int n_set, double tau_p
 int oracle_hhs_split_step(int n, int ld, double *pos, double *vel, const double *mass, double dt_top,
                           double G, double eps2, double eta_ff, double eta_fb, int eta_in_q,
                           int max_depth, const int32_t *frozen_level, int split_max,
-                          const int32_t *frozen_comp, oracle_hhs_stats *stats) {
+                          const int32_t *frozen_comp, int kepler, oracle_hhs_stats *stats) {
     if (n < 0 || ld < n || !pos || !vel || !mass || !(dt_top > 0.0) || split_max < 0) return ORACLE_EINVAL;
     hhs_env e;
     e.n = n; e.ld = ld; e.pos = pos; e.vel = vel; e.mass = mass;
     e.G = G; e.eps2 = eps2; e.eta_ff = eta_ff; e.eta_fb = eta_fb;
     e.eta_in_q = eta_in_q; e.max_depth = max_depth; e.frozen_level = frozen_level;
-    e.split_max = split_max; e.frozen_comp = frozen_comp;
+    e.split_max = split_max; e.frozen_comp = frozen_comp; e.kepler = kepler;
     e.acc = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
     e.grad = (double *)calloc((size_t)3 * ld + 1, sizeof(double));
     e.tau = (double *)calloc((size_t)ld + 1, sizeof(double));
@@ -749,7 +860,7 @@ int oracle_hhs_step(int n, int ld, double *pos, double *vel, const double *mass,
                     double G, double eps2, double eta_ff, double eta_fb, int eta_in_q,
                     int max_depth, const int32_t *frozen_level, oracle_hhs_stats *stats) {
     return oracle_hhs_split_step(n, ld, pos, vel, mass, dt_top, G, eps2, eta_ff, eta_fb, eta_in_q,
-                                 max_depth, frozen_level, 0, NULL, stats);
+                                 max_depth, frozen_level, 0, NULL, 0, stats);
 }
 
 /* ---------------------------------------------------------------------------------------------

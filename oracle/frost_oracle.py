@@ -23,14 +23,15 @@ class HHSStats(C.Structure):
                 ("entries", C.c_int64 * MAX_LEVELS), ("n_slow", C.c_int64 * MAX_LEVELS),
                 ("n_fast", C.c_int64 * MAX_LEVELS), ("pairs_newton", C.c_int64),
                 ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64),
-                ("n_comp", C.c_int64 * MAX_LEVELS)]
+                ("n_comp", C.c_int64 * MAX_LEVELS), ("n_kepler", C.c_int64)]
 
     def as_dict(self):
         d = self.depth
         return {"depth": d, "entries": list(self.entries[: d + 1]),
                 "n_slow": list(self.n_slow[: d + 1]), "n_fast": list(self.n_fast[: d + 1]),
                 "pairs_newton": self.pairs_newton, "pairs_gradient": self.pairs_gradient,
-                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1])}
+                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1]),
+                "n_kepler": self.n_kepler}
 
 
 def lib():
@@ -179,7 +180,7 @@ def fsi_step(pos, vel, mass, dt, idx=None, G=1.0, eps2=0.0):
 
 
 def hhs_step(pos, vel, mass, dt_top, G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2, eta_in_q=True,
-             max_depth=64, frozen_level=None, split_max=0, frozen_comp=None):
+             max_depth=64, frozen_level=None, split_max=0, frozen_comp=None, kepler=False):
     """One HHS-FSI step (Alg. 3).  split_max > 0: entries with at most split_max members split
     their fast set into the connected components of the fast pairs (O6s in frost_oracle.c)."""
     ld = pos.shape[1]
@@ -191,9 +192,18 @@ def hhs_step(pos, vel, mass, dt_top, G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2, et
                                      C.c_double(dt_top), C.c_double(G), C.c_double(eps2),
                                      C.c_double(eta_ff), C.c_double(eta_fb),
                                      C.c_int(1 if eta_in_q else 0), C.c_int(max_depth), _ptr(fl),
-                                     C.c_int(split_max), _ptr(fc), C.byref(st))
+                                     C.c_int(split_max), _ptr(fc), C.c_int(1 if kepler else 0),
+                                     C.byref(st))
     _check(rc, "oracle_hhs_split_step")
     return st.as_dict()
+
+
+def kepler_relative(mu, dt, r, v):
+    """Relative position and velocity (length-3 arrays) advanced by dt along the Kepler flow of mu."""
+    rr = np.ascontiguousarray(r, dtype=np.float64).copy()
+    vv = np.ascontiguousarray(v, dtype=np.float64).copy()
+    _check(lib().oracle_kepler_relative(C.c_double(mu), C.c_double(dt), _d(rr), _d(vv)), "oracle_kepler_relative")
+    return rr, vv
 
 
 def components(pos, vel, mass, tau_pivot, idx=None, G=1.0, eta_ff=0.2, eta_fb=0.2, eta_in_q=True):

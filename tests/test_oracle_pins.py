@@ -730,3 +730,78 @@ def test_split_step_on_a_cluster_with_binaries(oracle):
         assert np.abs((mass * (v - vel)).sum(1)).max() < 1e-15
     assert abs(de1) < 10 * abs(de0) + 1e-10, (de0, de1)
     assert np.abs(p1 - p0).max() < 1e-5, np.abs(p1 - p0).max()
+
+
+# ------------------------------------ O6k: two-body propagator of a split level's binary components
+def test_kepler_propagator_matches_the_classical_elements_solution(oracle):
+    """oracle_kepler_relative (universal variables, Stumpff functions) against the textbook route
+    through the eccentric anomaly (M = E - e sin E; _kepler_state above) -- an independent
+    parametrisation of the same orbit -- for e = 0 ... 0.99, fractions of a period and many periods."""
+    for e in (0.0, 0.3, 0.9, 0.99):
+        for mt, a in ((1.0, 1.0), (3.7e-5, 2.5e-4)):
+            G = 0.8
+            P = 2 * math.pi * math.sqrt(a ** 3 / (G * mt))
+            r0, v0 = _kepler_state(mt * 0.6, mt * 0.4, a, e, 0.0, G)
+            for frac in (1e-3, 0.37, 0.5, 1.0, 7.81, 123.456):
+                r1, v1 = oracle.kepler_relative(G * mt, frac * P, r0, v0)
+                rr, vr = _kepler_state(mt * 0.6, mt * 0.4, a, e, frac * P, G)
+                # the classical route loses digits near pericentre of e = 0.99 and over many periods
+                tol = 1e-12 * (1 + frac) / (1 - e) ** 2
+                assert np.abs(r1 - rr).max() < tol * a, (e, a, frac, r1, rr)
+                assert np.abs(v1 - vr).max() < tol * np.abs(v0).max() / (1 - e), (e, a, frac, v1, vr)
+
+
+def test_kepler_propagator_unbound_orbits_and_group_property(oracle):
+    """Hyperbolic and near-parabolic fly-bys: energy and angular momentum are invariant, two half
+    steps equal one full step, propagating the reversed state returns to the start, and the result
+    agrees with a fine FSI integration (O5, pinned above) of the same two bodies."""
+    rng = np.random.default_rng(4)
+    for k in range(6):
+        r0 = rng.normal(size=3); v0 = rng.normal(size=3) * (2.0 if k < 4 else 1.0)
+        mu = 0.9
+        if k >= 4:                                      # near-parabolic: v^2 = 2 mu / r (1 + 1e-9)
+            v0 *= math.sqrt(2 * mu / np.linalg.norm(r0) * (1 + 1e-9)) / np.linalg.norm(v0)
+        dt = 1.3
+        r1, v1 = oracle.kepler_relative(mu, dt, r0, v0)
+        E0 = 0.5 * v0 @ v0 - mu / np.linalg.norm(r0); E1 = 0.5 * v1 @ v1 - mu / np.linalg.norm(r1)
+        assert abs(E1 - E0) < 1e-14 * (abs(E0) + mu / np.linalg.norm(r0))
+        assert np.abs(np.cross(r1, v1) - np.cross(r0, v0)).max() < 1e-14 * np.linalg.norm(np.cross(r0, v0))
+        ra, va = oracle.kepler_relative(mu, 0.5 * dt, r0, v0)
+        rb, vb = oracle.kepler_relative(mu, 0.5 * dt, ra, va)
+        assert np.abs(rb - r1).max() < 1e-14 * np.abs(r1).max() and np.abs(vb - v1).max() < 1e-14 * np.abs(v0).max()
+        rback, vback = oracle.kepler_relative(mu, dt, r1, -v1)
+        assert np.abs(rback - r0).max() < 1e-13 * np.abs(r1).max() and np.abs(vback + v0).max() < 1e-13 * np.abs(v0).max()
+    # against FSI with a small step (two bodies of total mass 0.9, G = 1)
+    m = np.array([0.5, 0.4])
+    pos = np.ascontiguousarray(np.array([[0.0, 1.1], [0.0, 0.2], [0.0, -0.3]]))
+    vel = np.ascontiguousarray(np.array([[0.0, -0.4], [0.0, 1.5], [0.0, 0.2]]))
+    r1, v1 = oracle.kepler_relative(0.9, 0.8, pos[:, 1] - pos[:, 0], vel[:, 1] - vel[:, 0])
+    for _ in range(4000):
+        oracle.fsi_step(pos, vel, m, 0.8 / 4000)
+    assert np.abs((pos[:, 1] - pos[:, 0]) - r1).max() < 1e-10 and np.abs((vel[:, 1] - vel[:, 0]) - v1).max() < 1e-10
+
+
+def test_split_step_with_kepler_components(oracle):
+    """The split step with its two-body components on their Kepler orbits (O6k): momentum at
+    roundoff, the binaries no longer recursed into (far fewer entries), an energy error no larger than
+    the split step's own, and an end state within the truncation error of it; with softening, or
+    without the split, the option changes nothing."""
+    pos, vel, mass, pairs = fi.star_cluster(300, 4, binary_fraction=0.2, a_lo=1e-4, a_hi=1e-2, e_max=0.3)
+    e0 = oracle.diagnostics(pos, vel, mass)["E"]
+    out = []
+    for kep in (False, True):
+        p, v = pos.copy(), vel.copy()
+        st = oracle.hhs_step(p, v, mass, 2.0 ** -6, split_max=1 << 20, kepler=kep)
+        out.append((st, p, v, oracle.diagnostics(p, v, mass)["E"] / e0 - 1))
+        assert np.abs((mass * (v - vel)).sum(1)).max() < 1e-15
+    (st0, p0, v0, de0), (st1, p1, v1, de1) = out
+    assert st0["n_kepler"] == 0 and st1["n_kepler"] > 20
+    assert sum(st1["entries"]) < 0.2 * sum(st0["entries"]) and st1["depth"] < st0["depth"]
+    assert abs(de1) <= 1.1 * abs(de0) + 1e-10, (de0, de1)          # (8.76e-7 vs 8.70e-7: set by the other pairs)
+    assert np.abs(p1 - p0).max() < 1e-6
+    for kw in (dict(split_max=0, kepler=True), dict(split_max=1 << 20, kepler=True, eps2=1e-8)):
+        pa, va, pb, vb = pos.copy(), vel.copy(), pos.copy(), vel.copy()
+        sa = oracle.hhs_step(pa, va, mass, 2.0 ** -6, **kw)
+        kw["kepler"] = False
+        sb = oracle.hhs_step(pb, vb, mass, 2.0 ** -6, **kw)
+        assert sa == sb and (pa == pb).all() and (va == vb).all()
