@@ -215,10 +215,11 @@ def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
     if hhs:
         out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
         out["hhs_step_config5_split"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)
+        out["hhs_step_config5_split_kepler"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5, kepler=1)
     return out
 
 
-def hhs_config5(fr, torch, dev, n5=262144, split_max=0):
+def hhs_config5(fr, torch, dev, n5=262144, split_max=0, kepler=0):
     """Config 5: one whole HHS-FSI step over all time-step levels (latency-bound: DESIGN.md 7), with
     the numbers that make the timing valid: momentum, angular momentum and energy change read by
     frost_diagnostics before and after (SURVEY 8(c) last pin row; expected floors PAPER.md:646-656,
@@ -228,17 +229,20 @@ def hhs_config5(fr, torch, dev, n5=262144, split_max=0):
     fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
     d0 = fr.diagnostics(p5, v5, m5)
     fr.set_split(split_max)
+    fr.set_kepler(kepler)
     l0 = fr.launch_count()
     torch.cuda.synchronize(); t0 = time.perf_counter()
     try:
         st = fr.hhs_step(p5, v5, m5, 2.0 ** -7)
     finally:
         fr.set_split(0)
+        fr.set_kepler(0)
     torch.cuda.synchronize(); t1 = time.perf_counter()
     launches = int(fr.launch_count() - l0)
     d1 = fr.diagnostics(p5, v5, m5)
     L0, L1 = np.array(d0["L"]), np.array(d1["L"])
-    return {"n": n5, "dt_top": 2.0 ** -7, "split_max": split_max, "seconds": t1 - t0, "depth": st["depth"],
+    return {"n": n5, "dt_top": 2.0 ** -7, "split_max": split_max, "kepler": kepler, "kepler_calls": int(st["n_kepler"]),
+            "seconds": t1 - t0, "depth": st["depth"],
             "hierarchy_entries": int(sum(st["entries"])), "launches": launches,
             "pairs_newton": int(st["pairs_newton"]), "pairs_gradient": int(st["pairs_gradient"]),
             "pairs_timestep": int(st["pairs_timestep"]),
@@ -350,6 +354,7 @@ def run_hhs_only(arm):
         out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
     if arm in ("both", "split"):
         out["hhs_step_config5_split"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)
+        out["hhs_step_config5_split_kepler"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5, kepler=1)
     print(json.dumps(out))
     fr.close()
 

@@ -62,6 +62,7 @@ typedef struct {
     int64_t pairs_timestep;             /* ordered pairs swept by the time-step kernel */
     int64_t n_comp[FROST_MAX_LEVELS];   /* sum over those entries of the fast components recursed into
                                            (Alg. 3 as printed: 1 per entry with |F| > 0; frost_set_split) */
+    int64_t n_kepler;                   /* two-body components advanced by the Kepler propagator (frost_set_kepler) */
 } frost_hhs_stats;
 
 /* allocate_memory / free_memory of Alg. 4: creates a context bound to CUDA
@@ -254,6 +255,16 @@ int frost_set_overlap(frost_ctx *ctx, int on);
  * one CTA each; larger ones by the host recursion.  Result: deterministic; not the numbers of
  * split_max = 0 (a different, equally fourth-order splitting of the same Hamiltonian). */
 int frost_set_split(frost_ctx *ctx, int split_max);
+
+/* Two-body propagator for the binaries of a split level -- PAPER.md:759 lists "regularised integrators,
+ * Wisdom-Holman integrators and Kepler solvers" as the modules a spatially split level can hand its
+ * few-body systems to, and defines none (reading 25).  on = 1 (needs frost_set_split, eps2 = 0):
+ * hhs_fsi(C, tau/2) of a component C of exactly two particles is replaced by the exact two-body flow
+ * over tau/2 -- the relative vector along its Kepler orbit (universal variables: ellipse, parabola and
+ * hyperbola alike), the centre of mass uniformly -- instead of 2^k sub-steps.  H_C is then integrated
+ * exactly, the order of the splitting is unchanged; frost_hhs_stats.n_kepler counts the calls.
+ * Default 0. */
+int frost_set_kepler(frost_ctx *ctx, int on);
 
 /* Inside the device-resident subtree kernels a hierarchy entry of exactly two particles -- a binary,
  * the deepest and most often entered sets of a cluster with hard binaries -- is advanced by ONE thread

@@ -27,6 +27,7 @@ exported_symbols = [
     "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
     "frost_set_split", "frost_forces_masked", "frost_set_pair_path",
     "frost_set_gradient_guard", "frost_set_equal_mass_path",
+    "frost_set_kepler",
 ]
 
 
@@ -39,14 +40,15 @@ class HHSStats(C.Structure):
                 ("entries", C.c_int64 * MAX_LEVELS), ("n_slow", C.c_int64 * MAX_LEVELS),
                 ("n_fast", C.c_int64 * MAX_LEVELS), ("pairs_newton", C.c_int64),
                 ("pairs_gradient", C.c_int64), ("pairs_timestep", C.c_int64),
-                ("n_comp", C.c_int64 * MAX_LEVELS)]
+                ("n_comp", C.c_int64 * MAX_LEVELS), ("n_kepler", C.c_int64)]
 
     def as_dict(self):
         d = self.depth
         return {"depth": d, "entries": list(self.entries[: d + 1]),
                 "n_slow": list(self.n_slow[: d + 1]), "n_fast": list(self.n_fast[: d + 1]),
                 "pairs_newton": self.pairs_newton, "pairs_gradient": self.pairs_gradient,
-                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1])}
+                "pairs_timestep": self.pairs_timestep, "n_comp": list(self.n_comp[: d + 1]),
+                "n_kepler": self.n_kepler}
 
 
 def library_path() -> str:
@@ -75,6 +77,7 @@ def load_library():
     lib.frost_set_pair_path.argtypes = [vp, i32]
     lib.frost_set_gradient_guard.argtypes = [vp, i32]
     lib.frost_set_equal_mass_path.argtypes = [vp, i32]
+    lib.frost_set_kepler.argtypes = [vp, i32]
     lib.frost_forces_masked.argtypes = [vp, i32, i32, vp, vp, vp, i32, vp, vp, vp]
     lib.frost_diagnostics.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     lib.frost_forces.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, vp, i32, vp, vp, i32]
@@ -180,6 +183,11 @@ class Frost:
         """split_max > 0: hierarchy entries with at most split_max members recurse into the connected
         components of their fast pairs one by one (frost.h: frost_set_split); 0 (default): Alg. 3."""
         self._check(self.lib.frost_set_split(self.h, split_max), "frost_set_split")
+
+    def set_kepler(self, on=0):
+        """1: two-body components of a split entry follow their exact Kepler orbit over the entry's half
+        step instead of being recursed into (needs set_split, eps2 = 0); 0 (default)."""
+        self._check(self.lib.frost_set_kepler(self.h, on), "frost_set_kepler")
 
     def set_equal_mass_path(self, on=1):
         """1 (default): large pair-symmetric force sweeps take their equal-mass variant when every mass

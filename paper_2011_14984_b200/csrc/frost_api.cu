@@ -84,7 +84,7 @@ static int side_ctx(frost_ctx *c, int level, frost_ctx **out) {
     }
     s->G = c->G; s->eps2 = c->eps2; s->eta_ff = c->eta_ff; s->eta_fb = c->eta_fb; s->max_depth = c->max_depth;
     s->tune_k = c->tune_k; s->tune_slices = c->tune_slices; s->tune_small = c->tune_small;
-    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max; s->tune_pair = c->tune_pair; s->tune_guard = c->tune_guard; s->tune_eqmass = c->tune_eqmass;
+    s->tune_cluster = c->tune_cluster; s->tune_sym = c->tune_sym; s->split_max = c->split_max; s->kepler = c->kepler; s->tune_pair = c->tune_pair; s->tune_guard = c->tune_guard; s->tune_eqmass = c->tune_eqmass;
     s->sym_scratch = c->sym_scratch < ((size_t)1 << 30) ? c->sym_scratch : ((size_t)1 << 30);
     *out = s;
     return FROST_OK;
@@ -133,6 +133,12 @@ int frost_set_overlap(frost_ctx *c, int on) {
 int frost_set_split(frost_ctx *c, int split_max) {
     if (!c || split_max < 0) return FROST_EINVAL;
     c->split_max = split_max;
+    return FROST_OK;
+}
+
+int frost_set_kepler(frost_ctx *c, int on) {
+    if (!c || on < 0 || on > 1) return FROST_EINVAL;
+    c->kepler = on;
     return FROST_OK;
 }
 
@@ -424,28 +430,32 @@ static int cross_kick(frost_ctx *c, int n, int ld, double *pos, double *vel, con
 }
 
 static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
-                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st);
+                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st,
+                   bool is_comp = false);
 
 // hhs_fsi(C, tau/2) of every component of F (Alg. 3: hhs_fsi(F, tau/2))
 static int recurse_fast(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                         const int32_t *F, int nF, const SplitInfo &si, double h, int level,
                         frost_hhs_stats *st) {
-    if (si.m <= 1) return hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st);
+    if (si.m <= 1) return hhs_rec(c, n, ld, pos, vel, mass, F, nF, h, level + 1, st, si.split);
     FROST_TRY(launch_comp_batch(c, 1, ld, pos, vel, mass, si.C, si.desc_small, si.n_small_dev, si.n_small, h,
                                 level + 1, c->dev_stats.p));
     FROST_TRY(launch_comp_batch(c, 0, ld, pos, vel, mass, si.C, si.desc_med, si.n_med_dev, si.n_med, h,
                                 level + 1, c->dev_stats.p));
     for (int b = 0; b < si.n_big; ++b)
-        FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, si.C + si.big_off[b], si.big_size[b], h, level + 1, st));
+        FROST_TRY(hhs_rec(c, n, ld, pos, vel, mass, si.C + si.big_off[b], si.big_size[b], h, level + 1, st, true));
     return FROST_OK;
 }
 
 static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
-                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st) {
+                   const int32_t *set, int n_set, double tau_pivot, int level, frost_hhs_stats *st,
+                   bool is_comp) {
     if (n_set <= 0) return FROST_OK;
     if (level >= c->max_depth || level >= FROST_MAX_LEVELS) return FROST_EDEPTH;
-    if (n_set <= small_threshold(c))     // the whole subtree on the device, asynchronously (row 11)
-        return launch_small(c, 0, ld, pos, vel, mass, set, n_set, tau_pivot, level, c->dev_stats.p);
+    // the whole subtree on the device, asynchronously (row 11); a two-body component of a split entry
+    // under frost_set_kepler goes there whatever the threshold (the propagator lives in that kernel)
+    if (n_set <= small_threshold(c) || (is_comp && n_set == 2 && c->kepler && c->eps2 == 0.0))
+        return launch_small(c, 0, ld, pos, vel, mass, set, n_set, tau_pivot, level, c->dev_stats.p, 1, is_comp);
     double *tau = (double *)c->tau.p;
     const bool split = c->split_max > 0 && n_set <= c->split_max;
     int *forest = nullptr;
@@ -461,6 +471,7 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     FROST_TRY(launch_partition(c, tau, set, n_set, tau_pivot, S, F, cnt));
     const int nS = cnt[0], nF = cnt[1];
     SplitInfo si;
+    si.split = split;
     si.m = nF > 0 ? 1 : 0;
     si.sumsq = (long long)nF * nF;
     if (split && nF > 0) {
@@ -650,7 +661,7 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
         for (int k = 0; k < FROST_MAX_LEVELS; ++k) if (c->side[k]) cudaStreamSynchronize(c->side[k]->stream);
     // merge what the device-resident subtrees counted (also carries their status)
     struct { long long e[FROST_MAX_LEVELS], s[FROST_MAX_LEVELS], f[FROST_MAX_LEVELS], pn, pg, pt; int depth, status;
-             long long nc[FROST_MAX_LEVELS]; } d;
+             long long nc[FROST_MAX_LEVELS]; long long nk; } d;
     static_assert(sizeof(d) >= 1, "");
     if (sizeof(d) != small_stats_bytes()) return FROST_EINVAL;
     FROST_CUDA(c, cudaMemcpyAsync(&d, c->dev_stats.p, sizeof(d), cudaMemcpyDeviceToHost, c->stream));
@@ -662,6 +673,7 @@ int frost_hhs_step(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
         local.n_comp[k] += d.nc[k];
     }
     local.pairs_newton += d.pn; local.pairs_gradient += d.pg; local.pairs_timestep += d.pt;
+    local.n_kepler += d.nk;
     if (d.depth > local.depth) local.depth = d.depth;
     if (local.depth < 0) local.depth = 0;
     if (stats) *stats = local;

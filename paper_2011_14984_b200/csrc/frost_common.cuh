@@ -56,6 +56,7 @@ struct frost_ctx {
     int32_t *pinned_counts = nullptr;  // host pinned int32[4]
     frost::Buf shard_idx;              // 0..n-1, for sharding the sinks of a NULL index list
     int tune_pair = 1;             // two-body frames of the subtree kernels on one thread (frost_set_pair_path)
+    int kepler = 0;                // frost_set_kepler: two-body components of a split entry on their Kepler orbit
     int split_max = 0;             // frost_set_split: entries with <= split_max members split F into components
     frost::Buf uf, comp;           // union-find forest / labels, sort and descriptor scratch of a split entry
     frost::Buf lvlC[FROST_MAX_LEVELS];   // F of a split entry reordered by component
@@ -206,6 +207,7 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
 
 // frost_split.cu: the components of the fast pairs of a split hierarchy entry (reading 24)
 struct SplitInfo {
+    bool split = false;              // the entry is split-enabled (its components follow reading 24/25)
     int m = 0;                       // components of F
     int n_small = 0, n_med = 0, n_big = 0;   // of <= comp_warp_max(), <= small_max(), more particles
     long long sumsq = 0;             // sum of squared component sizes
@@ -222,7 +224,8 @@ int split_components(frost_ctx *c, int level, int ld, const double *tau, const i
 int small_max();
 size_t small_stats_bytes();
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
-                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps = 1);
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps = 1,
+                 int root_is_comp = 0);
 int comp_warp_max();
 int launch_comp_batch(frost_ctx *c, int warp_team, int ld, double *pos, double *vel, const double *mass,
                       const int32_t *idx, const void *desc, const int *n_desc, int max_desc, double tau,

@@ -24,6 +24,7 @@ struct SmallStats {                 // device-side mirror of frost_hhs_stats (+ 
     long long pairs_newton, pairs_gradient, pairs_timestep;
     int depth, status;
     long long n_comp[FROST_MAX_LEVELS];
+    long long n_kepler;
 };
 
 struct SmallParams {
@@ -45,6 +46,8 @@ struct SmallParams {
     const int2 *desc;
     const int *n_desc;
     int pair_path;                  // two-body frames on one thread (binary_subtree); 0: team path (tests)
+    int kepler;                     // two-body COMPONENTS of a split entry follow their Kepler orbit (reading 25)
+    int root_is_comp;               // the set of this launch is itself such a component
 };
 
 template <int CAP>
@@ -64,6 +67,7 @@ struct SmallSmemT {
     int f_start[FROST_MAX_LEVELS], f_n[FROST_MAX_LEVELS], f_ns[FROST_MAX_LEVELS], f_stage[FROST_MAX_LEVELS];
     int f_cpos[FROST_MAX_LEVELS];   // next component of F to recurse into (offset inside F)
     int f_m[FROST_MAX_LEVELS];      // number of components of F
+    int f_iscomp[FROST_MAX_LEVELS]; // the frame's set is a component of a split entry
     long long f_sumsq[FROST_MAX_LEVELS];          // sum of squared component sizes
     unsigned f_bnd[FROST_MAX_LEVELS][kWords];     // bit r: a component starts at position r of F
     double f_tau[FROST_MAX_LEVELS];
@@ -74,7 +78,7 @@ using SmallSmem = SmallSmemT<kSmallMax>;
 struct SmStats {                    // per CTA, shared by its teams (atomics)
     unsigned long long entries[FROST_MAX_LEVELS], slow[FROST_MAX_LEVELS], fast[FROST_MAX_LEVELS],
         comps[FROST_MAX_LEVELS];
-    unsigned long long pn, pg, pt;
+    unsigned long long pn, pg, pt, kep;
     int depth;
 };
 
@@ -601,6 +605,97 @@ __device__ __forceinline__ void pair_fsi(Body &p, Body &q, const SweepParams &pN
     body_kick(p, ap, dt / 6.0); body_kick(q, aq, dt / 6.0);
 }
 
+// ------------------------------------------------------------------------------------------------
+// Two-body propagator (reading 25; the paper lists Kepler solvers among the modules a split
+// level can hand its few-body systems to): the relative vector follows the Kepler flow of
+// mu = G (m_1 + m_2), advanced over dt in universal variables -- one formula for ellipses, parabolas and
+// hyperbolas -- and the centre of mass moves uniformly.
+//     c_k(z) = sum_n (-z)^n / (2n + k)!,  z = alpha s^2,  alpha = 2 mu / r_0 - v_0^2
+//     r_0 s c_1 + (r_0.v_0) s^2 c_2 + mu s^3 c_3 = dt            (increasing in s: bracketed Newton)
+//     dr = -(mu/r_0) s^2 c_2 r_0 + (dt - mu s^3 c_3) v_0
+//     dv = -(mu/(r r_0)) s c_1 r_0 - (mu/r) s^2 c_2 v_0,   r = r_0 c_0 + (r_0.v_0) s c_1 + mu s^2 c_2
+// The bodies are moved by DISPLACEMENTS (x_1 += V dt - (m_2/M) dr, ...), never rebuilt from the centre
+// of mass, so that a binary of size 1e-5 at |x| ~ 1 keeps its relative accuracy.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void stumpff(double z, double &c0, double &c1, double &c2, double &c3) {
+    int k = 0;
+    while (fabs(z) > 0.1) { z *= 0.25; ++k; }
+    // nested form of the two series to z^9 (|z| <= 0.1: the neglected terms are below 1e-30)
+    double h2 = 1.0, h3 = 1.0;
+#pragma unroll
+    for (int n = 9; n >= 1; --n) {
+        h2 = 1.0 - z * h2 / (double)((2 * n + 1) * (2 * n + 2));
+        h3 = 1.0 - z * h3 / (double)((2 * n + 2) * (2 * n + 3));
+    }
+    c2 = 0.5 * h2; c3 = h3 / 6.0;
+    c1 = 1.0 - z * c3; c0 = 1.0 - z * c2;
+    for (; k > 0; --k) {          // c_k(4z) from c_k(z)
+        c3 = 0.25 * (c2 + c0 * c3);
+        c2 = 0.5 * c1 * c1;
+        c1 = c0 * c1;
+        c0 = 2.0 * c0 * c0 - 1.0;
+    }
+}
+
+__device__ void kepler_bodies(Body &p, Body &q, double G, double dt) {
+    const double rx = q.x - p.x, ry = q.y - p.y, rz = q.z - p.z;
+    const double vx = q.vx - p.vx, vy = q.vy - p.vy, vz = q.vz - p.vz;
+    const double mt = p.m + q.m, mu = G * mt;
+    const double r0 = sqrt(rx * rx + ry * ry + rz * rz);
+    const double v2 = vx * vx + vy * vy + vz * vz, u = rx * vx + ry * vy + rz * vz;
+    const double alpha = 2.0 * mu / r0 - v2;
+    double t = dt;
+    if (alpha > 0.0) {                                  // bound: whole periods change nothing
+        const double P = 6.283185307179586476925 * mu / (alpha * sqrt(alpha));
+        t -= floor(t / P) * P;
+    }
+    double c0, c1, c2, c3, lo = 0.0, hi = t / r0, s;
+    for (int it = 0; it < 1100; ++it) {                 // bracket the root
+        stumpff(alpha * hi * hi, c0, c1, c2, c3);
+        if (r0 * hi * c1 + u * hi * hi * c2 + mu * hi * hi * hi * c3 - t > 0.0) break;
+        lo = hi; hi = 2.0 * hi + 1e-300;
+    }
+    s = 0.5 * (lo + hi);
+    for (int it = 0; it < 100; ++it) {
+        stumpff(alpha * s * s, c0, c1, c2, c3);
+        const double F = r0 * s * c1 + u * s * s * c2 + mu * s * s * s * c3 - t;
+        if (F == 0.0) break;
+        const double dF = r0 * c0 + u * s * c1 + mu * s * s * c2;
+        if (F > 0.0) hi = s; else lo = s;
+        double sn = s - F / dF;
+        if (!(sn >= lo && sn <= hi)) sn = 0.5 * (lo + hi);
+        const bool done = fabs(sn - s) <= 2.3e-16 * fabs(s);
+        s = sn;
+        if (done) break;
+    }
+    stumpff(alpha * s * s, c0, c1, c2, c3);
+    const double rr = r0 * c0 + u * s * c1 + mu * s * s * c2;
+    const double fm1 = -(mu / r0) * s * s * c2, g = t - mu * s * s * s * c3;
+    const double fd = -(mu / (rr * r0)) * s * c1, gdm1 = -(mu / rr) * s * s * c2;
+    const double drx = fm1 * rx + g * vx, dry = fm1 * ry + g * vy, drz = fm1 * rz + g * vz;
+    const double dvx = fd * rx + gdm1 * vx, dvy = fd * ry + gdm1 * vy, dvz = fd * rz + gdm1 * vz;
+    const double wp = q.m / mt, wq = p.m / mt;
+    const double Vx = wq * p.vx + wp * q.vx, Vy = wq * p.vy + wp * q.vy, Vz = wq * p.vz + wp * q.vz;
+    p.x += fma(Vx, dt, -wp * drx); p.y += fma(Vy, dt, -wp * dry); p.z += fma(Vz, dt, -wp * drz);
+    q.x += fma(Vx, dt, wq * drx); q.y += fma(Vy, dt, wq * dry); q.z += fma(Vz, dt, wq * drz);
+    p.vx -= wp * dvx; p.vy -= wp * dvy; p.vz -= wp * dvz;
+    q.vx += wq * dvx; q.vy += wq * dvy; q.vz += wq * dvz;
+}
+
+template <class SM>
+__device__ void kepler_frame(SM &sm, SmStats &st, const SmallParams &P, int sp) {
+    const int start = sm.f_start[sp];
+    const int i1 = sm.perm[start], i2 = sm.perm[start + 1];
+    Body p, q;
+    { const double4 x = sm.xm[i1], v = sm.vv[i1]; p.x = x.x; p.y = x.y; p.z = x.z; p.m = x.w; p.vx = v.x; p.vy = v.y; p.vz = v.z; }
+    { const double4 x = sm.xm[i2], v = sm.vv[i2]; q.x = x.x; q.y = x.y; q.z = x.z; q.m = x.w; q.vx = v.x; q.vy = v.y; q.vz = v.z; }
+    kepler_bodies(p, q, P.G, sm.f_tau[sp]);
+    sm.xm[i1] = make_double4(p.x, p.y, p.z, p.m); sm.vv[i1] = make_double4(p.vx, p.vy, p.vz, 1.0);
+    sm.xm[i2] = make_double4(q.x, q.y, q.z, q.m); sm.vv[i2] = make_double4(q.vx, q.vy, q.vz, 1.0);
+    atomicAdd(&st.kep, 1ull);
+    sm.sp = sp - 1;
+}
+
 template <class SM>
 __device__ void binary_subtree(SM &sm, SmStats &st, const SmallParams &P, const SweepParams &pN,
                                const SweepParams &pG, int sp) {
@@ -662,6 +757,11 @@ __device__ void hhs_loop(SM &sm, SmStats &st, const SmallParams &P, const SweepP
         const int start = sm.f_start[sp], cnt = sm.f_n[sp], stage = sm.f_stage[sp];
         const double tau = sm.f_tau[sp];
         const int level = P.level0 + sp;
+        if (stage == 0 && cnt == 2 && P.kepler && sm.f_iscomp[sp] && P.eps2 == 0.0) {
+            // a two-body component of a split entry: exact two-body motion over its span (reading 25)
+            if (T::tid() == 0) kepler_frame(sm, st, P, sp);
+            continue;
+        }
         if (stage == 0 && cnt == 2 && P.pair_path) {      // a binary: one thread, both bodies in registers
             if (T::tid() == 0) binary_subtree(sm, st, P, pN, pG, sp);
             continue;
@@ -715,6 +815,7 @@ __device__ void hhs_loop(SM &sm, SmStats &st, const SmallParams &P, const SweepP
                     sm.f_cpos[sp] = cpos + size;
                     sm.f_start[sp + 1] = start + nS + cpos; sm.f_n[sp + 1] = size; sm.f_ns[sp + 1] = 0;
                     sm.f_stage[sp + 1] = 0; sm.f_tau[sp + 1] = 0.5 * tau;
+                    sm.f_iscomp[sp + 1] = (P.split_max > 0 && cnt <= P.split_max) ? 1 : 0;
                     sm.sp = sp + 1;
                 }
             } else if (stage == 1) {
@@ -741,7 +842,7 @@ __device__ __forceinline__ void stats_zero(SmStats &st, int tid, int nthreads) {
     for (int k = tid; k < FROST_MAX_LEVELS; k += nthreads) {
         st.entries[k] = 0; st.slow[k] = 0; st.fast[k] = 0; st.comps[k] = 0;
     }
-    if (tid == 0) { st.pn = st.pg = st.pt = 0; st.depth = -1; }
+    if (tid == 0) { st.pn = st.pg = st.pt = st.kep = 0; st.depth = -1; }
 }
 
 // atomics: an fsi(S) launch on a side stream, or other CTAs of a batch, run concurrently
@@ -759,6 +860,7 @@ __device__ __forceinline__ void stats_flush(const SmStats &st, SmallStats *out, 
         atomicAdd((ull *)&out->pairs_newton, st.pn);
         atomicAdd((ull *)&out->pairs_gradient, st.pg);
         atomicAdd((ull *)&out->pairs_timestep, st.pt);
+        if (st.kep) atomicAdd((ull *)&out->n_kepler, st.kep);
         atomicMax(&out->depth, st.depth);
         if (err) atomicCAS(&out->status, 0, err);
     }
@@ -777,6 +879,7 @@ __device__ __forceinline__ void set_load(SM &sm, const SmallParams &P, const int
     if (tid == 0) {
         sm.sp = 0; sm.err = 0;
         sm.f_start[0] = 0; sm.f_n[0] = n; sm.f_ns[0] = 0; sm.f_stage[0] = 0; sm.f_tau[0] = P.tau_pivot;
+        sm.f_iscomp[0] = P.root_is_comp;
     }
 }
 
@@ -883,6 +986,7 @@ static SmallParams small_params(frost_ctx *c, int mode, int ld, double *pos, dou
     P.stats = (SmallStats *)dev_stats;
     P.split_max = c->split_max;
     P.pair_path = c->tune_pair;
+    P.kepler = c->kepler;
     return P;
 }
 
@@ -898,11 +1002,13 @@ static int small_attrs(frost_ctx *c) {
 
 // mode 0: hhs_fsi(set, tau) subtree rooted at hierarchy level `level0`; mode 1: fsi(set, dt).
 int launch_small(frost_ctx *c, int mode, int ld, double *pos, double *vel, const double *mass,
-                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps) {
+                 const int32_t *idx, int n, double tau_or_dt, int level0, void *dev_stats, int n_steps,
+                 int root_is_comp) {
     if (n <= 0) return FROST_OK;
     if (n > kSmallMax) return FROST_EINVAL;
     FROST_TRY(small_attrs(c));
-    const SmallParams P = small_params(c, mode, ld, pos, vel, mass, idx, n, tau_or_dt, level0, dev_stats, n_steps);
+    SmallParams P = small_params(c, mode, ld, pos, vel, mass, idx, n, tau_or_dt, level0, dev_stats, n_steps);
+    P.root_is_comp = root_is_comp;
     const size_t bytes = sizeof(SmallSmem) + sizeof(SmStats);
     if (n >= kClusterMinSet && c->tune_cluster != 1) {   // one cluster of kClusterSize replicas
         cudaLaunchConfig_t cfg{};
@@ -928,7 +1034,7 @@ int launch_comp_batch(frost_ctx *c, int warp_team, int ld, double *pos, double *
     if (max_desc <= 0) return FROST_OK;
     FROST_TRY(small_attrs(c));
     SmallParams P = small_params(c, 0, ld, pos, vel, mass, idx, 0, tau, level0, dev_stats, 1);
-    P.desc = (const int2 *)desc; P.n_desc = n_desc;
+    P.desc = (const int2 *)desc; P.n_desc = n_desc; P.root_is_comp = 1;
     if (warp_team) {
         const int grid = (max_desc + kCompWarps - 1) / kCompWarps;
         hhs_comp_kernel<<<grid, kCompWarps * 32, kCompWarps * sizeof(CompSmem) + sizeof(SmStats), c->stream>>>(P);

@@ -223,3 +223,36 @@ def test_split_multi_step_run_conserves_like_alg3(fr, capsys):
     assert np.abs(de0).max() < 1e-6 and np.abs(de1).max() < 1e-6
     assert np.abs(de1).max() < 10 * np.abs(de0).max() + 1e-9
     assert np.abs(out[0][1] - out[BIG][1]).max() < 1e-4
+
+
+@pytest.mark.parametrize("n,small,log2dt", [(256, -1, 7), (256, 0, 9), (3000, -1, 8), (3000, 100, 8)])
+def test_split_step_with_kepler_components_matches_oracle(fr, oracle, n, small, log2dt, capsys):
+    """frost_set_kepler on top of the split step: every two-body component follows its exact Kepler orbit
+    (reading 25; oracle O6k) -- bookkeeping identical to the oracle's (fewer and shallower entries, the
+    same number of propagator calls), trajectory inside the oracle's 1-ulp envelope, momentum at
+    rounding level: inside the subtree kernel (small = -1, n = 256), through the batched component
+    launches, and from the host recursion alone (small = 0)."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
+    dt = 2.0 ** -log2dt
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    pr, vr, st_ref, env_p, env_v, sts = oracle_hhs_with_envelope(oracle, pos, vel, mass, dt, split_max=BIG, kepler=True)
+    assert all(s == st_ref for s in sts)
+    fr.set_tuning(0, 0, small)
+    fr.set_split(BIG)
+    fr.set_kepler(1)
+    p, v = dev(pos), dev(vel)
+    try:
+        st = fr.hhs_step(p, v, dev(mass), dt)
+    finally:
+        fr.set_kepler(0)
+        fr.set_split(0)
+        fr.set_tuning(0, 0, -1)
+    assert st == st_ref and st["n_kepler"] > 0
+    pg, vg = p.cpu().numpy(), v.cpu().numpy()
+    rp, rv = envelope_ratio(pg, vg, pr, vr, env_p, env_v)
+    with capsys.disabled():
+        print(f"\n[split + kepler n={n} small={small}] depth {st['depth']}, {st['n_kepler']} propagator calls, "
+              f"{sum(st['entries'])} entries; max |dx| {np.abs(pg - pr).max():.2e} (envelope {env_p.max():.2e}); "
+              f"ratio x {rp:.3f}, v {rv:.3f}")
+    assert rp <= 1.0 and rv <= 1.0, (rp, rv)
+    assert momentum_change(mass, vel, vg, vr) <= 1.0
