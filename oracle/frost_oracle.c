@@ -37,6 +37,10 @@
  *                            independent graph routine; 4th-order convergence with a frozen
  *                            partition into components; momentum at roundoff; energy error of the
  *                            size of Alg. 3's on a cluster with binaries.
+ *   O6k two-body propagator: (PAPER.md:759 lists Kepler solvers as plug-ins; reading 25) the
+ *                            classical-elements solution through the eccentric anomaly for
+ *                            e = 0 ... 0.99 and up to 123 periods; energy, angular momentum, the
+ *                            group property and time reversal on unbound orbits; a fine FSI run.
  *   O7 oracle_diagnostics  : textbook definitions (Eq. 23); used by the pins.
  *
  * Array convention (same as include/frost.h, restated independently): positions, velocities,
