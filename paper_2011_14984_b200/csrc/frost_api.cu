@@ -319,6 +319,8 @@ static int timesteps_impl(frost_ctx *c, int n, int ld, const double *pos, const 
                           double *out_tau, int32_t *out_bin, int *forest = nullptr) {
     if (!idx) n_idx = n;
     if (n_idx <= 0) return FROST_OK;
+    if (forest && c->tune_sym != 1 && c->tune_sym != 3 && n_idx >= 32768)     // pruned sweep with edge output
+        return tau_pruned(c, ld, pos, vel, mass, idx, n_idx, tau_pivot, out_tau, out_bin, c->tune_sym != 4, forest);
     if (forest) {
         const int pad = pad_rec(n_idx);
         FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
@@ -412,13 +414,38 @@ static int cross_kick(frost_ctx *c, int n, int ld, double *pos, double *vel, con
                       const SplitInfo &si, bool with_g, double cc, double kappa) {
     double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
     if (si.m > 1) {
-        const int pad = pad_rec(n_set);
-        FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
-        FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
-        double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
-        FROST_TRY(launch_pack_xm(c, ld, pos, mass, set, n_set, pad, xm, 1.0, 0, av));
-        FROST_TRY(launch_pack_label(c, si.labpos, n_set, pad, av));
-        FROST_TRY(sweep_masked(c, xm, av, n_set, set, ld, acc, with_g ? grad : nullptr));
+        // P = S x F  u  G x R  u  { pairs of R in different components }, with G the largest component
+        // above 1024 particles (if any) and R the rest of F: two pair-symmetric mutual sweeps and one
+        // masked self sweep of R, the accelerations of all three added up before any gradient sweep
+        // (Eq. 43-44 need the a of the whole pair set).  Every member of the set is a sink of at least
+        // one overwriting sweep: S and F of the first (when S is not empty), else R and G.
+        const int32_t *G = si.C + si.g_off;
+        const int nG = si.g_size, nR = si.nR;
+        const int pad = pad_rec(nR);
+        for (int phase = 0; phase < (with_g ? 2 : 1); ++phase) {
+            const int fl = phase == 0 ? FROST_ACC : FROST_GRAD;
+            double *out = phase == 0 ? acc : grad;
+            bool fresh = true;                                        // nothing written to `out` yet
+            if (nS > 0) {
+                FROST_TRY(forces_impl(c, n, ld, pos, mass, S, nS, F, nF, acc, grad, fl | FROST_MUTUAL));
+                fresh = false;
+            }
+            if (nG > 0 && nR > 0) {
+                FROST_TRY(forces_impl(c, n, ld, pos, mass, G, nG, si.R, nR, acc, grad,
+                                      fl | FROST_MUTUAL | (fresh ? 0 : FROST_ACCUMULATE)));
+                fresh = false;
+            }
+            if (nR > 0) {
+                FROST_TRY(ensure(c, c->recA_xm, (size_t)pad * kRecBytes));
+                FROST_TRY(ensure(c, c->recA_v, (size_t)pad * kRecBytes));
+                double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
+                FROST_TRY(launch_pack_xm(c, ld, pos, mass, si.R, nR, pad, xm, 1.0, 0, av));
+                if (phase == 1) FROST_TRY(launch_pack_vec(c, ld, acc, si.R, nR, pad, av));     // the total a of P
+                FROST_TRY(launch_pack_label(c, si.labR, nR, pad, av));
+                FROST_TRY(sweep_masked(c, xm, av, nR, si.R, ld, phase == 0 ? out : nullptr,
+                                       phase == 1 ? out : nullptr, fresh ? 0 : 1));
+            }
+        }
         return launch_kick(c, ld, vel, acc, with_g ? grad : nullptr, set, n_set, cc, kappa);
     }
     if (nS > 0 && nF > 0) {

@@ -180,8 +180,10 @@ int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set,
                    int *forest = nullptr);
 // Self sweep of one list over the pairs whose component labels differ (low word of a_lab[k].w; the
 // kicked pair set of a split hierarchy entry): accelerations, then (grad != NULL) gradient accelerations.
+// out_acc != NULL: the Newton sweep (its sums are also written to the packed stream a_lab, labels kept);
+// out_grad != NULL: the gradient sweep from the accelerations in a_lab.  accumulate: add to the planes.
 int sweep_masked(frost_ctx *c, const double *xm, double *a_lab, int n_set, const int32_t *idx, int ld,
-                 double *out_acc, double *out_grad);
+                 double *out_acc, double *out_grad, int accumulate = 0);
 
 // frost_sym.cu: pair-symmetric sweeps (one evaluation serves i<-j and j<-i).  self: B == A.
 int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,
@@ -203,7 +205,8 @@ int launch_zero_outside(frost_ctx *c, int ld, double *planes, const int32_t *idx
 
 // frost_tau.cu: time-step sweep in Morton order with exact block pruning (prune = 0: evaluate all)
 int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const double *mass,
-               const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune);
+               const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune,
+               int *forest = nullptr);
 
 // frost_split.cu: the components of the fast pairs of a split hierarchy entry (reading 24)
 struct SplitInfo {
@@ -216,6 +219,10 @@ struct SplitInfo {
     const void *desc_small = nullptr, *desc_med = nullptr;   // int2 {offset into C, size} (device)
     const int *n_small_dev = nullptr, *n_med_dev = nullptr;
     int big_off[64], big_size[64];   // the big components (host)
+    // kick decomposition: G = the largest big component (C[g_off .. g_off + g_size)), R = the rest of F
+    int g_off = 0, g_size = 0, nR = 0;
+    const int32_t *R = nullptr;      // R as one list (device; = C when there is no G)
+    const int *labR = nullptr;       // component label of every position of R (device)
 };
 int split_components(frost_ctx *c, int level, int ld, const double *tau, const int32_t *set, int n_set,
                      double pivot, const int *forest, const int32_t *F, int nF, SplitInfo *out);

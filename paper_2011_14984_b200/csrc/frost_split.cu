@@ -62,13 +62,16 @@ int split_components(frost_ctx *c, int level, int ld, const double *tau, const i
     // persistent part (lives as long as the entry): C, labpos, descriptors, header
     const size_t oC = 0, oLab = align256(oC + (size_t)nF * 4), oDs = align256(oLab + (size_t)n_set * 4);
     const size_t oDm = align256(oDs + (size_t)(nF / 2 + 1) * 8), oDb = align256(oDm + (size_t)(nF / 2 + 1) * 8);
-    const size_t oHdr = align256(oDb + (size_t)kBigCap * 8), persist = oHdr + 256;
+    const size_t oHdr = align256(oDb + (size_t)kBigCap * 8), oR = oHdr + 256;
+    const size_t oLR = align256(oR + (size_t)nF * 4), persist = align256(oLR + (size_t)nF * 4);
     FROST_TRY(ensure(c, c->lvlC[level], persist));
     char *pb = (char *)c->lvlC[level].p;
     int32_t *C = (int32_t *)(pb + oC);
     int *labpos = (int *)(pb + oLab);
     int2 *d_small = (int2 *)(pb + oDs), *d_med = (int2 *)(pb + oDm), *d_big = (int2 *)(pb + oDb);
     int *hdr = (int *)(pb + oHdr);
+    int32_t *Rl = (int32_t *)(pb + oR);
+    int *labR = (int *)(pb + oLR);
     // transient part: global-indexed labels, keys, run-length encoding, cub scratch
     size_t t_sort = 0, t_rle = 0, t_scan = 0;
     int *nul = nullptr;
@@ -122,6 +125,25 @@ int split_components(frost_ctx *c, int level, int ld, const double *tau, const i
                 if (big[b].x < big[a].x) { const int2 t = big[a]; big[a] = big[b]; big[b] = t; }
         for (int a = 0; a < out->n_big; ++a) { out->big_off[a] = big[a].x; out->big_size[a] = big[a].y; }
     }
+    // kick decomposition (frost_api.cu: cross_kick): G = the largest component above 1024 particles, if
+    // any; R = every other fast particle as one list with its labels (the sorted keys)
+    int gb = -1;
+    for (int a = 0; a < out->n_big; ++a)
+        if (gb < 0 || out->big_size[a] > out->big_size[gb]) gb = a;
+    if (gb >= 0) { out->g_off = out->big_off[gb]; out->g_size = out->big_size[gb]; }
+    const int head = out->g_off, tail = nF - out->g_off - out->g_size;
+    out->nR = head + tail;
+    if (head > 0) {
+        FROST_CUDA(c, cudaMemcpyAsync(Rl, C, (size_t)head * 4, cudaMemcpyDeviceToDevice, c->stream));
+        FROST_CUDA(c, cudaMemcpyAsync(labR, keys_s, (size_t)head * 4, cudaMemcpyDeviceToDevice, c->stream));
+    }
+    if (tail > 0) {
+        FROST_CUDA(c, cudaMemcpyAsync(Rl + head, C + out->g_off + out->g_size, (size_t)tail * 4,
+                                      cudaMemcpyDeviceToDevice, c->stream));
+        FROST_CUDA(c, cudaMemcpyAsync(labR + head, keys_s + out->g_off + out->g_size, (size_t)tail * 4,
+                                      cudaMemcpyDeviceToDevice, c->stream));
+    }
+    out->R = Rl; out->labR = labR;
     out->C = C; out->labpos = labpos; out->desc_small = d_small; out->desc_med = d_med;
     out->n_small_dev = hdr + 1; out->n_med_dev = hdr + 2;
     return FROST_OK;

@@ -258,10 +258,11 @@ int sweep_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, c
 // whose component labels differ (reading 24).  One-sided self sweep of the list; the label
 // stream shares the records of the packed accelerations.
 int sweep_masked(frost_ctx *c, const double *xm, double *a_lab, int n_set, const int32_t *idx, int ld,
-                 double *out_acc, double *out_grad) {
+                 double *out_acc, double *out_grad, int accumulate) {
     if (n_set <= 0) return FROST_OK;
     const int n_pad = pad1024(n_set);
-    for (int pass = 0; pass < (out_grad ? 2 : 1); ++pass) {
+    for (int pass = 0; pass < 2; ++pass) {
+        if ((pass == 0 && !out_acc) || (pass == 1 && !out_grad)) continue;
         const Plan pl = make_plan(c, n_set, n_set, pass == 0 ? 4 : 2);
         FROST_TRY(ensure(c, c->partial, (size_t)pl.slices * 3 * n_pad * sizeof(double)));
         SweepParams prm{};
@@ -272,15 +273,17 @@ int sweep_masked(frost_ctx *c, const double *xm, double *a_lab, int n_set, const
         if (pass == 0) {
             prm.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
             FROST_TRY(launch_sweep<MaskedNewtonPolicy>(c, prm, pl));
+            // (with accumulate the packed stream would need the total, which only the planes hold: the
+            //  caller re-packs before a gradient sweep)
             reduce_vec_kernel<<<(n_set + 255) / 256, 256, 0, c->stream>>>(
                 (const double *)c->partial.p, n_pad, pl.slices, n_set, c->G, idx, ld, out_acc,
-                (double4 *)a_lab, 0, 1);
+                accumulate ? nullptr : (double4 *)a_lab, accumulate, 1);
         } else {
             prm.eps2 = c->eps2;
             FROST_TRY(launch_sweep<MaskedGradientPolicy>(c, prm, pl));
             reduce_vec_kernel<<<(n_set + 255) / 256, 256, 0, c->stream>>>(
                 (const double *)c->partial.p, n_pad, pl.slices, n_set, 2.0 * c->G, idx, ld, out_grad,
-                nullptr, 0, 0);
+                nullptr, accumulate, 0);
         }
         FROST_TRY(check_launch(c));
     }

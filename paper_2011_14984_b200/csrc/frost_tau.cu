@@ -50,6 +50,11 @@ struct TauParams {
     int diag_only;                   // pass 1
     int prune;                       // 0: evaluate everything (tests)
     double eta_ff, eta_fb;
+    // a split hierarchy entry (reading 24): every pair with a candidate below `pivot` is united
+    // in the union-find forest over the SORTED positions; such a pair must never be discarded, so the
+    // discard test then runs against max(running minimum, pivot)
+    double pivot;                    // 0 when forest is NULL
+    int *forest;
 };
 
 __device__ __forceinline__ double tau_from_bits(unsigned long long b) { return __longlong_as_double((long long)b); }
@@ -336,7 +341,7 @@ __global__ void __launch_bounds__(kTauNT, 4) tau_sym_kernel(const TauParams prm)
                     for (int k = 0; k < KA; ++k) {
                         const double ux = j1.x - avx[k], uy = j1.y - avy[k], uz = j1.z - avz[k];
                         const double v2 = fma(uz, uz, fma(uy, uy, ux * ux));
-                        const double T = fmax(at[k], tb);
+                        const double T = fmax(fmax(at[k], tb), prm.pivot);
                         const double T2 = T * T;
                         ok = ok && (T2 < tc.K) && (v2 * T2 < tc.C) && (v2 > tc.D * T2) && (v2 > tc.V0) && (v2 < tc.V1);
                     }
@@ -348,6 +353,7 @@ __global__ void __launch_bounds__(kTauNT, 4) tau_sym_kernel(const TauParams prm)
                                                               j0, j1, prm.eta_ff, prm.eta_fb);
                             at[k] = fmin(at[k], cand);
                             b = fmin(b, cand);
+                            if (cand < prm.pivot) uf_union(prm.forest, a_first + k * NT, tile * NT + c * 32 + src);
                         }
                     }
                     b = __shfl_sync(0xffffffffu, b, from);
@@ -363,6 +369,7 @@ __global__ void __launch_bounds__(kTauNT, 4) tau_sym_kernel(const TauParams prm)
                                                           j0, j1, prm.eta_ff, prm.eta_fb);
                         at[k] = fmin(at[k], cand);
                         b = fmin(b, cand);
+                        if (cand < prm.pivot) uf_union(prm.forest, a_first + k * NT, tile * NT + c * 32 + src);
                     }
                     b = __shfl_sync(0xffffffffu, b, from);
                 }
@@ -395,9 +402,29 @@ __global__ void tau_finish_kernel(const unsigned long long *__restrict__ tau64, 
     }
 }
 
+// The forest over sorted positions -> a forest over LIST positions whose roots are the smallest list
+// position of each component (what split_components expects): two passes over the sorted positions.
+__global__ void tau_forest_min_kernel(const int *__restrict__ fs, const int32_t *__restrict__ perm, int n,
+                                      int *__restrict__ minlist) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) atomicMin(&minlist[uf_find(fs, p)], perm[p]);
+}
+__global__ void tau_forest_out_kernel(const int *__restrict__ fs, const int32_t *__restrict__ perm, int n,
+                                      const int *__restrict__ minlist, int *__restrict__ forest_list) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n) forest_list[perm[p]] = minlist[uf_find(fs, p)];
+}
+__global__ void tau_forest_init_kernel(int *__restrict__ fs, int *__restrict__ minlist, int n_pad) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p < n_pad) { fs[p] = p; minlist[p] = 0x7fffffff; }
+}
+
 // Host driver.  prune = 0 evaluates every block (tests: the pruned result must be bitwise the same).
+// forest != NULL (length >= n, over list positions): the fast pairs of the level (candidate < tau_pivot)
+// are united in it -- the component search of a split hierarchy entry.
 int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const double *mass,
-               const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune) {
+               const int32_t *idx, int n, double tau_pivot, double *out_tau, int32_t *out_bin, int prune,
+               int *forest) {
     if (n <= 0) return FROST_OK;
     constexpr int TA = kTauNT * kTauKA;
     const int n_pad = round_up(n, TA);
@@ -410,7 +437,8 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
     const size_t o_vals2 = o_vals + (size_t)n_pad * 4, o_sidx = o_vals2 + (size_t)n_pad * 4;
     const size_t o_box6 = o_sidx + (size_t)n_pad * 4, o_boxes = o_box6 + 64;
     const size_t o_tau = o_boxes + (size_t)(n_pad / 32) * sizeof(TauBox);
-    const size_t o_cub = o_tau + (size_t)n_pad * 8;
+    const size_t o_fs = o_tau + (size_t)n_pad * 8, o_min = o_fs + (forest ? (size_t)n_pad * 4 : 0);
+    const size_t o_cub = o_min + (forest ? (size_t)n_pad * 4 : 0);
     FROST_TRY(ensure(c, c->tau_scratch, o_cub + cub_bytes + 256));
     FROST_TRY(ensure(c, c->recA_xm, (size_t)n_pad * kRecBytes));
     FROST_TRY(ensure(c, c->recA_v, (size_t)n_pad * kRecBytes));
@@ -451,6 +479,12 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
     TauParams prm{};
     prm.xm = (const double4 *)xm; prm.vv = (const double4 *)vv; prm.box = boxes; prm.tau64 = tau64;
     prm.n_tiles = n_tiles; prm.prune = prune; prm.eta_ff = c->eta_ff; prm.eta_fb = c->eta_fb;
+    int *fs = (int *)(base + o_fs), *minlist = (int *)(base + o_min);
+    prm.pivot = forest ? tau_pivot : 0.0; prm.forest = forest ? fs : nullptr;
+    if (forest) {
+        tau_forest_init_kernel<<<(n_pad + 255) / 256, 256, 0, c->stream>>>(fs, minlist, n_pad);
+        FROST_TRY(check_launch(c));
+    }
     const int a_tiles = n_pad / TA;
     prm.diag_only = 1; prm.seg_tiles = kTauKA;
     tau_sym_kernel<<<dim3(a_tiles, 1), kTauNT, smem, c->stream>>>(prm);
@@ -464,6 +498,12 @@ int tau_pruned(frost_ctx *c, int ld, const double *pos, const double *vel, const
         prm.diag_only = 0; prm.seg_tiles = (int)seg;
         const int segs = (int)((n_tiles - kTauKA + seg - 1) / seg);
         tau_sym_kernel<<<dim3(a_tiles, segs), kTauNT, smem, c->stream>>>(prm);
+        FROST_TRY(check_launch(c));
+    }
+    if (forest) {
+        tau_forest_min_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(fs, vals2, n, minlist);
+        FROST_TRY(check_launch(c));
+        tau_forest_out_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(fs, vals2, n, minlist, forest);
         FROST_TRY(check_launch(c));
     }
     tau_finish_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(tau64, sidx, n, tau_pivot, out_tau, out_bin);
