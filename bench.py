@@ -42,7 +42,7 @@ SLOTS_NEWTON, SLOTS_GRAD = 10, 16
 SLOTS_NEWTON_EQ, SLOTS_GRAD_EQ = 9.5, 15.5
 SLOTS_NEWTON_1S, SLOTS_GRAD_1S = 16, 28
 SM_COUNT, FP64_LANES_PER_SM = 148, 64      # B200: 64 FP64 FMA lanes per SM
-SPLIT_MAX_CONFIG5 = 32768                  # frost_set_split for the split arm of the config-5 step
+SPLIT_MAX_CONFIG5 = 1 << 20                # frost_set_split for the split arms of the config-5 step: every level
 METRIC = "pair interactions/s (acc+gradient, fp64) at N=2^20"
 UNIT = "pair interactions/s"
 

@@ -223,10 +223,12 @@ def test_config5_full_step_gate_n262144(fr):
     assert abs(e1 / e0 - 1) <= 2 * max(abs(rep["base"]["dE_rel"]), abs(rep["ulp_perturbed"]["dE_rel"]))
 
 
-def test_config5_full_step_with_split_levels_n262144(fr):
-    """The same step with the fast levels split into components (frost_set_split(32768), the launch
-    configuration bench.py times as `hhs_step_config5_split`).  Level 0 has 262144
-    members and runs Alg. 3 as printed: |S|, |F| equal the oracle's golden values.  The split levels
+@pytest.mark.parametrize("split_max,kepler", [(32768, 0), (1 << 20, 0), (1 << 20, 1)])
+def test_config5_full_step_with_split_levels_n262144(fr, split_max, kepler):
+    """The same step with the fast levels split into components (frost_set_split; 2^20 = every level,
+    the launch configuration bench.py times as `hhs_step_config5_split`, with frost_set_kepler as
+    `hhs_step_config5_split_kepler`).  The slow / fast partition of level 0 is the one
+    of Alg. 3: |S|, |F| equal the oracle's golden values.  The split levels
     cannot be run by the oracle at this size (its element-by-element parity is tests/test_gpu_split.py,
     n <= 3000); here: every level entered by as many components as its parent recursed into (twice
     each), sum m dv at roundoff, |dL|/|L| < 1e-12, energy error below the replica gate of the
@@ -238,21 +240,26 @@ def test_config5_full_step_with_split_levels_n262144(fr):
     fr.set_params(eta_ff=g0["eta"], eta_fb=g0["eta"])
     p, v, m = dev(pos), dev(vel), dev(mass)
     e0, p0, l0 = _conserved(fr, p, v, m)
-    fr.set_split(32768)
+    fr.set_split(split_max)
+    fr.set_kepler(kepler)
     l_before = fr.launch_count()
     try:
         st = fr.hhs_step(p, v, m, g0["dt_top"])
     finally:
         fr.set_split(0)
+        fr.set_kepler(0)
     launches = fr.launch_count() - l_before
     e1, p1, l1 = _conserved(fr, p, v, m)
     assert st["n_slow"][0] == g0["n_slow"] and st["n_fast"][0] == g0["n_fast"] and st["entries"][0] == 1
     e, c, s, f = st["entries"], st["n_comp"], st["n_slow"], st["n_fast"]
     for k in range(st["depth"]):
-        assert e[k + 1] <= 2 * c[k] and s[k + 1] + f[k + 1] == 2 * f[k], k
+        # (two-body components on their Kepler orbits enter no level)
+        assert e[k + 1] <= 2 * c[k], k
+        assert (s[k + 1] + f[k + 1] <= 2 * f[k]) if kepler else (s[k + 1] + f[k + 1] == 2 * f[k]), k
     assert max(ck / ek for ck, ek in zip(c, e)) > 100          # thousands of binaries side by side
-    assert st["depth"] >= 20 and bool(torch.isfinite(p).all()) and bool(torch.isfinite(v).all())
-    assert launches < 10000 < sum(e)
+    assert st["depth"] >= (5 if kepler else 20) and bool(torch.isfinite(p).all()) and bool(torch.isfinite(v).all())
+    assert (st["n_kepler"] > 100000) == bool(kepler)
+    assert launches < 10000 and (kepler or sum(e) > 10000)
     assert np.abs(p1 - p0).max() < 1e-15
     assert np.linalg.norm(l1 - l0) < 1e-12 * np.linalg.norm(l0)
     rep = gold["replica"]
