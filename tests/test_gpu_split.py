@@ -256,3 +256,29 @@ def test_split_step_with_kepler_components_matches_oracle(fr, oracle, n, small, 
               f"ratio x {rp:.3f}, v {rv:.3f}")
     assert rp <= 1.0 and rv <= 1.0, (rp, rv)
     assert momentum_change(mass, vel, vg, vr) <= 1.0
+
+
+def test_pruned_time_step_sweep_finds_every_fast_pair(fr):
+    """Levels of >= 32768 particles take the pruned time-step sweep, which in a split entry must still
+    meet every pair below the pivot (it discards against max(running minimum, tau_pivot)).  The same
+    split step with the pruning machinery off (frost_set_symmetric mode 3: the plain pair-symmetric
+    sweep evaluates all pairs) must give the same components and bookkeeping, and the same state up to
+    the last bit of a few sums (mode 3 also sends the small force sweeps through the symmetric kernels,
+    which add in another order: 81 velocity components differ by one ulp)."""
+    n = 40000
+    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-4, a_hi=1e-2)
+    fr.set_params(eta_ff=0.2, eta_fb=0.2)
+    out = []
+    try:
+        for mode in (0, 3):
+            fr.set_symmetric(mode)
+            fr.set_split(BIG)
+            p, v = dev(pos), dev(vel)
+            st = fr.hhs_step(p, v, dev(mass), 2.0 ** -8)
+            out.append((st, p, v))
+    finally:
+        fr.set_symmetric(0)
+        fr.set_split(0)
+    assert out[0][0] == out[1][0]
+    assert out[0][0]["n_comp"][0] > 100 and out[0][0]["depth"] >= 8
+    assert (out[0][1] - out[1][1]).abs().max() < 1e-14 and (out[0][2] - out[1][2]).abs().max() < 1e-13
