@@ -15,6 +15,10 @@ counts, |dE/E|, |dP|, |dL|/|L| -- and the same step from inputs moved by +-1 ulp
 (seeded), which shows down to which level the bookkeeping is a reproducible function of the input
 (reading 23: eccentric hard binaries sweep their time-step across pivots thousands of
 times per top step, and the deepest levels' entry counts then depend on the last bit).
+
+Part "replica_split": the same replica, one whole oracle step with every level split into the connected
+components of its fast pairs and the two-body components on their Kepler orbits (SURVEY 8(f).4;
+oracle O6s + O6k), again from the inputs as they are and from inputs 1 ulp away.
 """
 import argparse
 import json
@@ -50,10 +54,11 @@ def conserved(pos, vel, mass):
     return d["E"], d["P"], d["L"]
 
 
-def replica(n):
+def replica(n, **kw):
     pos, vel, mass, _ = fi.star_cluster(n, SEED)
     e0, p0, l0 = conserved(pos, vel, mass)
     out = {"n": n, "seed": SEED, "dt_top": DT_TOP, "eta": ETA}
+    out.update(kw)
     rng = np.random.default_rng(0)
     for name in ("base", "ulp_perturbed"):
         p, v = pos.copy(), vel.copy()
@@ -61,7 +66,7 @@ def replica(n):
             p = np.ascontiguousarray(np.nextafter(p, rng.choice([-1.0, 1.0], size=p.shape) * np.inf))
             v = np.ascontiguousarray(np.nextafter(v, rng.choice([-1.0, 1.0], size=v.shape) * np.inf))
         t0 = time.time()
-        st = oracle.hhs_step(p, v, mass, DT_TOP, eta_ff=ETA, eta_fb=ETA)
+        st = oracle.hhs_step(p, v, mass, DT_TOP, eta_ff=ETA, eta_fb=ETA, **kw)
         e1, p1, l1 = conserved(p, v, mass)
         out[name] = {"stats": st, "dE_rel": float(e1 / e0 - 1.0),
                      "dP_max": float(np.abs(p1 - p0).max()),
@@ -69,7 +74,7 @@ def replica(n):
                      "oracle_seconds": time.time() - t0}
     a, b = out["base"]["stats"], out["ulp_perturbed"]["stats"]
     k = 0
-    while k <= min(a["depth"], b["depth"]) and all(a[q][k] == b[q][k] for q in ("entries", "n_slow", "n_fast")):
+    while k <= min(a["depth"], b["depth"]) and all(a[q][k] == b[q][k] for q in ("entries", "n_slow", "n_fast", "n_comp")):
         k += 1
     out["levels_reproducible_under_1ulp"] = k
     return out
@@ -81,12 +86,20 @@ def main():
     ap.add_argument("--skip-full", action="store_true")
     ap.add_argument("--full-n", type=int, default=262144)
     ap.add_argument("--replica-n", type=int, default=32768)
+    ap.add_argument("--only-split", action="store_true", help="(re)write only the replica_split part")
     args = ap.parse_args()
     if args.threads > 0:
         oracle.set_num_threads(args.threads)
     doc = json.load(open(OUT)) if os.path.exists(OUT) else {}
     doc["generated_by"] = "tests/golden/make_config5_gate.py (oracle/ only)"
     doc["cites"] = "SURVEY.md 8(c) last pin row; Alg. 3 PAPER.md:572-587; Eq. 49-54 PAPER.md:429-474"
+    # Part "replica_split": the same replica with every level split into the components of its fast pairs
+    # and the two-body components on their Kepler orbits (oracle O6s + O6k; readings 24-25)
+    doc["replica_split"] = replica(args.replica_n, split_max=1 << 20, kepler=True)
+    json.dump(doc, open(OUT, "w"), indent=1)
+    if args.only_split:
+        print("wrote", OUT)
+        return
     doc["replica"] = replica(args.replica_n)
     json.dump(doc, open(OUT, "w"), indent=1)
     if not args.skip_full:

@@ -296,3 +296,35 @@ def test_config5_replica_step_against_golden_n32768(fr):
     assert np.abs(p1 - p0).max() <= max(4 * rep["base"]["dP_max"], 1e-15)
     assert np.linalg.norm(l1 - l0) < 1e-12 * np.linalg.norm(l0)
     assert abs(e1 / e0 - 1) <= 4 * max(abs(rep["base"]["dE_rel"]), abs(rep["ulp_perturbed"]["dE_rel"]))
+
+
+def test_config5_replica_split_kepler_step_against_golden_n32768(fr):
+    """The N = 32768 replica with every level split into the components of its fast pairs and the
+    two-body components on their Kepler orbits (frost_set_split(2^20) + frost_set_kepler)
+    against the oracle's WHOLE step of the same definition (golden `replica_split`, written by
+    tests/golden/make_config5_gate.py from oracle/ alone).  Without the deep binary recursion the
+    oracle's bookkeeping is reproducible under a 1-ulp change of its input on every level, so the
+    device's must be IDENTICAL: entries, |S|, |F|, components and propagator calls per level, pair
+    counts -- through the pruned time-step sweep with edge output (level 0 has 32768 members), the
+    S x F + G x R + masked-R kick decomposition and the batched component kernels.  Energy error equal
+    to the oracle's to 1 %, momentum at roundoff."""
+    rep = json.load(open(GOLDEN))["replica_split"]
+    base, pert = rep["base"]["stats"], rep["ulp_perturbed"]["stats"]
+    assert base == pert and rep["levels_reproducible_under_1ulp"] == base["depth"] + 1
+    n = rep["n"]
+    pos, vel, mass, pairs = fi.star_cluster(n, rep["seed"])
+    fr.set_params(eta_ff=rep["eta"], eta_fb=rep["eta"])
+    p, v, m = dev(pos), dev(vel), dev(mass)
+    e0, p0, l0 = _conserved(fr, p, v, m)
+    fr.set_split(rep["split_max"])
+    fr.set_kepler(1 if rep["kepler"] else 0)
+    try:
+        st = fr.hhs_step(p, v, m, rep["dt_top"])
+    finally:
+        fr.set_split(0)
+        fr.set_kepler(0)
+    e1, p1, l1 = _conserved(fr, p, v, m)
+    assert st == base
+    assert abs((e1 / e0 - 1) / rep["base"]["dE_rel"] - 1) < 1e-2
+    assert np.abs(p1 - p0).max() <= max(4 * rep["base"]["dP_max"], 1e-16)
+    assert np.linalg.norm(l1 - l0) < 1e-13 * np.linalg.norm(l0)
