@@ -17,6 +17,7 @@ no torchrun environment the script re-launches itself under torch.distributed.ru
     --rows-only      launch every O(N) kernel and the three time-step sweeps once or twice (for ncu)
     --subtree K      the device-resident subtree kernel on K/2 hard binaries (for ncu)
     --hhs-only       one HHS-FSI step of config 5 (N = 262144) with its validity numbers
+    --hhs-plummer N  one HHS-FSI step of an equal-mass Plummer sphere of N particles (Alg. 3 / split + Kepler)
 """
 import argparse
 import json
@@ -359,6 +360,39 @@ def run_hhs_only(arm):
     fr.close()
 
 
+def run_hhs_plummer(n):
+    """--hhs-plummer N: one whole HHS-FSI step (dt_top = 2^-7, eta = 0.2) of an equal-mass Plummer sphere of
+    N particles -- the paper's million-body setting in synthetic form -- with Alg. 3 as
+    printed and with every level split + Kepler components; conserved quantities by frost_diagnostics."""
+    import torch
+    import paper_2011_14984_b200 as frost
+    fr = frost.Frost(0)
+    dev = torch.device("cuda", 0)
+    pos, vel, mass = fi.plummer(n, 2)
+    out = {}
+    for name, split, kep in (("alg3", 0, 0), ("split_kepler", 1 << 20, 1)):
+        p, v, m = (torch.as_tensor(x).to(dev) for x in (pos, vel, mass))
+        fr.set_params(G=1.0, eps2=0.0, eta_ff=0.2, eta_fb=0.2)
+        d0 = fr.diagnostics(p, v, m)
+        fr.set_split(split); fr.set_kepler(kep)
+        l0 = fr.launch_count()
+        torch.cuda.synchronize(); t0 = time.perf_counter()
+        st = fr.hhs_step(p, v, m, 2.0 ** -7)
+        torch.cuda.synchronize(); t1 = time.perf_counter()
+        fr.set_split(0); fr.set_kepler(0)
+        d1 = fr.diagnostics(p, v, m)
+        L0, L1 = np.array(d0["L"]), np.array(d1["L"])
+        out[name] = {"n": n, "seconds": t1 - t0, "launches": int(fr.launch_count() - l0), "depth": st["depth"],
+                     "hierarchy_entries": int(sum(st["entries"])), "kepler_calls": int(st["n_kepler"]),
+                     "pairs_newton": int(st["pairs_newton"]), "pairs_gradient": int(st["pairs_gradient"]),
+                     "pairs_timestep": int(st["pairs_timestep"]),
+                     "dE_rel": float(d1["E"] / d0["E"] - 1.0),
+                     "dP": float(np.abs(np.array(d1["P"]) - np.array(d0["P"])).max()),
+                     "dL_rel": float(np.linalg.norm(L1 - L0) / np.linalg.norm(L0))}
+    print(json.dumps({"hhs_step_plummer": out}))
+    fr.close()
+
+
 def run_frost(args):
     import torch
     import torch.distributed as dist
@@ -593,6 +627,7 @@ def main():
     ap.add_argument("--rows-only", action="store_true", help="launch the O(N) kernels and time-step sweeps (for ncu)")
     ap.add_argument("--subtree", type=int, default=0, help="run the subtree kernel on K/2 hard binaries (for ncu)")
     ap.add_argument("--hhs-only", action="store_true", help="one HHS-FSI step of config 5 with its validity numbers")
+    ap.add_argument("--hhs-plummer", type=int, default=0, help="one HHS-FSI step of a Plummer sphere of N particles")
     ap.add_argument("--no-eqmass", action="store_true", help="general kernels even on equal masses (frost_set_equal_mass_path(0))")
     ap.add_argument("--hhs-arm", default="both", choices=["both", "alg3", "split"],
                     help="--hhs-only: Alg. 3 as printed, the split fast levels (frost_set_split), or both")
@@ -605,6 +640,8 @@ def main():
         return run_subtree(args.subtree)
     if args.hhs_only:
         return run_hhs_only(args.hhs_arm)
+    if args.hhs_plummer:
+        return run_hhs_plummer(args.hhs_plummer)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # not under torchrun: launch one rank per GPU ourselves (rank 0 prints the JSON line)
         import socket
