@@ -354,9 +354,11 @@ static int small_threshold(const frost_ctx *c) { return c->tune_small < 0 ? smal
 // n_steps consecutive fsi steps (Alg. 2).  The trailing Newton sweep of one step is at the
 // positions of the leading sweep of the next, so from the second step on the leading sweep is
 // skipped: 3 all-pairs sweeps per step instead of 4, bitwise the same result.
+// skip_leading: the context's acc planes already hold a^{SS} of this set at the current positions (the
+// trailing sweep of an earlier fsi on the same set, nothing moved since): the first sweep is skipped.
 static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const double *mass,
                     const int32_t *idx, int n_idx, double dt, frost_hhs_stats *st, void *dev_stats,
-                    int n_steps = 1) {
+                    int n_steps = 1, bool skip_leading = false) {
     if (!idx) n_idx = n;
     if (n_idx <= 0 || n_steps <= 0) return FROST_OK;
     if (n_idx <= small_threshold(c))     // device-resident, set in shared memory (row 11)
@@ -365,7 +367,7 @@ static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const
     FROST_TRY(ensure(c, c->grad, (size_t)3 * ld * sizeof(double)));
     double *acc = (double *)c->acc.p, *grad = (double *)c->grad.p;
     for (int k = 0; k < n_steps; ++k) {
-        if (k == 0)
+        if (k == 0 && !skip_leading)
             FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, nullptr, FROST_ACC));
         FROST_TRY(launch_kick_drift(c, ld, pos, vel, acc, nullptr, idx, n_idx, dt / 6.0, 0.0, dt / 2.0));
         FROST_TRY(forces_impl(c, n, ld, pos, mass, idx, n_idx, idx, n_idx, acc, grad, FROST_ACC | FROST_GRAD));
@@ -385,8 +387,12 @@ static int fsi_impl(frost_ctx *c, int n, int ld, double *pos, double *vel, const
 // fsi(S, h) of an entry at `level`.  With overlap on it is enqueued on the level's side stream after
 // everything enqueued so far on the parent's stream (fork); join_side() makes the parent's stream
 // wait for it.  Same kernels, same inputs, disjoint particles: bitwise the serial result.
+// second: the second fsi(S, h) of the entry.  Between the two, S is only kicked (the recursion moves F),
+// and the side context's acc planes are touched by nobody else: they still hold the trailing a^{SS} of
+// the first call at the positions S still has, so the leading sweep of the second call is skipped --
+// the same values, one all-pairs sweep of S less per entry.
 static int fsi_side(frost_ctx *c, int level, int n, int ld, double *pos, double *vel, const double *mass,
-                    const int32_t *S, int nS, double h, frost_hhs_stats *st, bool *forked) {
+                    const int32_t *S, int nS, double h, frost_hhs_stats *st, bool *forked, bool second = false) {
     *forked = false;
     if (nS <= 0) return FROST_OK;
     if (!c->overlap) return fsi_impl(c, n, ld, pos, vel, mass, S, nS, h, st, c->dev_stats.p);
@@ -394,7 +400,7 @@ static int fsi_side(frost_ctx *c, int level, int n, int ld, double *pos, double 
     FROST_TRY(side_ctx(c, level, &s));
     FROST_CUDA(c, cudaEventRecord(c->ev_fork[level], c->stream));
     FROST_CUDA(c, cudaStreamWaitEvent(s->stream, c->ev_fork[level], 0));
-    const int rc = fsi_impl(s, n, ld, pos, vel, mass, S, nS, h, st, c->dev_stats.p);
+    const int rc = fsi_impl(s, n, ld, pos, vel, mass, S, nS, h, st, c->dev_stats.p, 1, second);
     if (rc != FROST_OK) { c->last_cuda = s->last_cuda; return rc; }
     *forked = true;
     return FROST_OK;
@@ -521,7 +527,7 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     FROST_TRY(join_side(c, level, forked));
     FROST_TRY(cross_kick(c, n, ld, pos, vel, mass, set, n_set, S, nS, F, nF, si, true, 2.0 * tau_pivot / 3.0,
                          tau_pivot * tau_pivot / 48.0));
-    FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked));
+    FROST_TRY(fsi_side(c, level, n, ld, pos, vel, mass, S, nS, h, st, &forked, true));
     FROST_TRY(recurse_fast(c, n, ld, pos, vel, mass, F, nF, si, h, level, st));
     FROST_TRY(join_side(c, level, forked));
     FROST_TRY(cross_kick(c, n, ld, pos, vel, mass, set, n_set, S, nS, F, nF, si, false, tau_pivot / 6.0, 0.0));
