@@ -509,6 +509,7 @@ static int hhs_rec(frost_ctx *c, int n, int ld, double *pos, double *vel, const 
     si.sumsq = (long long)nF * nF;
     if (split && nF > 0) {
         FROST_TRY(split_components(c, level, ld, tau, set, n_set, tau_pivot, forest, F, nF, &si));
+        si.split = true;
         F = const_cast<int32_t *>(si.C);       // same members, components contiguous
     }
     if (st) {

@@ -150,7 +150,7 @@ def test_pair_path_is_bitwise_the_team_path(fr, n, split):
 
 def test_split_tiny_and_degenerate_systems(fr, oracle):
     """Edge cases of the split step against the oracle: one, two, three and five bodies (no fast pair,
-    one fast pair, a chain), softening, the five-body Solar system (F = {Sun, Jupiter}: one component,
+    one fast pair, a chain), softening, the Kepler propagator on and off, the five-body Solar system (F = {Sun, Jupiter}: one component,
     several levels), an empty fast set at the top (everything slow)."""
     rng = np.random.default_rng(11)
     cases = []
@@ -169,20 +169,22 @@ def test_split_tiny_and_degenerate_systems(fr, oracle):
     sp, sv, sm, sG = fi.solar_system()
     cases.append((sp, sv, sm, 512.0, dict(G=sG, eps2=0.0)))
     for pos, vel, mass, dt, kw in cases:
-        for small in (-1, 0):
+        for small, kepler in ((-1, 0), (0, 0), (-1, 1), (0, 1)):
             fr.set_params(G=kw["G"], eps2=kw["eps2"], eta_ff=0.1, eta_fb=0.1)
             fr.set_tuning(0, 0, small)
             fr.set_split(BIG)
+            fr.set_kepler(kepler)                 # (ignored with softening, by both sides)
             pr, vr = pos.copy(), vel.copy()
-            st_ref = oracle.hhs_step(pr, vr, mass, dt, eta_ff=0.1, eta_fb=0.1, split_max=BIG, **kw)
+            st_ref = oracle.hhs_step(pr, vr, mass, dt, eta_ff=0.1, eta_fb=0.1, split_max=BIG, kepler=bool(kepler), **kw)
             p, v = dev(pos), dev(vel)
             try:
                 st = fr.hhs_step(p, v, dev(mass), dt)
             finally:
                 fr.set_split(0)
+                fr.set_kepler(0)
                 fr.set_tuning(0, 0, -1)
                 fr.set_params()
-            assert st == st_ref, (mass.size, dt, small)
+            assert st == st_ref, (mass.size, dt, small, kepler)
             scale = max(1.0, np.abs(pr).max())
             # (a tight pair turns a rounding difference into an orbital phase difference: |dv| ~ v dphi)
             assert np.abs(p.cpu().numpy() - pr).max() < 1e-10 * scale
