@@ -61,7 +61,8 @@ def _split_case(fr, oracle, pos, vel, mass, dt, small, one_cta=0, **kw):
 
 
 @pytest.mark.parametrize("n,small,one_cta,log2dt", [(256, -1, 0, 7), (256, -1, 1, 7), (256, 48, 0, 7), (256, 0, 0, 9),
-                                                    (1024, -1, 0, 8), (3000, -1, 0, 8), (3000, 100, 0, 8)])
+                                                    (1024, -1, 0, 8), (3000, -1, 0, 8), (3000, 100, 0, 8),
+                                                    (2000, 0, 0, 9)])
 def test_split_step_matches_split_oracle(fr, oracle, n, small, one_cta, log2dt, capsys):
     """One split HHS-FSI step of config 5's recipe (binaries a = 1e-5..1e-3, e <= 0.1 so that no pair
     step oscillates across a pivot): n <= 1024 with small = -1 runs entirely inside the subtree kernel
@@ -227,7 +228,7 @@ def test_split_multi_step_run_conserves_like_alg3(fr, capsys):
     assert np.abs(out[0][1] - out[BIG][1]).max() < 1e-4
 
 
-@pytest.mark.parametrize("n,small,log2dt", [(256, -1, 7), (256, 0, 9), (3000, -1, 8), (3000, 100, 8)])
+@pytest.mark.parametrize("n,small,log2dt", [(256, -1, 7), (256, 0, 9), (3000, -1, 8), (3000, 100, 8), (2000, 0, 9)])
 def test_split_step_with_kepler_components_matches_oracle(fr, oracle, n, small, log2dt, capsys):
     """frost_set_kepler on top of the split step: every two-body component follows its exact Kepler orbit
     (reading 25; oracle O6k) -- bookkeeping identical to the oracle's (fewer and shallower entries, the
