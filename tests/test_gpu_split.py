@@ -228,13 +228,15 @@ def test_split_multi_step_run_conserves_like_alg3(fr, capsys):
     assert np.abs(out[0][1] - out[BIG][1]).max() < 1e-4
 
 
-@pytest.mark.parametrize("n,small,log2dt", [(256, -1, 7), (256, 0, 9), (3000, -1, 8), (3000, 100, 8), (2000, 0, 9)])
+@pytest.mark.parametrize("n,small,log2dt", [(256, -1, 7), (256, 0, 9), (3000, -1, 8), (3000, 100, 8), (2000, 0, 9), (3000, -1, 4)])
 def test_split_step_with_kepler_components_matches_oracle(fr, oracle, n, small, log2dt, capsys):
     """frost_set_kepler on top of the split step: every two-body component follows its exact Kepler orbit
     (reading 25; oracle O6k) -- bookkeeping identical to the oracle's (fewer and shallower entries, the
     same number of propagator calls), trajectory inside the oracle's 1-ulp envelope, momentum at
     rounding level: inside the subtree kernel (small = -1, n = 256), through the batched component
-    launches, and from the host recursion alone (small = 0)."""
+    launches, and from the host recursion alone (small = 0).  dt_top = 2^-4 at n = 3000 makes level 0
+    percolate (one component of ~2800 particles beside a few small ones): the S x F + G x R + masked-R
+    kick and the host recursion into the giant component, against the oracle."""
     pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
     dt = 2.0 ** -log2dt
     fr.set_params(eta_ff=0.2, eta_fb=0.2)
