@@ -448,8 +448,13 @@ static int cross_kick(frost_ctx *c, int n, int ld, double *pos, double *vel, con
                 FROST_TRY(launch_pack_xm(c, ld, pos, mass, si.R, nR, pad, xm, 1.0, 0, av));
                 if (phase == 1) FROST_TRY(launch_pack_vec(c, ld, acc, si.R, nR, pad, av));     // the total a of P
                 FROST_TRY(launch_pack_label(c, si.labR, nR, pad, av));
-                FROST_TRY(sweep_masked(c, xm, av, nR, si.R, ld, phase == 0 ? out : nullptr,
-                                       phase == 1 ? out : nullptr, fresh ? 0 : 1));
+                // pair-symmetric from the same size as the unmasked self sweeps, else one-sided
+                if (use_sym(c, nR, nR, 0))
+                    FROST_TRY(sym_masked(c, xm, av, nR, si.R, ld, phase == 0 ? out : nullptr,
+                                         phase == 1 ? out : nullptr, fresh ? 0 : 1));
+                else
+                    FROST_TRY(sweep_masked(c, xm, av, nR, si.R, ld, phase == 0 ? out : nullptr,
+                                           phase == 1 ? out : nullptr, fresh ? 0 : 1));
             }
         }
         return launch_kick(c, ld, vel, acc, with_g ? grad : nullptr, set, n_set, cc, kappa);

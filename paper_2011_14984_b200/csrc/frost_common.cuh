@@ -196,6 +196,8 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
                  double tau_pivot, double *out_tau, int32_t *out_bin, int *forest = nullptr);
 
 int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
+int sym_masked(frost_ctx *c, const double *xm, const double *a_lab, int n, const int32_t *idx, int ld,
+               double *out_acc, double *out_grad, int accumulate);
 // frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)
 int launch_diag(frost_ctx *c, int n, int ld, const double *pos, const double *vel, const double *mass,
                 const double *phi, double *out8);

@@ -178,6 +178,68 @@ struct SymGradientFastT : SymGradient {
 
 using SymGradientFast = SymGradientFastT<false>;
 
+// The kick sweeps of a split hierarchy entry over the debris list R: pairs whose component
+// labels are equal contribute nothing.  The label of a record travels in the low word of .w of its
+// second record (as in the one-sided MaskedNewtonPolicy / MaskedGradientPolicy); the weight of a
+// same-label pair is replaced by zero (ISETP + 2 SEL per pair).  Self sweeps only, guarded gradient.
+struct SymNewtonMasked {
+    static constexpr int kRecs = 2, kPlanes = 3;
+    static constexpr bool kMin = false;
+    struct A : SymNewton::A { int lab; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        SymNewton::load(a, p, i);
+        a.lab = __double2loint(p.a1[i].w);
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[3]) { b[0] = b[1] = b[2] = 0.0; }
+    __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
+        const double y = rsqrt_seed(s2);
+        const double y2 = y * y;
+        const double e = fma(-s2, y2, 1.0);
+        const double w0 = y2 * y;
+        const double q = fma(1.875, e, 1.5);
+        const double qe = q * e;
+        double w = fma(w0, qe, w0);
+        if (__double2loint(j1.w) == a.lab) w = 0.0;
+        const double wa = w * j0.w;
+        const double wb = w * a.nm;
+        fma3_shared(a.s[0], a.s[1], a.s[2], wa, dx, dy, dz);
+        fma3_shared(b[0], b[1], b[2], wb, dx, dy, dz);
+    }
+};
+
+struct SymGradientMasked {
+    static constexpr int kRecs = 2, kPlanes = 3;
+    static constexpr bool kMin = false;
+    struct A : SymGradient::A { int lab; };
+    __device__ static __forceinline__ void load(A &a, const SymParams &p, int i) {
+        SymGradient::load(a, p, i);
+        a.lab = __double2loint(p.a1[i].w);
+    }
+    __device__ static __forceinline__ void init_b(double (&b)[3]) { b[0] = b[1] = b[2] = 0.0; }
+    __device__ static __forceinline__ void pair(A &a, double (&b)[3], const double4 &j0,
+                                                const double4 &j1, const SymParams &p) {
+        const double dx = j0.x - a.x, dy = j0.y - a.y, dz = j0.z - a.z;
+        const double ax = j1.x - a.ax, ay = j1.y - a.ay, az = j1.z - a.az;
+        const double s2 = fma(dz, dz, fma(dy, dy, fma(dx, dx, p.eps2)));
+        const double ri = rsqrt_full_or_zero(s2);
+        const double dot = fma(dz, az, fma(dy, ay, dx * ax));
+        const double q = ri * ri;
+        double w3 = ri * q;
+        if (__double2loint(j1.w) == a.lab) w3 = 0.0;
+        const double t = q * dot;
+        const double u = t * -3.0;
+        double vx = ax, vy = ay, vz = az;
+        fma3_shared(vx, vy, vz, u, dx, dy, dz);
+        const double wa = w3 * j0.w;
+        const double wb = w3 * a.nm;
+        fma3_shared(a.s[0], a.s[1], a.s[2], wa, vx, vy, vz);
+        fma3_shared(b[0], b[1], b[2], wb, vx, vy, vz);
+    }
+};
+
 template <class P, class = void> struct UnrollOf { static constexpr int value = 2; };
 template <class P> struct UnrollOf<P, std::enable_if_t<(P::kUnroll > 0)>> { static constexpr int value = P::kUnroll; };
 template <class P, class = void> struct DiagGuard { static constexpr bool value = false; };
@@ -665,6 +727,29 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
     }
     if (n_set < kSymSmallN) return run_sym<SymTimestep, kSymKSmall, kSymNT, kSymMinBSmall>(c, j);
     return run_sym<SymTimestep, kSymKTau, kSymNT, kSymMinB>(c, j);
+}
+
+// Masked self sweep of one list (labels in the low word of a_lab[k].w): out_acc != NULL the Newton sweep,
+// out_grad != NULL the gradient sweep from the accelerations in a_lab.  accumulate: add to the planes.
+int sym_masked(frost_ctx *c, const double *xm, const double *a_lab, int n, const int32_t *idx, int ld,
+               double *out_acc, double *out_grad, int accumulate) {
+    if (n <= 0) return FROST_OK;
+    for (int pass = 0; pass < 2; ++pass) {
+        if ((pass == 0 && !out_acc) || (pass == 1 && !out_grad)) continue;
+        SymJob j{};
+        j.A0 = xm; j.A1 = a_lab; j.nA = n; j.nB = n; j.self = true; j.A_idx = idx; j.ld = ld;
+        j.accumulate = accumulate;
+        if (pass == 0) {
+            j.out = out_acc; j.scale = c->G; j.eps2 = c->eps2 > 0x1p-400 ? c->eps2 : 0x1p-400;
+            if (n < kSymSmallN) FROST_TRY((run_sym<SymNewtonMasked, kSymKSmall, kSymNT, kSymMinBSmall>(c, j)));
+            else FROST_TRY((run_sym<SymNewtonMasked, kSymKNewton, kSymNT, kSymMinB>(c, j)));
+        } else {
+            j.out = out_grad; j.scale = 2.0 * c->G; j.eps2 = c->eps2;
+            if (n < kSymSmallN) FROST_TRY((run_sym<SymGradientMasked, kSymKSmall, kSymNT, kSymMinBSmall>(c, j)));
+            else FROST_TRY((run_sym<SymGradientMasked, kSymKGrad, kSymNTGrad, kSymMinBGrad>(c, j)));
+        }
+    }
+    return FROST_OK;
 }
 
 // phi_i = -G sum_{j != i} m_j / s_ij for all particles of the packed stream (always symmetric).
