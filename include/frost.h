@@ -251,9 +251,9 @@ int frost_set_overlap(frost_ctx *ctx, int on);
  * split_max > 0 applies this to every entry with at most split_max members (larger entries run Alg. 3
  * as printed); 0 (default) switches it off.  A level that still percolates -- one giant component G plus
  * debris R -- gains too: the next level then holds G alone, and the kick is swept as S x F + G x R
- * (pair-symmetric) plus the pairs of R in different components.  Components of at most 32 particles -- binaries, triples -- are advanced side by
- * side, one warp each, by one batched launch per recursion pass; components of up to 1024 particles
- * one CTA each; larger ones by the host recursion.  Result: deterministic; not the numbers of
+ * (pair-symmetric) plus the pairs of R in different components.  Components of at most 32 particles --
+ * binaries, triples -- are advanced side by side, one warp each, by one batched launch per recursion
+ * pass; components of up to 1024 particles one CTA each; larger ones by the host recursion.  Result: deterministic; not the numbers of
  * split_max = 0 (a different, equally fourth-order splitting of the same Hamiltonian). */
 int frost_set_split(frost_ctx *ctx, int split_max);
 
