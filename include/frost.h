@@ -39,6 +39,7 @@ extern "C" {
 #define FROST_ENOMEM (-3)     /* scratch allocation failed */
 #define FROST_EDEPTH (-4)     /* frost_hhs_step recursed beyond max_depth */
 #define FROST_ENONFINITE (-5) /* reserved: non-finite input detected (debug scans) */
+#define FROST_ETOOBIG (-6)    /* frost_acc_noalloc: n exceeds FROST_NOALLOC_MAX_N (its scratch is a fixed array) */
 
 /* flags of frost_forces */
 #define FROST_ACC 1    /* compute Newtonian accelerations of the sinks */
@@ -301,6 +302,41 @@ int frost_set_equal_mass_path(frost_ctx *ctx, int on);
 int frost_forces_masked(frost_ctx *ctx, int n, int ld, const double *pos, const double *mass,
                         const int32_t *idx, int n_idx, const int32_t *label, double *out_acc,
                         double *out_grad);
+
+/* ---- The entry point that allocates nothing -------------------------------------------------------
+ * Every call above may grow the context's scratch with cudaMalloc (and frost_create itself allocates).
+ * Some callers cannot have that: a host application whose memory pool owns the whole device, a
+ * latency-critical loop that cannot take the device-wide synchronisation a cudaFree implies, a program
+ * that runs under a memory budget fixed at start-up.  For them:
+ *
+ *   out_acc[c*ld + i] <- G sum_{j != i} m_j (x_j - x_i)_c / (|x_j - x_i|^2 + eps2)^(3/2),  0 <= i < n
+ *
+ * (Eq. 24: the Newtonian accelerations of all n particles from all n particles, the
+ * FROST_ACC self sweep of frost_forces) with no context and no allocation of any kind: the call issues
+ * no cudaMalloc, cudaFree or allocating library routine, on the host or on the device.  Its scratch --
+ * the packed source records and the per-slice partial sums of the one-sided Newton sweep it is a
+ * variant of -- is a static __device__ array of 6.5 MiB compiled into the library, which every GPU
+ * that loads the library's module keeps until the process exits.  Hence the limit:
+ * n <= FROST_NOALLOC_MAX_N, otherwise FROST_ETOOBIG and nothing is launched (frost_noalloc_max_n()
+ * returns the limit of the loaded build).
+ *   device, stream : the CUDA device the pointers live on and the stream (cudaStream_t as void*, NULL =
+ *                    legacy default stream) the three kernels are enqueued on; the device is made
+ *                    current for the call and the caller's current device restored.  Asynchronous.
+ *   pos, mass      : DEVICE inputs, layout as everywhere in this header; out_acc: DEVICE output, three
+ *                    planes of stride ld, entries i >= n untouched.  Caller-owned; nothing is retained.
+ *   cuda_error     : HOST, nullable: receives the cudaError_t when the status is FROST_ECUDA, else 0.
+ * Sharing: all calls on a device use the one array and it keeps the previous call's contents.  A call
+ * rewrites everything it later reads, so consecutive calls of any sizes on ordered streams are
+ * independent -- but two calls that OVERLAP on the GPU (different streams without an event between
+ * them, or two host threads) race on it and both results are garbage.  Serialise them.
+ * First call: the first call on each device looks up the array's device address (cudaGetSymbolAddress,
+ * which may load the module).  Make that call before starting any stream capture.
+ * Same pair arithmetic as frost_forces (results agree to rounding, ~1e-15 |a_i|; the slice count, and
+ * so the summation order, differs); coincident pairs contribute nothing, as above. */
+#define FROST_NOALLOC_MAX_N 16384
+int frost_acc_noalloc(int device, void *stream, int n, int ld, const double *pos, const double *mass,
+                      double G, double eps2, double *out_acc, int *cuda_error);
+int frost_noalloc_max_n(void);
 
 #ifdef __cplusplus
 }

@@ -5,8 +5,8 @@ Every step of the path runs in the CUDA kernels behind include/frost.h; this pac
 arguments (torch tensors -> device pointers).  There is no CPU fallback and no dependency on
 oracle/: if the shared library is missing or no CUDA device is usable, calls raise.
 """
-from .binding import (ACC, ACCUMULATE, GRAD, MUTUAL, Frost, FrostError, exported_symbols, library_path,
-                      load_library)
+from .binding import (ACC, ACCUMULATE, GRAD, MUTUAL, Frost, FrostError, acc_noalloc, exported_symbols,
+                      library_path, load_library, noalloc_max_n)
 
-__all__ = ["ACC", "ACCUMULATE", "GRAD", "MUTUAL", "Frost", "FrostError", "exported_symbols", "library_path",
-           "load_library"]
+__all__ = ["ACC", "ACCUMULATE", "GRAD", "MUTUAL", "Frost", "FrostError", "acc_noalloc", "exported_symbols",
+           "library_path", "load_library", "noalloc_max_n"]

@@ -27,7 +27,7 @@ exported_symbols = [
     "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
     "frost_set_split", "frost_forces_masked", "frost_set_pair_path",
     "frost_set_gradient_guard", "frost_set_equal_mass_path",
-    "frost_set_kepler",
+    "frost_set_kepler", "frost_acc_noalloc", "frost_noalloc_max_n",
 ]
 
 
@@ -91,6 +91,8 @@ def load_library():
     lib.frost_hhs_step.argtypes = [vp, i32, i32, vp, vp, vp, f64, vp]
     lib.frost_gather_pack.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp]
     lib.frost_fp64_probe.argtypes = [vp, i32, i32, i32, vp, vp]
+    lib.frost_acc_noalloc.argtypes = [i32, vp, i32, i32, vp, vp, f64, f64, vp, C.POINTER(C.c_int)]
+    lib.frost_noalloc_max_n.argtypes = []
     lib.frost_launch_count.argtypes = [vp]
     lib.frost_launch_count.restype = C.c_int64
     lib.frost_last_cuda_error.argtypes = [vp]
@@ -120,6 +122,34 @@ def _idx(t: Optional[torch.Tensor], name: str):
     if t.numel() == 0:      # an empty list is not "all particles": pass a non-NULL pointer, count 0
         return torch.zeros(1, dtype=torch.int32, device=t.device), 0
     return t, t.numel()
+
+
+def noalloc_max_n() -> int:
+    """Largest n frost_acc_noalloc accepts (its scratch is a fixed static device array)."""
+    return int(load_library().frost_noalloc_max_n())
+
+
+def acc_noalloc(pos, mass, out_acc, G=1.0, eps2=0.0, stream: Optional[torch.cuda.Stream] = None):
+    """frost_acc_noalloc: Newtonian accelerations of all particles (Eq. 24) written into the
+    caller's out_acc, for callers that must not allocate device memory (a pool that owns the device, a
+    loop that cannot afford cudaFree's synchronisation, a fixed memory budget).  No context, no
+    cudaMalloc anywhere on the path -- which is why out_acc is a required argument here: this wrapper
+    creates no tensor either.  n <= noalloc_max_n(); calls that overlap on the GPU race on the library's
+    one static scratch array; make the first call on a device outside stream capture (frost.h)."""
+    lib = load_library()
+    _vec(pos, "pos"); _vec(out_acc, "out_acc")
+    if out_acc.shape != pos.shape or out_acc.device != pos.device or mass.device != pos.device:
+        raise FrostError("acc_noalloc: pos, mass and out_acc must share device and plane stride")
+    dev = pos.device.index
+    if stream is None:
+        stream = torch.cuda.current_stream(dev)
+    err = C.c_int(0)
+    rc = lib.frost_acc_noalloc(dev, C.c_void_p(stream.cuda_stream), mass.numel(), pos.shape[1], _p(pos),
+                               _p(mass), G, eps2, _p(out_acc), C.byref(err))
+    if rc != 0:
+        raise FrostError(f"frost_acc_noalloc: {lib.frost_strerror(rc).decode()} "
+                         f"(status {rc}, cudaError {err.value})")
+    return out_acc
 
 
 class Frost:

@@ -177,6 +177,7 @@ const char *frost_strerror(int status) {
         case FROST_ENOMEM: return "out of memory";
         case FROST_EDEPTH: return "hierarchy deeper than max_depth";
         case FROST_ENONFINITE: return "non-finite input";
+        case FROST_ETOOBIG: return "n exceeds FROST_NOALLOC_MAX_N (frost_acc_noalloc has a fixed static scratch)";
         default: return "unknown status";
     }
 }
