@@ -40,6 +40,8 @@ extern "C" {
 #define FROST_EDEPTH (-4)     /* frost_hhs_step recursed beyond max_depth */
 #define FROST_ENONFINITE (-5) /* reserved: non-finite input detected (debug scans) */
 #define FROST_ETOOBIG (-6)    /* frost_acc_noalloc: n exceeds FROST_NOALLOC_MAX_N (its scratch is a fixed array) */
+#define FROST_ELIMIT (-7)     /* frost_hhs_step with frost_set_split: one entry has more than 64 components of
+                                 more than 1024 particles (a fixed list; no allocation failed) */
 
 /* flags of frost_forces */
 #define FROST_ACC 1    /* compute Newtonian accelerations of the sinks */
@@ -255,7 +257,12 @@ int frost_set_overlap(frost_ctx *ctx, int on);
  * (pair-symmetric) plus the pairs of R in different components.  Components of at most 32 particles --
  * binaries, triples -- are advanced side by side, one warp each, by one batched launch per recursion
  * pass; components of up to 1024 particles one CTA each; larger ones by the host recursion.  Result: deterministic; not the numbers of
- * split_max = 0 (a different, equally fourth-order splitting of the same Hamiltonian). */
+ * split_max = 0 (a different, equally fourth-order splitting of the same Hamiltonian).
+ * Limits: the components of a split entry are classified by these fixed sizes (32 / 1024), NOT by
+ * frost_set_tuning's small_set_max -- that knob moves the hand-over of whole ENTRIES to the subtree kernel
+ * only, so small_set_max = 0 still advances components of <= 1024 particles in the batched kernels.  An
+ * entry may have at most 64 components above 1024 particles (a system of many sub-clusters can exceed
+ * this); beyond that frost_hhs_step returns FROST_ELIMIT with the particles partly advanced. */
 int frost_set_split(frost_ctx *ctx, int split_max);
 
 /* Two-body propagator for the binaries of a split level -- PAPER.md:759 lists "regularised integrators,
@@ -298,7 +305,9 @@ int frost_set_equal_mass_path(frost_ctx *ctx, int on);
  *   out_grad[i] <- 2G sum over the same j of m_j s^-5 (s^2 a_ji - 3 (x_ji.a_ji) x_ji) with the a of this call
  * for every i of the list idx (DEVICE int32[n_idx], NULL = all).  label (DEVICE int32[n_idx]) is
  * indexed by LIST POSITION; equal labels = same component, so the pair is skipped (frost_hhs_step
- * gives every slow particle -1).  out_grad nullable.  One-sided sweeps; asynchronous. */
+ * gives every slow particle -1).  out_grad nullable.  Served by the kernels frost_hhs_step uses for the
+ * debris list of a split entry: pair-symmetric masked sweeps from ~6000 list members (or whenever
+ * frost_set_symmetric mode >= 2), one-sided masked sweeps below.  Asynchronous. */
 int frost_forces_masked(frost_ctx *ctx, int n, int ld, const double *pos, const double *mass,
                         const int32_t *idx, int n_idx, const int32_t *label, double *out_acc,
                         double *out_grad);

@@ -1,6 +1,7 @@
 // frost_api.cu -- the C-ABI of include/frost.h: argument checks, scratch, and the host-side
 // sequencing of Alg. 2 (fsi) and Alg. 3 (hhs_fsi).  All arithmetic is in the kernels of
 // frost_sweeps.cu / frost_update.cu.
+#include <cstdio>
 #include <new>
 
 #include "frost_common.cuh"
@@ -167,7 +168,12 @@ int64_t frost_launch_count(const frost_ctx *c) {
     return t;
 }
 int frost_last_cuda_error(const frost_ctx *c) { return c ? c->last_cuda : 0; }
-const char *frost_version(void) { return "frost-b200 0.1 (sm_100a)"; }
+const char *frost_version(void) {
+    static char buf[192];
+    static const int n = snprintf(buf, sizeof(buf), "frost-b200 0.3 (sm_100a; pair-symmetric sweeps: %s)", frost::sym_geometry());
+    (void)n;
+    return buf;
+}
 
 const char *frost_strerror(int status) {
     switch (status) {
@@ -177,6 +183,7 @@ const char *frost_strerror(int status) {
         case FROST_ENOMEM: return "out of memory";
         case FROST_EDEPTH: return "hierarchy deeper than max_depth";
         case FROST_ENONFINITE: return "non-finite input";
+        case FROST_ELIMIT: return "more than 64 components above 1024 particles in one split entry (frost_set_split)";
         case FROST_ETOOBIG: return "n exceeds FROST_NOALLOC_MAX_N (frost_acc_noalloc has a fixed static scratch)";
         default: return "unknown status";
     }
@@ -756,6 +763,15 @@ int frost_forces_masked(frost_ctx *c, int n, int ld, const double *pos, const do
     double *xm = (double *)c->recA_xm.p, *av = (double *)c->recA_v.p;
     FROST_TRY(launch_pack_xm(c, ld, pos, mass, idx, n_idx, pad, xm, 1.0, 0, av));
     FROST_TRY(launch_pack_label(c, label, n_idx, pad, av));
+    // the same decision, and for the pair-symmetric kernels the same sequence, as the masked self sweep
+    // of R in cross_kick: accelerations, re-pack of the total accelerations beside the labels, gradient
+    if (use_sym(c, n_idx, n_idx, 0)) {
+        FROST_TRY(sym_masked(c, xm, av, n_idx, idx, ld, out_acc, nullptr, 0));
+        if (!out_grad) return FROST_OK;
+        FROST_TRY(launch_pack_vec(c, ld, out_acc, idx, n_idx, pad, av));
+        FROST_TRY(launch_pack_label(c, label, n_idx, pad, av));
+        return sym_masked(c, xm, av, n_idx, idx, ld, nullptr, out_grad, 0);
+    }
     return sweep_masked(c, xm, av, n_idx, idx, ld, out_acc, out_grad);
 }
 

@@ -196,6 +196,7 @@ int sym_timestep(frost_ctx *c, const double *xm, const double *v, int n_set, con
                  double tau_pivot, double *out_tau, int32_t *out_bin, int *forest = nullptr);
 
 int sym_potential(frost_ctx *c, const double *xm, int n, double *out_phi);
+const char *sym_geometry();   // tile geometry of the large force sweeps (frost_version)
 int sym_masked(frost_ctx *c, const double *xm, const double *a_lab, int n, const int32_t *idx, int ld,
                double *out_acc, double *out_grad, int accumulate);
 // frost_update.cu: T, U, P, L (one CTA, compensated sums, fixed order) -> out8 (device)

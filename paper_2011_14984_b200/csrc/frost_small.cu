@@ -759,10 +759,17 @@ __device__ void hhs_loop(SM &sm, SmStats &st, const SmallParams &P, const SweepP
         const int level = P.level0 + sp;
         if (stage == 0 && cnt == 2 && P.kepler && sm.f_iscomp[sp] && P.eps2 == 0.0) {
             // a two-body component of a split entry: exact two-body motion over its span (reading 25)
+            T::sync();                                    // everyone has read sm.sp before it is popped
             if (T::tid() == 0) kepler_frame(sm, st, P, sp);
             continue;
         }
-        if (stage == 0 && cnt == 2 && P.pair_path) {      // a binary: one thread, both bodies in registers
+        // a binary: one thread, both bodies in registers.  Not when its fast levels belong to the Kepler
+        // propagator: a two-body frame that is not itself a component (the root of a two-body step, a
+        // two-body F below an unsplit parent) is then split by the team path like any other entry, and
+        // its one component -- the same two bodies -- takes kepler_frame above (reading 25).
+        const bool kepler_owns_pairs = P.kepler && P.split_max >= 2 && P.eps2 == 0.0;
+        if (stage == 0 && cnt == 2 && P.pair_path && !kepler_owns_pairs) {
+            T::sync();
             if (T::tid() == 0) binary_subtree(sm, st, P, pN, pG, sp);
             continue;
         }

@@ -98,6 +98,8 @@ int split_components(frost_ctx *c, int level, int ld, const double *tau, const i
     FROST_TRY(check_launch(c));
     FROST_CUDA(c, cub::DeviceRadixSort::SortPairs(tmp, t_cub, keys, keys_s, F, C, nF, 0, bits, c->stream));
     c->launches += 2;
+    // (the scan below runs over nF entries of `sizes`, the encoder writes only the first *n_runs)
+    FROST_CUDA(c, cudaMemsetAsync(sizes, 0, (size_t)nF * sizeof(int), c->stream));
     FROST_CUDA(c, cub::DeviceRunLengthEncode::Encode(tmp, t_cub, keys_s, uniq, sizes, n_runs, nF, c->stream));
     c->launches += 2;
     FROST_CUDA(c, cub::DeviceScan::ExclusiveSum(tmp, t_cub, sizes, offs, nF, c->stream));
@@ -113,7 +115,7 @@ int split_components(frost_ctx *c, int level, int ld, const double *tau, const i
     unsigned long long ss;
     memcpy(&ss, h + 4, sizeof(ss));
     out->sumsq = (long long)ss;
-    if (out->n_big > kBigCap) return FROST_ENOMEM;       // more than 64 components above 1024 particles
+    if (out->n_big > kBigCap) return FROST_ELIMIT;       // more than 64 components above 1024 particles
     if (out->n_big > 0) {
         int2 big[kBigCap];
         FROST_CUDA(c, cudaMemcpyAsync(big, d_big, (size_t)out->n_big * sizeof(int2), cudaMemcpyDeviceToHost, c->stream));

@@ -25,6 +25,7 @@
 // diagonal block is evaluated one-sided (its B-side sums are dropped), everything beyond it
 // two-sided.  For the bipartite case (slow/fast sets of Alg. 3) every tile pair
 // is two-sided and one sweep yields both directions of acc_sf_*.
+#include <cstdio>
 #include <type_traits>
 
 // Rotation steps per iteration of the main loop of sym_kernel, and whether the Newton seed takes its low
@@ -656,23 +657,20 @@ static int run_sym(frost_ctx *c, const SymJob &job) {
 // More A particles per thread amortise the per-step SHFL / LDS / address instructions; the A tile
 // is 1024 (Newton) or 512 (gradient, time step) particles, the B tile 128.
 constexpr int kSymNT = 128, kSymMinB = 2;
-#ifndef FROST_GRAD_KA
-#define FROST_GRAD_KA 6
-#endif
-#ifndef FROST_GRAD_MINB
-#define FROST_GRAD_MINB 2
-#endif
-#ifndef FROST_NEWTON_KA
-#define FROST_NEWTON_KA 8
-#endif
-constexpr int kSymKNewton = FROST_NEWTON_KA, kSymKGrad = FROST_GRAD_KA, kSymKTau = 4;
-constexpr int kSymMinBGrad = FROST_GRAD_MINB;
-#ifndef FROST_GRAD_NT
-#define FROST_GRAD_NT 128
-#endif
-constexpr int kSymNTGrad = FROST_GRAD_NT;
+constexpr int kSymKNewton = 8, kSymKGrad = 6, kSymKTau = 4;
+constexpr int kSymMinBGrad = 2, kSymNTGrad = 128;
 // sets below kSymSmallN particles: A tiles of 256 so that there are enough tile pairs to fill the GPU
 constexpr int kSymSmallN = 16384, kSymKSmall = 2, kSymMinBSmall = 4;
+
+// The tile geometry of the large force sweeps, as text: part of frost_version(), so that a stored
+// measurement (profiles/sym_gradient_traffic.csv) can be tied to the build it was taken on.
+const char *sym_geometry() {
+    static char buf[96];
+    static const int n = snprintf(buf, sizeof(buf), "newton A%dxB%d; gradient A%dxB%d, %d CTAs/SM", kSymKNewton * kSymNT,
+                                  kSymNT, kSymKGrad * kSymNTGrad, kSymNTGrad, kSymMinBGrad);
+    (void)n;
+    return buf;
+}
 
 // Newton sweep, both directions at once (Eq. 24 / 42).  self: B == A (B arguments ignored).
 int sym_newton(frost_ctx *c, const double *A_xm, int nA, const double *B_xm, int nB, bool self,

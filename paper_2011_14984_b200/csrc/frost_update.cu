@@ -33,8 +33,9 @@ __global__ void pack_xm_kernel(const double *__restrict__ pos, const double *__r
     out[k] = r;
 }
 
-// out[k] = {p_x, p_y, p_z, 1} of particle idx[k] (accelerations or velocities); zero padding.
-// The 1 marks a real record (the time-step sweep skips records whose flag is 0).
+// out[k] = {p_x, p_y, p_z, w} of particle idx[k] (accelerations or velocities); zero padding.
+// w = 1.0, or with w_index the list position k in the low word (the time-step sweeps that enter their
+// fast pairs into a union-find forest; position 0 is a valid value, so .w is not a "real record" flag).
 __global__ void pack_vec_kernel(const double *__restrict__ planes, int ld,
                                 const int32_t *__restrict__ idx, int n_idx, int n_pad,
                                 double4 *__restrict__ out, int w_index) {

@@ -8,7 +8,7 @@ import pytest
 import torch
 
 import frost_inputs as fi
-from test_gpu_parity import (TOL_A, TOL_G, dev, envelope_ratio, momentum_change, oracle_hhs_with_envelope,
+from test_gpu_parity import (C_FWD, TOL_A, TOL_G, dev, envelope_ratio, momentum_change, oracle_hhs_with_envelope,
                              vec_err)
 
 pytestmark = pytest.mark.gpu
@@ -23,27 +23,116 @@ def fr():
     f.close()
 
 
+def masked_termsum(pos, mass, acc, idx, label_g, G, eps2, sinks):
+    """T_i of DESIGN.md reading 22 (the magnitude sum of Eq. 27's terms, as oracle_gradient_termsum forms
+    it) over the MASKED pair set, for the listed sinks.  A bound for the forward-error gate, not an
+    expected value: plain fp64 numpy."""
+    xj, mj, aj, lj = pos[:, idx], mass[idx], acc[:, idx], label_g[idx]
+    T = np.zeros(len(sinks))
+    for c0 in range(0, len(sinks), 256):
+        ii = sinks[c0:c0 + 256]
+        dx = xj[:, None, :] - pos[:, ii, None]
+        da = aj[:, None, :] - acc[:, ii, None]
+        s2 = (dx * dx).sum(0) + eps2
+        xa = (dx * da).sum(0)
+        ok = (s2 > 0) & (lj[None, :] != label_g[ii, None])
+        s2 = np.where(ok, s2, 1.0)
+        t = s2[None] * da - 3.0 * xa[None] * dx
+        T[c0:c0 + 256] = 2.0 * G * np.where(ok, mj[None, :] * np.sqrt((t * t).sum(0)) / (s2 * s2 * np.sqrt(s2)), 0.0).sum(1)
+    return T
+
+
+def check_masked(fr, oracle, pos, mass, idx, label_g, G, eps2):
+    """frost_forces_masked against oracle_forces_masked, every sink of the list: a to 1e-12 |a_i|; g to
+    1e-10 |g_i|, and where a hard binary inside the swept pair set makes Eq. 27 itself ill-conditioned
+    (reading 22) to 1e-10 |g_i| + C_FWD 2^-53 T_i with T_i over the masked pairs."""
+    n = mass.size
+    fr.set_params(G=G, eps2=eps2)
+    a_ref, g_ref = oracle.forces_masked(pos, mass, idx, label_g, G=G, eps2=eps2)
+    out_a = torch.full((3, n), 5.0, dtype=torch.float64, device="cuda")
+    out_g = torch.full((3, n), 6.0, dtype=torch.float64, device="cuda")
+    a, g = fr.forces_masked(dev(pos), dev(mass), torch.as_tensor(label_g[idx]).cuda(),
+                            idx=torch.as_tensor(idx).cuda(), out_acc=out_a, out_grad=out_g)
+    torch.cuda.synchronize()
+    fr.set_params()
+    a, g = a.cpu().numpy(), g.cpu().numpy()
+    out = np.setdiff1d(np.arange(n), idx)
+    assert (a[:, out] == 5.0).all() and (g[:, out] == 6.0).all()         # untouched outside the list
+    assert np.isfinite(a).all() and np.isfinite(g).all()
+    ea = vec_err(a[:, idx], a_ref[:, idx])
+    assert ea <= TOL_A, ea
+    d = np.abs(g - g_ref).max(0)[idx]
+    nrm = np.linalg.norm(g_ref, axis=0)[idx]
+    bad = np.nonzero(d > TOL_G * nrm)[0]
+    assert bad.size <= 4096, bad.size             # the ill-conditioned sinks are the few next to a hard binary
+    ratio = 0.0
+    if bad.size:
+        T = masked_termsum(pos, mass, a_ref, idx, label_g, G, eps2, idx[bad])
+        ratio = float((d[bad] / (TOL_G * nrm[bad] + C_FWD * 2.0 ** -53 * T)).max())
+        assert ratio <= 1.0, ratio
+    return ea, bad.size, ratio
+
+
 @pytest.mark.parametrize("n,eps2", [(700, 0.0), (5000, 0.0), (5000, 1e-6)])
 def test_masked_kick_sweeps_match_oracle(fr, oracle, n, eps2):
     """frost_forces_masked (the kick sweeps of a split entry, Eq. 42-44 on "labels differ") against
-    oracle_forces_masked on a sub-list with slow particles (-1), two-body and larger components."""
-    pos, vel, mass, pairs = fi.star_cluster(n, 4, a_lo=1e-3, a_hi=1e-2)
+    oracle_forces_masked on a sub-list with slow particles (-1), two-body and larger components; the
+    one-sided kernels (lists below ~6000), config 5's recipe at its default hardness."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4)
     rng = np.random.default_rng(n)
     idx = np.sort(rng.choice(n, size=n - n // 7, replace=False)).astype(np.int32)
     lab_pos = rng.integers(0, idx.size // 3, size=idx.size).astype(np.int32)       # ~3 members per label
     lab_pos[rng.random(idx.size) < 0.4] = -1
     label_g = np.full(n, -7, dtype=np.int32)
     label_g[idx] = lab_pos
-    fr.set_params(G=0.9, eps2=eps2)
-    a_ref, g_ref = oracle.forces_masked(pos, mass, idx, label_g, G=0.9, eps2=eps2)
-    a, g = fr.forces_masked(dev(pos), dev(mass), torch.as_tensor(lab_pos).cuda(), idx=torch.as_tensor(idx).cuda())
-    torch.cuda.synchronize()
-    fr.set_params()
-    a, g = a.cpu().numpy(), g.cpu().numpy()
-    out = np.setdiff1d(np.arange(n), idx)
-    assert (a[:, out] == 0).all() and (g[:, out] == 0).all()
-    assert vec_err(a[:, idx], a_ref[:, idx]) <= TOL_A
-    assert vec_err(g[:, idx], g_ref[:, idx]) <= TOL_G
+    fr.set_symmetric(1)
+    try:
+        check_masked(fr, oracle, pos, mass, idx, label_g, 0.9, eps2)
+    finally:
+        fr.set_symmetric(0)
+
+
+@pytest.mark.parametrize("n,eps2,labels,mib", [(129, 0.0, "random", 0), (3000, 0.0, "random", 1), (3000, 1e-6, "binaries", 0),
+                                                (9000, 0.0, "binaries", 1), (9000, 1e-6, "random", 0),
+                                                (20000, 0.0, "binaries", 1), (20000, 0.0, "random", 0),
+                                                (20000, 1e-6, "random", 1)])
+def test_masked_pair_symmetric_sweeps_match_oracle(fr, oracle, n, eps2, labels, mib, capsys):
+    """The pair-symmetric masked kernels (SymNewtonMasked / SymGradientMasked: the debris list of every
+    large split entry of frost_hhs_step) element by element against oracle_forces_masked, Eq. 42-44
+    (PAPER.md:365-387): the small-tile geometry (n < 16384) and the large one, the B list in one band and
+    in several (scratch cap 1 MiB), labels -1, two-body and large components, two coincident particles in
+    different components, with and without softening, on config 5's recipe at its default hardness.
+    labels = "binaries": every binary is one component (what a split entry produces: the hard pairs are
+    masked out); "random": labels drawn at random, so hard binaries sit INSIDE the swept pair set and the
+    sinks around them take the forward-error gate of reading 22."""
+    pos, vel, mass, pairs = fi.star_cluster(n, 4)
+    rng = np.random.default_rng(n + 1)
+    idx = np.sort(rng.choice(n, size=n - n // 9, replace=False)).astype(np.int32)
+    k = idx.size
+    lab_pos = rng.integers(0, max(k // 3, 2), size=k).astype(np.int32)             # ~3 members per label
+    lab_pos[rng.random(k) < 0.3] = -1                                              # "slow" members
+    big = rng.random(k) < 0.25
+    lab_pos[big] = k + 1                                                           # one component of ~k/4
+    label_g = np.full(n, -7, dtype=np.int32)
+    label_g[idx] = lab_pos
+    if labels == "binaries":
+        for b, (i1, i2) in enumerate(pairs):
+            label_g[i1] = label_g[i2] = 2 * k + b
+    # two coincident particles of the list in different components (reading 11: the pair adds nothing)
+    free = idx[np.isin(idx, pairs.ravel(), invert=True) & (idx > 0)]
+    i, j = free[3], free[11]
+    pos = pos.copy()
+    pos[:, j] = pos[:, i]
+    label_g[i], label_g[j] = 3 * k + 1, 3 * k + 2
+    fr.set_symmetric(2, mib)
+    l0 = fr.launch_count()
+    try:
+        ea, nbad, ratio = check_masked(fr, oracle, pos, mass, idx, label_g, 0.9, eps2)
+    finally:
+        fr.set_symmetric(0)
+    with capsys.disabled():
+        print(f"\n[masked sym n={n} eps2={eps2} {labels} cap={mib}] launches {fr.launch_count() - l0}, "
+              f"a err {ea:.1e}, sinks beyond 1e-10|g| {nbad}, worst gate ratio {ratio:.2f}")
 
 
 def _split_case(fr, oracle, pos, vel, mass, dt, small, one_cta=0, **kw):
@@ -84,8 +173,9 @@ def test_split_step_matches_split_oracle(fr, oracle, n, small, one_cta, log2dt, 
 
 def test_split_with_one_component_is_the_unsplit_step_bitwise(fr):
     """A hard binary among distant slow stars: F is the binary (one component) at every level, so the
-    split step must be Alg. 3's bits -- from the host-driven levels (small = 0) and inside the subtree
-    kernel alike."""
+    split step must be Alg. 3's bits -- with every entry driven from the host (small = 0; the components
+    themselves still run in the batched kernels: frost.h, frost_set_split) and inside the subtree kernel
+    alike."""
     b_pos, b_vel, b_mass, P = fi.kepler_binary(1.0, 0.7, 1e-3, 0.3)
     rng = np.random.default_rng(3)
     pos = np.ascontiguousarray(np.concatenate([b_pos, rng.normal(size=(3, 6)) * 3.0], axis=1))
@@ -192,6 +282,45 @@ def test_split_tiny_and_degenerate_systems(fr, oracle):
             assert np.abs(v.cpu().numpy() - vr).max() < 1e-7 * max(1.0, np.abs(vr).max())
 
 
+def test_fast_two_body_frames_take_the_kepler_propagator_on_every_path(fr, oracle):
+    """A two-body frame that is fast but not itself a component -- the root of a two-body step, or a
+    two-body F below a parent too large to be split (split_max = 2) -- is split like any entry: its one
+    component is the pair, which the Kepler propagator advances over tau/2 twice (reading 25).  The
+    one-thread binary path must not swallow such a frame: bookkeeping (n_kepler included) equal to the
+    oracle's with the pair path on and off, on the device-resident and on the host recursion."""
+    rng = np.random.default_rng(23)
+    cases = []
+    for n, split_max in ((2, BIG), (2, 2), (5, 2)):
+        pos = np.ascontiguousarray(rng.normal(size=(3, n)))
+        vel = np.ascontiguousarray(rng.normal(size=(3, n)) * 0.3)
+        mass = rng.uniform(0.5, 2.0, n)
+        r = np.array([1e-3, 2e-3, 0.0])                 # a close pair on a circular orbit
+        pos[:, 1] = pos[:, 0] + r
+        vc = np.sqrt((mass[0] + mass[1]) / np.linalg.norm(r))
+        vel[:, 1] = vel[:, 0] + vc * np.array([-r[1], r[0], 0.0]) / np.linalg.norm(r)
+        cases.append((pos, vel, mass, split_max))
+    dt = 2.0 ** -5
+    for pos, vel, mass, split_max in cases:
+        pr, vr = pos.copy(), vel.copy()
+        st_ref = oracle.hhs_step(pr, vr, mass, dt, eta_ff=0.1, eta_fb=0.1, split_max=split_max, kepler=True)
+        assert st_ref["n_kepler"] >= 2, st_ref
+        for small, pair in ((-1, 1), (-1, 0), (0, 1), (0, 0)):
+            fr.set_params(eta_ff=0.1, eta_fb=0.1)
+            fr.set_tuning(0, 0, small)
+            fr.set_split(split_max)
+            fr.set_kepler(1)
+            fr.set_pair_path(pair)
+            p, v = dev(pos), dev(vel)
+            try:
+                st = fr.hhs_step(p, v, dev(mass), dt)
+            finally:
+                fr.set_split(0); fr.set_kepler(0); fr.set_pair_path(1)
+                fr.set_tuning(0, 0, -1); fr.set_params()
+            assert st == st_ref, (mass.size, split_max, small, pair)
+            assert np.abs(p.cpu().numpy() - pr).max() < 1e-10 * max(1.0, np.abs(pr).max())
+            assert np.abs(v.cpu().numpy() - vr).max() < 1e-7 * max(1.0, np.abs(vr).max())
+
+
 def test_split_multi_step_run_conserves_like_alg3(fr, capsys):
     """Sixteen steps of a 6000-star cluster with a central mass and binaries down to a = 1e-4, with the
     fast levels split and with Alg. 3 as printed, from the same start: linear momentum at rounding
@@ -234,7 +363,8 @@ def test_split_step_with_kepler_components_matches_oracle(fr, oracle, n, small, 
     (reading 25; oracle O6k) -- bookkeeping identical to the oracle's (fewer and shallower entries, the
     same number of propagator calls), trajectory inside the oracle's 1-ulp envelope, momentum at
     rounding level: inside the subtree kernel (small = -1, n = 256), through the batched component
-    launches, and from the host recursion alone (small = 0).  dt_top = 2^-4 at n = 3000 makes level 0
+    launches, and with every entry driven from the host (small = 0; components of <= 1024 particles still
+    run in the batched kernels).  dt_top = 2^-4 at n = 3000 makes level 0
     percolate (one component of ~2800 particles beside a few small ones): the S x F + G x R + masked-R
     kick and the host recursion into the giant component, against the oracle."""
     pos, vel, mass, pairs = fi.star_cluster(n, 4, e_max=0.1)
