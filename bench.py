@@ -48,17 +48,20 @@ METRIC = "pair interactions/s (acc+gradient, fp64) at N=2^20"
 UNIT = "pair interactions/s"
 
 
-def _sweep_traffic(one_sided, n):
+def _sweep_traffic(variant, n, version):
     """dram__bytes_read.sum + dram__bytes_write.sum of one whole gradient sweep (all its band launches
-    and reductions) from the committed ncu --set full capture, if one exists for this configuration;
-    else None.  profiles/sym_gradient_traffic.csv: n,one_sided,dram_bytes,source."""
+    and reductions) from a committed ncu capture -- only if that capture was taken on the same size, the
+    same kernel variant (eqmass | general | one_sided) and the same tile geometry as the running build
+    (the geometry is part of frost_version()); else None with the reason.
+    profiles/sym_gradient_traffic.csv: n,variant,geometry,dram_bytes,source."""
     path = os.path.join(ROOT, "profiles", "sym_gradient_traffic.csv")
     if os.path.exists(path):
         for ln in open(path):
-            f = [x.strip() for x in ln.split(",")]
-            if len(f) >= 4 and f[0].isdigit() and int(f[0]) == n and int(f[1]) == int(bool(one_sided)):
-                return float(f[2]), f[3]
-    return None, "no ncu capture committed for this configuration (see profiles/)"
+            f = [x.strip() for x in ln.split(",", 4)]
+            if len(f) >= 5 and f[0].isdigit() and int(f[0]) == n and f[1] == variant \
+                    and f[2].replace(",", "") in version.replace(",", ""):
+                return float(f[3]), f[4]
+    return None, f"no ncu capture committed for n={n}, variant={variant}, build '{version}' (see profiles/)"
 
 
 def _peaks():
@@ -168,8 +171,8 @@ def run_reference(args):
 
 def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
     """Side measurements of the other SURVEY.md 8(a) rows (not part of `value`): the time-step sweep
-    on config 2 and the HBM-bound O(N) kernels at N = 2^20 (L2 flushed before every timed launch;
-    algorithmic bytes per particle as in DESIGN.md)."""
+    on config 2, the HBM-bound O(N) kernels at N = 2^20 (algorithmic bytes per particle as in DESIGN.md),
+    and a timed row with its oracle error for each of BASELINE.json's configs 1, 2, 4 and 5."""
     def ev():
         return torch.cuda.Event(enable_timing=True)
 
@@ -192,31 +195,165 @@ def measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=True):
     bins = torch.empty(n2, dtype=torch.int32, device=dev)
     ms = best(lambda: fr.timesteps(p, v, m, tau_pivot=1.0 / 128, out_tau=tau, out_bin=bins), 3, False)
     out["timestep_sweep_config2"] = {"n": n2, "ms": ms, "pairs_per_s": float(n2) * n2 / (ms * 1e-3)}
+    # O(N) kernels at N = 2^20: kReps launches back to back inside ONE event pair, each on its own set of
+    # buffers (kSets x 24-32 MB per operand >> 126 MB of L2 in total, so every launch streams from HBM);
+    # the launch gaps are inside the timed region, as they are in a step
     n = 1 << 20
-    x = torch.randn((3, n), dtype=torch.float64, device=dev)
-    w = torch.randn((3, n), dtype=torch.float64, device=dev)
-    a = torch.randn((3, n), dtype=torch.float64, device=dev)
-    g = torch.randn((3, n), dtype=torch.float64, device=dev)
-    mm = torch.rand(n, dtype=torch.float64, device=dev)
-    rec = torch.empty((n, 4), dtype=torch.float64, device=dev)
+    kSets, kReps = 8, 24
+    mk = lambda: [torch.randn((3, n), dtype=torch.float64, device=dev) for _ in range(kSets)]
+    xs, ws, as_, gs = mk(), mk(), mk(), mk()
+    mms = [torch.rand(n, dtype=torch.float64, device=dev) for _ in range(kSets)]
+    recs = [torch.empty((n, 4), dtype=torch.float64, device=dev) for _ in range(kSets)]
     lib, h = fr.lib, fr.h
     import ctypes as C
     P = lambda t: C.c_void_p(t.data_ptr())
     cases = {
-        "kick_with_gradient": (96, lambda: fr.kick(w, a, g, c=1e-9, kappa=1e-9)),
-        "kick": (72, lambda: fr.kick(w, a, None, c=1e-9, kappa=0.0)),
-        "drift": (72, lambda: fr.drift(x, w, c=1e-12)),
-        "gather_pack": (64, lambda: lib.frost_gather_pack(h, n, n, P(x), P(mm), None, 0, n, P(rec))),
+        "kick_with_gradient": (96, lambda k: fr.kick(ws[k], as_[k], gs[k], c=1e-9, kappa=1e-9)),
+        "kick": (72, lambda k: fr.kick(ws[k], as_[k], None, c=1e-9, kappa=0.0)),
+        "drift": (72, lambda k: fr.drift(xs[k], ws[k], c=1e-12)),
+        "gather_pack": (64, lambda k: lib.frost_gather_pack(h, n, n, P(xs[k]), P(mms[k]), None, 0, n, P(recs[k]))),
     }
     for name, (bpp, f) in cases.items():
-        ms = best(f)
+        def many():
+            for r in range(kReps):
+                f(r % kSets)
+        ms = best(many, 3) / kReps
         gbs = n * bpp / (ms * 1e-3) / 1e9
         out[name] = {"n": n, "us": ms * 1e3, "bytes_per_particle": bpp, "GB_per_s": gbs,
-                     "frac_of_hbm_peak": gbs / hbm_peak}
+                     "frac_of_hbm_peak": gbs / hbm_peak,
+                     "timing": f"{kReps} back-to-back launches over {kSets} rotating buffer sets, one event pair"}
+    del xs, ws, as_, gs, mms, recs
+    out.update(config_rows(fr, frost, torch, dev, flush))
     if hhs:
         out["hhs_step_config5"] = hhs_config5(fr, torch, dev)
         out["hhs_step_config5_split"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5)
         out["hhs_step_config5_split_kepler"] = hhs_config5(fr, torch, dev, split_max=SPLIT_MAX_CONFIG5, kepler=1)
+    return out
+
+
+def _rel_err(x, ref):
+    return float((np.abs(x - ref).max(0) / np.linalg.norm(ref, axis=0)).max())
+
+
+def config_rows(fr, frost, torch, dev, flush):
+    """Driver-timed rows for BASELINE.json's configs 1, 2 and 4 (config 3 is the headline, config 5 the
+    hhs_step_* rows), each with its error against the oracle on a sample so that the number carries its
+    validity.  CUDA events on the context's stream; best of 3 after a warm-up call."""
+    import oracle
+    SLOT_PEAK = SM_COUNT * FP64_LANES_PER_SM * _peaks()[1] * 1e6
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    def timed(f, reps=3, do_flush=False):
+        f(); torch.cuda.synchronize()
+        ts = []
+        for _ in range(reps):
+            if do_flush:
+                flush.fill_(1.0)
+            a, b = ev(), ev()
+            l0 = fr.launch_count()
+            a.record(); f(); b.record(); torch.cuda.synchronize()
+            ts.append((a.elapsed_time(b), fr.launch_count() - l0))
+        return min(ts)
+
+    T = lambda x: torch.as_tensor(np.ascontiguousarray(x)).to(dev)
+    out = {}
+    fr.set_params(G=1.0, eps2=0.0)
+
+    # ---- config 1: N = 1024, seed 0: one acc+gradient evaluation; 10 FSI steps, dt = 1/1024 ----------
+    n1, dt1 = 1024, 1.0 / 1024
+    pos, vel, mass = fi.plummer(n1, 0)
+    p, v, m = T(pos), T(vel), T(mass)
+    acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+    ms, nl = timed(lambda: fr.forces(p, m, out_acc=acc, out_grad=grad), 5)
+    a_ref, g_ref = oracle.forces(pos, mass)
+    row = {"n": n1, "acc_grad_us": ms * 1e3, "acc_grad_launches": int(nl),
+           "acc_rel_err": _rel_err(acc.cpu().numpy(), a_ref), "grad_rel_err": _rel_err(grad.cpu().numpy(), g_ref)}
+    pr, vr = pos.copy(), vel.copy()
+    for _ in range(10):
+        oracle.fsi_step(pr, vr, mass, dt1)
+    for name, small in (("resident", -1), ("streaming", 0)):
+        fr.set_tuning(0, 0, small)
+        state = {}
+
+        def ten():
+            state["p"], state["v"] = p.clone(), v.clone()
+            fr.fsi_steps(state["p"], state["v"], m, dt1, 10)
+        ms, nl = timed(ten, 3)          # (two 24 KB clones inside the timed region: < 1 % of either path)
+        row[f"fsi10_{name}_us_per_step"] = ms * 1e2
+        row[f"fsi10_{name}_launches"] = int(nl)
+        row[f"fsi10_{name}_max_abs_dx_vs_oracle"] = float(np.abs(state["p"].cpu().numpy() - pr).max())
+    fr.set_tuning(0, 0, -1)
+    out["config1_n1024"] = row
+
+    # ---- config 2: N = 65536, seed 1: full self acc+gradient pass (the time-step pass is its own row) --
+    n2 = 65536
+    pos, vel, mass = fi.plummer(n2, 1)
+    p, m = T(pos), T(mass)
+    acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+    ms, nl = timed(lambda: fr.forces(p, m, out_acc=acc, out_grad=grad), 3, True)
+    s = fi.active_subset(n2, 256 / n2, 101)
+    a_r = np.zeros((3, n2)); g_r = np.zeros((3, n2))
+    oracle.forces(pos, mass, sink_idx=s, flags=oracle.ACC, acc=a_r, grad=g_r)
+    a_in = acc.cpu().numpy().copy()
+    oracle.forces(pos, mass, sink_idx=s, flags=oracle.GRAD, acc=a_in, grad=g_r)
+    pairs = float(n2) * n2
+    out["config2_acc_grad_n65536"] = {
+        "n": n2, "ms": ms, "launches": int(nl), "pairs_per_s": pairs / (ms * 1e-3),
+        "fp64_pipe_frac_at_max_clock": pairs * (SLOTS_NEWTON_EQ + SLOTS_GRAD_EQ) / (ms * 1e-3) / SLOT_PEAK,
+        "acc_rel_err_256_sinks": _rel_err(acc.cpu().numpy()[:, s], a_r[:, s]),
+        "grad_rel_err_256_sinks": _rel_err(grad.cpu().numpy()[:, s], g_r[:, s])}
+
+    # ---- config 4: N = 2^20, seed 3: active subset A (0.1 / 1 / 10 %), pair set {i in A or j in A} ------
+    n4, dt4 = 1 << 20, 1.0 / 1024
+    pos, vel, mass = fi.plummer(n4, 3)
+    p, m, v0 = T(pos), T(mass), T(vel)
+    rows4 = {}
+    for frac in (0.001, 0.01, 0.1):
+        A = fi.active_subset(n4, frac, 3)
+        rest = np.setdiff1d(np.arange(n4, dtype=np.int32), A).astype(np.int32)
+        dA, dR = T(A), T(rest)
+        acc = torch.zeros_like(p); grad = torch.zeros_like(p)
+
+        def one_directional():      # A <- all, rest <- A (one-sided kernels with source slices)
+            fr.forces(p, m, sink_idx=dA, source_idx=None, out_acc=acc, out_grad=grad, flags=frost.ACC)
+            fr.forces(p, m, sink_idx=dR, source_idx=dA, out_acc=acc, out_grad=grad, flags=frost.ACC)
+            fr.forces(p, m, sink_idx=dA, source_idx=None, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+            fr.forces(p, m, sink_idx=dR, source_idx=dA, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+
+        def self_plus_mutual():     # self(A) + mutual(A, rest) with FROST_ACCUMULATE (pair-symmetric kernels)
+            acc.zero_(); grad.zero_()   # (the accumulating piece adds to whatever the rest holds)
+            fr.forces(p, m, dA, dA, out_acc=acc, out_grad=grad, flags=frost.ACC)
+            fr.forces(p, m, dA, dR, out_acc=acc, out_grad=grad, flags=frost.ACC | frost.MUTUAL | frost.ACCUMULATE)
+            fr.forces(p, m, dA, dA, out_acc=acc, out_grad=grad, flags=frost.GRAD)
+            fr.forces(p, m, dA, dR, out_acc=acc, out_grad=grad, flags=frost.GRAD | frost.MUTUAL | frost.ACCUMULATE)
+
+        # ordered pairs of the set: A x all (minus self) + rest x A
+        pairs = float(A.size) * n4 + float(rest.size) * A.size
+        sA, sR = A[:: max(1, A.size // 64)][:64], rest[:: rest.size // 64][:64]
+        a_ref = np.zeros((3, n4)); g_ref = np.zeros((3, n4))
+        oracle.forces(pos, mass, sink_idx=sA, source_idx=None, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+        oracle.forces(pos, mass, sink_idx=sR, source_idx=A, flags=oracle.ACC, acc=a_ref, grad=g_ref)
+        ss = np.concatenate([sA, sR])
+        r = {"n_active": int(A.size), "ordered_pairs": pairs}
+        for name, f in (("one_directional", one_directional), ("self_plus_mutual", self_plus_mutual)):
+            ms, nl = timed(f, 2, True)
+            a = acc.cpu().numpy()
+            a_in = a.copy()
+            oracle.forces(pos, mass, sink_idx=sA, source_idx=None, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+            oracle.forces(pos, mass, sink_idx=sR, source_idx=A, flags=oracle.GRAD, acc=a_in, grad=g_ref)
+            vk = v0.clone()
+            fr.kick(vk, acc, grad, idx=None, c=2 * dt4 / 3, kappa=dt4 * dt4 / 48)
+            dv = vk.cpu().numpy() - vel
+            r[name] = {"ms": ms, "launches": int(nl), "pairs_per_s": pairs / (ms * 1e-3),
+                       "acc_rel_err_128_sinks": _rel_err(a[:, ss], a_ref[:, ss]),
+                       "grad_rel_err_128_sinks": _rel_err(grad.cpu().numpy()[:, ss], g_ref[:, ss]),
+                       "sum_m_dv_over_sum_m_abs_dv": float(np.abs((mass * dv).sum(1)).max() /
+                                                           (mass * np.abs(dv)).sum(1).max())}
+        rows4[f"active_{frac:g}"] = r
+    out["config4_active_subsets_n2pow20"] = rows4
+    fr.set_params()
     return out
 
 
@@ -402,9 +539,14 @@ def run_frost(args):
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.same_device:
+        local = 0            # every rank on cuda:0 (one-GPU execution of the N > 1 path; needs --backend gloo)
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")      # exchanges staged through the host (sharding.py)
     n, seed, dt = args.n, 2, 1.0 / 1024
     hbm_peak, sm_max_mhz, peak_src = _peaks()
 
@@ -436,10 +578,9 @@ def run_frost(args):
     def ev():
         return torch.cuda.Event(enable_timing=True)
 
-    def step(record=None):
-        """One pass of the path; returns nothing, records events if asked."""
-        e = [ev() for _ in range(4)] if record is not None else None
-        if e: e[0].record()
+    def force_pass(pos, acc, grad, e=None):
+        """Newton sweep, exchange of a, gradient sweep, exchange of g: this rank's share of the pairs
+        (or of the sinks) and the one real exchange step of the path after each sweep."""
         fr.forces(pos, mass, sink_idx=sink_idx, source_idx=None, out_acc=acc, out_grad=grad,
                   flags=frost.ACC)
         if pair_sharded:
@@ -451,6 +592,12 @@ def run_frost(args):
                   flags=frost.GRAD)
         if pair_sharded:
             sharding.all_reduce_planes(grad, world)
+
+    def step(record=None):
+        """One pass of the path; returns nothing, records events if asked."""
+        e = [ev() for _ in range(4)] if record is not None else None
+        if e: e[0].record()
+        force_pass(pos, acc, grad, e)
         if e: e[2].record()
         fr.kick(vel, acc, grad, idx=sink_idx, c=2.0 * dt / 3.0, kappa=dt * dt / 48.0)
         fr.drift(pos, vel, idx=sink_idx, c=dt / 2.0)
@@ -484,10 +631,13 @@ def run_frost(args):
     t_newton = [e[0].elapsed_time(e[1]) for e in recs]
     t_grad = [e[1].elapsed_time(e[2]) for e in recs]
     t_upd = [e[2].elapsed_time(e[3]) for e in recs]
-    total_ms = torch.tensor([sum(t_step)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_ms = float(total_ms.item())
+    def max_over_ranks(x):
+        t = torch.tensor([x], dtype=torch.float64, device=dev if args.backend == "nccl" else "cpu")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    total_ms = max_over_ranks(sum(t_step))
     pairs_step = float(n) * float(n)
     value = pairs_step * args.steps / (total_ms * 1e-3)
 
@@ -509,8 +659,44 @@ def run_frost(args):
                "d2h_bytes_per_step": int(ha.numel() * 8 + hg.numel() * 8),
                "steps": len(ts), "ms_per_step": float(np.mean(ts)) * 1e3}
 
+    if world > 1:
+        # N > 1: the state is replicated, so every rank copies pos and mass from its pinned host buffers,
+        # sweeps its share, takes part in the two exchanges, and rank 0 reads a and g back; wall clock
+        # between barriers, max over ranks
+        hp = torch.as_tensor(pos_h).pin_memory(); hm = torch.as_tensor(mass_h).pin_memory()
+        ha = torch.zeros((3, n), dtype=torch.float64).pin_memory()
+        hg = torch.zeros((3, n), dtype=torch.float64).pin_memory()
+        dp = torch.empty_like(pos0)
+        da, dg = torch.zeros_like(pos0), torch.zeros_like(pos0)
+        ts = []
+        for it in range(1 + max(1, args.e2e_steps)):
+            flush.fill_(1.0); barrier()
+            t0 = time.perf_counter()
+            dp.copy_(hp, non_blocking=True); mass.copy_(hm, non_blocking=True)
+            force_pass(dp, da, dg)
+            if rank == 0:
+                ha.copy_(da, non_blocking=True); hg.copy_(dg, non_blocking=True)
+            barrier()
+            if it > 0:
+                ts.append(max_over_ranks(time.perf_counter() - t0))
+        e2e = {"value": pairs_step / float(np.mean(ts)), "unit": UNIT,
+               "h2d_bytes_per_step": int(world * (hp.numel() + hm.numel()) * 8),
+               "d2h_bytes_per_step": int((ha.numel() + hg.numel()) * 8),
+               "steps": len(ts), "ms_per_step": float(np.mean(ts)) * 1e3,
+               "note": "per-rank H2D of the replicated state + sharded sweeps + exchanges + D2H on rank 0"}
+        # every rank: the sharded pass at the ORIGINAL positions (rank 0 compares it with the oracle and
+        # with the unsharded pass below; --dump-dir keeps every rank's copy for tests/)
+        a_sh, g_sh = torch.zeros_like(pos0), torch.zeros_like(pos0)
+        force_pass(pos0, a_sh, g_sh)
+        torch.cuda.synchronize()
+        if args.dump_dir:
+            os.makedirs(args.dump_dir, exist_ok=True)
+            np.savez(os.path.join(args.dump_dir, f"rank{rank}.npz"), acc=a_sh.cpu().numpy(), grad=g_sh.cpu().numpy(),
+                     lo=lo, hi=hi)
+
     if rank != 0:
         if world > 1:
+            dist.barrier()                       # stay until rank 0 has printed its line
             dist.destroy_process_group()
         return
 
@@ -530,14 +716,17 @@ def run_frost(args):
     g_ms = float(np.mean(t_grad)); n_ms = float(np.mean(t_newton))
     sinks_here = hi - lo
     pairs_rank = float(n) * n / world if pair_sharded else float(sinks_here) * n
+    variant = "general"
     if args.one_sided:      # forced: the one-sided sweeps run
+        variant = "one_sided"
         slots_n, slots_g, kname = SLOTS_NEWTON_1S, SLOTS_GRAD_1S, "sweep_kernel<GradientPolicy> (one-sided gradient sweep, Eq. 27)"
     elif bool((mass_h == mass_h[0]).all()) and not args.no_eqmass:
+        variant = "eqmass"
         slots_n, slots_g = SLOTS_NEWTON_EQ, SLOTS_GRAD_EQ
         kname = "sym_kernel<SymGradientFastT<true>> (pair-symmetric gradient sweep, Eq. 27; equal-mass variant, no coincidence guard)"
     else:
         slots_n, slots_g, kname = SLOTS_NEWTON, SLOTS_GRAD, "sym_kernel<SymGradientFastT<false>> (pair-symmetric gradient sweep, Eq. 27)"
-    traffic, traffic_src = _sweep_traffic(args.one_sided, n)
+    traffic, traffic_src = _sweep_traffic(variant, n, fr.lib.frost_version().decode())
     # measured FP64 rate of this run's probe (MEASURED_PEAKS.json carries no fp64 entry): a DFMA with two
     # loop-invariant operands issues every 2 cycles, i.e. thread instructions/s x 2 flop
     peak_measured = probe.get("dfma_thread_inst_per_s", 0.0) * 2 / 1e12
@@ -585,6 +774,12 @@ def run_frost(args):
         ea = (np.abs(a_g[:, s] - a_r[:, s]).max(0) / np.linalg.norm(a_r[:, s], axis=0)).max()
         eg = (np.abs(g_chk.cpu().numpy()[:, s] - g_r[:, s]).max(0) / np.linalg.norm(g_r[:, s], axis=0)).max()
         cpu["parity_on_256_sampled_sinks"] = {"acc_rel_err": float(ea), "grad_rel_err": float(eg)}
+        if world > 1:      # the sharded + exchanged pass of this rank against the same oracle sample
+            own = s if pair_sharded else s[(s >= lo) & (s < hi)]
+            cpu["parity_of_the_sharded_pass"] = {
+                "acc_rel_err": float((np.abs(a_sh.cpu().numpy()[:, s] - a_r[:, s]).max(0) / np.linalg.norm(a_r[:, s], axis=0)).max()),
+                "grad_rel_err": float((np.abs(g_sh.cpu().numpy()[:, own] - g_r[:, own]).max(0) /
+                                       np.linalg.norm(g_r[:, own], axis=0)).max()) if own.size else None}
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": total_ms / args.steps, "higher_is_better": True,
@@ -595,7 +790,8 @@ def run_frost(args):
                       "parallelism": "1 GPU" if world == 1 else (
                           f"tile pairs of the symmetric sweeps sharded over {world} ranks, all-reduce of a "
                           "and of g" if pair_sharded else
-                          f"sinks sharded over {world} ranks, all-gather of a between the sweeps")},
+                          f"sinks sharded over {world} ranks, all-gather of a between the sweeps"),
+                      "backend": None if world == 1 else args.backend + (", all ranks on cuda:0" if args.same_device else "")},
            "gflops": value * (FLOPS_NEWTON + FLOPS_GRAD) / 1e9,
            "flops_convention": "Newton 18 + gradient 34 = 52 flops per ordered pair (FMA=2, add/mul=1, rsqrt=1)",
            "breakdown_ms": {"newton+pack+reduce": n_ms, "gradient+pack+reduce": g_ms,
@@ -604,8 +800,9 @@ def run_frost(args):
            "cpu_baseline": cpu, "e2e": e2e}
     if world == 1 and not args.no_rows:
         out["other_rows"] = measure_rows(fr, frost, torch, dev, flush, hbm_peak, hhs=not args.no_hhs)
-    print(json.dumps(out))
+    print(json.dumps(out), flush=True)
     if world > 1:
+        dist.barrier()
         dist.destroy_process_group()
 
 
@@ -614,12 +811,17 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--n", type=int, default=1 << 20)
+    ap.add_argument("--n", "--particles", dest="n", type=int, default=1 << 20)
     ap.add_argument("--impl", default="frost", choices=["frost", "reference"])
     ap.add_argument("--cpu-sinks", type=int, default=6144)
     ap.add_argument("--one-sided", action="store_true", help="force the one-sided sweeps (no pair symmetry)")
     ap.add_argument("--ref-sinks", type=int, default=1024)
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="process-group backend for --gpus N > 1 (gloo: exchanges staged through the host)")
+    ap.add_argument("--same-device", action="store_true",
+                    help="all ranks on cuda:0 (executes the N > 1 path on a one-GPU box; needs --backend gloo)")
+    ap.add_argument("--dump-dir", default="", help="N > 1: every rank saves its sharded acc / grad at the initial positions here")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-rows", action="store_true", help="skip the side measurements of the O(N) rows")
     ap.add_argument("--no-hhs", action="store_true", help="skip the config-5 HHS-FSI step (about 15 s)")
@@ -632,6 +834,8 @@ def main():
     ap.add_argument("--hhs-arm", default="both", choices=["both", "alg3", "split"],
                     help="--hhs-only: Alg. 3 as printed, the split fast levels (frost_set_split), or both")
     args = ap.parse_args()
+    if args.same_device and args.backend != "gloo":
+        ap.error("--same-device needs --backend gloo (NCCL refuses two ranks on one device)")
     if args.probe:
         return run_probe()
     if args.rows_only:
@@ -649,7 +853,11 @@ def main():
             sk.bind(("127.0.0.1", 0))
             port = sk.getsockname()[1]
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
-               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)]
+        # (torch.distributed.run's own parser rejects "--n" even behind the script name: it is an ambiguous
+        #  prefix of --nnodes / --nproc-per-node / ...; the long spelling is not)
+        cmd += ["--particles" if a == "--n" else a.replace("--n=", "--particles=", 1) if a.startswith("--n=") else a
+                for a in sys.argv[1:]]
         env = dict(os.environ)
         env.setdefault("NCCL_DEBUG", "INFO")              # the communicator log shows the N ranks ...
         env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")

@@ -103,6 +103,59 @@ __global__ void drift_kernel(double *__restrict__ pos, const double *__restrict_
     }
 }
 
+// Dense lists (idx == NULL): y[i] = fma(c, GRAD ? fma(kappa, g[i], x[i]) : x[i], y[i]) on the three planes --
+// the kick (y = vel, x = acc, g = grad) and the drift (y = pos, x = vel) -- with four particles per thread
+// (kDenseU = 2; two with the gradient term, whose third operand would otherwise cost the occupancy) as
+// 16-byte accesses, every load issued before the first store.  Measured at N = 2^20, back to back over
+// rotating buffers (bench.py other_rows; profiles/rows_ncu_r3.md): see there.  Same fma per element as the
+// one-particle kernels: same bits.  The gather/pack kernel stays one record per thread: two records per
+// thread store 64 contiguous bytes as strided 16-byte pieces and measured 15 % slower.
+// n2 = n / 2 double2 per plane; an odd last particle is done by thread 0 of block 0.
+constexpr int kDenseNT = 256;
+template <bool GRAD, int kDenseU>
+__global__ void __launch_bounds__(kDenseNT) update_dense_kernel(double *__restrict__ y, const double *__restrict__ x,
+                                                               const double *__restrict__ g, int ld, int n,
+                                                               double c, double kappa) {
+    const int n2 = n >> 1, ld2 = ld >> 1;
+    const int k0 = blockIdx.x * (kDenseNT * kDenseU) + threadIdx.x;
+    double2 vy[3][kDenseU], vx[3][kDenseU], vg[3][kDenseU];
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+        for (int u = 0; u < kDenseU; ++u) {
+            const int k = k0 + u * kDenseNT;
+            if (k < n2) {
+                const size_t o = (size_t)d * ld2 + k;
+                vx[d][u] = reinterpret_cast<const double2 *>(x)[o];
+                if (GRAD) vg[d][u] = reinterpret_cast<const double2 *>(g)[o];
+                vy[d][u] = reinterpret_cast<const double2 *>(y)[o];
+            }
+        }
+#pragma unroll
+    for (int d = 0; d < 3; ++d)
+#pragma unroll
+        for (int u = 0; u < kDenseU; ++u) {
+            const int k = k0 + u * kDenseNT;
+            if (k < n2) {
+                double2 a = vx[d][u];
+                if (GRAD) { a.x = fma(kappa, vg[d][u].x, a.x); a.y = fma(kappa, vg[d][u].y, a.y); }
+                double2 r;
+                r.x = fma(c, a.x, vy[d][u].x); r.y = fma(c, a.y, vy[d][u].y);
+                reinterpret_cast<double2 *>(y)[(size_t)d * ld2 + k] = r;
+            }
+        }
+    if ((n & 1) && blockIdx.x == 0 && threadIdx.x == 0) {
+        const int i = n - 1;
+#pragma unroll
+        for (int d = 0; d < 3; ++d) {
+            const size_t o = (size_t)d * ld + i;
+            double a = x[o];
+            if (GRAD) a = fma(kappa, g[o], a);
+            y[o] = fma(c, a, y[o]);
+        }
+    }
+}
+
 __global__ void iota_kernel(int32_t *__restrict__ out, int n, int k0) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k < n) out[k] = k0 + k;
@@ -238,6 +291,12 @@ diag_kernel(const double *__restrict__ pos, const double *__restrict__ vel, cons
 }
 
 // ---- launchers ---------------------------------------------------------------------------------
+// The dense kernels need an even plane stride and 16-byte aligned planes; lists below kDenseMin particles
+// keep the one-particle kernels (more CTAs to spread over the SMs).
+constexpr int kDenseMin = 65536;
+static bool dense_ok(int ld, const void *a, const void *b, const void *c3) {
+    return (ld & 1) == 0 && (((uintptr_t)a | (uintptr_t)b | (uintptr_t)c3) & 15u) == 0;
+}
 int launch_pack_xm(frost_ctx *c, int ld, const double *pos, const double *mass, const int32_t *idx,
                    int n_idx, int n_pad, double *out, double wscale, int nan_pad, double *zero_tail,
                    int *eq_flag, const int32_t *eq_ref) {
@@ -265,8 +324,14 @@ int launch_pack_label(frost_ctx *c, const int *lab, int n_idx, int n_pad, double
 int launch_kick(frost_ctx *c, int ld, double *vel, const double *acc, const double *grad,
                 const int32_t *idx, int n_idx, double cc, double kappa) {
     if (n_idx <= 0) return FROST_OK;
-    kick_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(vel, acc, kappa != 0.0 ? grad : nullptr,
-                                                          ld, idx, n_idx, cc, kappa);
+    const double *g = kappa != 0.0 ? grad : nullptr;
+    if (!idx && n_idx >= kDenseMin && dense_ok(ld, vel, acc, g)) {
+        const int n2 = n_idx >> 1;
+        if (g) update_dense_kernel<true, 1><<<(n2 + kDenseNT - 1) / kDenseNT, kDenseNT, 0, c->stream>>>(vel, acc, g, ld, n_idx, cc, kappa);
+        else update_dense_kernel<false, 2><<<(n2 + 2 * kDenseNT - 1) / (2 * kDenseNT), kDenseNT, 0, c->stream>>>(vel, acc, nullptr, ld, n_idx, cc, 0.0);
+        return check_launch(c);
+    }
+    kick_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(vel, acc, g, ld, idx, n_idx, cc, kappa);
     return check_launch(c);
 }
 
@@ -281,6 +346,11 @@ int launch_kick_drift(frost_ctx *c, int ld, double *pos, double *vel, const doub
 int launch_drift(frost_ctx *c, int ld, double *pos, const double *vel, const int32_t *idx,
                  int n_idx, double cc) {
     if (n_idx <= 0) return FROST_OK;
+    if (!idx && n_idx >= kDenseMin && dense_ok(ld, pos, vel, nullptr)) {
+        const int n2 = n_idx >> 1;
+        update_dense_kernel<false, 2><<<(n2 + 2 * kDenseNT - 1) / (2 * kDenseNT), kDenseNT, 0, c->stream>>>(pos, vel, nullptr, ld, n_idx, cc, 0.0);
+        return check_launch(c);
+    }
     drift_kernel<<<(n_idx + 255) / 256, 256, 0, c->stream>>>(pos, vel, ld, idx, n_idx, cc);
     return check_launch(c);
 }

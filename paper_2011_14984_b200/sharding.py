@@ -27,6 +27,12 @@ def shard_range(n: int, rank: int, world: int) -> Tuple[int, int]:
     return lo, lo + base + (1 if rank < rem else 0)
 
 
+def _staged_through_host(t: torch.Tensor) -> bool:
+    """gloo moves host memory: a CUDA tensor is exchanged through a host copy (the backend used to run
+    several ranks on ONE device, bench.py --backend gloo --same-device; NCCL exchanges device memory)."""
+    return t.is_cuda and dist.get_backend() == "gloo"
+
+
 def all_gather_planes(local: torch.Tensor, n: int, rank: int, world: int,
                       out: torch.Tensor) -> torch.Tensor:
     """Assemble out[:, 0:n] from every rank's block out[:, lo:hi]; `local` is this rank's (3, hi-lo)."""
@@ -36,7 +42,8 @@ def all_gather_planes(local: torch.Tensor, n: int, rank: int, world: int,
         return out
     sizes = [shard_range(n, r, world) for r in range(world)]
     blk = max(hi - lo for lo, hi in sizes)
-    send = torch.zeros((3, blk), dtype=local.dtype, device=local.device)
+    dev = torch.device("cpu") if _staged_through_host(local) else local.device
+    send = torch.zeros((3, blk), dtype=local.dtype, device=dev)
     send[:, : local.shape[1]] = local
     recv = [torch.empty_like(send) for _ in range(world)]
     dist.all_gather(recv, send)
@@ -63,7 +70,12 @@ def sharded_acc_grad(n: int, rank: int, world: int, acc_fn: Callable, grad_fn: C
 def all_reduce_planes(t: torch.Tensor, world: int) -> torch.Tensor:
     """Sum the partial planes of all ranks in place (NCCL on GPUs, gloo in the CPU test)."""
     if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
+        if _staged_through_host(t):
+            h = t.cpu()
+            dist.all_reduce(h, op=dist.ReduceOp.SUM)
+            t.copy_(h)
+        else:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM)
     return t
 
 

@@ -235,6 +235,48 @@ def test_kick_drift_gather(fr, oracle):
     assert (rec[idx.size:] == 0).all()
 
 
+@pytest.mark.parametrize("n,ld", [(65536, 65536), (70001, 70002), (70001, 70001), (200003, 200010)])
+def test_dense_update_kernels_are_bitwise_the_indexed_ones(fr, oracle, n, ld):
+    """Dense lists (idx = None) of >= 65536 particles take the four-particles-per-thread kernels with
+    16-byte accesses (even plane stride; an odd stride keeps the one-particle kernels): kick with and
+    without the gradient term, drift and gather/pack must give the bits of the one-particle kernels --
+    reached through the explicit index list 0..n-1 -- and the oracle's values, for even and odd n,
+    leaving the entries n..ld-1 untouched."""
+    rng = np.random.default_rng(n)
+    mk = lambda: np.ascontiguousarray(rng.normal(size=(3, ld)))
+    pos, vel, acc, grad = mk(), mk(), mk(), mk()
+    mass = rng.uniform(0.5, 2.0, n)
+    iota = torch.arange(n, dtype=torch.int32, device="cuda")
+    m = dev(mass)
+    out = {}
+    for name, ii in (("dense", None), ("indexed", iota)):
+        v, p, a, g = dev(vel), dev(pos), dev(acc), dev(grad)
+        lib = fr.lib
+        import ctypes as C
+        P = lambda t: None if t is None else C.c_void_p(t.data_ptr())
+        # (through the C-ABI directly: the binding passes ld for n)
+        assert lib.frost_kick(fr.h, n, ld, P(v), P(a), P(g), P(ii), n, 0.37, 0.011) == 0
+        assert lib.frost_kick(fr.h, n, ld, P(v), P(a), None, P(ii), n, -0.2, 0.0) == 0
+        assert lib.frost_drift(fr.h, n, ld, P(p), P(v), P(ii), n, 0.21) == 0
+        rec = torch.full((n + 5, 4), 7.0, dtype=torch.float64, device="cuda")
+        assert lib.frost_gather_pack(fr.h, n, ld, P(p), P(m), None if ii is None else P(ii), n, n + 5, P(rec)) == 0
+        torch.cuda.synchronize()
+        out[name] = (v, p, rec)
+    for a, b in zip(out["dense"], out["indexed"]):
+        assert torch.equal(a, b)
+    v, p, rec = (t.cpu().numpy() for t in out["dense"])
+    v_ref, p_ref = vel.copy(), pos.copy()
+    sub = lambda x: np.ascontiguousarray(x[:, :n])
+    vr, pr = sub(v_ref), sub(p_ref)
+    oracle.kick(vr, sub(acc), sub(grad), c=0.37, kappa=0.011)
+    oracle.kick(vr, sub(acc), None, c=-0.2, kappa=0.0)
+    oracle.drift(pr, vr, c=0.21)
+    np.testing.assert_allclose(v[:, :n], vr, rtol=0, atol=4e-16 * np.abs(vr).max())
+    np.testing.assert_allclose(p[:, :n], pr, rtol=0, atol=4e-16 * np.abs(pr).max())
+    assert np.array_equal(v[:, n:], vel[:, n:]) and np.array_equal(p[:, n:], pos[:, n:])
+    assert np.array_equal(rec[:n, :3], p[:, :n].T) and np.array_equal(rec[:n, 3], mass) and (rec[n:] == 0).all()
+
+
 @pytest.mark.parametrize("n,eps2", [(1, 0.0), (2, 0.0), (1000, 0.0), (5000, 1e-4), (20000, 0.0)])
 def test_diagnostics_match_oracle(fr, oracle, n, eps2):
     """frost_diagnostics (on-device E, P, L with an O(N^2) potential sweep) against

@@ -4,6 +4,8 @@ in seconds: ragged A tiles (1024 / 512 particles) and B tiles (128), several ban
 (scratch cap of 1-3 MiB), self, mutual (slow/fast) and time-step sweeps, softening, coincident
 particles, the central-mass-at-the-origin case that meets the zero padding, determinism.
 Tolerances as in test_gpu_parity.py (north_star; reading 19)."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -461,3 +463,59 @@ def test_equal_mass_variant_is_bitwise_the_general_kernels(frs, oracle):
         a, g = res[0][0].cpu().numpy(), res[0][1].cpu().numpy()
         assert (np.abs(a - a_ref).max(0) / np.linalg.norm(a_ref, axis=0)).max() < 1e-12
         assert (np.abs(g - g_ref).max(0) / np.linalg.norm(g_ref, axis=0)).max() < 1e-10
+
+
+@pytest.mark.parametrize("world,extra", [(2, []), (3, []), (2, ["--one-sided"])])
+def test_multi_rank_bench_path_on_one_device(oracle, tmp_path, world, extra):
+    """The N > 1 path of bench.py EXECUTED on the one GPU of the box: `world`
+    ranks under torch.distributed.run, all on cuda:0, process group gloo (NCCL refuses two ranks on a
+    device; the exchanges are staged through the host).  Every rank runs bench.py's own step -- its
+    share of the tile pairs (frost_set_shard) + all-reduce of a and of g, or with --one-sided its block
+    of sinks + all-gather of a -- and saves the sharded pass at the initial positions.  Checked: one JSON
+    line with n_gpus = world and an end-to-end number; every rank holds the same complete a (bitwise);
+    a and g equal the unsharded call to 1e-12 / 1e-10 and the oracle (scatter, compute,
+    gather)."""
+    import json
+    import subprocess
+    import sys
+    import paper_2011_14984_b200 as frost
+    n = 20000
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    cmd = [sys.executable, os.path.join(root, "bench.py"), "--gpus", str(world), "--backend", "gloo",
+           "--same-device", "--n", str(n), "--steps", "1", "--warmup", "1", "--e2e-steps", "1", "--no-rows",
+           "--cpu-sinks", "256", "--dump-dir", str(tmp_path)] + extra
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=900)
+    assert r.returncode == 0, r.stderr[-3000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1, r.stdout[-2000:]
+    out = json.loads(lines[0])
+    assert out["n_gpus"] == world and out["value"] > 0 and out["e2e"]["value"] > 0
+    assert out["e2e"]["h2d_bytes_per_step"] == world * 32 * n and out["e2e"]["d2h_bytes_per_step"] == 48 * n
+    par = out["cpu_baseline"]["parity_of_the_sharded_pass"]
+    assert par["acc_rel_err"] < 1e-12 and par["grad_rel_err"] < 1e-10
+
+    pos, vel, mass = fi.plummer(n, 2)                     # bench.py's input: seed 2
+    a_ref, g_ref = oracle.forces(pos, mass)
+    fr = frost.Frost()
+    try:
+        if extra:
+            fr.set_symmetric(1)
+        one_a, one_g = fr.forces(dev(pos), dev(mass))
+        torch.cuda.synchronize()
+        one_a, one_g = one_a.cpu().numpy(), one_g.cpu().numpy()
+    finally:
+        fr.close()
+    na, ng = np.linalg.norm(a_ref, axis=0), np.linalg.norm(g_ref, axis=0)
+    dumps = [np.load(os.path.join(tmp_path, f"rank{k}.npz")) for k in range(world)]
+    for d in dumps:
+        assert np.array_equal(d["acc"], dumps[0]["acc"])            # the exchange leaves every rank with the same a
+        assert (np.abs(d["acc"] - a_ref).max(0) / na).max() < 1e-12
+        assert (np.abs(d["acc"] - one_a).max(0) / na).max() < 1e-12
+        lo, hi = (0, n) if not extra else (int(d["lo"]), int(d["hi"]))   # sink sharding: g of the own block only
+        assert (np.abs(d["grad"] - g_ref)[:, lo:hi].max(0) / ng[lo:hi]).max() < 1e-10
+        assert (np.abs(d["grad"] - one_g)[:, lo:hi].max(0) / ng[lo:hi]).max() < 1e-10
+        if extra:                                                       # one-sided kernels: same bits per sink
+            assert np.array_equal(d["acc"], one_a) and np.array_equal(d["grad"][:, lo:hi], one_g[:, lo:hi])
+    if not extra:
+        for d in dumps:
+            assert np.array_equal(d["grad"], dumps[0]["grad"])
