@@ -13,7 +13,7 @@ One "pair interaction" = one ordered pair visited once by each of the two sweeps
 Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.  With --gpus N > 1 and
 no torchrun environment the script re-launches itself under torch.distributed.run with N ranks
 (one per GPU, NCCL).  Side modes used by the commands in profiles/*.md (no JSON line):
-    --probe          print the FP64 issue-model table of this GPU (frost_fp64_probe, CUDA events)
+    --probe          print the FP64 issue-model table of this GPU (libfrost_probe.so, CUDA events)
     --rows-only      launch every O(N) kernel and the three time-step sweeps once or twice (for ncu)
     --subtree K      the device-resident subtree kernel on K/2 hard binaries (for ncu)
     --hhs-only       one HHS-FSI step of config 5 (N = 262144) with its validity numbers
@@ -70,6 +70,27 @@ def _peaks():
         d = json.load(open(path))
         return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured"
     return 6650.0, 1965.0, "fallback"
+
+
+_probe_lib = None
+
+
+def fp64_probe(device, stream, mode, iters, blocks_per_sm, scratch):
+    """frost_fp64_probe of libfrost_probe.so (paper_2011_14984_b200/probe/: measurement code, its own
+    library, not part of the product ABI); returns the thread-level FP64 instructions it executes."""
+    global _probe_lib
+    import ctypes as C
+    if _probe_lib is None:
+        from paper_2011_14984_b200 import build as b
+        _probe_lib = C.CDLL(b.build_probe())
+        _probe_lib.frost_fp64_probe.argtypes = [C.c_int, C.c_void_p, C.c_int, C.c_int, C.c_int, C.c_void_p,
+                                                C.POINTER(C.c_int64)]
+    n = C.c_int64()
+    rc = _probe_lib.frost_fp64_probe(device, C.c_void_p(stream.cuda_stream), mode, iters, blocks_per_sm,
+                                     C.c_void_p(scratch.data_ptr()), C.byref(n))
+    if rc != 0:
+        raise RuntimeError(f"frost_fp64_probe: status {rc}")
+    return int(n.value)
 
 
 class ClockSampler:
@@ -416,18 +437,18 @@ def run_probe():
     print(f"# {'probe':78s} cyc/FP64-inst  extra cyc per extra instr")
     base = None
     for mode, name, extras in modes:
-        fr.fp64_probe(mode, 2000, 4, scratch); torch.cuda.synchronize()
+        fp64_probe(fr.device, fr.stream, mode, 2000, 4, scratch); torch.cuda.synchronize()
         a, b = ev(), ev()
-        a.record(); ninst = fr.fp64_probe(mode, 40000, 4, scratch); b.record(); torch.cuda.synchronize()
+        a.record(); ninst = fp64_probe(fr.device, fr.stream, mode, 40000, 4, scratch); b.record(); torch.cuda.synchronize()
         cyc = a.elapsed_time(b) * 1e-3 * mhz * 1e6 / (ninst / 32 / (sms * 4))
         if mode == 1:
             base = cyc
         extra = "" if not extras else f"{(cyc - base) * 16 / extras:6.2f}"
         print(f"  {name:78s} {cyc:6.3f}        {extra}")
     for mode, name in ((10, "DFMA"), (11, "DADD")):      # latency: 1 CTA of 8 warps per SM, one chain per thread
-        fr.fp64_probe(mode, 2000, 1, scratch); torch.cuda.synchronize()
+        fp64_probe(fr.device, fr.stream, mode, 2000, 1, scratch); torch.cuda.synchronize()
         a, b = ev(), ev()
-        a.record(); fr.fp64_probe(mode, 40000, 1, scratch); b.record(); torch.cuda.synchronize()
+        a.record(); fp64_probe(fr.device, fr.stream, mode, 40000, 1, scratch); b.record(); torch.cuda.synchronize()
         cyc = a.elapsed_time(b) * 1e-3 * mhz * 1e6 / (40000 * 64)
         print(f"  dependent {name} chain, 2 warps per sub-partition: {cyc:6.2f} cycles per instruction (latency)")
     fr.close()
@@ -705,9 +726,9 @@ def run_frost(args):
     scratch = torch.zeros(torch.cuda.get_device_properties(local).multi_processor_count * 8 * 256,
                           dtype=torch.float64, device=dev)
     for mode, nm in ((0, "dfma"), (3, "mixed")):
-        fr.fp64_probe(mode, 2000, 4, scratch); torch.cuda.synchronize()
+        fp64_probe(fr.device, fr.stream, mode, 2000, 4, scratch); torch.cuda.synchronize()
         a, b = ev(), ev()
-        a.record(); ninst = fr.fp64_probe(mode, 60000, 4, scratch); b.record(); torch.cuda.synchronize()
+        a.record(); ninst = fp64_probe(fr.device, fr.stream, mode, 60000, 4, scratch); b.record(); torch.cuda.synchronize()
         probe[nm + "_thread_inst_per_s"] = ninst / (a.elapsed_time(b) * 1e-3)
 
     sm_mhz = (clocks or {}).get("sm_mhz") or sm_max_mhz

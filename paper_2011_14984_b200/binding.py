@@ -23,7 +23,7 @@ exported_symbols = [
     "frost_create", "frost_destroy", "frost_set_params", "frost_forces", "frost_forces_host",
     "frost_timesteps", "frost_partition", "frost_kick", "frost_drift", "frost_fsi_step",
     "frost_hhs_step", "frost_gather_pack", "frost_launch_count", "frost_last_cuda_error",
-    "frost_strerror", "frost_version", "frost_set_tuning", "frost_fp64_probe", "frost_set_symmetric",
+    "frost_strerror", "frost_version", "frost_set_tuning", "frost_set_symmetric",
     "frost_diagnostics", "frost_set_shard", "frost_fsi_steps", "frost_set_overlap",
     "frost_set_split", "frost_forces_masked", "frost_set_pair_path",
     "frost_set_gradient_guard", "frost_set_equal_mass_path",
@@ -90,7 +90,6 @@ def load_library():
     lib.frost_fsi_steps.argtypes = [vp, i32, i32, vp, vp, vp, vp, i32, f64, i32]
     lib.frost_hhs_step.argtypes = [vp, i32, i32, vp, vp, vp, f64, vp]
     lib.frost_gather_pack.argtypes = [vp, i32, i32, vp, vp, vp, i32, i32, vp]
-    lib.frost_fp64_probe.argtypes = [vp, i32, i32, i32, vp, vp]
     lib.frost_acc_noalloc.argtypes = [i32, vp, i32, i32, vp, vp, f64, f64, vp, C.POINTER(C.c_int)]
     lib.frost_noalloc_max_n.argtypes = []
     lib.frost_launch_count.argtypes = [vp]
@@ -348,16 +347,6 @@ class Frost:
                                                _p(mass), _p(out_phi), out), "frost_diagnostics")
         o = list(out)
         return {"T": o[0], "U": o[1], "E": o[0] + o[1], "P": o[2:5], "L": o[5:8]}
-
-    def fp64_probe(self, mode=0, iters=4096, blocks_per_sm=4, scratch=None):
-        if scratch is None:
-            sms = torch.cuda.get_device_properties(self.device).multi_processor_count
-            scratch = torch.zeros(sms * max(blocks_per_sm, 1) * 256, dtype=torch.float64,
-                                  device=torch.device("cuda", self.device))
-        n = C.c_int64()
-        self._check(self.lib.frost_fp64_probe(self.h, mode, iters, blocks_per_sm, _p(scratch),
-                                              C.byref(n)), "frost_fp64_probe")
-        return int(n.value)
 
     def gather_pack(self, pos, mass, idx=None, n_pad=None):
         _vec(pos, "pos")

@@ -1,7 +1,9 @@
 """Build libfrost_b200.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
 Every csrc/*.cu is compiled to its own object (in parallel, only when stale) under
-paper_2011_14984_b200/build/, then linked with the static CUDA runtime."""
+paper_2011_14984_b200/build/, then linked with the static CUDA runtime.  probe/frost_probe.cu (the
+FP64 issue-rate probe bench.py times) becomes its own libfrost_probe.so: measurement code stays out
+of the product library."""
 import glob
 import os
 import subprocess
@@ -12,6 +14,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libfrost_b200.so")
+PROBE_SRC = os.path.join(HERE, "probe", "frost_probe.cu")
+PROBE_LIB = os.path.join(HERE, "libfrost_probe.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 CFLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
           "-Xcompiler", "-fPIC"]
@@ -38,7 +42,15 @@ def _newer(deps, target):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+def build_probe(force: bool = False) -> str:
+    deps = [PROBE_SRC, os.path.join(HERE, "probe", "frost_probe.h")]
+    if force or _newer(deps, PROBE_LIB):
+        subprocess.check_call([NVCC] + CFLAGS + ["-shared", "-cudart", "static", "-o", PROBE_LIB, PROBE_SRC])
+    return PROBE_LIB
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    build_probe(force)
     hdr = _headers()
     if not force and not _newer(sources() + hdr, LIB):
         return LIB                      # (a box that received the built library never recompiles)
@@ -53,7 +65,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 1)) as ex:
             list(ex.map(compile_one, todo))
     objs = [_obj(s) for s in sources()]
-    if todo or _newer(objs, LIB):
+    stale = [o for o in glob.glob(os.path.join(OBJ, "*.o")) if o not in objs]
+    for o in stale:                     # the object of a source file that no longer exists
+        os.remove(o)
+    if todo or stale or _newer(objs, LIB):
         subprocess.check_call([NVCC] + LFLAGS + ["-o", LIB] + objs)
     return LIB
 

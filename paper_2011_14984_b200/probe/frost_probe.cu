@@ -3,8 +3,11 @@
 // plain "one warp instruction per 2 cycles" unit: these probes measure what the sweep kernels
 // are bounded by.  bench.py times modes 0/3 next to the headline
 // number; `python bench.py --probe` prints the whole table.
-#include "../../include/frost_probe.h"
-#include "frost_common.cuh"
+//
+// Built into its own library (libfrost_probe.so, bench only): not part of the product's C-ABI.
+#include <cuda_runtime.h>
+
+#include "frost_probe.h"
 
 namespace frost {
 
@@ -84,14 +87,18 @@ __global__ void __launch_bounds__(256) fp64_probe_kernel(double *out, int iters,
 
 }  // namespace frost
 
-extern "C" int frost_fp64_probe(frost_ctx *c, int mode, int iters, int blocks_per_sm, double *scratch,
+extern "C" int frost_fp64_probe(int device, void *stream, int mode, int iters, int blocks_per_sm, double *scratch,
                                 int64_t *out_instr) {
     using namespace frost;
-    if (!c || !scratch || iters < 1 || blocks_per_sm < 1 || mode < 0 || mode > 11) return FROST_EINVAL;
-    FROST_DEVICE(c);
-    const int grid = c->num_sms * blocks_per_sm;
+    if (!scratch || iters < 1 || blocks_per_sm < 1 || mode < 0 || mode > 11) return -1;
+    int prev = -1, sms = 0;
+    if (cudaGetDevice(&prev) != cudaSuccess) return -2;
+    if (prev != device && cudaSetDevice(device) != cudaSuccess) return -2;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) return -2;
+    const int grid = sms * blocks_per_sm;
+    cudaStream_t st = (cudaStream_t)stream;
 #define FROST_PROBE_CASE(M) \
-    case M: fp64_probe_kernel<M><<<grid, 256, 0, c->stream>>>(scratch, iters, 0.5); break;
+    case M: fp64_probe_kernel<M><<<grid, 256, 0, st>>>(scratch, iters, 0.5); break;
     switch (mode) {
         FROST_PROBE_CASE(0) FROST_PROBE_CASE(1) FROST_PROBE_CASE(2) FROST_PROBE_CASE(3)
         FROST_PROBE_CASE(4) FROST_PROBE_CASE(5) FROST_PROBE_CASE(6) FROST_PROBE_CASE(7)
@@ -99,5 +106,7 @@ extern "C" int frost_fp64_probe(frost_ctx *c, int mode, int iters, int blocks_pe
     }
 #undef FROST_PROBE_CASE
     if (out_instr) *out_instr = (int64_t)grid * 256 * (int64_t)iters * 64;   // thread-level FP64 instructions
-    return check_launch(c);
+    const cudaError_t e = cudaGetLastError();
+    if (prev != device) cudaSetDevice(prev);
+    return e == cudaSuccess ? 0 : -2;
 }
